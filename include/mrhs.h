@@ -1,0 +1,190 @@
+/*
+ * mrhs.h -- C ABI of the B200-native MRHS Wilson-clover stencil library.
+ *
+ * One data-parallel hot path of arxiv 2211.13719 ("MRHS multigrid solver for
+ * Wilson-clover fermions"): the Wilson-clover stencil operators applied to
+ * N_rhs right-hand sides at once, with the RHS index innermost so that each
+ * gauge link, clover block or coarse link matrix fetched from HBM serves every
+ * RHS (PAPER.md:23 benefit (i), "RHS index in the fifth dimension").
+ * The paper prints no formula; the definitions implemented are the readings
+ * S1-S8 of SURVEY.md Sec. 8(c), restated in DESIGN.md.
+ *
+ * Conventions common to every entry point
+ *  - "d_" pointers are DEVICE pointers, "h_" pointers are HOST pointers.
+ *  - All field data is single precision complex (two fp32).
+ *  - Return value: MRHS_OK or an error code; never throws, never aborts.
+ *    mrhs_last_error() returns a thread-local message for the last failure.
+ *  - Applies enqueue work on the handle's stream and return without
+ *    synchronising.  Asynchronous faults surface at the caller's next sync.
+ *  - Handles are not thread-safe.  The current device at create time is the
+ *    handle's device.  One GPU, periodic boundaries handled in-kernel, no
+ *    communication (BASELINE.json north_star).
+ *  - create copies/repacks gauge, clover and coarse links into device memory
+ *    OWNED by the handle; the caller may free its buffers after create returns
+ *    (create synchronises the stream before returning).  Field buffers are
+ *    caller-owned, 16-byte aligned, and d_in must not alias d_out.
+ *
+ * Canonical layouts (C order, last index fastest):
+ *   site    lex = x + X*(y + Y*(z + Z*t)), extents even and >= 2, periodic
+ *   spinor  psi[lex][spin 4][colour 3][rhs N]   complex64 (re,im interleaved)
+ *   checkerboarded spinor of parity p: the V/2 sites with (x+y+z+t)%2 == p in
+ *           increasing lex order (index lex >> 1)
+ *   gauge   U[lex][mu 4][row 3][col 3], mu = x,y,z,t; U_mu(x) links x -> x+mu
+ *   clover  C[lex][chirality 2][6][6], block index 3*(spin%2)+colour
+ *   coarse links  A[lex][p 9][row nb][col nb]; p=0 self, 1..4 = +x..+t, 5..8 = -x..-t
+ *   coarse vector v[lex][nb][rhs N]
+ *
+ * Native layouts (what the timed applies read and write).
+ * Fine fields (ncomp == 12):
+ *   x-lines are cut in blocks of XB = mrhs_xblock(X_eff, N) sites (largest divisor of X_eff
+ *   with XB <= 16 and XB * threads-per-site <= 48), X_eff = X
+ *   for a full field and X/2 for a checkerboarded one (site xh of a parity-p
+ *   line has x = 2*xh + ((p+y+z+t)&1)).  Block b = xb + (X_eff/XB)*(y + Y*(z + Z*t)).
+ *   float index = ((b*12 + comp)*XB + x_in)*2N + e, comp = 3*spin + colour, with
+ *     N even: e = 4*(r/2) + (r&1) + 2*im   (RHS pairs stored re0 re1 im0 im1)
+ *     N odd : e = 2*r + im
+ *   i.e. the RHS index is fastest, then the site inside the block, then the
+ *   spin-colour component, so that a warp reads 512 contiguous bytes per load.
+ * Coarse fields (ncomp == nbasis): v[lex][nb][rhs] with the same RHS-pair
+ *   element order e as above (site-contiguous, fetched by bulk copies).
+ * The helpers below convert; the applies never do.
+ */
+#ifndef MRHS_H
+#define MRHS_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mrhs_wilson mrhs_wilson_t;   /* opaque: owns packed gauge + clover  */
+typedef struct mrhs_coarse mrhs_coarse_t;   /* opaque: owns packed coarse links    */
+
+typedef enum {
+    MRHS_OK = 0,
+    MRHS_ERR_INVALID_ARG = 1,   /* NULL pointer, odd or < 2 extent, bad parity, misalignment, aliasing */
+    MRHS_ERR_UNSUPPORTED = 2,   /* N_rhs or nbasis without a compiled specialisation */
+    MRHS_ERR_ALLOC = 3,         /* device or host allocation failed */
+    MRHS_ERR_CUDA = 4           /* a CUDA runtime call or kernel launch failed */
+} mrhs_status_t;
+
+/* Parity arguments: 0 = even sites, 1 = odd sites, 2 = full lattice. */
+#define MRHS_EVEN 0
+#define MRHS_ODD 1
+#define MRHS_FULL 2
+
+/* ------------------------------------------------------------------ fine level */
+
+/* Build a fine-level handle for lattice dims = {X,Y,Z,T} and N_rhs = nrhs
+ * (1..128; UNSUPPORTED above).
+ *   d_gauge : device, canonical gauge field, required.
+ *   d_clover: device, canonical clover blocks, or NULL.  NULL => the blocks
+ *             M_ooee(x) = (4+mass) - (csw/2) sum_{mu<nu} sigma_munu F_munu(x)
+ *             (readings S5-S7) are built on the device from d_gauge, mass, csw.
+ *             When given, mass and csw are not used by mrhs_mooee.
+ *   cuda_stream: a cudaStream_t (NULL = default stream); every later apply on
+ *             this handle is enqueued on it.
+ * PAPER.md:43 (D_hop, M_eooe), PAPER.md:47,:53 (precomputed clover term). */
+mrhs_status_t mrhs_wilson_create(mrhs_wilson_t **out, const int dims[4], int nrhs,
+                                 float mass, float csw,
+                                 const void *d_gauge, const void *d_clover,
+                                 void *cuda_stream);
+
+/* D_hop on the full lattice (reading S3):
+ *   out(x) = sum_mu (1-gamma_mu) U_mu(x) in(x+mu) + (1+gamma_mu) U_mu(x-mu)^+ in(x-mu)
+ * bare sum (no -1/2, no mass), 1320 flops per site per RHS.
+ * d_in, d_out: native full-lattice fields, mrhs_field_bytes(dims,12,nrhs,0) each. */
+mrhs_status_t mrhs_dhop(mrhs_wilson_t *h, const void *d_in, void *d_out);
+
+/* M_eooe (reading S4): the same sum evaluated at the V/2 sites of
+ * parity out_parity (0 or 1), reading the checkerboarded field of the other
+ * parity.  d_in, d_out: native checkerboarded fields. */
+mrhs_status_t mrhs_meooe(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity);
+
+/* M_ooee (readings S6, S7): out(x) = C(x) in(x), two 6x6
+ * Hermitian chiral blocks per site, includes the (4+mass) diagonal.
+ * parity 0/1: checkerboarded fields of that parity; 2: full-lattice fields. */
+mrhs_status_t mrhs_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity);
+
+/* Schur-style sequence of config 5, three launches
+ * back to back on the handle's stream with no host synchronisation:
+ *   tmp_o = M_eooe(in_e -> odd); tmp2_o = M_ooee(tmp_o); out_e = M_eooe(tmp2_o -> even).
+ * d_in, d_out: even checkerboarded native fields; d_tmp0, d_tmp1: odd ones. */
+mrhs_status_t mrhs_schur_sequence(mrhs_wilson_t *h, const void *d_in, void *d_tmp0,
+                                  void *d_tmp1, void *d_out);
+
+/* Copy the handle's native clover blocks back in canonical form
+ * d_clover_out[lex][2][6][6] complex64 (parity check of the device-side
+ * construction, row a0). */
+mrhs_status_t mrhs_wilson_export_clover(mrhs_wilson_t *h, void *d_clover_out);
+
+/* Optional tuning knobs (defaults are chosen at create from the lattice, N_rhs
+ * and the L2 size).  which: 0 = D_hop (full), 1 = M_eooe (checkerboarded).
+ * tile = {by, bz, bt}: sites per thread-block tile in y,z,t (x extent is the
+ * layout block XB); chunk = {cy, cz}: tiles per L2 sweep chunk in y and z.
+ * Each must divide the lattice accordingly; INVALID_ARG otherwise. */
+mrhs_status_t mrhs_wilson_set_tiling(mrhs_wilson_t *h, int which, const int tile[3], const int chunk[2]);
+mrhs_status_t mrhs_wilson_get_tiling(mrhs_wilson_t *h, int which, int tile[3], int chunk[2]);
+
+mrhs_status_t mrhs_wilson_destroy(mrhs_wilson_t *h);
+
+/* ---------------------------------------------------------------- coarse level */
+
+/* Coarse-level handle (reading S8; PAPER.md:61 nbasis, PAPER.md:75 coarse hopping).
+ *   cdims: coarse lattice extents (>= 2; need not be even), nbasis in {24, 40},
+ *   nrhs in {1,2,4,8,12,16,24,32,48,64,96};
+ *   d_links: device, canonical A[lex][9][nb][nb];
+ *   math_mode: 0 = FP32 FMA, 1 = tensor-core split precision (same tolerance). */
+mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nbasis, int nrhs,
+                                 const void *d_links, int math_mode, void *cuda_stream);
+
+/* out_i(x) = sum_{p=0..8} sum_j A_p(x)_ij in_j(x + delta_p), periodic;
+ * 72 nb^2 flops per site per RHS.  d_in, d_out: native coarse vectors. */
+mrhs_status_t mrhs_coarse_apply(mrhs_coarse_t *h, const void *d_in, void *d_out);
+
+mrhs_status_t mrhs_coarse_destroy(mrhs_coarse_t *h);
+
+/* ------------------------------------------------- layout helpers (untimed) */
+
+/* Layout block extent along x for a line of x_eff sites and N_rhs = nrhs. */
+int mrhs_xblock(int x_eff, int nrhs);
+
+/* Bytes of a native field: ncomp = 12 (fine) or nbasis (coarse);
+ * checkerboarded != 0 => one parity (V/2 sites).  0 on invalid arguments. */
+size_t mrhs_field_bytes(const int dims[4], int ncomp, int nrhs, int checkerboarded);
+
+/* canonical -> native and back.  parity 0/1: checkerboarded field of that
+ * parity (canonical side has V/2 sites in lex>>1 order); 2: full field.
+ * Pure data movement, bit-exact round trip. */
+mrhs_status_t mrhs_field_import(const int dims[4], int ncomp, int nrhs, int parity,
+                                const void *d_canonical, void *d_native, void *cuda_stream);
+mrhs_status_t mrhs_field_export(const int dims[4], int ncomp, int nrhs, int parity,
+                                const void *d_native, void *d_canonical, void *cuda_stream);
+
+/* full native <-> (even native, odd native). */
+mrhs_status_t mrhs_cb_split(const int dims[4], int ncomp, int nrhs, const void *d_full,
+                            void *d_even, void *d_odd, void *cuda_stream);
+mrhs_status_t mrhs_cb_merge(const int dims[4], int ncomp, int nrhs, const void *d_even,
+                            const void *d_odd, void *d_full, void *cuda_stream);
+
+/* ------------------------------------------- host-buffer (end-to-end) entries */
+
+/* One operator apply with HOST buffers in CANONICAL layout: host->device copy,
+ * import, the same kernel the device entry launches, export, device->host copy,
+ * then a stream synchronise.  op: 0 = D_hop, 1 = M_eooe, 2 = M_ooee.
+ * parity: out parity for op 1; field parity (0,1,2) for op 2; ignored for op 0.
+ * Staging buffers are owned by the handle and allocated on first use. */
+mrhs_status_t mrhs_wilson_apply_host(mrhs_wilson_t *h, int op, int parity,
+                                     const void *h_in, void *h_out);
+mrhs_status_t mrhs_coarse_apply_host(mrhs_coarse_t *h, const void *h_in, void *h_out);
+
+/* ------------------------------------------------------------------- errors */
+
+const char *mrhs_last_error(void);   /* thread-local, valid until the next call */
+const char *mrhs_version(void);      /* build string incl. target arch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MRHS_H */

@@ -1,0 +1,299 @@
+"""Python binding of the B200-native MRHS Wilson-clover stencil library (include/mrhs.h).
+
+Argument marshalling only: every operator step runs in the CUDA kernels of ``libmrhs.so``
+(built in-tree by ``python -m paper_2211_13719_b200.build``).  PyTorch supplies device memory
+and streams.  There is no CPU fallback: loading fails loudly if the library is missing.
+
+The functions carry the names of the C entry points without the ``mrhs_`` prefix
+(``wilson_create``, ``dhop``, ``meooe``, ``mooee``, ``coarse_create``, ``coarse_apply``, ...);
+``Wilson`` and ``Coarse`` are thin handle owners around them.
+
+Canonical layouts (complex64 torch tensors): spinor [sites][4][3][N], gauge [V][4][3][3],
+clover [V][2][6][6], coarse links [V][9][nb][nb], coarse vector [V][nb][N]; the timed applies
+work on NATIVE fields (opaque float32 tensors made by ``field_import``).  PAPER.md:25, :43-53, :75.
+"""
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libmrhs.so")
+_lib = None
+
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA = 0, 1, 2, 3, 4
+EVEN, ODD, FULL = 0, 1, 2
+OP_DHOP, OP_MEOOE, OP_MOOEE = 0, 1, 2
+
+_vp = ctypes.c_void_p
+_int4 = ctypes.c_int * 4
+_int3 = ctypes.c_int * 3
+_int2 = ctypes.c_int * 2
+
+_SIGNATURES = {
+    "mrhs_wilson_create": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, ctypes.c_int, ctypes.c_float, ctypes.c_float, _vp, _vp, _vp]),
+    "mrhs_dhop": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_meooe": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
+    "mrhs_mooee": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
+    "mrhs_schur_sequence": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "mrhs_wilson_export_clover": (ctypes.c_int, [_vp, _vp]),
+    "mrhs_wilson_set_tiling": (ctypes.c_int, [_vp, ctypes.c_int, _int3, _int2]),
+    "mrhs_wilson_get_tiling": (ctypes.c_int, [_vp, ctypes.c_int, _int3, _int2]),
+    "mrhs_wilson_destroy": (ctypes.c_int, [_vp]),
+    "mrhs_coarse_create": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, ctypes.c_int, ctypes.c_int, _vp, ctypes.c_int, _vp]),
+    "mrhs_coarse_apply": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_coarse_destroy": (ctypes.c_int, [_vp]),
+    "mrhs_xblock": (ctypes.c_int, [ctypes.c_int, ctypes.c_int]),
+    "mrhs_field_bytes": (ctypes.c_size_t, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "mrhs_field_import": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]),
+    "mrhs_field_export": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]),
+    "mrhs_cb_split": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
+    "mrhs_cb_merge": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
+    "mrhs_wilson_apply_host": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _vp, _vp]),
+    "mrhs_coarse_apply_host": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_last_error": (ctypes.c_char_p, []),
+    "mrhs_version": (ctypes.c_char_p, []),
+}
+EXPORTED_SYMBOLS = tuple(_SIGNATURES)
+
+
+class MrhsError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("mrhs status %d: %s" % (status, message))
+        self.status = status
+
+
+def lib():
+    """The loaded C-ABI library.  Raises if it has not been built (no fallback exists)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError("libmrhs.so is missing: run `python -m paper_2211_13719_b200.build` "
+                              "(nvcc, sm_100a); there is no CPU fallback")
+        l = ctypes.CDLL(_LIB_PATH)
+        for name, (res, args) in _SIGNATURES.items():
+            f = getattr(l, name)
+            f.restype = res
+            f.argtypes = args
+        _lib = l
+    return _lib
+
+
+def last_error():
+    return lib().mrhs_last_error().decode()
+
+
+def version():
+    return lib().mrhs_version().decode()
+
+
+def _check(status):
+    if status != OK:
+        raise MrhsError(status, last_error())
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    return _vp(t.data_ptr())
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return None
+    return _vp(stream.cuda_stream)
+
+
+def _dims(dims):
+    return _int4(*[int(d) for d in dims])
+
+
+# ------------------------------------------------------------------ layout helpers
+
+def xblock(x_eff, nrhs):
+    return lib().mrhs_xblock(int(x_eff), int(nrhs))
+
+
+def field_bytes(dims, ncomp, nrhs, checkerboarded):
+    return lib().mrhs_field_bytes(_dims(dims), int(ncomp), int(nrhs), int(bool(checkerboarded)))
+
+
+def empty_field(dims, ncomp, nrhs, parity, device="cuda"):
+    """Uninitialised native field (float32 tensor of field_bytes/4 elements)."""
+    import torch
+    nbytes = field_bytes(dims, ncomp, nrhs, parity != FULL)
+    if nbytes == 0:
+        raise MrhsError(ERR_INVALID_ARG, "invalid field shape")
+    return torch.empty(nbytes // 4, dtype=torch.float32, device=device)
+
+
+def field_import(dims, ncomp, nrhs, parity, canonical, native=None, stream=None):
+    """canonical complex64 tensor -> native field (allocated if not given)."""
+    if native is None:
+        native = empty_field(dims, ncomp, nrhs, parity, canonical.device)
+    _check(lib().mrhs_field_import(_dims(dims), ncomp, nrhs, parity, _ptr(canonical), _ptr(native), _stream_ptr(stream)))
+    return native
+
+
+def field_export(dims, ncomp, nrhs, parity, native, canonical=None, stream=None):
+    """native field -> canonical complex64 tensor [sites][ncomp][nrhs] (allocated if not given)."""
+    import torch
+    if canonical is None:
+        nsites = int(dims[0]) * int(dims[1]) * int(dims[2]) * int(dims[3])
+        if parity != FULL:
+            nsites //= 2
+        canonical = torch.empty((nsites, ncomp, nrhs), dtype=torch.complex64, device=native.device)
+    _check(lib().mrhs_field_export(_dims(dims), ncomp, nrhs, parity, _ptr(native), _ptr(canonical), _stream_ptr(stream)))
+    return canonical
+
+
+def cb_split(dims, ncomp, nrhs, full, even, odd, stream=None):
+    _check(lib().mrhs_cb_split(_dims(dims), ncomp, nrhs, _ptr(full), _ptr(even), _ptr(odd), _stream_ptr(stream)))
+
+
+def cb_merge(dims, ncomp, nrhs, even, odd, full, stream=None):
+    _check(lib().mrhs_cb_merge(_dims(dims), ncomp, nrhs, _ptr(even), _ptr(odd), _ptr(full), _stream_ptr(stream)))
+
+
+# ------------------------------------------------------------------ fine level
+
+def wilson_create(dims, nrhs, mass, csw, gauge, clover=None, stream=None):
+    h = _vp()
+    _check(lib().mrhs_wilson_create(ctypes.byref(h), _dims(dims), int(nrhs), float(mass), float(csw),
+                                    _ptr(gauge), _ptr(clover), _stream_ptr(stream)))
+    return h
+
+
+def dhop(h, d_in, d_out):
+    _check(lib().mrhs_dhop(h, _ptr(d_in), _ptr(d_out)))
+
+
+def meooe(h, d_in, d_out, out_parity):
+    _check(lib().mrhs_meooe(h, _ptr(d_in), _ptr(d_out), int(out_parity)))
+
+
+def mooee(h, d_in, d_out, parity):
+    _check(lib().mrhs_mooee(h, _ptr(d_in), _ptr(d_out), int(parity)))
+
+
+def schur_sequence(h, d_in, d_tmp0, d_tmp1, d_out):
+    _check(lib().mrhs_schur_sequence(h, _ptr(d_in), _ptr(d_tmp0), _ptr(d_tmp1), _ptr(d_out)))
+
+
+def wilson_export_clover(h, clover_out):
+    _check(lib().mrhs_wilson_export_clover(h, _ptr(clover_out)))
+
+
+def wilson_set_tiling(h, which, tile, chunk):
+    _check(lib().mrhs_wilson_set_tiling(h, int(which), _int3(*[int(v) for v in tile]), _int2(*[int(v) for v in chunk])))
+
+
+def wilson_get_tiling(h, which):
+    tile, chunk = _int3(), _int2()
+    _check(lib().mrhs_wilson_get_tiling(h, int(which), tile, chunk))
+    return list(tile), list(chunk)
+
+
+def wilson_apply_host(h, op, parity, h_in, h_out):
+    """h_in / h_out: HOST tensors (canonical complex64, ideally pinned)."""
+    _check(lib().mrhs_wilson_apply_host(h, int(op), int(parity), _ptr(h_in), _ptr(h_out)))
+
+
+def wilson_destroy(h):
+    _check(lib().mrhs_wilson_destroy(h))
+
+
+# ------------------------------------------------------------------ coarse level
+
+def coarse_create(cdims, nbasis, nrhs, links, math_mode=0, stream=None):
+    h = _vp()
+    _check(lib().mrhs_coarse_create(ctypes.byref(h), _dims(cdims), int(nbasis), int(nrhs), _ptr(links),
+                                    int(math_mode), _stream_ptr(stream)))
+    return h
+
+
+def coarse_apply(h, d_in, d_out):
+    _check(lib().mrhs_coarse_apply(h, _ptr(d_in), _ptr(d_out)))
+
+
+def coarse_apply_host(h, h_in, h_out):
+    _check(lib().mrhs_coarse_apply_host(h, _ptr(h_in), _ptr(h_out)))
+
+
+def coarse_destroy(h):
+    _check(lib().mrhs_coarse_destroy(h))
+
+
+# ------------------------------------------------------------------ handle owners
+
+class Wilson:
+    """Owns a fine-level handle (packed gauge + clover on the device)."""
+
+    def __init__(self, dims, nrhs, mass, csw, gauge, clover=None, stream=None):
+        self.dims = [int(d) for d in dims]
+        self.nrhs = int(nrhs)
+        self.h = wilson_create(dims, nrhs, mass, csw, gauge, clover, stream)
+
+    def close(self):
+        if self.h is not None:
+            wilson_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def empty(self, parity, device="cuda"):
+        return empty_field(self.dims, 12, self.nrhs, parity, device)
+
+    def import_field(self, canonical, parity):
+        return field_import(self.dims, 12, self.nrhs, parity, canonical)
+
+    def export_field(self, native, parity):
+        out = field_export(self.dims, 12, self.nrhs, parity, native)
+        return out.reshape(out.shape[0], 4, 3, self.nrhs)
+
+    def dhop(self, d_in, d_out):
+        dhop(self.h, d_in, d_out)
+
+    def meooe(self, d_in, d_out, out_parity):
+        meooe(self.h, d_in, d_out, out_parity)
+
+    def mooee(self, d_in, d_out, parity):
+        mooee(self.h, d_in, d_out, parity)
+
+    def schur_sequence(self, d_in, d_tmp0, d_tmp1, d_out):
+        schur_sequence(self.h, d_in, d_tmp0, d_tmp1, d_out)
+
+
+class Coarse:
+    """Owns a coarse-level handle (packed link matrices on the device)."""
+
+    def __init__(self, cdims, nbasis, nrhs, links, math_mode=0, stream=None):
+        self.cdims = [int(d) for d in cdims]
+        self.nbasis = int(nbasis)
+        self.nrhs = int(nrhs)
+        self.h = coarse_create(cdims, nbasis, nrhs, links, math_mode, stream)
+
+    def close(self):
+        if self.h is not None:
+            coarse_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def empty(self, device="cuda"):
+        return empty_field(self.cdims, self.nbasis, self.nrhs, FULL, device)
+
+    def import_field(self, canonical):
+        return field_import(self.cdims, self.nbasis, self.nrhs, FULL, canonical)
+
+    def export_field(self, native):
+        return field_export(self.cdims, self.nbasis, self.nrhs, FULL, native)
+
+    def apply(self, d_in, d_out):
+        coarse_apply(self.h, d_in, d_out)

@@ -1,0 +1,353 @@
+// api.cu -- the C ABI of include/mrhs.h: handles, argument checks, error strings and the
+// host-buffer (end-to-end) entries.  Every operator step runs in the kernels of fine_hop.cu,
+// clover.cu and coarse.cu; nothing here computes.
+#include <cstring>
+#include <new>
+
+#include "coarse.cuh"
+#include "fine_hop.cuh"
+
+namespace mrhs {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+mrhs_status_t cuda_fail(cudaError_t e, const char *what, const char *file, int line) {
+    set_error("CUDA error %d (%s) at %s:%d in %s", (int)e, cudaGetErrorString(e), file, line, what);
+    return (e == cudaErrorMemoryAllocation) ? MRHS_ERR_ALLOC : MRHS_ERR_CUDA;
+}
+
+static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace mrhs
+
+using namespace mrhs;
+
+struct mrhs_wilson {
+    int dims[4];
+    int nrhs;
+    float mass, csw;
+    cudaStream_t st;
+    FieldGeom gfull, gcb[2];
+    float4 *gauge_full, *gauge_cb[2];
+    float4 *clov_full, *clov_cb[2];
+    HopParams hp_full, hp_cb[2];   // hp_cb[p]: output parity p
+    size_t l2_bytes;
+    // staging for the host-buffer entry
+    void *st_canon, *st_in, *st_out;
+    size_t st_bytes;
+};
+
+struct mrhs_coarse {
+    CoarseGeom g;
+    int mode;
+    cudaStream_t st;
+    float2 *links;
+    void *st_canon, *st_in, *st_out;
+    size_t st_bytes;
+};
+
+namespace {
+
+mrhs_status_t wilson_free(mrhs_wilson *h) {
+    if (!h) return MRHS_OK;
+    cudaFree(h->gauge_full); cudaFree(h->gauge_cb[0]); cudaFree(h->gauge_cb[1]);
+    cudaFree(h->clov_full); cudaFree(h->clov_cb[0]); cudaFree(h->clov_cb[1]);
+    cudaFree(h->st_canon); cudaFree(h->st_in); cudaFree(h->st_out);
+    delete h;
+    return MRHS_OK;
+}
+
+mrhs_status_t wilson_build(mrhs_wilson *h, const void *d_gauge, const void *d_clover) {
+    const size_t site_bytes = 72 * sizeof(float);
+    const size_t V = (size_t)h->gfull.nsites;
+    MRHS_CUDA(cudaMalloc(&h->gauge_full, V * site_bytes));
+    MRHS_CUDA(cudaMalloc(&h->clov_full, V * site_bytes));
+    for (int p = 0; p < 2; p++) {
+        MRHS_CUDA(cudaMalloc(&h->gauge_cb[p], V / 2 * site_bytes));
+        MRHS_CUDA(cudaMalloc(&h->clov_cb[p], V / 2 * site_bytes));
+    }
+    // the canonical gauge field already is [lex][72 floats]
+    mrhs_status_t s;
+    if ((s = pack_site_data(h->gfull, (const float *)d_gauge, h->gauge_full, h->st)) != MRHS_OK) return s;
+    for (int p = 0; p < 2; p++)
+        if ((s = pack_site_data(h->gcb[p], (const float *)d_gauge, h->gauge_cb[p], h->st)) != MRHS_OK) return s;
+    float *tmp = nullptr;
+    MRHS_CUDA(cudaMalloc(&tmp, V * site_bytes));
+    if (d_clover) s = pack_clover_blocks((long long)V, (const float2 *)d_clover, tmp, h->st);
+    else s = build_clover(h->dims, h->mass, h->csw, (const float2 *)d_gauge, tmp, h->st);
+    if (s == MRHS_OK) s = pack_site_data(h->gfull, tmp, h->clov_full, h->st);
+    for (int p = 0; p < 2 && s == MRHS_OK; p++) s = pack_site_data(h->gcb[p], tmp, h->clov_cb[p], h->st);
+    cudaError_t e = cudaStreamSynchronize(h->st);
+    cudaFree(tmp);
+    if (s != MRHS_OK) return s;
+    MRHS_CUDA(e);
+    return MRHS_OK;
+}
+
+mrhs_status_t wilson_set_default_tiling(mrhs_wilson *h) {
+    const size_t budget = h->l2_bytes * 2 / 5;
+    HopTiling tf = default_tiling(h->gfull, budget);
+    if (!build_hop_params(h->gfull, 0, tf, h->hp_full)) {
+        set_error("wilson create: no valid tiling for the full lattice");
+        return MRHS_ERR_UNSUPPORTED;
+    }
+    h->hp_full.gauge_out = h->hp_full.gauge_in = h->gauge_full;
+    for (int p = 0; p < 2; p++) {
+        HopTiling tc = default_tiling(h->gcb[p], budget);
+        if (!build_hop_params(h->gcb[p], p, tc, h->hp_cb[p])) {
+            set_error("wilson create: no valid tiling for the checkerboarded lattice");
+            return MRHS_ERR_UNSUPPORTED;
+        }
+        h->hp_cb[p].gauge_out = h->gauge_cb[p];
+        h->hp_cb[p].gauge_in = h->gauge_cb[1 - p];
+    }
+    return MRHS_OK;
+}
+
+bool fine_dims_ok(const int dims[4]) {
+    for (int i = 0; i < 4; i++)
+        if (dims[i] < 2 || (dims[i] & 1)) return false;
+    return true;
+}
+
+mrhs_status_t ensure_stage(void **canon, void **in, void **out, size_t *have, size_t need) {
+    if (*have >= need) return MRHS_OK;
+    cudaFree(*canon); cudaFree(*in); cudaFree(*out);
+    *canon = *in = *out = nullptr; *have = 0;
+    MRHS_CUDA(cudaMalloc(canon, need));
+    MRHS_CUDA(cudaMalloc(in, need));
+    MRHS_CUDA(cudaMalloc(out, need));
+    *have = need;
+    return MRHS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+mrhs_status_t mrhs_wilson_create(mrhs_wilson_t **out, const int dims[4], int nrhs, float mass, float csw,
+                                 const void *d_gauge, const void *d_clover, void *cuda_stream) {
+    MRHS_REQUIRE(out, "wilson create: out is NULL");
+    *out = nullptr;
+    MRHS_REQUIRE(dims && d_gauge, "wilson create: NULL argument");
+    MRHS_REQUIRE(fine_dims_ok(dims), "wilson create: extents must be even and >= 2");
+    MRHS_REQUIRE(nrhs >= 1, "wilson create: nrhs must be positive");
+    MRHS_REQUIRE(aligned16(d_gauge) && aligned16(d_clover), "wilson create: buffers must be 16-byte aligned");
+    if (nrhs > 128) {
+        set_error("wilson create: nrhs=%d unsupported (1..128)", nrhs);
+        return MRHS_ERR_UNSUPPORTED;
+    }
+    mrhs_wilson *h = new (std::nothrow) mrhs_wilson();
+    if (!h) { set_error("wilson create: host allocation failed"); return MRHS_ERR_ALLOC; }
+    memset(h, 0, sizeof(*h));
+    for (int i = 0; i < 4; i++) h->dims[i] = dims[i];
+    h->nrhs = nrhs; h->mass = mass; h->csw = csw;
+    h->st = (cudaStream_t)cuda_stream;
+    h->gfull = make_geom(dims, 12, nrhs, MRHS_FULL);
+    h->gcb[0] = make_geom(dims, 12, nrhs, MRHS_EVEN);
+    h->gcb[1] = make_geom(dims, 12, nrhs, MRHS_ODD);
+    int dev = 0, l2 = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev);
+    if (e != cudaSuccess) { wilson_free(h); return cuda_fail(e, "device query", __FILE__, __LINE__); }
+    h->l2_bytes = (size_t)l2;
+    mrhs_status_t s = wilson_build(h, d_gauge, d_clover);
+    if (s == MRHS_OK) s = wilson_set_default_tiling(h);
+    if (s != MRHS_OK) { wilson_free(h); return s; }
+    *out = h;
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_dhop(mrhs_wilson_t *h, const void *d_in, void *d_out) {
+    MRHS_REQUIRE(h && d_in && d_out, "dhop: NULL argument");
+    MRHS_REQUIRE(d_in != d_out, "dhop: in and out must not alias");
+    MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "dhop: buffers must be 16-byte aligned");
+    return launch_hop(h->hp_full, h->nrhs, d_in, d_out, h->st);
+}
+
+mrhs_status_t mrhs_meooe(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity) {
+    MRHS_REQUIRE(h && d_in && d_out, "meooe: NULL argument");
+    MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "meooe: out_parity must be 0 or 1");
+    MRHS_REQUIRE(d_in != d_out, "meooe: in and out must not alias");
+    MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "meooe: buffers must be 16-byte aligned");
+    return launch_hop(h->hp_cb[out_parity], h->nrhs, d_in, d_out, h->st);
+}
+
+mrhs_status_t mrhs_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity) {
+    MRHS_REQUIRE(h && d_in && d_out, "mooee: NULL argument");
+    MRHS_REQUIRE(parity >= 0 && parity <= 2, "mooee: parity must be 0, 1 or 2");
+    MRHS_REQUIRE(d_in != d_out, "mooee: in and out must not alias");
+    MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "mooee: buffers must be 16-byte aligned");
+    if (parity == MRHS_FULL) return launch_mooee(h->gfull, h->clov_full, d_in, d_out, h->st);
+    return launch_mooee(h->gcb[parity], h->clov_cb[parity], d_in, d_out, h->st);
+}
+
+mrhs_status_t mrhs_schur_sequence(mrhs_wilson_t *h, const void *d_in, void *d_tmp0, void *d_tmp1, void *d_out) {
+    MRHS_REQUIRE(h && d_in && d_tmp0 && d_tmp1 && d_out, "schur sequence: NULL argument");
+    MRHS_REQUIRE(d_in != d_out && d_tmp0 != d_tmp1 && d_in != d_tmp0 && d_in != d_tmp1 && d_out != d_tmp0 && d_out != d_tmp1,
+                 "schur sequence: the four buffers must be distinct");
+    mrhs_status_t s = mrhs_meooe(h, d_in, d_tmp0, MRHS_ODD);
+    if (s == MRHS_OK) s = mrhs_mooee(h, d_tmp0, d_tmp1, MRHS_ODD);
+    if (s == MRHS_OK) s = mrhs_meooe(h, d_tmp1, d_out, MRHS_EVEN);
+    return s;
+}
+
+mrhs_status_t mrhs_wilson_export_clover(mrhs_wilson_t *h, void *d_clover_out) {
+    MRHS_REQUIRE(h && d_clover_out, "export clover: NULL argument");
+    float *tmp = nullptr;
+    const size_t V = (size_t)h->gfull.nsites;
+    MRHS_CUDA(cudaMalloc(&tmp, V * 72 * sizeof(float)));
+    mrhs_status_t s = unpack_site_data(h->gfull, h->clov_full, tmp, h->st);
+    if (s == MRHS_OK) s = unpack_clover_blocks((long long)V, tmp, (float2 *)d_clover_out, h->st);
+    cudaError_t e = cudaStreamSynchronize(h->st);
+    cudaFree(tmp);
+    if (s != MRHS_OK) return s;
+    MRHS_CUDA(e);
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_wilson_set_tiling(mrhs_wilson_t *h, int which, const int tile[3], const int chunk[2]) {
+    MRHS_REQUIRE(h && tile && chunk, "set tiling: NULL argument");
+    MRHS_REQUIRE(which == 0 || which == 1, "set tiling: which must be 0 (D_hop) or 1 (M_eooe)");
+    HopTiling t = {tile[0], tile[1], tile[2], chunk[0], chunk[1]};
+    if (which == 0) {
+        HopParams p;
+        MRHS_REQUIRE(build_hop_params(h->gfull, 0, t, p), "set tiling: tiling does not fit the full lattice");
+        p.gauge_out = p.gauge_in = h->gauge_full;
+        h->hp_full = p;
+    } else {
+        HopParams p[2];
+        for (int q = 0; q < 2; q++) {
+            MRHS_REQUIRE(build_hop_params(h->gcb[q], q, t, p[q]), "set tiling: tiling does not fit the checkerboarded lattice");
+            p[q].gauge_out = h->gauge_cb[q];
+            p[q].gauge_in = h->gauge_cb[1 - q];
+        }
+        h->hp_cb[0] = p[0];
+        h->hp_cb[1] = p[1];
+    }
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_wilson_get_tiling(mrhs_wilson_t *h, int which, int tile[3], int chunk[2]) {
+    MRHS_REQUIRE(h && tile && chunk, "get tiling: NULL argument");
+    MRHS_REQUIRE(which == 0 || which == 1, "get tiling: which must be 0 (D_hop) or 1 (M_eooe)");
+    const HopParams &p = which == 0 ? h->hp_full : h->hp_cb[0];
+    tile[0] = p.by; tile[1] = p.bz; tile[2] = p.bt;
+    chunk[0] = p.cy; chunk[1] = p.cz;
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_wilson_destroy(mrhs_wilson_t *h) { return wilson_free(h); }
+
+mrhs_status_t mrhs_wilson_apply_host(mrhs_wilson_t *h, int op, int parity, const void *h_in, void *h_out) {
+    MRHS_REQUIRE(h && h_in && h_out, "apply host: NULL argument");
+    MRHS_REQUIRE(op >= 0 && op <= 2, "apply host: op must be 0 (D_hop), 1 (M_eooe) or 2 (M_ooee)");
+    int in_par = MRHS_FULL, out_par = MRHS_FULL;
+    if (op == 1) {
+        MRHS_REQUIRE(parity == 0 || parity == 1, "apply host: out parity must be 0 or 1");
+        out_par = parity; in_par = 1 - parity;
+    } else if (op == 2) {
+        MRHS_REQUIRE(parity >= 0 && parity <= 2, "apply host: parity must be 0, 1 or 2");
+        in_par = out_par = parity;
+    }
+    const size_t bytes = mrhs_field_bytes(h->dims, 12, h->nrhs, in_par != MRHS_FULL);
+    mrhs_status_t s = ensure_stage(&h->st_canon, &h->st_in, &h->st_out, &h->st_bytes, bytes);
+    if (s != MRHS_OK) return s;
+    MRHS_CUDA(cudaMemcpyAsync(h->st_canon, h_in, bytes, cudaMemcpyHostToDevice, h->st));
+    s = mrhs_field_import(h->dims, 12, h->nrhs, in_par, h->st_canon, h->st_in, h->st);
+    if (s != MRHS_OK) return s;
+    if (op == 0) s = mrhs_dhop(h, h->st_in, h->st_out);
+    else if (op == 1) s = mrhs_meooe(h, h->st_in, h->st_out, out_par);
+    else s = mrhs_mooee(h, h->st_in, h->st_out, parity);
+    if (s != MRHS_OK) return s;
+    s = mrhs_field_export(h->dims, 12, h->nrhs, out_par, h->st_out, h->st_canon, h->st);
+    if (s != MRHS_OK) return s;
+    MRHS_CUDA(cudaMemcpyAsync(h_out, h->st_canon, bytes, cudaMemcpyDeviceToHost, h->st));
+    MRHS_CUDA(cudaStreamSynchronize(h->st));
+    return MRHS_OK;
+}
+
+/* ---------------------------------------------------------------- coarse level */
+
+mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nbasis, int nrhs, const void *d_links,
+                                 int math_mode, void *cuda_stream) {
+    MRHS_REQUIRE(out, "coarse create: out is NULL");
+    *out = nullptr;
+    MRHS_REQUIRE(cdims && d_links, "coarse create: NULL argument");
+    for (int i = 0; i < 4; i++) MRHS_REQUIRE(cdims[i] >= 2, "coarse create: extents must be >= 2");
+    MRHS_REQUIRE(nbasis >= 1 && nrhs >= 1, "coarse create: nbasis and nrhs must be positive");
+    MRHS_REQUIRE(math_mode == 0 || math_mode == 1, "coarse create: math_mode must be 0 or 1");
+    MRHS_REQUIRE(aligned16(d_links), "coarse create: links must be 16-byte aligned");
+    if (!coarse_fma_supported(nbasis, nrhs)) {
+        set_error("coarse create: no specialisation for nbasis=%d nrhs=%d (nbasis 24|40, nrhs 1,2,4,8,12,16,24,32,48,64,96)", nbasis, nrhs);
+        return MRHS_ERR_UNSUPPORTED;
+    }
+    if (math_mode == 1) {
+        set_error("coarse create: the tensor-core variant is not built in this version");
+        return MRHS_ERR_UNSUPPORTED;
+    }
+    mrhs_coarse *h = new (std::nothrow) mrhs_coarse();
+    if (!h) { set_error("coarse create: host allocation failed"); return MRHS_ERR_ALLOC; }
+    memset(h, 0, sizeof(*h));
+    h->g.X = cdims[0]; h->g.Y = cdims[1]; h->g.Z = cdims[2]; h->g.T = cdims[3];
+    h->g.nb = nbasis; h->g.N = nrhs;
+    h->g.nsites = (long long)cdims[0] * cdims[1] * cdims[2] * cdims[3];
+    h->mode = math_mode;
+    h->st = (cudaStream_t)cuda_stream;
+    const size_t bytes = (size_t)h->g.nsites * 9 * nbasis * nbasis * sizeof(float2);
+    cudaError_t e = cudaMalloc(&h->links, bytes);
+    if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaMalloc(links)", __FILE__, __LINE__); }
+    mrhs_status_t s = pack_coarse_links(h->g, (const float2 *)d_links, h->links, h->st);
+    if (s == MRHS_OK) s = coarse_fma_prepare(h->g);
+    if (s == MRHS_OK) {
+        e = cudaStreamSynchronize(h->st);
+        if (e != cudaSuccess) s = cuda_fail(e, "cudaStreamSynchronize", __FILE__, __LINE__);
+    }
+    if (s != MRHS_OK) { cudaFree(h->links); delete h; return s; }
+    *out = h;
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_coarse_apply(mrhs_coarse_t *h, const void *d_in, void *d_out) {
+    MRHS_REQUIRE(h && d_in && d_out, "coarse apply: NULL argument");
+    MRHS_REQUIRE(d_in != d_out, "coarse apply: in and out must not alias");
+    MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "coarse apply: buffers must be 16-byte aligned");
+    return launch_coarse_fma(h->g, h->links, d_in, d_out, h->st);
+}
+
+mrhs_status_t mrhs_coarse_destroy(mrhs_coarse_t *h) {
+    if (!h) return MRHS_OK;
+    cudaFree(h->links);
+    cudaFree(h->st_canon); cudaFree(h->st_in); cudaFree(h->st_out);
+    delete h;
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_coarse_apply_host(mrhs_coarse_t *h, const void *h_in, void *h_out) {
+    MRHS_REQUIRE(h && h_in && h_out, "coarse apply host: NULL argument");
+    const int dims[4] = {h->g.X, h->g.Y, h->g.Z, h->g.T};
+    const size_t bytes = mrhs_field_bytes(dims, h->g.nb, h->g.N, 0);
+    mrhs_status_t s = ensure_stage(&h->st_canon, &h->st_in, &h->st_out, &h->st_bytes, bytes);
+    if (s != MRHS_OK) return s;
+    MRHS_CUDA(cudaMemcpyAsync(h->st_canon, h_in, bytes, cudaMemcpyHostToDevice, h->st));
+    s = mrhs_field_import(dims, h->g.nb, h->g.N, MRHS_FULL, h->st_canon, h->st_in, h->st);
+    if (s == MRHS_OK) s = mrhs_coarse_apply(h, h->st_in, h->st_out);
+    if (s == MRHS_OK) s = mrhs_field_export(dims, h->g.nb, h->g.N, MRHS_FULL, h->st_out, h->st_canon, h->st);
+    if (s != MRHS_OK) return s;
+    MRHS_CUDA(cudaMemcpyAsync(h_out, h->st_canon, bytes, cudaMemcpyDeviceToHost, h->st));
+    MRHS_CUDA(cudaStreamSynchronize(h->st));
+    return MRHS_OK;
+}
+
+const char *mrhs_last_error(void) { return g_err; }
+
+const char *mrhs_version(void) { return "mrhs-wilson-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

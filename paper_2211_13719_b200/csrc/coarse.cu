@@ -1,0 +1,252 @@
+// coarse.cu -- coarse-level 9-point stencil, FP32-FMA variant:
+//   out_i(x) = sum_{p=0..8} sum_j A_p(x)_ij v_j(x + delta_p)          (reading S8)
+// with nine independent dense nb x nb complex matrices per site, applied to N_rhs vectors at
+// once: each matrix entry fetched from HBM serves every RHS (PAPER.md:23 (i)).
+//
+// One thread block per coarse site.  The nine (A_p, v(x+delta_p)) pairs are streamed through a
+// ring of shared-memory stages with bulk async copies (one contiguous copy per matrix and per
+// neighbour vector) signalled on mbarriers.  A thread owns a TI x TP register tile of (rows, RHS
+// pairs) and, for small N_rhs, one of KS slices of the column range; slices are summed through
+// shared memory at the end.
+#include "coarse.cuh"
+#include "layout.cuh"
+
+namespace mrhs {
+
+namespace {
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok)
+                     : "r"(smem_u32(bar)), "r"(parity)
+                     : "memory");
+    } while (!ok);
+}
+
+template <int R> __device__ __forceinline__ CVec<R> czero_c();
+template <> __device__ __forceinline__ CVec<1> czero_c<1>() { return {{0.f}, {0.f}}; }
+template <> __device__ __forceinline__ CVec<2> czero_c<2>() { return {{0ull}, {0ull}}; }
+
+constexpr int largest_ks(int nb, int groups) {
+    int best = 1;
+    for (int k = 1; k <= nb; k++)
+        if (nb % k == 0 && groups * k <= 256) best = k;
+    return best;
+}
+
+template <int NB, int N>
+struct CoarseCfg {
+    static constexpr int R = (N % 2 == 0) ? 2 : 1;
+    static constexpr int NP = N / R;                       // RHS lanes (elements) per component
+    static constexpr int ITEMS = NB * NP;
+    static constexpr int TP = (ITEMS / 2 > 256 && NP % 2 == 0) ? 2 : 1;
+    static constexpr int TI = (ITEMS / (2 * TP) > 256) ? 4 : 2;
+    static constexpr int NPG = NP / TP;                    // pair groups
+    static constexpr int NRG = NB / TI;                    // row groups
+    static constexpr int GROUPS = NPG * NRG;
+    static constexpr int KS = largest_ks(NB, GROUPS);
+    static constexpr int THREADS = GROUPS * KS;
+    static constexpr int JS = NB / KS;                     // columns per slice
+    static constexpr int A_BYTES = NB * NB * 8;
+    static constexpr int V_BYTES = NB * N * 8;
+    static constexpr int STAGE_BYTES = A_BYTES + V_BYTES;
+    static constexpr int NSTAGE = STAGE_BYTES < 24 * 1024 ? 4 : 3;
+    static constexpr int RED_BYTES = (KS - 1) * GROUPS * TI * TP * R * 8;
+    static constexpr int DATA_BYTES = NSTAGE * STAGE_BYTES > RED_BYTES ? NSTAGE * STAGE_BYTES : RED_BYTES;
+    static constexpr int SMEM_BYTES = DATA_BYTES + 64;     // + mbarriers
+    static_assert(NB % TI == 0 && NP % TP == 0, "tile must divide the site");
+    static_assert(GROUPS <= 256 && THREADS <= 256, "too many work items for one block");
+    static_assert(A_BYTES % 16 == 0 && V_BYTES % 16 == 0, "bulk copies need 16-byte multiples");
+};
+
+template <int NB, int N>
+__global__ void __launch_bounds__(CoarseCfg<NB, N>::THREADS)
+coarse_fma_kernel(int X, int Y, int Z, int T, const float2 *__restrict__ links,
+                  const typename Elem<CoarseCfg<NB, N>::R>::type *__restrict__ in,
+                  typename Elem<CoarseCfg<NB, N>::R>::type *__restrict__ out) {
+    typedef CoarseCfg<NB, N> C;
+    constexpr int R = C::R, TI = C::TI, TP = C::TP;
+    typedef typename Elem<R>::type E;
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + C::DATA_BYTES);
+
+    const int tid = threadIdx.x;
+    const int pg = tid % C::NPG;
+    const int rg = (tid / C::NPG) % C::NRG;
+    const int ks = tid / C::GROUPS;
+
+    const long long site = blockIdx.x;
+    // neighbour sites of the nine stencil points: 0 self, 1..4 = +x..+t, 5..8 = -x..-t
+    auto neighbour = [&](int p) -> long long {
+        if (p == 0) return site;
+        int c[4];
+        long long s = site;
+        c[0] = (int)(s % X); s /= X;
+        c[1] = (int)(s % Y); s /= Y;
+        c[2] = (int)(s % Z);
+        c[3] = (int)(s / Z);
+        const int ext[4] = {X, Y, Z, T};
+        const int mu = (p - 1) & 3;
+        const int d = p <= 4 ? 1 : -1;
+        c[mu] = (c[mu] + d + ext[mu]) % ext[mu];
+        return c[0] + (long long)X * (c[1] + (long long)Y * (c[2] + (long long)Z * c[3]));
+    };
+    auto issue = [&](int p) {
+        const int slot = p % C::NSTAGE;
+        unsigned char *dst = smem + (size_t)slot * C::STAGE_BYTES;
+        mbar_expect_tx(&full[slot], C::STAGE_BYTES);
+        bulk_g2s(dst, links + ((size_t)site * 9 + p) * NB * NB, C::A_BYTES, &full[slot]);
+        bulk_g2s(dst + C::A_BYTES, in + (size_t)neighbour(p) * NB * C::NP, C::V_BYTES, &full[slot]);
+    };
+
+    if (tid == 0) {
+        for (int s = 0; s < C::NSTAGE; s++) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0)
+        for (int p = 0; p < C::NSTAGE && p < 9; p++) issue(p);
+
+    CVec<R> acc[TI][TP];
+#pragma unroll
+    for (int a = 0; a < TI; a++)
+#pragma unroll
+        for (int b = 0; b < TP; b++) acc[a][b] = czero_c<R>();
+
+    for (int p = 0; p < 9; p++) {
+        const int slot = p % C::NSTAGE;
+        mbar_wait(&full[slot], (p / C::NSTAGE) & 1);
+        const float2 *As = reinterpret_cast<const float2 *>(smem + (size_t)slot * C::STAGE_BYTES);   // [col][row]
+        const E *vs = reinterpret_cast<const E *>(smem + (size_t)slot * C::STAGE_BYTES + C::A_BYTES);  // [col][lane]
+        const float2 *ap = As + (size_t)(ks * C::JS) * NB + rg * TI;
+        const E *vp = vs + (size_t)(ks * C::JS) * C::NP + pg * TP;
+#pragma unroll 4
+        for (int j = 0; j < C::JS; j++) {
+            float2 a[TI];
+#pragma unroll
+            for (int i = 0; i < TI; i += 2) {
+                float4 t = *reinterpret_cast<const float4 *>(ap + j * NB + i);
+                a[i] = make_float2(t.x, t.y);
+                a[i + 1] = make_float2(t.z, t.w);
+            }
+            CVec<R> v[TP];
+#pragma unroll
+            for (int b = 0; b < TP; b++) v[b] = to_cvec(vp[j * C::NP + b]);
+#pragma unroll
+            for (int i = 0; i < TI; i++)
+#pragma unroll
+                for (int b = 0; b < TP; b++) acc[i][b] = cfma(a[i].x, a[i].y, v[b], acc[i][b]);
+        }
+        __syncthreads();   // every thread is done with this slot
+        if (tid == 0 && p + C::NSTAGE < 9) issue(p + C::NSTAGE);
+    }
+
+    // sum the column slices (the stage ring is free: the last __syncthreads above covers it)
+    if (C::KS > 1) {
+        E *red = reinterpret_cast<E *>(smem);
+        if (ks > 0) {
+            E *r = red + ((size_t)(ks - 1) * C::GROUPS + (tid % C::GROUPS)) * (TI * TP);
+#pragma unroll
+            for (int i = 0; i < TI; i++)
+#pragma unroll
+                for (int b = 0; b < TP; b++) r[i * TP + b] = from_cvec(acc[i][b]);
+        }
+        __syncthreads();
+        if (ks == 0) {
+            for (int k = 1; k < C::KS; k++) {
+                const E *r = red + ((size_t)(k - 1) * C::GROUPS + tid) * (TI * TP);
+#pragma unroll
+                for (int i = 0; i < TI; i++)
+#pragma unroll
+                    for (int b = 0; b < TP; b++) acc[i][b] = cadd(acc[i][b], to_cvec(r[i * TP + b]));
+            }
+        }
+    }
+    if (ks == 0) {
+        E *o = out + ((size_t)site * NB + rg * TI) * C::NP + pg * TP;
+#pragma unroll
+        for (int i = 0; i < TI; i++)
+#pragma unroll
+            for (int b = 0; b < TP; b++) o[(size_t)i * C::NP + b] = from_cvec(acc[i][b]);
+    }
+}
+
+__global__ void pack_links_kernel(int nb, const float2 *__restrict__ src, float2 *__restrict__ dst, long long total) {
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // native order: [mat][col][row]
+    if (idx >= total) return;
+    int row = (int)(idx % nb);
+    long long q = idx / nb;
+    int col = (int)(q % nb);
+    long long mat = q / nb;
+    dst[idx] = src[(mat * nb + row) * nb + col];
+}
+
+template <int NB, int N>
+mrhs_status_t launch_t(const CoarseGeom &g, const float2 *links, const void *in, void *out, cudaStream_t st) {
+    typedef CoarseCfg<NB, N> C;
+    typedef typename Elem<C::R>::type E;
+    coarse_fma_kernel<NB, N><<<(unsigned)g.nsites, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, links, (const E *)in, (E *)out);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+template <int NB, int N>
+mrhs_status_t prepare_t() {
+    typedef CoarseCfg<NB, N> C;
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_fma_kernel<NB, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    return MRHS_OK;
+}
+
+#define MRHS_COARSE_N_LIST(F, NB) \
+    F(NB, 1) F(NB, 2) F(NB, 4) F(NB, 8) F(NB, 12) F(NB, 16) F(NB, 24) F(NB, 32) F(NB, 48) F(NB, 64) F(NB, 96)
+
+}  // namespace
+
+bool coarse_fma_supported(int nb, int nrhs) {
+#define MRHS_CASE(NB, NN) if (nb == NB && nrhs == NN) return true;
+    MRHS_COARSE_N_LIST(MRHS_CASE, 24)
+    MRHS_COARSE_N_LIST(MRHS_CASE, 40)
+#undef MRHS_CASE
+    return false;
+}
+
+mrhs_status_t coarse_fma_prepare(const CoarseGeom &g) {
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return prepare_t<NB, NN>();
+    MRHS_COARSE_N_LIST(MRHS_CASE, 24)
+    MRHS_COARSE_N_LIST(MRHS_CASE, 40)
+#undef MRHS_CASE
+    set_error("coarse apply: no FP32-FMA specialisation for nbasis=%d nrhs=%d", g.nb, g.N);
+    return MRHS_ERR_UNSUPPORTED;
+}
+
+mrhs_status_t launch_coarse_fma(const CoarseGeom &g, const float2 *d_links, const void *d_in, void *d_out, cudaStream_t st) {
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return launch_t<NB, NN>(g, d_links, d_in, d_out, st);
+    MRHS_COARSE_N_LIST(MRHS_CASE, 24)
+    MRHS_COARSE_N_LIST(MRHS_CASE, 40)
+#undef MRHS_CASE
+    set_error("coarse apply: no FP32-FMA specialisation for nbasis=%d nrhs=%d", g.nb, g.N);
+    return MRHS_ERR_UNSUPPORTED;
+}
+
+mrhs_status_t pack_coarse_links(const CoarseGeom &g, const float2 *d_canonical, float2 *d_native, cudaStream_t st) {
+    long long total = g.nsites * 9 * g.nb * g.nb;
+    long long blocks = (total + 255) / 256;
+    pack_links_kernel<<<(unsigned)blocks, 256, 0, st>>>(g.nb, d_canonical, d_native, total);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+}  // namespace mrhs

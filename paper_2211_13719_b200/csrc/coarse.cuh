@@ -1,0 +1,23 @@
+// coarse.cuh -- host-side interface of the coarse-level 9-point stencil (SURVEY.md Sec. 8(a)
+// rows a5, a6; reading S8; PAPER.md:61 nbasis, PAPER.md:75 coarse hopping term).
+#pragma once
+#include "common.cuh"
+
+namespace mrhs {
+
+struct CoarseGeom {
+    int X, Y, Z, T;
+    int nb, N;
+    long long nsites;
+};
+
+// canonical A[site][p][row][col] -> native A[site][p][col][row] (one bulk copy per stencil point
+// lands the matrix so that a thread's TI consecutive rows of one column are contiguous).
+mrhs_status_t pack_coarse_links(const CoarseGeom &g, const float2 *d_canonical, float2 *d_native, cudaStream_t st);
+
+// true if an FP32-FMA specialisation for (nbasis, nrhs) is compiled
+bool coarse_fma_supported(int nb, int nrhs);
+mrhs_status_t coarse_fma_prepare(const CoarseGeom &g);   // opt in to large dynamic shared memory
+mrhs_status_t launch_coarse_fma(const CoarseGeom &g, const float2 *d_links, const void *d_in, void *d_out, cudaStream_t st);
+
+}  // namespace mrhs

@@ -1,0 +1,361 @@
+// fine_hop.cu -- the fine-level hopping kernel:
+//   out(x) = sum_mu (1-gamma_mu) U_mu(x) in(x+mu) + (1+gamma_mu) U_mu(x-mu)^+ in(x-mu)
+// (reading S3) for N_rhs right-hand sides at once.  One thread owns one output
+// site and R right-hand sides (R = 2 packed in FFMA2 lanes for even N_rhs), so the 18 reals of
+// a link are fetched once per site and reused by every RHS (PAPER.md:23 (i)).  Gamma matrices:
+// Hermitian chiral basis of reading S2; the spin projection to two-component half spinors and
+// the reconstruction are written out per direction below.
+#include "fine_hop.cuh"
+
+namespace mrhs {
+
+namespace {
+
+template <int R> __device__ __forceinline__ CVec<R> czero();
+template <> __device__ __forceinline__ CVec<1> czero<1>() { return {{0.f}, {0.f}}; }
+template <> __device__ __forceinline__ CVec<2> czero<2>() { return {{0ull}, {0ull}}; }
+
+__device__ __forceinline__ float2 ldg_nc(const float2 *p) { return __ldg(p); }
+__device__ __forceinline__ float4 ldg_nc(const float4 *p) { return __ldg(p); }
+
+// The 9 complex entries of link MU of one site.  Site data is [18][xin] float4 = 36 complex
+// entries e = 9*mu + 3*row + col, two per float4; g points at float4 0 of the site, stride XB.
+template <int MU>
+__device__ __forceinline__ void load_link(const float4 *__restrict__ g, int XB, float (&u)[18]) {
+    constexpr int e0 = 9 * MU;
+    if constexpr ((e0 & 1) == 0) {
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            float4 v = __ldg(g + (size_t)(e0 / 2 + j) * XB);
+            u[4 * j + 0] = v.x; u[4 * j + 1] = v.y; u[4 * j + 2] = v.z; u[4 * j + 3] = v.w;
+        }
+        float2 w = __ldg(reinterpret_cast<const float2 *>(g + (size_t)(e0 / 2 + 4) * XB));
+        u[16] = w.x; u[17] = w.y;
+    } else {
+        float2 w = __ldg(reinterpret_cast<const float2 *>(g + (size_t)((e0 - 1) / 2) * XB) + 1);
+        u[0] = w.x; u[1] = w.y;
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            float4 v = __ldg(g + (size_t)((e0 + 1) / 2 + j) * XB);
+            u[2 + 4 * j + 0] = v.x; u[2 + 4 * j + 1] = v.y; u[2 + 4 * j + 2] = v.z; u[2 + 4 * j + 3] = v.w;
+        }
+    }
+}
+
+// One of the eight hops.  FWD: (1 - gamma_MU) U_MU(x) psi(x+MU); else (1 + gamma_MU) U_MU(x-MU)^+ psi(x-MU).
+// nb: component 0 of the neighbour's element for this thread; cs: component stride (elements).
+// g: the link's site data (own site for FWD, the neighbour's for backward hops).
+template <int R, int MU, bool FWD>
+__device__ __forceinline__ void hop_dir(const typename Elem<R>::type *__restrict__ nb, size_t cs,
+                                        const float4 *__restrict__ g, int XB, CVec<R> (&acc)[12]) {
+    CVec<R> psi[12];
+#pragma unroll
+    for (int c = 0; c < 12; c++) psi[c] = to_cvec(ldg_nc(nb + c * cs));
+    float u[18];
+    load_link<MU>(g, XB, u);
+
+    // spin projection: h = upper two spin components of (1 -+ gamma_MU) psi  (S = +1 for FWD)
+    CVec<R> h[6];
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        if constexpr (MU == 0) {          // h0 = psi0 + S i psi3 ; h1 = psi1 + S i psi2
+            h[c]     = FWD ? cadd_i(psi[c], psi[9 + c])     : csub_i(psi[c], psi[9 + c]);
+            h[3 + c] = FWD ? cadd_i(psi[3 + c], psi[6 + c]) : csub_i(psi[3 + c], psi[6 + c]);
+        } else if constexpr (MU == 1) {   // h0 = psi0 + S psi3 ; h1 = psi1 - S psi2
+            h[c]     = FWD ? cadd(psi[c], psi[9 + c])     : csub(psi[c], psi[9 + c]);
+            h[3 + c] = FWD ? csub(psi[3 + c], psi[6 + c]) : cadd(psi[3 + c], psi[6 + c]);
+        } else if constexpr (MU == 2) {   // h0 = psi0 + S i psi2 ; h1 = psi1 - S i psi3
+            h[c]     = FWD ? cadd_i(psi[c], psi[6 + c])     : csub_i(psi[c], psi[6 + c]);
+            h[3 + c] = FWD ? csub_i(psi[3 + c], psi[9 + c]) : cadd_i(psi[3 + c], psi[9 + c]);
+        } else {                          // h0 = psi0 - S psi2 ; h1 = psi1 - S psi3
+            h[c]     = FWD ? csub(psi[c], psi[6 + c])     : cadd(psi[c], psi[6 + c]);
+            h[3 + c] = FWD ? csub(psi[3 + c], psi[9 + c]) : cadd(psi[3 + c], psi[9 + c]);
+        }
+    }
+
+    // colour multiply: r = U h (FWD) or U^+ h
+    CVec<R> r[6];
+#pragma unroll
+    for (int s = 0; s < 2; s++) {
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            if constexpr (FWD) {
+                CVec<R> t = cmul(u[2 * (3 * c + 0)], u[2 * (3 * c + 0) + 1], h[3 * s + 0]);
+                t = cfma(u[2 * (3 * c + 1)], u[2 * (3 * c + 1) + 1], h[3 * s + 1], t);
+                r[3 * s + c] = cfma(u[2 * (3 * c + 2)], u[2 * (3 * c + 2) + 1], h[3 * s + 2], t);
+            } else {
+                CVec<R> t = cmul_conj(u[2 * (0 + c)], u[2 * (0 + c) + 1], h[3 * s + 0]);
+                t = cfma_conj(u[2 * (3 + c)], u[2 * (3 + c) + 1], h[3 * s + 1], t);
+                r[3 * s + c] = cfma_conj(u[2 * (6 + c)], u[2 * (6 + c) + 1], h[3 * s + 2], t);
+            }
+        }
+    }
+
+    // reconstruction: upper components get r, lower ones -S i sigma_MU r (spatial) or -S r (time)
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        acc[c] = cadd(acc[c], r[c]);
+        acc[3 + c] = cadd(acc[3 + c], r[3 + c]);
+        if constexpr (MU == 0) {          // out2 += -S i r1 ; out3 += -S i r0
+            acc[6 + c] = FWD ? csub_i(acc[6 + c], r[3 + c]) : cadd_i(acc[6 + c], r[3 + c]);
+            acc[9 + c] = FWD ? csub_i(acc[9 + c], r[c])     : cadd_i(acc[9 + c], r[c]);
+        } else if constexpr (MU == 1) {   // out2 += -S r1 ; out3 += S r0
+            acc[6 + c] = FWD ? csub(acc[6 + c], r[3 + c]) : cadd(acc[6 + c], r[3 + c]);
+            acc[9 + c] = FWD ? cadd(acc[9 + c], r[c])     : csub(acc[9 + c], r[c]);
+        } else if constexpr (MU == 2) {   // out2 += -S i r0 ; out3 += S i r1
+            acc[6 + c] = FWD ? csub_i(acc[6 + c], r[c])     : cadd_i(acc[6 + c], r[c]);
+            acc[9 + c] = FWD ? cadd_i(acc[9 + c], r[3 + c]) : csub_i(acc[9 + c], r[3 + c]);
+        } else {                          // out2 += -S r0 ; out3 += -S r1
+            acc[6 + c] = FWD ? csub(acc[6 + c], r[c])     : cadd(acc[6 + c], r[c]);
+            acc[9 + c] = FWD ? csub(acc[9 + c], r[3 + c]) : cadd(acc[9 + c], r[3 + c]);
+        }
+    }
+}
+
+// XB_, NP_: compile-time layout block and threads per site (0 = take them from p at run time).
+// With both fixed every component and link load is base register + immediate offset.
+template <int R, bool CB, int XB_, int NP_>
+__global__ void __launch_bounds__(kHopMaxThreads, 1)
+hop_kernel(const HopParams p, const typename Elem<R>::type *__restrict__ in, typename Elem<R>::type *__restrict__ out) {
+    typedef typename Elem<R>::type E;
+    const int XB = XB_ ? XB_ : p.XB;
+    const int NP = NP_ ? NP_ : p.NP;
+    // thread -> (site in tile, rhs lane)
+    uint32_t q, pair, xin, row, ty, tz, tt;
+    if (NP_) { q = threadIdx.x / (uint32_t)NP; pair = threadIdx.x - q * NP; }
+    else p.d_np.divmod(threadIdx.x, q, pair);
+    if (XB_) { row = q / (uint32_t)XB; xin = q - row * XB; }
+    else p.d_xb.divmod(q, row, xin);
+    p.d_by.divmod(row, q, ty);
+    p.d_bz.divmod(q, tt, tz);
+    // block -> tile, in sweep order: x-blocks, then y and z tiles inside a chunk, then t, then chunks
+    uint32_t xb, yc, zc, ttile, chy, chz;
+    p.d_nxb.divmod(blockIdx.x, q, xb);
+    p.d_cy.divmod(q, q, yc);
+    p.d_cz.divmod(q, q, zc);
+    p.d_ntt.divmod(q, q, ttile);
+    p.d_ncy.divmod(q, chz, chy);
+    const int y = (int)((chy * p.cy + yc) * p.by + ty);
+    const int z = (int)((chz * p.cz + zc) * p.bz + tz);
+    const int t = (int)(ttile * p.bt + tt);
+
+    const int nxb = p.nxb;
+    const int sy = nxb, sz = nxb * p.Y, st = nxb * p.Y * p.Z;   // block strides
+    const int b = (int)xb + sy * y + sz * z + st * t;
+    const size_t cs = (size_t)XB * NP;                        // component stride in elements
+    const size_t lane = pair;
+
+    // x neighbours: (block, xin) of x+1 and x-1 in the input field
+    int bxp = b, xinp = (int)xin, bxm = b, xinm = (int)xin;
+    {
+        bool stepp = true, stepm = true;   // does the site index along the line change?
+        if (CB) {
+            int s = (p.out_parity + y + z + t) & 1;   // x = 2 xe + s on this line of the output field
+            stepp = s != 0;                           // x+1 -> xe + s
+            stepm = s == 0;                           // x-1 -> xe + s - 1
+        }
+        if (stepp) {
+            if (xinp + 1 < XB) xinp++;
+            else { xinp = 0; bxp = ((int)xb + 1 == nxb) ? b - (nxb - 1) : b + 1; }
+        }
+        if (stepm) {
+            if (xinm > 0) xinm--;
+            else { xinm = XB - 1; bxm = (xb == 0) ? b + (nxb - 1) : b - 1; }
+        }
+    }
+    const int byp = (y + 1 == p.Y) ? b - (p.Y - 1) * sy : b + sy;
+    const int bym = (y == 0) ? b + (p.Y - 1) * sy : b - sy;
+    const int bzp = (z + 1 == p.Z) ? b - (p.Z - 1) * sz : b + sz;
+    const int bzm = (z == 0) ? b + (p.Z - 1) * sz : b - sz;
+    const int btp = (t + 1 == p.T) ? b - (p.T - 1) * st : b + st;
+    const int btm = (t == 0) ? b + (p.T - 1) * st : b - st;
+
+#define MRHS_ELEM(bb, xx) (in + ((size_t)(bb) * 12 * XB + (xx)) * NP + lane)
+#define MRHS_LINK(base, bb, xx) ((base) + (size_t)(bb) * kSiteF4 * XB + (xx))
+
+    CVec<R> acc[12];
+#pragma unroll
+    for (int c = 0; c < 12; c++) acc[c] = czero<R>();
+
+    const float4 *gown = MRHS_LINK(p.gauge_out, b, xin);
+    hop_dir<R, 0, true >(MRHS_ELEM(bxp, xinp), cs, gown, XB, acc);
+    hop_dir<R, 0, false>(MRHS_ELEM(bxm, xinm), cs, MRHS_LINK(p.gauge_in, bxm, xinm), XB, acc);
+    hop_dir<R, 1, true >(MRHS_ELEM(byp, xin), cs, gown, XB, acc);
+    hop_dir<R, 1, false>(MRHS_ELEM(bym, xin), cs, MRHS_LINK(p.gauge_in, bym, xin), XB, acc);
+    hop_dir<R, 2, true >(MRHS_ELEM(bzp, xin), cs, gown, XB, acc);
+    hop_dir<R, 2, false>(MRHS_ELEM(bzm, xin), cs, MRHS_LINK(p.gauge_in, bzm, xin), XB, acc);
+    hop_dir<R, 3, true >(MRHS_ELEM(btp, xin), cs, gown, XB, acc);
+    hop_dir<R, 3, false>(MRHS_ELEM(btm, xin), cs, MRHS_LINK(p.gauge_in, btm, xin), XB, acc);
+
+    E *o = out + ((size_t)b * 12 * XB + xin) * NP + lane;
+#pragma unroll
+    for (int c = 0; c < 12; c++) o[c * cs] = from_cvec(acc[c]);
+#undef MRHS_ELEM
+#undef MRHS_LINK
+}
+
+// ------------------------------------------------------------- site data packing
+// one thread per float of the native array
+__global__ void pack_site_kernel(FieldGeom g, const float *__restrict__ src, float *__restrict__ dst, long long total) {
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    int k = (int)(idx & 3);
+    long long q = idx >> 2;
+    int xin = (int)(q % g.XB); q /= g.XB;
+    int j = (int)(q % kSiteF4);
+    long long b = q / kSiteF4;
+    int xb = (int)(b % g.nxb); b /= g.nxb;
+    int y = (int)(b % g.Y); b /= g.Y;
+    int z = (int)(b % g.Z);
+    int t = (int)(b / g.Z);
+    int x = x_of(g, xb * g.XB + xin, y, z, t);
+    long long lex = x + (long long)g.X * (y + (long long)g.Y * (z + (long long)g.Z * t));
+    dst[idx] = src[lex * 72 + 4 * j + k];
+}
+__global__ void unpack_site_kernel(FieldGeom g, const float *__restrict__ src, float *__restrict__ dst, long long total) {
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    int k = (int)(idx & 3);
+    long long q = idx >> 2;
+    int xin = (int)(q % g.XB); q /= g.XB;
+    int j = (int)(q % kSiteF4);
+    long long b = q / kSiteF4;
+    int xb = (int)(b % g.nxb); b /= g.nxb;
+    int y = (int)(b % g.Y); b /= g.Y;
+    int z = (int)(b % g.Z);
+    int t = (int)(b / g.Z);
+    int x = x_of(g, xb * g.XB + xin, y, z, t);
+    long long lex = x + (long long)g.X * (y + (long long)g.Y * (z + (long long)g.Z * t));
+    dst[lex * 72 + 4 * j + k] = src[idx];
+}
+
+}  // namespace
+
+mrhs_status_t pack_site_data(const FieldGeom &g, const float *d_src, float4 *d_dst, cudaStream_t st) {
+    long long total = g.nsites * 72;
+    long long blocks = (total + 255) / 256;
+    pack_site_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, d_src, (float *)d_dst, total);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+mrhs_status_t unpack_site_data(const FieldGeom &g, const float4 *d_src, float *d_dst, cudaStream_t st) {
+    long long total = g.nsites * 72;
+    long long blocks = (total + 255) / 256;
+    unpack_site_kernel<<<(unsigned)blocks, 256, 0, st>>>(g, (const float *)d_src, d_dst, total);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+// ------------------------------------------------------------------ tiling
+HopTiling default_tiling(const FieldGeom &g, size_t l2_budget) {
+    const int np = threads_per_site(g.N);
+    const int per_row = g.XB * np;
+    int rows_max = kHopMaxThreads / per_row;
+    if (rows_max < 1) rows_max = 1;
+    HopTiling best = {1, 1, 1, 1, 1};
+    double best_score = -1.0;
+    for (int by = 1; by <= g.Y; by++) {
+        if (g.Y % by) continue;
+        for (int bz = 1; bz <= g.Z; bz++) {
+            if (g.Z % bz) continue;
+            for (int bt = 1; bt <= g.T; bt++) {
+                if (g.T % bt) continue;
+                int rows = by * bz * bt;
+                if (rows > rows_max) continue;
+                // prefer full warps and many rows, then the smallest surface (neighbour rows outside the tile)
+                int thr = rows * per_row;
+                double fill = (double)thr / (double)(((thr + 31) / 32) * 32);
+                double surf = 1.0 / by + 1.0 / bz + 1.0 / bt;
+                double score = rows * fill * 16.0 - surf;
+                if (score > best_score) { best_score = score; best.by = by; best.bz = bz; best.bt = bt; }
+            }
+        }
+    }
+    // L2 sweep chunk: the kernel walks t inside a (y,z) chunk; about six t-slices of the chunk are
+    // live (t-1, t, t+1 of the tiles in flight), each site costing 96 N bytes of input.
+    const int nty = g.Y / best.by, ntz = g.Z / best.bz;
+    const double slice_site_bytes = 96.0 * g.N * 6.0;
+    double best_c = -1.0;
+    for (int cy = 1; cy <= nty; cy++) {
+        if (nty % cy) continue;
+        for (int cz = 1; cz <= ntz; cz++) {
+            if (ntz % cz) continue;
+            double sites = (double)g.Xe * cy * best.by * cz * best.bz;
+            bool fits = sites * slice_site_bytes <= (double)l2_budget;
+            if (!fits && !(cy == 1 && cz == 1)) continue;
+            // halo re-read of the chunk faces: 2/extent per chunked direction
+            double ey = cy * best.by, ez = cz * best.bz;
+            double over = (cy == nty ? 0.0 : 2.0 / ey) + (cz == ntz ? 0.0 : 2.0 / ez);
+            double score = 1.0 / (1.0 + over) + 1e-9 * sites;
+            if (score > best_c) { best_c = score; best.cy = cy; best.cz = cz; }
+        }
+    }
+    return best;
+}
+
+bool build_hop_params(const FieldGeom &g, int out_parity, const HopTiling &t, HopParams &p) {
+    if (t.by < 1 || t.bz < 1 || t.bt < 1 || t.cy < 1 || t.cz < 1) return false;
+    if (g.Y % t.by || g.Z % t.bz || g.T % t.bt) return false;
+    const int nty = g.Y / t.by, ntz = g.Z / t.bz, ntt = g.T / t.bt;
+    if (nty % t.cy || ntz % t.cz) return false;
+    const int np = threads_per_site(g.N);
+    const long long threads = (long long)t.by * t.bz * t.bt * g.XB * np;
+    if (threads > kHopMaxThreads) return false;
+    const long long grid = (long long)g.nxb * nty * ntz * ntt;
+    if (grid >= (1ll << 31)) return false;
+    p.Y = g.Y; p.Z = g.Z; p.T = g.T;
+    p.XB = g.XB; p.nxb = g.nxb; p.NP = np;
+    p.cb = g.cb; p.out_parity = out_parity;
+    p.by = t.by; p.bz = t.bz; p.bt = t.bt; p.cy = t.cy; p.cz = t.cz;
+    bool ok = true;
+    ok &= make_fastdiv(np, kHopMaxThreads, p.d_np);
+    ok &= make_fastdiv(g.XB, kHopMaxThreads, p.d_xb);
+    ok &= make_fastdiv(t.by, kHopMaxThreads, p.d_by);
+    ok &= make_fastdiv(t.bz, kHopMaxThreads, p.d_bz);
+    ok &= make_fastdiv(g.nxb, grid, p.d_nxb);
+    ok &= make_fastdiv(t.cy, grid, p.d_cy);
+    ok &= make_fastdiv(t.cz, grid, p.d_cz);
+    ok &= make_fastdiv(ntt, grid, p.d_ntt);
+    ok &= make_fastdiv(nty / t.cy, grid, p.d_ncy);
+    if (!ok) return false;
+    p.gauge_out = p.gauge_in = nullptr;
+    p.grid = (unsigned)grid;
+    p.threads = (unsigned)threads;
+    return true;
+}
+
+namespace {
+template <int R, int XB_, int NP_>
+void launch_hop_t(const HopParams &p, const void *d_in, void *d_out, cudaStream_t st) {
+    typedef typename Elem<R>::type E;
+    if (p.cb) hop_kernel<R, true, XB_, NP_><<<p.grid, p.threads, 0, st>>>(p, (const E *)d_in, (E *)d_out);
+    else      hop_kernel<R, false, XB_, NP_><<<p.grid, p.threads, 0, st>>>(p, (const E *)d_in, (E *)d_out);
+}
+}  // namespace
+
+mrhs_status_t launch_hop(const HopParams &p, int nrhs, const void *d_in, void *d_out, cudaStream_t st) {
+    const int key = p.XB * 1000 + p.NP;
+    if (nrhs & 1) {
+        switch (key) {
+            case 16001: launch_hop_t<1, 16, 1>(p, d_in, d_out, st); break;
+            case 12001: launch_hop_t<1, 12, 1>(p, d_in, d_out, st); break;
+            default:    launch_hop_t<1, 0, 0>(p, d_in, d_out, st); break;
+        }
+    } else {
+        switch (key) {
+            case 8006:  launch_hop_t<2, 8, 6>(p, d_in, d_out, st); break;     // N = 12
+            case 6006:  launch_hop_t<2, 6, 6>(p, d_in, d_out, st); break;     // N = 12, 24^4 checkerboarded
+            case 4012:  launch_hop_t<2, 4, 12>(p, d_in, d_out, st); break;    // N = 24
+            case 2024:  launch_hop_t<2, 2, 24>(p, d_in, d_out, st); break;    // N = 48
+            case 1048:  launch_hop_t<2, 1, 48>(p, d_in, d_out, st); break;    // N = 96
+            case 16002: launch_hop_t<2, 16, 2>(p, d_in, d_out, st); break;    // N = 4
+            case 12002: launch_hop_t<2, 12, 2>(p, d_in, d_out, st); break;    // N = 4
+            default:    launch_hop_t<2, 0, 0>(p, d_in, d_out, st); break;
+        }
+    }
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+}  // namespace mrhs

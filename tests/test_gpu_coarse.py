@@ -1,0 +1,81 @@
+"""GPU parity of the coarse-level 9-point stencil against the fp64 oracle (SURVEY.md
+Sec. 8(a) row a5; configs 3 and 4 of BASELINE.json).  Through the C-ABI binding."""
+import numpy as np
+import pytest
+
+import synth_inputs as syn
+from helpers import rel_l2_per_rhs
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+if not torch.cuda.is_available():
+    pytest.skip("needs a CUDA device", allow_module_level=True)
+
+import oracle                      # noqa: E402
+import paper_2211_13719_b200 as mrhs   # noqa: E402
+from gpu_common import TOL, dev, host   # noqa: E402
+
+
+def gpu_coarse(c, v):
+    d_in = c.import_field(dev(v))
+    d_out = c.empty()
+    c.apply(d_in, d_out)
+    torch.cuda.synchronize()
+    return host(c.export_field(d_out))
+
+
+SMALL = [([2, 2, 2, 2], 24, n) for n in (1, 2, 4, 8, 12, 16, 24, 32, 48, 64, 96)] + \
+        [([3, 2, 4, 2], 40, n) for n in (1, 2, 4, 8, 12, 16, 24, 32, 48, 64, 96)] + \
+        [([5, 3, 2, 4], 24, 12), ([4, 4, 4, 6], 40, 12)]
+
+
+@pytest.mark.parametrize("cdims,nb,nrhs", SMALL)
+def test_coarse_apply_matches_oracle_small(cdims, nb, nrhs):
+    A = syn.coarse_links_np(cdims, nb, 3)
+    v = syn.coarse_vector_np(cdims, nb, nrhs, 3)
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A))
+    err = rel_l2_per_rhs(gpu_coarse(c, v), oracle.coarse_apply(cdims, A, v))
+    assert err.max() < TOL, err
+    c.close()
+
+
+@pytest.mark.parametrize("nrhs", [1, 12, 24, 64])
+def test_config3_intermediate_level(nrhs):
+    cdims, nb = [8, 8, 8, 8], 24
+    A = syn.coarse_links_np(cdims, nb, 3)
+    v = syn.coarse_vector_np(cdims, nb, nrhs, 3)
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A))
+    err = rel_l2_per_rhs(gpu_coarse(c, v), oracle.coarse_apply(cdims, A, v))
+    assert err.max() < TOL, err
+    c.close()
+
+
+@pytest.mark.parametrize("nrhs", [12, 96])
+def test_config4_coarsest_level(nrhs):
+    cdims, nb = [6, 6, 6, 32], 40
+    A = syn.coarse_links_np(cdims, nb, 4)
+    v = syn.coarse_vector_np(cdims, nb, nrhs, 4)
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A))
+    err = rel_l2_per_rhs(gpu_coarse(c, v), oracle.coarse_apply(cdims, A, v))
+    assert err.max() < TOL, err
+    # host-buffer entry
+    h_in = torch.from_numpy(v).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    mrhs.coarse_apply_host(c.h, h_in, h_out)
+    err = rel_l2_per_rhs(h_out.numpy(), oracle.coarse_apply(cdims, A, v))
+    assert err.max() < TOL, err
+    c.close()
+
+
+def test_coarse_errors():
+    cdims, nb = [2, 2, 2, 2], 24
+    A = dev(syn.coarse_links_np(cdims, nb, 3))
+    with pytest.raises(mrhs.MrhsError) as e:
+        mrhs.Coarse(cdims, nb, 5, A)
+    assert e.value.status == mrhs.ERR_UNSUPPORTED
+    c = mrhs.Coarse(cdims, nb, 4, A)
+    f = c.empty()
+    with pytest.raises(mrhs.MrhsError):
+        c.apply(f, f)
+    c.close()

@@ -1,0 +1,183 @@
+"""GPU parity of the fine-level kernels against the fp64 oracle (SURVEY.md Sec. 8(a) rows
+a0-a4, a7; configs 1, 2 and 5 of BASELINE.json).  Everything goes through the C-ABI binding."""
+import numpy as np
+import pytest
+
+import synth_inputs as syn
+from helpers import rel_l2_per_rhs
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+if not torch.cuda.is_available():
+    pytest.skip("needs a CUDA device", allow_module_level=True)
+
+import oracle                      # noqa: E402
+import paper_2211_13719_b200 as mrhs   # noqa: E402
+from gpu_common import TOL, dev, gpu_dhop, gpu_meooe, gpu_mooee, host, make_wilson   # noqa: E402
+
+
+def _fine_case(dims, nrhs, seed, mass, csw):
+    U = syn.gauge_np(dims, seed)
+    psi = syn.spinor_np(syn.volume(dims), nrhs, seed)
+    return U, psi
+
+
+# config 1 first; then shapes that exercise x-blocks with several blocks per line, ragged thread
+# blocks (threads not a multiple of 32), extent-2 directions, odd N (scalar path) and N = 1.
+FINE_CASES = [
+    ([4, 4, 4, 4], 4, 0, -0.1, 1.0),
+    ([4, 4, 4, 4], 1, 1, -0.1, 1.0),
+    ([8, 4, 6, 2], 3, 2, 0.2, 1.3),
+    ([2, 2, 2, 2], 2, 3, 0.0, 1.0),
+    ([12, 6, 4, 10], 12, 4, -0.05, 1.5),
+    ([48, 4, 2, 4], 12, 5, -0.05, 1.5),
+    ([16, 8, 2, 4], 24, 6, -0.05, 1.5),
+    ([8, 4, 4, 4], 96, 7, -0.05, 1.5),
+    ([32, 2, 4, 6], 1, 8, -0.05, 1.5),
+]
+
+
+@pytest.mark.parametrize("dims,nrhs,seed,mass,csw", FINE_CASES)
+def test_dhop_meooe_mooee_match_oracle(dims, nrhs, seed, mass, csw):
+    U, psi = _fine_case(dims, nrhs, seed, mass, csw)
+    w = make_wilson(dims, nrhs, mass, csw, U)
+    # D_hop, full lattice (row a2)
+    want = oracle.dhop(dims, U, psi)
+    got = gpu_dhop(w, psi)
+    err = rel_l2_per_rhs(got, want)
+    assert err.max() < TOL, ("dhop", err)
+    # M_eooe, both parities (row a3)
+    pe, po = oracle.cb_split(dims, psi)
+    for out_parity, src in ((0, po), (1, pe)):
+        want = oracle.meooe(dims, U, src, out_parity)
+        got = gpu_meooe(w, src, out_parity)
+        err = rel_l2_per_rhs(got, want)
+        assert err.max() < TOL, ("meooe", out_parity, err)
+    # clover construction on the device (row a0) and M_ooee on full / even / odd fields (row a4)
+    C, _ = oracle.clover_blocks(dims, U, mass, csw)
+    Cg = torch.empty((syn.volume(dims), 2, 6, 6), dtype=torch.complex64, device="cuda")
+    mrhs.wilson_export_clover(w.h, Cg)
+    cerr = np.linalg.norm(host(Cg) - C) / np.linalg.norm(C)
+    assert cerr < 1e-6, cerr
+    want = oracle.mooee(C, psi)
+    err = rel_l2_per_rhs(gpu_mooee(w, psi, mrhs.FULL), want)
+    assert err.max() < TOL, ("mooee full", err)
+    Ce, Co = oracle.cb_split(dims, C)
+    for parity, Cp, src in ((0, Ce, pe), (1, Co, po)):
+        err = rel_l2_per_rhs(gpu_mooee(w, src, parity), oracle.mooee(Cp, src))
+        assert err.max() < TOL, ("mooee", parity, err)
+    w.close()
+
+
+def test_user_supplied_clover_is_used():
+    dims, nrhs = [4, 4, 4, 4], 4
+    U, psi = _fine_case(dims, nrhs, 11, 0.0, 1.0)
+    rng = np.random.default_rng(5)
+    A = rng.standard_normal((256, 2, 6, 6)) + 1j * rng.standard_normal((256, 2, 6, 6))
+    C = (A + np.conj(np.swapaxes(A, 2, 3))).astype(np.complex64)     # Hermitian blocks
+    w = make_wilson(dims, nrhs, 0.0, 1.0, U, clover=C)
+    err = rel_l2_per_rhs(gpu_mooee(w, psi, mrhs.FULL), oracle.mooee(C, psi))
+    assert err.max() < TOL, err
+    w.close()
+
+
+def test_layout_round_trips_are_bit_exact():
+    dims, nrhs = [12, 4, 6, 2], 12
+    psi = syn.spinor_np(syn.volume(dims), nrhs, 21)
+    d = dev(psi)
+    nat = mrhs.field_import(dims, 12, nrhs, mrhs.FULL, d)
+    back = mrhs.field_export(dims, 12, nrhs, mrhs.FULL, nat)
+    assert torch.equal(back.reshape(d.shape), d)
+    # full native -> even/odd native -> canonical equals the oracle-side canonical split
+    ev = mrhs.empty_field(dims, 12, nrhs, mrhs.EVEN)
+    od = mrhs.empty_field(dims, 12, nrhs, mrhs.ODD)
+    mrhs.cb_split(dims, 12, nrhs, nat, ev, od)
+    pe, po = oracle.cb_split(dims, psi)
+    assert np.array_equal(host(mrhs.field_export(dims, 12, nrhs, mrhs.EVEN, ev)).reshape(pe.shape), pe)
+    assert np.array_equal(host(mrhs.field_export(dims, 12, nrhs, mrhs.ODD, od)).reshape(po.shape), po)
+    full2 = torch.zeros_like(nat)
+    mrhs.cb_merge(dims, 12, nrhs, ev, od, full2)
+    assert torch.equal(full2, nat)
+
+
+def test_tilings_give_identical_results():
+    dims, nrhs = [16, 8, 8, 8], 12
+    U, psi = _fine_case(dims, nrhs, 31, -0.05, 1.5)
+    w = make_wilson(dims, nrhs, -0.05, 1.5, U)
+    ref = gpu_dhop(w, psi)
+    pe, po = oracle.cb_split(dims, psi)
+    ref_e = gpu_meooe(w, po, 0)
+    for tile, chunk in (([1, 1, 1], [1, 1]), ([2, 2, 2], [2, 1]), ([4, 2, 1], [1, 2]), ([2, 4, 1], [2, 2])):
+        mrhs.wilson_set_tiling(w.h, 0, tile, chunk)
+        mrhs.wilson_set_tiling(w.h, 1, tile, chunk)
+        assert mrhs.wilson_get_tiling(w.h, 0) == (tile, chunk)
+        assert np.array_equal(gpu_dhop(w, psi), ref)
+        assert np.array_equal(gpu_meooe(w, po, 0), ref_e)
+    with pytest.raises(mrhs.MrhsError):
+        mrhs.wilson_set_tiling(w.h, 0, [3, 2, 2], [1, 1])       # 3 does not divide 8
+    with pytest.raises(mrhs.MrhsError):
+        mrhs.wilson_set_tiling(w.h, 0, [8, 8, 8], [1, 1])       # too many threads
+    w.close()
+
+
+def test_argument_errors():
+    dims, nrhs = [4, 4, 4, 4], 4
+    U, psi = _fine_case(dims, nrhs, 41, 0.0, 1.0)
+    w = make_wilson(dims, nrhs, 0.0, 1.0, U)
+    f = w.empty(mrhs.FULL)
+    with pytest.raises(mrhs.MrhsError) as e:
+        w.dhop(f, f)
+    assert e.value.status == mrhs.ERR_INVALID_ARG
+    with pytest.raises(mrhs.MrhsError):
+        w.meooe(f, w.empty(mrhs.EVEN), 2)
+    with pytest.raises(mrhs.MrhsError):
+        w.mooee(f, w.empty(mrhs.FULL), 3)
+    with pytest.raises(mrhs.MrhsError):
+        w.dhop(f[1:], w.empty(mrhs.FULL))       # misaligned
+    w.close()
+
+
+def test_schur_sequence_and_host_entry():
+    dims, nrhs, mass, csw = [8, 8, 4, 4], 12, -0.05, 1.5
+    U, psi = _fine_case(dims, nrhs, 51, mass, csw)
+    w = make_wilson(dims, nrhs, mass, csw, U)
+    C, _ = oracle.clover_blocks(dims, U, mass, csw)
+    Ce, Co = oracle.cb_split(dims, C)
+    pe, po = oracle.cb_split(dims, psi)
+    want = oracle.meooe(dims, U, oracle.mooee(Co, oracle.meooe(dims, U, pe, 1)), 0)
+    d_in = w.import_field(dev(pe), mrhs.EVEN)
+    t0, t1, d_out = w.empty(mrhs.ODD), w.empty(mrhs.ODD), w.empty(mrhs.EVEN)
+    w.schur_sequence(d_in, t0, t1, d_out)
+    torch.cuda.synchronize()
+    err = rel_l2_per_rhs(host(w.export_field(d_out, mrhs.EVEN)), want)
+    assert err.max() < TOL, err
+    # host-buffer entry: canonical host in -> canonical host out
+    h_in = torch.from_numpy(psi).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    mrhs.wilson_apply_host(w.h, mrhs.OP_DHOP, 0, h_in, h_out)
+    err = rel_l2_per_rhs(h_out.numpy(), oracle.dhop(dims, U, psi))
+    assert err.max() < TOL, err
+    h_in = torch.from_numpy(po).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    mrhs.wilson_apply_host(w.h, mrhs.OP_MEOOE, 0, h_in, h_out)
+    err = rel_l2_per_rhs(h_out.numpy(), oracle.meooe(dims, U, po, 0))
+    assert err.max() < TOL, err
+    w.close()
+
+
+@pytest.mark.parametrize("nrhs", [1, 12])
+def test_config2_24x24_full_field(nrhs):
+    """Config 2 (24^4, mass -0.05, c_sw 1.5): full-field parity for D_hop, M_eooe and M_ooee."""
+    dims, mass, csw = [24, 24, 24, 24], -0.05, 1.5
+    U, psi = _fine_case(dims, nrhs, 2, mass, csw)
+    w = make_wilson(dims, nrhs, mass, csw, U)
+    err = rel_l2_per_rhs(gpu_dhop(w, psi), oracle.dhop(dims, U, psi))
+    assert err.max() < TOL, err
+    pe, po = oracle.cb_split(dims, psi)
+    err = rel_l2_per_rhs(gpu_meooe(w, pe, 1), oracle.meooe(dims, U, pe, 1))
+    assert err.max() < TOL, err
+    C, _ = oracle.clover_blocks(dims, U, mass, csw)
+    err = rel_l2_per_rhs(gpu_mooee(w, psi, mrhs.FULL), oracle.mooee(C, psi))
+    assert err.max() < TOL, err
+    w.close()
