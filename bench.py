@@ -1,0 +1,550 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the MRHS Wilson-clover stencil hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--sweep OUT.jsonl]
+
+One "step" is one pass of the whole hot path over one batch
+of seeded synthetic input, at BASELINE.json's target workload (config 5: 48^4 fine lattice,
+N_rhs = 12, mass -0.05, c_sw 1.5; plus config 4's coarsest-style level 6^3x32, nbasis 40,
+N_rhs = 12):
+
+    D_hop (full lattice)                                   row a2
+    M_eooe (odd <- even) and M_eooe (even <- odd)          row a3
+    M_ooee (full lattice)                                  row a4
+    Schur sequence M_eooe, M_ooee, M_eooe                  row a7
+    coarse 9-point apply, FP32 FMA                         row a5
+
+All fields are resident in HBM in the library's native layout when the timed region starts; the
+working set of every launch (>= 0.85 GB) is far larger than the 126 MB L2, so no flush is needed
+between iterations.  The metric is nominal GFLOP/s (1320 flops/site/RHS for the hop, 504 for the
+clover term, 72 nb^2 for the coarse apply); each kernel's algorithmic GB/s against the measured
+HBM copy bandwidth (MEASURED_PEAKS.json) is reported beside it.
+
+--impl reference times the fp64 CPU oracle (oracle/), as it stands, on a bounded sample of the
+same workload.  --sweep writes one JSON line per (operator, lattice, N_rhs) for configs 2-5.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOPS_HOP = 1320.0      # per output site per RHS (BASELINE.json north_star)
+FLOPS_CLOVER = 504.0    # per site per RHS (reading S10)
+FINE_DIMS = [48, 48, 48, 48]
+COARSE_DIMS = [6, 6, 6, 32]
+NBASIS = 40
+NRHS = 12
+MASS, CSW = -0.05, 1.5
+SEED = 5
+
+# bounded sample of the same workload for the CPU oracle (cpu_baseline and --impl reference)
+CPU_FINE_DIMS = [16, 16, 16, 16]
+CPU_COARSE_DIMS = [6, 6, 6, 8]
+CPU_SAMPLE = ("same operators, distributions and N_rhs=12 on a 16^4 fine lattice (1/81 of the 48^4 sites) "
+              "and a 6^3x8 coarse lattice (1/4 of the 6^3x32 sites), fp64 oracle, OpenMP over sites")
+
+
+def coarse_flops(nb):
+    return 72.0 * nb * nb
+
+
+def bytes_dhop(V, N):
+    return V * (288.0 + 192.0 * N)
+
+
+def bytes_meooe(V, N):
+    return (V / 2) * (576.0 + 192.0 * N)
+
+
+def bytes_mooee(nsites, N):
+    return nsites * (288.0 + 192.0 * N)
+
+
+def bytes_coarse(V, nb, N):
+    return V * (72.0 * nb * nb + 16.0 * nb * N)
+
+
+def vol(dims):
+    return dims[0] * dims[1] * dims[2] * dims[3]
+
+
+def step_work(fdims, cdims, nb, N):
+    """Nominal flops and algorithmic bytes of each launch of one step, in launch order."""
+    V, Vc = vol(fdims), vol(cdims)
+    hop_f, hop_b = FLOPS_HOP * (V / 2) * N, bytes_meooe(V, N)
+    clv_h_f, clv_h_b = FLOPS_CLOVER * (V / 2) * N, bytes_mooee(V / 2, N)
+    return [
+        ("dhop", FLOPS_HOP * V * N, bytes_dhop(V, N)),
+        ("meooe_oe", hop_f, hop_b),
+        ("meooe_eo", hop_f, hop_b),
+        ("mooee", FLOPS_CLOVER * V * N, bytes_mooee(V, N)),
+        ("schur_meooe_oe", hop_f, hop_b),
+        ("schur_mooee_oo", clv_h_f, clv_h_b),
+        ("schur_meooe_eo", hop_f, hop_b),
+        ("coarse_fma", coarse_flops(nb) * Vc * N, bytes_coarse(Vc, nb, N)),
+    ]
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(key):
+    """DRAM bytes per launch from the committed ncu capture (profiles/dram_traffic.json), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "dram_traffic.json")) as f:
+            return json.load(f).get(key)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line)
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.lines:
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                smax = float(parts[1])
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------ CPU oracle arm
+
+def oracle_step_setup():
+    import numpy as np
+    import oracle
+    import synth_inputs as syn
+    fd, cd = CPU_FINE_DIMS, CPU_COARSE_DIMS
+    U = syn.gauge_np(fd, SEED).astype(np.complex128)
+    psi = syn.spinor_np(vol(fd), NRHS, SEED).astype(np.complex128)
+    C, _ = oracle.clover_blocks(fd, U, MASS, CSW)          # setup (row a0), untimed like the GPU side
+    pe, po = oracle.cb_split(fd, psi)
+    Ce, Co = oracle.cb_split(fd, C)
+    A = syn.coarse_links_np(cd, NBASIS, 4).astype(np.complex128)
+    v = syn.coarse_vector_np(cd, NBASIS, NRHS, 4).astype(np.complex128)
+    return dict(fd=fd, cd=cd, U=U, psi=psi, C=C, pe=pe, po=po, Co=Co, A=A, v=v)
+
+
+def oracle_step(s):
+    import oracle
+    oracle.dhop(s["fd"], s["U"], s["psi"])
+    oracle.meooe(s["fd"], s["U"], s["pe"], 1)
+    oracle.meooe(s["fd"], s["U"], s["po"], 0)
+    oracle.mooee(s["C"], s["psi"])
+    t = oracle.meooe(s["fd"], s["U"], s["pe"], 1)
+    t = oracle.mooee(s["Co"], t)
+    oracle.meooe(s["fd"], s["U"], t, 0)
+    oracle.coarse_apply(s["cd"], s["A"], s["v"])
+
+
+def time_oracle(steps, warmup):
+    import oracle
+    s = oracle_step_setup()
+    flops = sum(w[1] for w in step_work(CPU_FINE_DIMS, CPU_COARSE_DIMS, NBASIS, NRHS))
+    for _ in range(warmup):
+        oracle_step(s)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_step(s)
+    dt = (time.perf_counter() - t0) / steps
+    return flops / dt / 1e9, dt * 1e3, oracle.get_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    gf, ms, cores = time_oracle(args.steps, args.warmup)
+    line = {
+        "impl": "reference", "metric": "MRHS Wilson-clover stencil hot path, nominal GFLOP/s", "value": gf,
+        "unit": "GFLOP/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(),
+        "cpu_baseline": {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": CPU_SAMPLE},
+        "e2e": {"value": gf, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config():
+    return {"workload": "config 5 (48^4 fine, N_rhs=12, mass -0.05, c_sw 1.5: D_hop, M_eooe x2, M_ooee, Schur sequence) "
+                        "+ config 4 (6^3x32 coarse, nbasis 40, N_rhs=12: 9-point apply, FP32 FMA)",
+            "fine_dims": FINE_DIMS, "coarse_dims": COARSE_DIMS, "nbasis": NBASIS, "n_rhs": NRHS,
+            "precision": "complex64 fields, fp32 FMA",
+            "l2": "every launch touches >= 0.85 GB, far above the 126 MB L2; no flush between iterations",
+            "parallelism": "replicas only (one GPU per lattice, no collectives; north_star)"}
+
+
+# ------------------------------------------------------------------------ GPU arm
+
+class Workload:
+    """Device-resident inputs and handles of one step (native layout), plus host staging for e2e."""
+
+    def __init__(self, torch, mrhs, syn, device, stream, fdims, cdims, nb, N):
+        self.torch, self.mrhs, self.fdims, self.cdims, self.nb, self.N = torch, mrhs, fdims, cdims, nb, N
+        V = vol(fdims)
+        U = syn.gauge_torch(fdims, SEED, device)
+        self.w = mrhs.Wilson(fdims, N, MASS, CSW, U, stream=stream)
+        del U
+        psi = syn.spinor_torch(V, N, SEED, device)
+        self.psi = self.w.import_field(psi, mrhs.FULL)
+        del psi
+        self.out_full = self.w.empty(mrhs.FULL)
+        self.in_e, self.in_o = self.w.empty(mrhs.EVEN), self.w.empty(mrhs.ODD)
+        mrhs.cb_split(fdims, 12, N, self.psi, self.in_e, self.in_o)
+        self.out_e, self.out_o = self.w.empty(mrhs.EVEN), self.w.empty(mrhs.ODD)
+        self.t0, self.t1 = self.w.empty(mrhs.ODD), self.w.empty(mrhs.ODD)
+        A = syn.coarse_links_torch(cdims, nb, 4, device)
+        self.c = mrhs.Coarse(cdims, nb, N, A, stream=stream)
+        del A
+        v = syn.spinor_torch(vol(cdims), N, 4, device, ncomp=(nb,))
+        self.v = self.c.import_field(v)
+        self.v_out = self.c.empty()
+        torch.cuda.synchronize()
+
+    def launches(self):
+        w, c, m = self.w, self.c, self.mrhs
+        return [
+            ("dhop", lambda: w.dhop(self.psi, self.out_full)),
+            ("meooe_oe", lambda: w.meooe(self.in_e, self.out_o, m.ODD)),
+            ("meooe_eo", lambda: w.meooe(self.in_o, self.out_e, m.EVEN)),
+            ("mooee", lambda: w.mooee(self.psi, self.out_full, m.FULL)),
+            ("schur", lambda: w.schur_sequence(self.in_e, self.t0, self.t1, self.out_e)),
+            ("coarse_fma", lambda: c.apply(self.v, self.v_out)),
+        ]
+
+
+def run_gpu(args):
+    import torch
+    import paper_2211_13719_b200 as mrhs
+    import synth_inputs as syn
+
+    mrhs.lib()   # fails loudly if libmrhs.so is missing: there is no fallback
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    fdims, cdims, nb, N = FINE_DIMS, COARSE_DIMS, NBASIS, NRHS
+    if args.small:
+        fdims, cdims = [16, 16, 16, 16], [4, 4, 4, 4]
+    stream = torch.cuda.Stream(device)
+    wl = Workload(torch, mrhs, syn, device, stream, fdims, cdims, nb, N)
+    launches = wl.launches()
+    work = step_work(fdims, cdims, nb, N)
+    flops_step = sum(w[1] for w in work)
+    K, W = args.steps, args.warmup
+
+    # one event pair per launch group per step, recorded on the stream the kernels run on
+    nseg = len(launches)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(nseg + 1)] for _ in range(K)]
+    for _ in range(W):
+        for _, f in launches:
+            f()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    t_wall = time.perf_counter()
+    for k in range(K):
+        evs[k][0].record(stream)
+        for i, (_, f) in enumerate(launches):
+            f()
+            evs[k][i + 1].record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = evs[0][0].elapsed_time(evs[K - 1][nseg])
+    seg_ms = [sum(evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)) / K for i in range(nseg)]
+    t = torch.tensor([total_ms], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / K
+    value = world * flops_step / (ms_per_step * 1e-3) / 1e9
+
+    # ------------------------------------------------------------ end to end, host buffers
+    e2e = run_e2e(torch, mrhs, wl, args, barrier, dist, device, world, flops_step)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = measured_peaks()
+    V = vol(fdims)
+    seg_names = [n for n, _ in launches]
+    kernels = {}
+    for name, ms in zip(seg_names, seg_ms):
+        if name == "schur":
+            fl = sum(w[1] for w in work if w[0].startswith("schur"))
+            by = sum(w[2] for w in work if w[0].startswith("schur"))
+        else:
+            fl, by = [(w[1], w[2]) for w in work if w[0] == name][0]
+        gbs = by / (ms * 1e-3) / 1e9
+        kernels[name] = {"ms": ms, "gflops": fl / (ms * 1e-3) / 1e9, "gbs": gbs, "hbm_frac": gbs / peak,
+                         "share_of_step": ms / sum(seg_ms)}
+    d = kernels["dhop"]
+    roofline = {"kernel": "hop_kernel (D_hop, full lattice %dx%dx%dx%d, N_rhs=%d)" % (*fdims, N), "bound": "hbm",
+                "achieved": d["gbs"], "peak": peak, "unit": "GB/s", "frac": d["gbs"] / peak,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_dhop(V, N),
+                "avg_launch_ms": d["ms"], "traffic": ncu_traffic("dhop_48x48x48x48_n12") if not args.small else None}
+    cpu = None
+    if not args.no_cpu:
+        gf, ms, cores = time_oracle(args.cpu_steps, 1)
+        cpu = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": CPU_SAMPLE, "ms_per_sample_step": ms}
+    cfg = workload_config()
+    if args.small:
+        cfg["workload"] = "SMALL smoke workload (16^4 fine, 4^4 coarse) -- not the benchmark configuration"
+        cfg["fine_dims"], cfg["coarse_dims"] = fdims, cdims
+    line = {
+        "metric": "MRHS Wilson-clover stencil hot path, nominal GFLOP/s", "value": value, "unit": "GFLOP/s",
+        "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": cfg, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
+        "gpu_launches": 8 * K, "kernels": kernels, "wall_ms_per_step": t_wall * 1e3 / K,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_e2e(torch, mrhs, wl, args, barrier, dist, device, world, flops_step):
+    """The same step through the host-buffer C-ABI entries: pinned canonical host fields in,
+    canonical host fields out, host<->device copies and layout conversion inside the timed region."""
+    if args.no_e2e:
+        return None
+    fdims, N, nb, cdims = wl.fdims, wl.N, wl.nb, wl.cdims
+    V = vol(fdims)
+    full_shape, half_shape = (V, 4, 3, N), (V // 2, 4, 3, N)
+    h_full_in = torch.empty(full_shape, dtype=torch.complex64).pin_memory()
+    h_full_out = torch.empty(full_shape, dtype=torch.complex64).pin_memory()
+    # canonical host inputs: export the device fields the device-timed arm uses
+    h_full_in.copy_(wl.w.export_field(wl.psi, mrhs.FULL))
+    h_e_in = torch.empty(half_shape, dtype=torch.complex64).pin_memory()
+    h_o_in = torch.empty(half_shape, dtype=torch.complex64).pin_memory()
+    h_e_in.copy_(wl.w.export_field(wl.in_e, mrhs.EVEN))
+    h_o_in.copy_(wl.w.export_field(wl.in_o, mrhs.ODD))
+    h_half_out = torch.empty(half_shape, dtype=torch.complex64).pin_memory()
+    h_v_in = torch.empty((vol(cdims), nb, N), dtype=torch.complex64).pin_memory()
+    h_v_in.copy_(wl.c.export_field(wl.v))
+    h_v_out = torch.empty_like(h_v_in).pin_memory()
+    torch.cuda.synchronize()
+    w, c = wl.w.h, wl.c.h
+
+    def step():
+        mrhs.wilson_apply_host(w, mrhs.OP_DHOP, 0, h_full_in, h_full_out)
+        mrhs.wilson_apply_host(w, mrhs.OP_MEOOE, mrhs.ODD, h_e_in, h_half_out)
+        mrhs.wilson_apply_host(w, mrhs.OP_MEOOE, mrhs.EVEN, h_o_in, h_half_out)
+        mrhs.wilson_apply_host(w, mrhs.OP_MOOEE, mrhs.FULL, h_full_in, h_full_out)
+        mrhs.wilson_apply_host(w, mrhs.OP_SCHUR, 0, h_e_in, h_half_out)
+        mrhs.coarse_apply_host(c, h_v_in, h_v_out)
+
+    fb, hb, cb = h_full_in.numel() * 8, h_e_in.numel() * 8, h_v_in.numel() * 8
+    h2d = 2 * fb + 3 * hb + cb
+    d2h = 2 * fb + 3 * hb + cb
+    E = max(1, min(args.steps, args.e2e_steps))
+    step()   # warm-up: allocates the handle's staging buffers
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(E):
+        step()   # every host entry synchronises its stream before returning
+    barrier()
+    dt = time.perf_counter() - t0
+    t = torch.tensor([dt], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dt = float(t.item()) / E
+    return {"value": world * flops_step / dt / 1e9, "unit": "GFLOP/s", "h2d_bytes_per_step": h2d,
+            "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3, "steps": E,
+            "api": "mrhs_wilson_apply_host / mrhs_coarse_apply_host (pinned canonical host buffers)"}
+
+
+# ------------------------------------------------------------------------ N_rhs sweep
+
+def run_sweep(args):
+    """One JSON line per (operator, lattice, N_rhs) for configs 2-5: median and min time of
+    individually timed launches, L2 flushed between launches (a 512 MB memset), GFLOP/s, GB/s,
+    fraction of the measured HBM peak, speed-up per RHS over N_rhs = 1."""
+    import torch
+    import paper_2211_13719_b200 as mrhs
+    import synth_inputs as syn
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    peak, peak_src = measured_peaks()
+    stream = torch.cuda.Stream(device)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)
+    iters, warm = args.sweep_iters, 5
+    out = open(args.sweep, "w")
+
+    def timeit(f):
+        with torch.cuda.stream(stream):
+            for _ in range(warm):
+                f()
+            ts = []
+            for _ in range(iters):
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                f()
+                e1.record(stream)
+                e1.synchronize()
+                ts.append(e0.elapsed_time(e1))
+        ts.sort()
+        return ts[len(ts) // 2], ts[0]
+
+    def emit(cfg, op, dims, N, fl, by, med, mn, base, extra=None):
+        rec = {"config": cfg, "op": op, "dims": dims, "n_rhs": N, "ms_median": med, "ms_min": mn,
+               "gflops": fl / (med * 1e-3) / 1e9, "gbs": by / (med * 1e-3) / 1e9,
+               "hbm_frac": by / (med * 1e-3) / 1e9 / peak, "alg_bytes": by, "nominal_flops": fl}
+        key = (cfg, op)
+        if N == base.get(key, (N, None))[0] or key not in base:
+            base.setdefault(key, (N, med / N))
+        rec["speedup_per_rhs_vs_first_n"] = base[key][1] / (med / N)
+        if extra:
+            rec.update(extra)
+        out.write(json.dumps(rec) + "\n")
+        out.flush()
+        print("%-8s %-12s %-16s N=%-3d %8.4f ms  %9.1f GF/s  %7.1f GB/s  %5.1f%% HBM" %
+              (cfg, op, "x".join(map(str, dims)), N, med, rec["gflops"], rec["gbs"], 100 * rec["hbm_frac"]), flush=True)
+
+    base = {}
+    fine = [("config2", [24, 24, 24, 24], [1, 4, 12, 24, 48], 2), ("config5", [48, 48, 48, 48], [1, 12, 24], 5)]
+    for cfg, dims, ns, seed in fine:
+        V = vol(dims)
+        U = syn.gauge_torch(dims, seed, device)
+        for N in ns:
+            w = mrhs.Wilson(dims, N, MASS, CSW, U, stream=stream)
+            psi = w.import_field(syn.spinor_torch(V, N, seed, device), mrhs.FULL)
+            o_full = w.empty(mrhs.FULL)
+            ie, io = w.empty(mrhs.EVEN), w.empty(mrhs.ODD)
+            mrhs.cb_split(dims, 12, N, psi, ie, io)
+            oe, oo, t0 = w.empty(mrhs.EVEN), w.empty(mrhs.ODD), w.empty(mrhs.ODD)
+            torch.cuda.synchronize()
+            m, mn = timeit(lambda: w.dhop(psi, o_full))
+            emit(cfg, "dhop", dims, N, FLOPS_HOP * V * N, bytes_dhop(V, N), m, mn, base)
+            m, mn = timeit(lambda: w.meooe(ie, oo, mrhs.ODD))
+            emit(cfg, "meooe", dims, N, FLOPS_HOP * V / 2 * N, bytes_meooe(V, N), m, mn, base)
+            m, mn = timeit(lambda: w.mooee(psi, o_full, mrhs.FULL))
+            emit(cfg, "mooee", dims, N, FLOPS_CLOVER * V * N, bytes_mooee(V, N), m, mn, base)
+            m, mn = timeit(lambda: w.schur_sequence(ie, oo, t0, oe))
+            emit(cfg, "schur_seq", dims, N, (2 * FLOPS_HOP + FLOPS_CLOVER) * V / 2 * N,
+                 2 * bytes_meooe(V, N) + bytes_mooee(V / 2, N), m, mn, base)
+            w.close()
+            del psi, o_full, ie, io, oe, oo, t0
+        del U
+    coarse = [("config3", [8, 8, 8, 8], 24, [1, 12, 24, 64], 3), ("config4", [6, 6, 6, 32], 40, [12, 24, 48, 96], 4)]
+    for cfg, dims, nb, ns, seed in coarse:
+        V = vol(dims)
+        A = syn.coarse_links_torch(dims, nb, seed, device)
+        for N in ns:
+            for mode in mrhs.COARSE_MODES:
+                try:
+                    c = mrhs.Coarse(dims, nb, N, A, math_mode=mode, stream=stream)
+                except mrhs.MrhsError:
+                    continue
+                v = c.import_field(syn.spinor_torch(V, N, seed, device, ncomp=(nb,)))
+                vo = c.empty()
+                torch.cuda.synchronize()
+                m, mn = timeit(lambda: c.apply(v, vo))
+                emit(cfg, "coarse_mode%d" % mode, dims, N, coarse_flops(nb) * V * N, bytes_coarse(V, nb, N), m, mn, base,
+                     {"nbasis": nb, "fp32_fma_peak_frac": coarse_flops(nb) * V * N / (m * 1e-3) / 74.4e12})
+                c.close()
+        del A
+    out.close()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--small", action="store_true", help="tiny workload for a functional check (not a benchmark)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-steps", type=int, default=8, help="oracle sample steps timed for cpu_baseline")
+    ap.add_argument("--sweep", default=None, help="write the per-operator N_rhs sweep to this .jsonl and exit")
+    ap.add_argument("--sweep-iters", type=int, default=30)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours" and not args.sweep:
+        args.warmup = 3   # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

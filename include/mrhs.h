@@ -172,8 +172,9 @@ mrhs_status_t mrhs_cb_merge(const int dims[4], int ncomp, int nrhs, const void *
 
 /* One operator apply with HOST buffers in CANONICAL layout: host->device copy,
  * import, the same kernel the device entry launches, export, device->host copy,
- * then a stream synchronise.  op: 0 = D_hop, 1 = M_eooe, 2 = M_ooee.
- * parity: out parity for op 1; field parity (0,1,2) for op 2; ignored for op 0.
+ * then a stream synchronise.  op: 0 = D_hop, 1 = M_eooe, 2 = M_ooee, 3 = the Schur
+ * sequence of mrhs_schur_sequence (even field in, even field out).
+ * parity: out parity for op 1; field parity (0,1,2) for op 2; ignored for ops 0 and 3.
  * Staging buffers are owned by the handle and allocated on first use. */
 mrhs_status_t mrhs_wilson_apply_host(mrhs_wilson_t *h, int op, int parity,
                                      const void *h_in, void *h_out);

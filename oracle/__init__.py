@@ -64,6 +64,13 @@ def _dims(dims):
     return _c_int4(*dims)
 
 
+def _cdims(dims):
+    """Coarse lattices need not have even extents (nothing is checkerboarded there)."""
+    dims = [int(d) for d in dims]
+    assert len(dims) == 4 and all(d >= 2 for d in dims), "extents must be >= 2"
+    return _c_int4(*dims)
+
+
 def volume(dims):
     return int(dims[0]) * int(dims[1]) * int(dims[2]) * int(dims[3])
 
@@ -180,7 +187,7 @@ def coarse_apply(cdims, A, v, pmask=0x1FF):
     assert A.shape == (V, 9, nb, nb) and v.shape[:2] == (V, nb)
     N = v.shape[2]
     out = np.empty_like(v)
-    _load().orc_coarse_apply(_dims(cdims), ctypes.c_int(nb), ctypes.c_int(N), _ptr(A), _ptr(v), _ptr(out), ctypes.c_int(pmask))
+    _load().orc_coarse_apply(_cdims(cdims), ctypes.c_int(nb), ctypes.c_int(N), _ptr(A), _ptr(v), _ptr(out), ctypes.c_int(pmask))
     return out
 
 

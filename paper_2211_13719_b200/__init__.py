@@ -21,7 +21,9 @@ _lib = None
 
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA = 0, 1, 2, 3, 4
 EVEN, ODD, FULL = 0, 1, 2
-OP_DHOP, OP_MEOOE, OP_MOOEE = 0, 1, 2
+OP_DHOP, OP_MEOOE, OP_MOOEE, OP_SCHUR = 0, 1, 2, 3
+COARSE_FMA, COARSE_TENSOR = 0, 1
+COARSE_MODES = (COARSE_FMA, COARSE_TENSOR)
 
 _vp = ctypes.c_void_p
 _int4 = ctypes.c_int * 4

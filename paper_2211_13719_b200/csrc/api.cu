@@ -42,6 +42,8 @@ struct mrhs_wilson {
     // staging for the host-buffer entry
     void *st_canon, *st_in, *st_out;
     size_t st_bytes;
+    void *st_tmp[2];               // odd-parity temporaries of the Schur sequence
+    size_t st_tmp_bytes;
 };
 
 struct mrhs_coarse {
@@ -60,6 +62,7 @@ mrhs_status_t wilson_free(mrhs_wilson *h) {
     cudaFree(h->gauge_full); cudaFree(h->gauge_cb[0]); cudaFree(h->gauge_cb[1]);
     cudaFree(h->clov_full); cudaFree(h->clov_cb[0]); cudaFree(h->clov_cb[1]);
     cudaFree(h->st_canon); cudaFree(h->st_in); cudaFree(h->st_out);
+    cudaFree(h->st_tmp[0]); cudaFree(h->st_tmp[1]);
     delete h;
     return MRHS_OK;
 }
@@ -248,8 +251,9 @@ mrhs_status_t mrhs_wilson_destroy(mrhs_wilson_t *h) { return wilson_free(h); }
 
 mrhs_status_t mrhs_wilson_apply_host(mrhs_wilson_t *h, int op, int parity, const void *h_in, void *h_out) {
     MRHS_REQUIRE(h && h_in && h_out, "apply host: NULL argument");
-    MRHS_REQUIRE(op >= 0 && op <= 2, "apply host: op must be 0 (D_hop), 1 (M_eooe) or 2 (M_ooee)");
+    MRHS_REQUIRE(op >= 0 && op <= 3, "apply host: op must be 0 (D_hop), 1 (M_eooe), 2 (M_ooee) or 3 (Schur sequence)");
     int in_par = MRHS_FULL, out_par = MRHS_FULL;
+    if (op == 3) in_par = out_par = MRHS_EVEN;
     if (op == 1) {
         MRHS_REQUIRE(parity == 0 || parity == 1, "apply host: out parity must be 0 or 1");
         out_par = parity; in_par = 1 - parity;
@@ -260,10 +264,18 @@ mrhs_status_t mrhs_wilson_apply_host(mrhs_wilson_t *h, int op, int parity, const
     const size_t bytes = mrhs_field_bytes(h->dims, 12, h->nrhs, in_par != MRHS_FULL);
     mrhs_status_t s = ensure_stage(&h->st_canon, &h->st_in, &h->st_out, &h->st_bytes, bytes);
     if (s != MRHS_OK) return s;
+    if (op == 3 && h->st_tmp_bytes < bytes) {
+        cudaFree(h->st_tmp[0]); cudaFree(h->st_tmp[1]);
+        h->st_tmp[0] = h->st_tmp[1] = nullptr; h->st_tmp_bytes = 0;
+        MRHS_CUDA(cudaMalloc(&h->st_tmp[0], bytes));
+        MRHS_CUDA(cudaMalloc(&h->st_tmp[1], bytes));
+        h->st_tmp_bytes = bytes;
+    }
     MRHS_CUDA(cudaMemcpyAsync(h->st_canon, h_in, bytes, cudaMemcpyHostToDevice, h->st));
     s = mrhs_field_import(h->dims, 12, h->nrhs, in_par, h->st_canon, h->st_in, h->st);
     if (s != MRHS_OK) return s;
-    if (op == 0) s = mrhs_dhop(h, h->st_in, h->st_out);
+    if (op == 3) s = mrhs_schur_sequence(h, h->st_in, h->st_tmp[0], h->st_tmp[1], h->st_out);
+    else if (op == 0) s = mrhs_dhop(h, h->st_in, h->st_out);
     else if (op == 1) s = mrhs_meooe(h, h->st_in, h->st_out, out_par);
     else s = mrhs_mooee(h, h->st_in, h->st_out, parity);
     if (s != MRHS_OK) return s;
