@@ -126,6 +126,10 @@ mrhs_status_t mrhs_wilson_export_clover(mrhs_wilson_t *h, void *d_clover_out);
  * Each must divide the lattice accordingly; INVALID_ARG otherwise. */
 mrhs_status_t mrhs_wilson_set_tiling(mrhs_wilson_t *h, int which, const int tile[3], const int chunk[2]);
 mrhs_status_t mrhs_wilson_get_tiling(mrhs_wilson_t *h, int which, int tile[3], int chunk[2]);
+/* L2 prefetch distance of the hopping kernel, in thread-block tiles of its sweep order: a tile
+ * asks the copy engine to bring the rows of the tile distance_tiles later into L2 (0 = off).
+ * set_tiling resets it to the default (one t-step of the chunk plus two waves of tiles). */
+mrhs_status_t mrhs_wilson_set_prefetch(mrhs_wilson_t *h, int which, int distance_tiles);
 
 mrhs_status_t mrhs_wilson_destroy(mrhs_wilson_t *h);
 

@@ -39,6 +39,7 @@ _SIGNATURES = {
     "mrhs_wilson_export_clover": (ctypes.c_int, [_vp, _vp]),
     "mrhs_wilson_set_tiling": (ctypes.c_int, [_vp, ctypes.c_int, _int3, _int2]),
     "mrhs_wilson_get_tiling": (ctypes.c_int, [_vp, ctypes.c_int, _int3, _int2]),
+    "mrhs_wilson_set_prefetch": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
     "mrhs_wilson_destroy": (ctypes.c_int, [_vp]),
     "mrhs_coarse_create": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, ctypes.c_int, ctypes.c_int, _vp, ctypes.c_int, _vp]),
     "mrhs_coarse_apply": (ctypes.c_int, [_vp, _vp, _vp]),
@@ -192,6 +193,10 @@ def wilson_get_tiling(h, which):
     tile, chunk = _int3(), _int2()
     _check(lib().mrhs_wilson_get_tiling(h, int(which), tile, chunk))
     return list(tile), list(chunk)
+
+
+def wilson_set_prefetch(h, which, distance_tiles):
+    _check(lib().mrhs_wilson_set_prefetch(h, int(which), int(distance_tiles)))
 
 
 def wilson_apply_host(h, op, parity, h_in, h_out):

@@ -238,6 +238,15 @@ mrhs_status_t mrhs_wilson_set_tiling(mrhs_wilson_t *h, int which, const int tile
     return MRHS_OK;
 }
 
+mrhs_status_t mrhs_wilson_set_prefetch(mrhs_wilson_t *h, int which, int distance_tiles) {
+    MRHS_REQUIRE(h, "set prefetch: NULL handle");
+    MRHS_REQUIRE(which == 0 || which == 1, "set prefetch: which must be 0 (D_hop) or 1 (M_eooe)");
+    MRHS_REQUIRE(distance_tiles >= 0, "set prefetch: distance must be >= 0 (0 = off)");
+    if (which == 0) h->hp_full.pf_dist = (unsigned)distance_tiles;
+    else h->hp_cb[0].pf_dist = h->hp_cb[1].pf_dist = (unsigned)distance_tiles;
+    return MRHS_OK;
+}
+
 mrhs_status_t mrhs_wilson_get_tiling(mrhs_wilson_t *h, int which, int tile[3], int chunk[2]) {
     MRHS_REQUIRE(h && tile && chunk, "get tiling: NULL argument");
     MRHS_REQUIRE(which == 0 || which == 1, "get tiling: which must be 0 (D_hop) or 1 (M_eooe)");

@@ -42,17 +42,31 @@ __device__ __forceinline__ void load_link(const float4 *__restrict__ g, int XB, 
     }
 }
 
-// One of the eight hops.  FWD: (1 - gamma_MU) U_MU(x) psi(x+MU); else (1 + gamma_MU) U_MU(x-MU)^+ psi(x-MU).
+// Operands of one hop as loaded: the neighbour's 12 components for this thread's RHS and the 18 reals
+// of the link.  Keeping load and arithmetic apart lets the kernel body put the loads of a later hop
+// in front of the arithmetic of the current one (software pipelining in registers).
+template <int R> struct HopOperands {
+    typename Elem<R>::type psi[12];
+    float u[18];
+};
+
 // nb: component 0 of the neighbour's element for this thread; cs: component stride (elements).
-// g: the link's site data (own site for FWD, the neighbour's for backward hops).
+// g: the link's site data (own site for forward hops, the neighbour's for backward hops).
+template <int R, int MU>
+__device__ __forceinline__ void hop_load(HopOperands<R> &o, const typename Elem<R>::type *__restrict__ nb, size_t cs,
+                                         const float4 *__restrict__ g, int XB) {
+#pragma unroll
+    for (int c = 0; c < 12; c++) o.psi[c] = ldg_nc(nb + c * cs);
+    load_link<MU>(g, XB, o.u);
+}
+
+// One of the eight hops.  FWD: (1 - gamma_MU) U_MU(x) psi(x+MU); else (1 + gamma_MU) U_MU(x-MU)^+ psi(x-MU).
 template <int R, int MU, bool FWD>
-__device__ __forceinline__ void hop_dir(const typename Elem<R>::type *__restrict__ nb, size_t cs,
-                                        const float4 *__restrict__ g, int XB, CVec<R> (&acc)[12]) {
+__device__ __forceinline__ void hop_compute(const HopOperands<R> &o, CVec<R> (&acc)[12]) {
     CVec<R> psi[12];
 #pragma unroll
-    for (int c = 0; c < 12; c++) psi[c] = to_cvec(ldg_nc(nb + c * cs));
-    float u[18];
-    load_link<MU>(g, XB, u);
+    for (int c = 0; c < 12; c++) psi[c] = to_cvec(o.psi[c]);
+    const float (&u)[18] = o.u;
 
     // spin projection: h = upper two spin components of (1 -+ gamma_MU) psi  (S = +1 for FWD)
     CVec<R> h[6];
@@ -112,10 +126,36 @@ __device__ __forceinline__ void hop_dir(const typename Elem<R>::type *__restrict
     }
 }
 
+template <int R, int MU, bool FWD>
+__device__ __forceinline__ void hop_dir(const typename Elem<R>::type *__restrict__ nb, size_t cs,
+                                        const float4 *__restrict__ g, int XB, CVec<R> (&acc)[12]) {
+    HopOperands<R> o;
+    hop_load<R, MU>(o, nb, cs, g, XB);
+    hop_compute<R, MU, FWD>(o, acc);
+}
+
+// blk -> origin of its tile.  Sweep order: x-blocks, then y and z tiles inside a chunk, then t, then chunks.
+__device__ __forceinline__ void tile_origin(const HopParams &p, uint32_t blk, uint32_t &xb, uint32_t &y0, uint32_t &z0, uint32_t &t0) {
+    uint32_t q, yc, zc, ttile, chy, chz;
+    p.d_nxb.divmod(blk, q, xb);
+    p.d_cy.divmod(q, q, yc);
+    p.d_cz.divmod(q, q, zc);
+    p.d_ntt.divmod(q, q, ttile);
+    p.d_ncy.divmod(q, chz, chy);
+    y0 = (chy * p.cy + yc) * p.by;
+    z0 = (chz * p.cz + zc) * p.bz;
+    t0 = ttile * p.bt;
+}
+
+// one instruction asks the copy engine to bring [ptr, ptr+bytes) into L2 (bytes % 16 == 0)
+__device__ __forceinline__ void l2_prefetch(const void *ptr, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(ptr), "r"(bytes) : "memory");
+}
+
 // XB_, NP_: compile-time layout block and threads per site (0 = take them from p at run time).
 // With both fixed every component and link load is base register + immediate offset.
-template <int R, bool CB, int XB_, int NP_>
-__global__ void __launch_bounds__(kHopMaxThreads, 1)
+template <int R, bool CB, int XB_, int NP_, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1)
 hop_kernel(const HopParams p, const typename Elem<R>::type *__restrict__ in, typename Elem<R>::type *__restrict__ out) {
     typedef typename Elem<R>::type E;
     const int XB = XB_ ? XB_ : p.XB;
@@ -129,15 +169,26 @@ hop_kernel(const HopParams p, const typename Elem<R>::type *__restrict__ in, typ
     p.d_by.divmod(row, q, ty);
     p.d_bz.divmod(q, tt, tz);
     // block -> tile, in sweep order: x-blocks, then y and z tiles inside a chunk, then t, then chunks
-    uint32_t xb, yc, zc, ttile, chy, chz;
-    p.d_nxb.divmod(blockIdx.x, q, xb);
-    p.d_cy.divmod(q, q, yc);
-    p.d_cz.divmod(q, q, zc);
-    p.d_ntt.divmod(q, q, ttile);
-    p.d_ncy.divmod(q, chz, chy);
-    const int y = (int)((chy * p.cy + yc) * p.by + ty);
-    const int z = (int)((chz * p.cz + zc) * p.bz + tz);
-    const int t = (int)(ttile * p.bt + tt);
+    uint32_t xb, ty0, tz0, tt0;
+    tile_origin(p, blockIdx.x, xb, ty0, tz0, tt0);
+    const int y = (int)(ty0 + ty);
+    const int z = (int)(tz0 + tz);
+    const int t = (int)(tt0 + tt);
+
+    // L2 prefetch of the rows a later tile in the sweep owns (spinor row of the input field at the
+    // same coordinates plus the rows of both link arrays): every input byte of the launch is
+    // requested once, pf_dist tiles before its first use, by one bulk-prefetch instruction per
+    // contiguous row, so the loads below find their data in L2 instead of waiting on HBM.
+    if (p.pf_dist && threadIdx.x < (unsigned)(p.by * p.bz * p.bt) && blockIdx.x + p.pf_dist < gridDim.x) {
+        uint32_t fxb, fy0, fz0, ft0, r = threadIdx.x, ry, rz, rt, qq;
+        tile_origin(p, blockIdx.x + p.pf_dist, fxb, fy0, fz0, ft0);
+        p.d_by.divmod(r, qq, ry);
+        p.d_bz.divmod(qq, rt, rz);
+        const size_t fb = (size_t)fxb + (size_t)p.nxb * ((fy0 + ry) + (size_t)p.Y * ((fz0 + rz) + (size_t)p.Z * (ft0 + rt)));
+        l2_prefetch(in + fb * 12 * XB * NP, (uint32_t)(12 * XB * NP * sizeof(E)));
+        l2_prefetch(p.gauge_out + fb * kSiteF4 * XB, (uint32_t)(kSiteF4 * XB * sizeof(float4)));
+        if (CB) l2_prefetch(p.gauge_in + fb * kSiteF4 * XB, (uint32_t)(kSiteF4 * XB * sizeof(float4)));
+    }
 
     const int nxb = p.nxb;
     const int sy = nxb, sz = nxb * p.Y, st = nxb * p.Y * p.Z;   // block strides
@@ -178,14 +229,35 @@ hop_kernel(const HopParams p, const typename Elem<R>::type *__restrict__ in, typ
     for (int c = 0; c < 12; c++) acc[c] = czero<R>();
 
     const float4 *gown = MRHS_LINK(p.gauge_out, b, xin);
-    hop_dir<R, 0, true >(MRHS_ELEM(bxp, xinp), cs, gown, XB, acc);
-    hop_dir<R, 0, false>(MRHS_ELEM(bxm, xinm), cs, MRHS_LINK(p.gauge_in, bxm, xinm), XB, acc);
-    hop_dir<R, 1, true >(MRHS_ELEM(byp, xin), cs, gown, XB, acc);
-    hop_dir<R, 1, false>(MRHS_ELEM(bym, xin), cs, MRHS_LINK(p.gauge_in, bym, xin), XB, acc);
-    hop_dir<R, 2, true >(MRHS_ELEM(bzp, xin), cs, gown, XB, acc);
-    hop_dir<R, 2, false>(MRHS_ELEM(bzm, xin), cs, MRHS_LINK(p.gauge_in, bzm, xin), XB, acc);
-    hop_dir<R, 3, true >(MRHS_ELEM(btp, xin), cs, gown, XB, acc);
-    hop_dir<R, 3, false>(MRHS_ELEM(btm, xin), cs, MRHS_LINK(p.gauge_in, btm, xin), XB, acc);
+    const E *n0p = MRHS_ELEM(bxp, xinp), *n0m = MRHS_ELEM(bxm, xinm);
+    const E *n1p = MRHS_ELEM(byp, xin), *n1m = MRHS_ELEM(bym, xin);
+    const E *n2p = MRHS_ELEM(bzp, xin), *n2m = MRHS_ELEM(bzm, xin);
+    const E *n3p = MRHS_ELEM(btp, xin), *n3m = MRHS_ELEM(btm, xin);
+    const float4 *g0m = MRHS_LINK(p.gauge_in, bxm, xinm), *g1m = MRHS_LINK(p.gauge_in, bym, xin);
+    const float4 *g2m = MRHS_LINK(p.gauge_in, bzm, xin), *g3m = MRHS_LINK(p.gauge_in, btm, xin);
+    if constexpr (MAXT <= 288) {
+        // two hops' operands in flight: the loads of hop k+2 are issued before the arithmetic of hop k
+        HopOperands<R> A, B;
+        hop_load<R, 0>(A, n0p, cs, gown, XB);
+        hop_load<R, 0>(B, n0m, cs, g0m, XB);
+        hop_compute<R, 0, true >(A, acc);  hop_load<R, 1>(A, n1p, cs, gown, XB);
+        hop_compute<R, 0, false>(B, acc);  hop_load<R, 1>(B, n1m, cs, g1m, XB);
+        hop_compute<R, 1, true >(A, acc);  hop_load<R, 2>(A, n2p, cs, gown, XB);
+        hop_compute<R, 1, false>(B, acc);  hop_load<R, 2>(B, n2m, cs, g2m, XB);
+        hop_compute<R, 2, true >(A, acc);  hop_load<R, 3>(A, n3p, cs, gown, XB);
+        hop_compute<R, 2, false>(B, acc);  hop_load<R, 3>(B, n3m, cs, g3m, XB);
+        hop_compute<R, 3, true >(A, acc);
+        hop_compute<R, 3, false>(B, acc);
+    } else {
+        hop_dir<R, 0, true >(n0p, cs, gown, XB, acc);
+        hop_dir<R, 0, false>(n0m, cs, g0m, XB, acc);
+        hop_dir<R, 1, true >(n1p, cs, gown, XB, acc);
+        hop_dir<R, 1, false>(n1m, cs, g1m, XB, acc);
+        hop_dir<R, 2, true >(n2p, cs, gown, XB, acc);
+        hop_dir<R, 2, false>(n2m, cs, g2m, XB, acc);
+        hop_dir<R, 3, true >(n3p, cs, gown, XB, acc);
+        hop_dir<R, 3, false>(n3m, cs, g3m, XB, acc);
+    }
 
     E *o = out + ((size_t)b * 12 * XB + xin) * NP + lane;
 #pragma unroll
@@ -320,6 +392,8 @@ bool build_hop_params(const FieldGeom &g, int out_parity, const HopTiling &t, Ho
     ok &= make_fastdiv(nty / t.cy, grid, p.d_ncy);
     if (!ok) return false;
     p.gauge_out = p.gauge_in = nullptr;
+    // default prefetch distance: one t-step of the chunk (the t+1 rows a tile reads) plus two waves of tiles
+    p.pf_dist = (unsigned)(g.nxb * t.cy * t.cz) + 2u * 148u;
     p.grid = (unsigned)grid;
     p.threads = (unsigned)threads;
     return true;
@@ -329,8 +403,15 @@ namespace {
 template <int R, int XB_, int NP_>
 void launch_hop_t(const HopParams &p, const void *d_in, void *d_out, cudaStream_t st) {
     typedef typename Elem<R>::type E;
-    if (p.cb) hop_kernel<R, true, XB_, NP_><<<p.grid, p.threads, 0, st>>>(p, (const E *)d_in, (E *)d_out);
-    else      hop_kernel<R, false, XB_, NP_><<<p.grid, p.threads, 0, st>>>(p, (const E *)d_in, (E *)d_out);
+    // CTAs of 193..288 threads get the 224-register build (deeper load pipelining); everything else the
+    // 168-register one, which also lets several small CTAs share an SM.
+    if (p.threads > 192 && p.threads <= 288) {
+        if (p.cb) hop_kernel<R, true, XB_, NP_, 288><<<p.grid, p.threads, 0, st>>>(p, (const E *)d_in, (E *)d_out);
+        else      hop_kernel<R, false, XB_, NP_, 288><<<p.grid, p.threads, 0, st>>>(p, (const E *)d_in, (E *)d_out);
+    } else {
+        if (p.cb) hop_kernel<R, true, XB_, NP_, kHopMaxThreads><<<p.grid, p.threads, 0, st>>>(p, (const E *)d_in, (E *)d_out);
+        else      hop_kernel<R, false, XB_, NP_, kHopMaxThreads><<<p.grid, p.threads, 0, st>>>(p, (const E *)d_in, (E *)d_out);
+    }
 }
 }  // namespace
 

@@ -20,6 +20,7 @@ struct HopParams {
     int cb, out_parity;       // checkerboarded fields? parity of the output field
     int by, bz, bt;           // tile extents
     int cy, cz;               // chunk extents in tiles
+    unsigned pf_dist;         // L2 prefetch distance in tiles of the sweep order (0 = off)
     FastDiv d_np, d_xb, d_by, d_bz;             // thread index -> (row, xin, pair) -> (ty, tz, tt)
     FastDiv d_nxb, d_cy, d_cz, d_ntt, d_ncy;    // block index -> tile coordinates in sweep order
     const float4 *gauge_out;  // links living on the sites of the output field, [block][18][xin] float4
