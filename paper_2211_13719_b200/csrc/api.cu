@@ -95,7 +95,7 @@ mrhs_status_t wilson_build(mrhs_wilson *h, const void *d_gauge, const void *d_cl
 }
 
 mrhs_status_t wilson_set_default_tiling(mrhs_wilson *h) {
-    const size_t budget = h->l2_bytes * 2 / 5;
+    const size_t budget = h->l2_bytes / 5;
     HopTiling tf = default_tiling(h->gfull, budget);
     if (!build_hop_params(h->gfull, 0, tf, h->hp_full)) {
         set_error("wilson create: no valid tiling for the full lattice");

@@ -323,7 +323,10 @@ mrhs_status_t unpack_site_data(const FieldGeom &g, const float4 *d_src, float *d
 HopTiling default_tiling(const FieldGeom &g, size_t l2_budget) {
     const int np = threads_per_site(g.N);
     const int per_row = g.XB * np;
-    int rows_max = kHopMaxThreads / per_row;
+    // Small thread blocks (about three warps, several resident per SM) measured faster than one large
+    // block per SM at 48^4: their load and arithmetic phases drift apart instead of all warps of an
+    // SM waiting on the same neighbour rows at once (profiles/r1b_tiling.md).
+    int rows_max = kHopTargetThreads / per_row;
     if (rows_max < 1) rows_max = 1;
     HopTiling best = {1, 1, 1, 1, 1};
     double best_score = -1.0;
@@ -393,7 +396,9 @@ bool build_hop_params(const FieldGeom &g, int out_parity, const HopTiling &t, Ho
     if (!ok) return false;
     p.gauge_out = p.gauge_in = nullptr;
     // default prefetch distance: one t-step of the chunk (the t+1 rows a tile reads) plus two waves of tiles
-    p.pf_dist = (unsigned)(g.nxb * t.cy * t.cz) + 2u * 148u;
+    // default prefetch distance: about half of the tiles resident on the GPU at once (two per SM).  Farther
+    // ahead the prefetched rows are evicted again before their tile runs and DRAM reads double (measured).
+    p.pf_dist = 2u * 148u;
     p.grid = (unsigned)grid;
     p.threads = (unsigned)threads;
     return true;

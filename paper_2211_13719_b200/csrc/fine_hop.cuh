@@ -8,6 +8,8 @@ namespace mrhs {
 
 // Upper bound on threads per block the hop kernel is compiled for (register budget 65536 / 384).
 constexpr int kHopMaxThreads = 384;
+// Threads per block the default tiling aims for.
+constexpr int kHopTargetThreads = 96;
 
 struct HopTiling {
     int by, bz, bt;   // sites per thread-block tile in y, z, t (x extent of a tile is the layout block XB)
