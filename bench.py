@@ -103,12 +103,16 @@ def measured_peaks():
 
 
 def ncu_traffic(key):
-    """DRAM bytes per launch from the committed ncu capture (profiles/dram_traffic.json), or None."""
+    """DRAM bytes per launch from the committed ncu capture (profiles/dram_traffic.csv), or None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "dram_traffic.json")) as f:
-            return json.load(f).get(key)
+        with open(os.path.join(ROOT, "profiles", "dram_traffic.csv")) as f:
+            for line in f:
+                parts = line.strip().split(",")
+                if len(parts) == 2 and parts[0] == key:
+                    return float(parts[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
@@ -229,6 +233,22 @@ def workload_config():
             "parallelism": "replicas only (one GPU per lattice, no collectives; north_star)"}
 
 
+# ------------------------------------------------------------------------ replicas (N > 1)
+
+def max_over_ranks(x, dist, device):
+    """max of a per-rank scalar over all ranks (the slowest replica sets the job time)."""
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_gflops(flops_step, world, ms_per_step):
+    """Whole-job throughput of `world` independent replicas (weak scaling: one lattice per GPU)."""
+    return world * flops_step / (ms_per_step * 1e-3) / 1e9
+
+
 # ------------------------------------------------------------------------ GPU arm
 
 class Workload:
@@ -296,6 +316,15 @@ def run_gpu(args):
         fdims, cdims = [16, 16, 16, 16], [4, 4, 4, 4]
     stream = torch.cuda.Stream(device)
     wl = Workload(torch, mrhs, syn, device, stream, fdims, cdims, nb, N)
+    tiling_note = "library default"
+    for which in (0, 1):
+        if args.hop_tiling:
+            t = [int(x) for x in args.hop_tiling.split(",")]
+            mrhs.wilson_set_tiling(wl.w.h, which, t[:3], t[3:5])
+        if args.hop_prefetch is not None:
+            mrhs.wilson_set_prefetch(wl.w.h, which, args.hop_prefetch)
+    if args.hop_tiling or args.hop_prefetch is not None:
+        tiling_note = "override: tiling %s prefetch %s" % (args.hop_tiling, args.hop_prefetch)
     launches = wl.launches()
     work = step_work(fdims, cdims, nb, N)
     flops_step = sum(w[1] for w in work)
@@ -323,12 +352,9 @@ def run_gpu(args):
     clocks = sampler.stop() if rank == 0 else None
     total_ms = evs[0][0].elapsed_time(evs[K - 1][nseg])
     seg_ms = [sum(evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)) / K for i in range(nseg)]
-    t = torch.tensor([total_ms], dtype=torch.float64, device=device)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist, device)
     ms_per_step = total_ms / K
-    value = world * flops_step / (ms_per_step * 1e-3) / 1e9
+    value = job_gflops(flops_step, world, ms_per_step)
 
     # ------------------------------------------------------------ end to end, host buffers
     e2e = run_e2e(torch, mrhs, wl, args, barrier, dist, device, world, flops_step)
@@ -361,6 +387,7 @@ def run_gpu(args):
         gf, ms, cores = time_oracle(args.cpu_steps, 1)
         cpu = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": CPU_SAMPLE, "ms_per_sample_step": ms}
     cfg = workload_config()
+    cfg["hop_tiling"] = {"dhop": mrhs.wilson_get_tiling(wl.w.h, 0), "meooe": mrhs.wilson_get_tiling(wl.w.h, 1), "source": tiling_note}
     if args.small:
         cfg["workload"] = "SMALL smoke workload (16^4 fine, 4^4 coarse) -- not the benchmark configuration"
         cfg["fine_dims"], cfg["coarse_dims"] = fdims, cdims
@@ -419,11 +446,8 @@ def run_e2e(torch, mrhs, wl, args, barrier, dist, device, world, flops_step):
         step()   # every host entry synchronises its stream before returning
     barrier()
     dt = time.perf_counter() - t0
-    t = torch.tensor([dt], dtype=torch.float64, device=device)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    dt = float(t.item()) / E
-    return {"value": world * flops_step / dt / 1e9, "unit": "GFLOP/s", "h2d_bytes_per_step": h2d,
+    dt = max_over_ranks(dt, dist, device) / E
+    return {"value": job_gflops(flops_step, world, dt * 1e3), "unit": "GFLOP/s", "h2d_bytes_per_step": h2d,
             "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3, "steps": E,
             "api": "mrhs_wilson_apply_host / mrhs_coarse_apply_host (pinned canonical host buffers)"}
 
@@ -536,6 +560,8 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=8, help="oracle sample steps timed for cpu_baseline")
     ap.add_argument("--sweep", default=None, help="write the per-operator N_rhs sweep to this .jsonl and exit")
     ap.add_argument("--sweep-iters", type=int, default=30)
+    ap.add_argument("--hop-tiling", default=None, help="by,bz,bt,cy,cz for D_hop and M_eooe instead of the library default")
+    ap.add_argument("--hop-prefetch", type=int, default=None, help="L2 prefetch distance in tiles (0 = off)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours" and not args.sweep:
         args.warmup = 3   # timing rule: at least 3 warm-up steps

@@ -1,0 +1,133 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (library
+default tiling), on sampled output sites the oracle computes one by one (SURVEY.md Sec. 8(d)
+"Parity at 48^4"): config 5 (48^4, N_rhs = 12) for D_hop, M_eooe and M_ooee, and config 4
+(6^3x32, nb = 40) full-field is in test_gpu_coarse.py.  The stencils are local, so the oracle needs
+only the sampled sites' neighbours and links, gathered from the device inputs (never from outputs)."""
+import numpy as np
+import pytest
+
+import synth_inputs as syn
+from helpers import rel_l2_per_rhs
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+if not torch.cuda.is_available():
+    pytest.skip("needs a CUDA device", allow_module_level=True)
+
+import oracle                      # noqa: E402
+import paper_2211_13719_b200 as mrhs   # noqa: E402
+from gpu_common import TOL   # noqa: E402
+
+DIMS, NRHS, MASS, CSW, SEED = [48, 48, 48, 48], 12, -0.05, 1.5, 5
+NSAMPLE = 4096
+
+
+def _sample_sites(dims, n, seed):
+    """Seeded sample of lex indices that includes every corner and sites on every face."""
+    X, Y, Z, T = dims
+    rng = np.random.default_rng([seed, 0x9E])
+    c = rng.integers(0, [X, Y, Z, T], size=(n, 4))
+    k = 0
+    for cx in (0, X - 1):                       # 16 corners
+        for cy in (0, Y - 1):
+            for cz in (0, Z - 1):
+                for ct in (0, T - 1):
+                    c[k] = (cx, cy, cz, ct); k += 1
+    for mu in range(4):                         # 64 sites on each of the 8 faces
+        for edge in (0, dims[mu] - 1):
+            c[k:k + 64, mu] = edge; k += 64
+    lex = c[:, 0] + X * (c[:, 1] + Y * (c[:, 2] + Z * c[:, 3]))
+    return np.unique(lex)
+
+
+def _nbr_lex(dims, lex, mu, sign):
+    X, Y, Z, T = dims
+    c = [lex % X, (lex // X) % Y, (lex // (X * Y)) % Z, lex // (X * Y * Z)]
+    c[mu] = (c[mu] + sign) % dims[mu]
+    return c[0] + X * (c[1] + Y * (c[2] + Z * c[3]))
+
+
+def _gather_hop_inputs(dims, U_dev, psi_dev, lex, cb):
+    """links [n][8][3][3] (U_mu(x), then U_mu(x-mu)) and nbrs [n][8][4][3][N] (psi(x+mu), then psi(x-mu))
+    for oracle.dhop_sites; psi_dev is the canonical full field, or (cb) the field of the other parity."""
+    n = lex.size
+    links = np.empty((n, 8, 3, 3), dtype=np.complex64)
+    nbrs = np.empty((n, 8, 4, 3, psi_dev.shape[-1]), dtype=np.complex64)
+    t_lex = torch.from_numpy(lex).cuda()
+    links[:, 0:4] = U_dev[t_lex].cpu().numpy()
+    for mu in range(4):
+        fw = torch.from_numpy(_nbr_lex(dims, lex, mu, +1)).cuda()
+        bw = torch.from_numpy(_nbr_lex(dims, lex, mu, -1)).cuda()
+        links[:, 4 + mu] = U_dev[bw, mu].cpu().numpy()
+        nbrs[:, mu] = psi_dev[(fw >> 1) if cb else fw].cpu().numpy()
+        nbrs[:, 4 + mu] = psi_dev[(bw >> 1) if cb else bw].cpu().numpy()
+    return links, nbrs
+
+
+@pytest.fixture(scope="module")
+def config5():
+    dev = torch.device("cuda", 0)
+    U = syn.gauge_torch(DIMS, SEED, dev)
+    psi = syn.spinor_torch(syn.volume(DIMS), NRHS, SEED, dev)
+    w = mrhs.Wilson(DIMS, NRHS, MASS, CSW, U)
+    yield U, psi, w
+    w.close()
+
+
+def test_config5_dhop_sampled_sites(config5):
+    U, psi, w = config5
+    lex = _sample_sites(DIMS, NSAMPLE, 1)
+    d_in = w.import_field(psi, mrhs.FULL)
+    d_out = w.empty(mrhs.FULL)
+    w.dhop(d_in, d_out)
+    torch.cuda.synchronize()
+    got = w.export_field(d_out, mrhs.FULL)[torch.from_numpy(lex).cuda()].cpu().numpy()
+    del d_in, d_out
+    links, nbrs = _gather_hop_inputs(DIMS, U, psi, lex, cb=False)
+    want = oracle.dhop_sites(links, nbrs)
+    err = rel_l2_per_rhs(got, want)
+    assert err.max() < TOL, err
+
+
+@pytest.mark.parametrize("out_parity", [0, 1])
+def test_config5_meooe_sampled_sites(config5, out_parity):
+    U, psi, w = config5
+    X, Y, Z, T = DIMS
+    lex_all = torch.arange(syn.volume(DIMS), device="cuda")
+    par = (lex_all % X + (lex_all // X) % Y + (lex_all // (X * Y)) % Z + lex_all // (X * Y * Z)) % 2
+    psi_in = psi[par == (1 - out_parity)].contiguous()          # canonical checkerboarded input, index lex >> 1
+    del lex_all, par
+    lex = _sample_sites(DIMS, NSAMPLE, 2 + out_parity)
+    c = [lex % X, (lex // X) % Y, (lex // (X * Y)) % Z, lex // (X * Y * Z)]
+    lex = lex[(c[0] + c[1] + c[2] + c[3]) % 2 == out_parity]
+    d_in = w.import_field(psi_in, 1 - out_parity)
+    d_out = w.empty(out_parity)
+    w.meooe(d_in, d_out, out_parity)
+    torch.cuda.synchronize()
+    got = w.export_field(d_out, out_parity)[torch.from_numpy(lex >> 1).cuda()].cpu().numpy()
+    del d_in, d_out
+    links, nbrs = _gather_hop_inputs(DIMS, U, psi_in, lex, cb=True)
+    want = oracle.dhop_sites(links, nbrs)
+    err = rel_l2_per_rhs(got, want)
+    assert err.max() < TOL, err
+
+
+def test_config5_mooee_sampled_sites(config5):
+    U, psi, w = config5
+    lex = _sample_sites(DIMS, 256, 4)
+    d_in = w.import_field(psi, mrhs.FULL)
+    d_out = w.empty(mrhs.FULL)
+    w.mooee(d_in, d_out, mrhs.FULL)
+    torch.cuda.synchronize()
+    t_lex = torch.from_numpy(lex).cuda()
+    got = w.export_field(d_out, mrhs.FULL)[t_lex].cpu().numpy()
+    del d_in, d_out
+    Uh = U.cpu().numpy().astype(np.complex128)
+    C = np.empty((lex.size, 2, 6, 6), dtype=np.complex128)
+    for i, x in enumerate(lex):
+        M = oracle.clover_site_matrix(DIMS, Uh, MASS, CSW, int(x))     # 12x12, index 3*spin + colour
+        C[i, 0], C[i, 1] = M[0:6, 0:6], M[6:12, 6:12]
+    want = oracle.mooee(C, psi[t_lex].cpu().numpy())
+    err = rel_l2_per_rhs(got, want)
+    assert err.max() < TOL, err
