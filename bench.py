@@ -502,6 +502,8 @@ def run_sweep(args):
 
     base = {}
     fine = [("config2", [24, 24, 24, 24], [1, 4, 12, 24, 48], 2), ("config5", [48, 48, 48, 48], [1, 12, 24], 5)]
+    if "fine" not in args.sweep_ops.split(","):
+        fine = []
     for cfg, dims, ns, seed in fine:
         V = vol(dims)
         U = syn.gauge_torch(dims, seed, device)
@@ -526,6 +528,8 @@ def run_sweep(args):
             del psi, o_full, ie, io, oe, oo, t0
         del U
     coarse = [("config3", [8, 8, 8, 8], 24, [1, 12, 24, 64], 3), ("config4", [6, 6, 6, 32], 40, [12, 24, 48, 96], 4)]
+    if "coarse" not in args.sweep_ops.split(","):
+        coarse = []
     for cfg, dims, nb, ns, seed in coarse:
         V = vol(dims)
         A = syn.coarse_links_torch(dims, nb, seed, device)
@@ -560,6 +564,7 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=8, help="oracle sample steps timed for cpu_baseline")
     ap.add_argument("--sweep", default=None, help="write the per-operator N_rhs sweep to this .jsonl and exit")
     ap.add_argument("--sweep-iters", type=int, default=30)
+    ap.add_argument("--sweep-ops", default="fine,coarse", help="which operator families the sweep covers")
     ap.add_argument("--hop-tiling", default=None, help="by,bz,bt,cy,cz for D_hop and M_eooe instead of the library default")
     ap.add_argument("--hop-prefetch", type=int, default=None, help="L2 prefetch distance in tiles (0 = off)")
     args = ap.parse_args()

@@ -50,7 +50,8 @@ struct mrhs_coarse {
     CoarseGeom g;
     int mode;
     cudaStream_t st;
-    float2 *links;
+    float2 *links;                 // math_mode 0: [site][p][col][row] complex; math_mode 1: the tensor-core order (coarse.cuh)
+    int tc_grid;                   // persistent grid of the tensor-core kernel
     void *st_canon, *st_in, *st_out;
     size_t st_bytes;
 };
@@ -310,8 +311,8 @@ mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nb
         set_error("coarse create: no specialisation for nbasis=%d nrhs=%d (nbasis 24|40, nrhs 1,2,4,8,12,16,24,32,48,64,96)", nbasis, nrhs);
         return MRHS_ERR_UNSUPPORTED;
     }
-    if (math_mode == 1) {
-        set_error("coarse create: the tensor-core variant is not built in this version");
+    if (math_mode == 1 && !coarse_tc_supported(nbasis, nrhs)) {
+        set_error("coarse create: no tensor-core specialisation for nbasis=%d nrhs=%d (nbasis 24|40, even nrhs in 2,4,8,12,16,24,32,48,64,96)", nbasis, nrhs);
         return MRHS_ERR_UNSUPPORTED;
     }
     mrhs_coarse *h = new (std::nothrow) mrhs_coarse();
@@ -325,8 +326,14 @@ mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nb
     const size_t bytes = (size_t)h->g.nsites * 9 * nbasis * nbasis * sizeof(float2);
     cudaError_t e = cudaMalloc(&h->links, bytes);
     if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaMalloc(links)", __FILE__, __LINE__); }
-    mrhs_status_t s = pack_coarse_links(h->g, (const float2 *)d_links, h->links, h->st);
-    if (s == MRHS_OK) s = coarse_fma_prepare(h->g);
+    mrhs_status_t s;
+    if (math_mode == 1) {
+        s = pack_coarse_links_tc(h->g, (const float2 *)d_links, (float *)h->links, h->st);
+        if (s == MRHS_OK) s = coarse_tc_prepare(h->g, &h->tc_grid);
+    } else {
+        s = pack_coarse_links(h->g, (const float2 *)d_links, h->links, h->st);
+        if (s == MRHS_OK) s = coarse_fma_prepare(h->g);
+    }
     if (s == MRHS_OK) {
         e = cudaStreamSynchronize(h->st);
         if (e != cudaSuccess) s = cuda_fail(e, "cudaStreamSynchronize", __FILE__, __LINE__);
@@ -340,6 +347,7 @@ mrhs_status_t mrhs_coarse_apply(mrhs_coarse_t *h, const void *d_in, void *d_out)
     MRHS_REQUIRE(h && d_in && d_out, "coarse apply: NULL argument");
     MRHS_REQUIRE(d_in != d_out, "coarse apply: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "coarse apply: buffers must be 16-byte aligned");
+    if (h->mode == 1) return launch_coarse_tc(h->g, h->tc_grid, (const float *)h->links, d_in, d_out, h->st);
     return launch_coarse_fma(h->g, h->links, d_in, d_out, h->st);
 }
 

@@ -1,0 +1,384 @@
+// coarse_tc.cu -- coarse-level 9-point stencil, tensor-core variant:
+//   out_i(x) = sum_{p=0..8} sum_j A_p(x)_ij v_j(x + delta_p)          (reading S8)
+// evaluated on the 5th-generation tensor cores (tcgen05.mma kind::tf32, accumulator in TMEM)
+// with split-precision operands so that the fp32 tolerance of north_star holds (reading S15):
+//   a = a_hi + a_lo,  a_hi = tf32(a), a_lo = tf32(a - a_hi);   a*b ~ a_hi*b_hi + a_hi*b_lo + a_lo*b_hi
+// (three MMAs per K step, fp32 accumulation; the dropped a_lo*b_lo term is ~2^-22 relative).
+//
+// Per coarse site the complex contraction is written as ONE real GEMM accumulated over the nine
+// stencil points and the nb columns:
+//   D[128 x NT] += Aop[128 x nb] * Bop[nb x NT]
+//   Aop rows 0..nb-1      = Re A_p,   rows 64..64+nb-1 = Im A_p            (other rows unused)
+//   Bop cols 0..N-1       = Re v,     cols N..2N-1     = Im v              (NT = 2N rounded up to 16)
+// so D holds Re A Re v, Re A Im v, Im A Re v, Im A Im v and the epilogue forms
+//   Re out = D[i][n] - D[64+i][N+n],   Im out = D[i][N+n] + D[64+i][n].
+// Every matrix entry read from HBM serves all N_rhs columns (PAPER.md:23 (i)).
+//
+// Data path: fp32 links and vectors go global -> registers (coalesced 128-bit loads) -> hi/lo split
+// -> shared memory in the no-swizzle K-major core-matrix layout tcgen05.mma reads (8 rows x 16 bytes
+// per core matrix, 16-byte K chunks LBO apart).  One elected thread issues the MMAs; completion comes
+// back on an mbarrier via tcgen05.commit.  Several CTAs share an SM, so one CTA's operand conversion
+// overlaps another's MMAs.
+#include "coarse.cuh"
+
+namespace mrhs {
+
+namespace {
+
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok)
+                     : "r"(smem_addr(bar)), "r"(parity)
+                     : "memory");
+    } while (!ok);
+}
+
+// ---- tcgen05 wrappers (PTX ISA 8.6+, sm_100a)
+template <int COLS> __device__ __forceinline__ void tmem_alloc(uint32_t *slot) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_addr(slot)), "n"(COLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+template <int COLS> __device__ __forceinline__ void tmem_free(uint32_t taddr) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(COLS) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// generic-proxy writes to shared memory -> visible to the async proxy (the MMA's operand reads)
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// D[tmem] (+)= A[smem] * B[smem], tf32 inputs, fp32 accumulate, issued by one thread for the CTA
+__device__ __forceinline__ void mma_tf32(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n"
+        " tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// arrive on bar once every MMA issued so far by this thread has completed
+__device__ __forceinline__ void mma_commit(uint64_t *bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+// 16 consecutive fp32 columns of this thread's TMEM lane
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
+    uint32_t r[16];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 16; i++) v[i] = __uint_as_float(r[i]);
+}
+
+// Shared-memory matrix descriptor, K-major, no swizzle: core matrix = 8 rows x 16 bytes stored as
+// 128 contiguous bytes; SBO = distance between 8-row groups, LBO = distance between the two
+// 16-byte K chunks of one MMA (K = 8 tf32 = 32 bytes).  Bits: [0,14) address >> 4, [16,30) LBO >> 4,
+// [32,46) SBO >> 4, [46,48) descriptor version (1 on sm_100), [61,64) swizzle mode (0 = none).
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    uint64_t d = 0;
+    d |= (uint64_t)((addr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16;
+    d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32;
+    d |= (uint64_t)1 << 46;
+    return d;
+}
+// Instruction descriptor, kind::tf32: [4,6) D format (1 = f32), [7,10) A format (2 = tf32), [10,13) B
+// format (2 = tf32), bit 15 / 16 A / B major (0 = K-major), [17,23) N >> 3, [24,29) M >> 4.
+__host__ __device__ constexpr uint32_t instr_desc_tf32(int M, int N) {
+    return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
+// round-to-nearest tf32 (low 13 mantissa bits cleared) and the remainder, itself rounded to tf32
+__device__ __forceinline__ void split_tf32(float x, float &hi, float &lo) {
+    uint32_t h;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(h) : "f"(x));
+    hi = __uint_as_float(h);
+    uint32_t l;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(l) : "f"(x - hi));
+    lo = __uint_as_float(l);
+}
+__device__ __forceinline__ void split4(float4 x, float4 &hi, float4 &lo) {
+    split_tf32(x.x, hi.x, lo.x);
+    split_tf32(x.y, hi.y, lo.y);
+    split_tf32(x.z, hi.z, lo.z);
+    split_tf32(x.w, hi.w, lo.w);
+}
+
+constexpr int pow2_cols(int n) { return n <= 32 ? 32 : n <= 64 ? 64 : n <= 128 ? 128 : n <= 256 ? 256 : 512; }
+
+template <int NB, int N>
+struct TcCfg {
+    static_assert(N % 2 == 0, "the tensor-core variant uses the RHS-pair element layout (even N_rhs)");
+    static_assert(NB % 8 == 0 && NB <= 64, "nbasis must be a multiple of the MMA K (8) and fit 64 rows");
+    static constexpr int NP = N / 2;                          // float4 elements per component
+    static constexpr int NT = ((2 * N + 15) / 16) * 16;       // MMA N: Re and Im columns of every RHS
+    static constexpr int KC = NB / 4;                         // 16-byte K chunks per stencil point
+    static constexpr int KS = NB / 8;                         // MMA K steps per stencil point
+    static constexpr int THREADS = NT <= 64 ? 128 : 256;
+    static constexpr int A_LBO = 128 * 16;                    // bytes between K chunks of the A operand
+    static constexpr int B_LBO = NT * 16;
+    static constexpr int A_BYTES = KC * A_LBO;                // one of hi / lo
+    static constexpr int B_BYTES = KC * B_LBO;
+    static constexpr int OPER_BYTES = 2 * A_BYTES + 2 * B_BYTES;
+    static constexpr int S_PITCH = 129;                       // epilogue scratch S[col][lane], floats
+    static constexpr int S_BYTES = NT * S_PITCH * 4;
+    static constexpr int DATA_BYTES = OPER_BYTES > S_BYTES ? OPER_BYTES : S_BYTES;
+    static constexpr int SMEM_BYTES = DATA_BYTES + 32;        // + mbarrier + TMEM address slot
+    static constexpr int TMEM_COLS = pow2_cols(NT);
+    static constexpr int A_UNITS = 2 * KC * NB;               // 16-byte units of one link matrix
+    static constexpr int B_UNITS = KC * NP;                   // (K chunk, RHS pair) work items of one vector
+    static_assert(NT <= 256, "MMA N limit");
+};
+
+// links: native tensor-core layout [site][p][part Re/Im][K chunk][row][4 columns] fp32 (pack_coarse_links_tc)
+// in/out: coarse vectors [site][component][RHS pair] float4 = (re0 re1 im0 im1), as in the FMA variant
+template <int NB, int N>
+__global__ void __launch_bounds__(TcCfg<NB, N>::THREADS)
+coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, const float4 *__restrict__ links,
+                 const float4 *__restrict__ in, float4 *__restrict__ out) {
+    typedef TcCfg<NB, N> C;
+    constexpr int A_IT = (C::A_UNITS + C::THREADS - 1) / C::THREADS;
+    constexpr int B_IT = (C::B_UNITS + C::THREADS - 1) / C::THREADS;
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char *a_hi = smem, *a_lo = smem + C::A_BYTES;
+    unsigned char *b_hi = smem + 2 * C::A_BYTES, *b_lo = b_hi + C::B_BYTES;
+    float *S = reinterpret_cast<float *>(smem);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem + C::DATA_BYTES);
+    uint32_t *tslot = reinterpret_cast<uint32_t *>(smem + C::DATA_BYTES + 8);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    // one-time setup: barrier, zeroed operand area (pad rows / columns), TMEM accumulator
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int i = tid; i < C::OPER_BYTES / 16; i += C::THREADS) reinterpret_cast<float4 *>(smem)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (warp == 0) tmem_alloc<C::TMEM_COLS>(tslot);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tslot;
+    constexpr uint32_t idesc = instr_desc_tf32(128, C::NT);
+
+    uint32_t nstage = 0;   // operand stages handed to the tensor core so far (same in every thread)
+    for (long long site = blockIdx.x; site < nsites; site += gridDim.x) {
+        int c[4];
+        {
+            long long s = site;
+            c[0] = (int)(s % X); s /= X;
+            c[1] = (int)(s % Y); s /= Y;
+            c[2] = (int)(s % Z);
+            c[3] = (int)(s / Z);
+        }
+        const int ext[4] = {X, Y, Z, T};
+        for (int p = 0; p < 9; p++) {
+            // neighbour of stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
+            long long nbr = site;
+            if (p > 0) {
+                const int mu = (p - 1) & 3, d = p <= 4 ? 1 : -1;
+                int cc[4] = {c[0], c[1], c[2], c[3]};
+                cc[mu] = (cc[mu] + d + ext[mu]) % ext[mu];
+                nbr = cc[0] + (long long)X * (cc[1] + (long long)Y * (cc[2] + (long long)Z * cc[3]));
+            }
+            // raw fp32 operands into registers while the previous stage's MMAs still run
+            const float4 *lp = links + ((size_t)site * 9 + p) * C::A_UNITS;
+            const float4 *vp = in + (size_t)nbr * NB * C::NP;
+            float4 ra[A_IT];
+            float4 rb[B_IT][4];
+#pragma unroll
+            for (int it = 0; it < A_IT; it++) {
+                const int u = tid + it * C::THREADS;
+                if (u < C::A_UNITS) ra[it] = __ldg(lp + u);
+            }
+#pragma unroll
+            for (int it = 0; it < B_IT; it++) {
+                const int w = tid + it * C::THREADS;
+                if (w < C::B_UNITS) {
+                    const int kc = w / C::NP, q = w - kc * C::NP;
+#pragma unroll
+                    for (int e = 0; e < 4; e++) rb[it][e] = __ldg(vp + (size_t)(4 * kc + e) * C::NP + q);
+                }
+            }
+            // the single operand buffer is free once the previous stage's MMAs have completed
+            if (nstage > 0) mbar_wait(bar, (nstage - 1) & 1);
+#pragma unroll
+            for (int it = 0; it < A_IT; it++) {
+                const int u = tid + it * C::THREADS;
+                if (u < C::A_UNITS) {
+                    const int part = u / (C::KC * NB), r = u - part * (C::KC * NB);
+                    const int kc = r / NB, row = r - kc * NB;
+                    float4 hi, lo;
+                    split4(ra[it], hi, lo);
+                    const int off = kc * C::A_LBO + (part * 64 + row) * 16;
+                    *reinterpret_cast<float4 *>(a_hi + off) = hi;
+                    *reinterpret_cast<float4 *>(a_lo + off) = lo;
+                }
+            }
+#pragma unroll
+            for (int it = 0; it < B_IT; it++) {
+                const int w = tid + it * C::THREADS;
+                if (w < C::B_UNITS) {
+                    const int kc = w / C::NP, q = w - kc * C::NP;
+                    const float4 x0 = rb[it][0], x1 = rb[it][1], x2 = rb[it][2], x3 = rb[it][3];
+                    float4 hi, lo;
+                    const int base = kc * C::B_LBO;
+                    split4(make_float4(x0.x, x1.x, x2.x, x3.x), hi, lo);        // Re, RHS 2q
+                    *reinterpret_cast<float4 *>(b_hi + base + (2 * q) * 16) = hi;
+                    *reinterpret_cast<float4 *>(b_lo + base + (2 * q) * 16) = lo;
+                    split4(make_float4(x0.y, x1.y, x2.y, x3.y), hi, lo);        // Re, RHS 2q+1
+                    *reinterpret_cast<float4 *>(b_hi + base + (2 * q + 1) * 16) = hi;
+                    *reinterpret_cast<float4 *>(b_lo + base + (2 * q + 1) * 16) = lo;
+                    split4(make_float4(x0.z, x1.z, x2.z, x3.z), hi, lo);        // Im, RHS 2q
+                    *reinterpret_cast<float4 *>(b_hi + base + (N + 2 * q) * 16) = hi;
+                    *reinterpret_cast<float4 *>(b_lo + base + (N + 2 * q) * 16) = lo;
+                    split4(make_float4(x0.w, x1.w, x2.w, x3.w), hi, lo);        // Im, RHS 2q+1
+                    *reinterpret_cast<float4 *>(b_hi + base + (N + 2 * q + 1) * 16) = hi;
+                    *reinterpret_cast<float4 *>(b_lo + base + (N + 2 * q + 1) * 16) = lo;
+                }
+            }
+            fence_async_smem();
+            __syncthreads();
+            if (tid == 0) {
+                tc_fence_after();
+                const uint32_t ah = smem_addr(a_hi), al = smem_addr(a_lo), bh = smem_addr(b_hi), bl = smem_addr(b_lo);
+#pragma unroll
+                for (int ks = 0; ks < C::KS; ks++) {
+                    const uint64_t dah = smem_desc(ah + ks * 2 * C::A_LBO, C::A_LBO, 128);
+                    const uint64_t dal = smem_desc(al + ks * 2 * C::A_LBO, C::A_LBO, 128);
+                    const uint64_t dbh = smem_desc(bh + ks * 2 * C::B_LBO, C::B_LBO, 128);
+                    const uint64_t dbl = smem_desc(bl + ks * 2 * C::B_LBO, C::B_LBO, 128);
+                    mma_tf32(tmem, dal, dbh, idesc, (p | ks) != 0);
+                    mma_tf32(tmem, dah, dbl, idesc, 1);
+                    mma_tf32(tmem, dah, dbh, idesc, 1);
+                }
+                mma_commit(bar);
+            }
+            nstage++;
+        }
+        // all nine points accumulated: TMEM -> shared scratch S[col][lane] -> combine -> global
+        mbar_wait(bar, (nstage - 1) & 1);
+        tc_fence_after();
+        {
+            const int quarter = warp & 3;
+            for (int ch = warp >> 2; ch < C::NT / 16; ch += C::THREADS / 128) {
+                float v[16];
+                tmem_ld16(tmem + ((uint32_t)(quarter * 32) << 16) + ch * 16, v);
+#pragma unroll
+                for (int k = 0; k < 16; k++) S[(ch * 16 + k) * C::S_PITCH + quarter * 32 + lane] = v[k];
+            }
+        }
+        tc_fence_before();
+        __syncthreads();
+        for (int idx = tid; idx < NB * C::NP; idx += C::THREADS) {
+            const int i = idx / C::NP, q = idx - i * C::NP;
+            const int n0 = 2 * q, n1 = 2 * q + 1;
+            float4 o;
+            o.x = S[n0 * C::S_PITCH + i] - S[(N + n0) * C::S_PITCH + 64 + i];
+            o.y = S[n1 * C::S_PITCH + i] - S[(N + n1) * C::S_PITCH + 64 + i];
+            o.z = S[(N + n0) * C::S_PITCH + i] + S[n0 * C::S_PITCH + 64 + i];
+            o.w = S[(N + n1) * C::S_PITCH + i] + S[n1 * C::S_PITCH + 64 + i];
+            out[((size_t)site * NB + i) * C::NP + q] = o;
+        }
+        __syncthreads();   // S (aliasing the operand buffer) is free for the next site
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_free<C::TMEM_COLS>(tmem);
+}
+
+// canonical A[site][p][row][col] complex -> [site][p][part][K chunk][row][4 columns] fp32; one thread per float
+__global__ void pack_links_tc_kernel(int nb, const float2 *__restrict__ src, float *__restrict__ dst, long long total) {
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    const int kcn = nb / 4;
+    int e = (int)(idx & 3);
+    long long q = idx >> 2;
+    int row = (int)(q % nb); q /= nb;
+    int kc = (int)(q % kcn); q /= kcn;
+    int part = (int)(q & 1);
+    long long mat = q >> 1;
+    float2 a = src[(mat * nb + row) * nb + 4 * kc + e];
+    dst[idx] = part ? a.y : a.x;
+}
+
+template <int NB, int N>
+mrhs_status_t tc_prepare_t(int *ctas_per_sm) {
+    typedef TcCfg<NB, N> C;
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_tc_kernel<NB, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    int occ = 0;
+    MRHS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, coarse_tc_kernel<NB, N>, C::THREADS, C::SMEM_BYTES));
+    const int tmem_cap = 512 / C::TMEM_COLS;   // TMEM columns are not part of the occupancy calculation
+    if (occ > tmem_cap) occ = tmem_cap;
+    if (occ < 1) { set_error("coarse tensor-core kernel does not fit an SM (nbasis=%d nrhs=%d)", NB, N); return MRHS_ERR_UNSUPPORTED; }
+    *ctas_per_sm = occ;
+    return MRHS_OK;
+}
+template <int NB, int N>
+mrhs_status_t tc_launch_t(const CoarseGeom &g, int grid, const float *links, const void *in, void *out, cudaStream_t st) {
+    typedef TcCfg<NB, N> C;
+    coarse_tc_kernel<NB, N><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, g.nsites, (const float4 *)links,
+                                                                      (const float4 *)in, (float4 *)out);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+#define MRHS_TC_N_LIST(F, NB) F(NB, 2) F(NB, 4) F(NB, 8) F(NB, 12) F(NB, 16) F(NB, 24) F(NB, 32) F(NB, 48) F(NB, 64) F(NB, 96)
+
+}  // namespace
+
+bool coarse_tc_supported(int nb, int nrhs) {
+#define MRHS_CASE(NB, NN) if (nb == NB && nrhs == NN) return true;
+    MRHS_TC_N_LIST(MRHS_CASE, 24)
+    MRHS_TC_N_LIST(MRHS_CASE, 40)
+#undef MRHS_CASE
+    return false;
+}
+
+mrhs_status_t coarse_tc_prepare(const CoarseGeom &g, int *grid) {
+    int dev = 0, sms = 0, per_sm = 0;
+    MRHS_CUDA(cudaGetDevice(&dev));
+    MRHS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    mrhs_status_t s = MRHS_ERR_UNSUPPORTED;
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) s = tc_prepare_t<NB, NN>(&per_sm);
+    MRHS_TC_N_LIST(MRHS_CASE, 24)
+    MRHS_TC_N_LIST(MRHS_CASE, 40)
+#undef MRHS_CASE
+    if (s != MRHS_OK) {
+        if (per_sm == 0 && !coarse_tc_supported(g.nb, g.N))
+            set_error("coarse apply: no tensor-core specialisation for nbasis=%d nrhs=%d", g.nb, g.N);
+        return s;
+    }
+    long long want = (long long)per_sm * sms;
+    *grid = (int)(want < g.nsites ? want : g.nsites);
+    return MRHS_OK;
+}
+
+mrhs_status_t launch_coarse_tc(const CoarseGeom &g, int grid, const float *d_links, const void *d_in, void *d_out, cudaStream_t st) {
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return tc_launch_t<NB, NN>(g, grid, d_links, d_in, d_out, st);
+    MRHS_TC_N_LIST(MRHS_CASE, 24)
+    MRHS_TC_N_LIST(MRHS_CASE, 40)
+#undef MRHS_CASE
+    set_error("coarse apply: no tensor-core specialisation for nbasis=%d nrhs=%d", g.nb, g.N);
+    return MRHS_ERR_UNSUPPORTED;
+}
+
+mrhs_status_t pack_coarse_links_tc(const CoarseGeom &g, const float2 *d_canonical, float *d_native, cudaStream_t st) {
+    long long total = g.nsites * 9 * g.nb * g.nb * 2;
+    long long blocks = (total + 255) / 256;
+    pack_links_tc_kernel<<<(unsigned)blocks, 256, 0, st>>>(g.nb, d_canonical, d_native, total);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+}  // namespace mrhs

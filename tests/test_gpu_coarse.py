@@ -68,6 +68,62 @@ def test_config4_coarsest_level(nrhs):
     c.close()
 
 
+# ---- row a6: the tensor-core variant (tcgen05 kind::tf32, hi/lo split operands) is held to the same tolerance
+TC_SMALL = [([2, 2, 2, 2], 24, n) for n in (2, 4, 8, 12, 16, 24, 32, 48, 64, 96)] + \
+           [([3, 2, 4, 2], 40, n) for n in (2, 4, 8, 12, 16, 24, 32, 48, 64, 96)] + \
+           [([5, 3, 2, 4], 24, 12), ([4, 4, 4, 6], 40, 12), ([7, 5, 3, 11], 40, 24)]
+
+
+@pytest.mark.parametrize("cdims,nb,nrhs", TC_SMALL)
+def test_coarse_tensor_core_matches_oracle_small(cdims, nb, nrhs):
+    A = syn.coarse_links_np(cdims, nb, 3)
+    v = syn.coarse_vector_np(cdims, nb, nrhs, 3)
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=1)
+    want = oracle.coarse_apply(cdims, A, v)
+    err = rel_l2_per_rhs(gpu_coarse(c, v), want)
+    assert err.max() < TOL, err
+    # a second apply on the same handle (persistent barrier phases, reused TMEM) gives the same result
+    err = rel_l2_per_rhs(gpu_coarse(c, v), want)
+    assert err.max() < TOL, err
+    c.close()
+
+
+@pytest.mark.parametrize("nrhs", [12, 24, 48, 96])
+def test_config4_tensor_core(nrhs):
+    cdims, nb = [6, 6, 6, 32], 40
+    A = syn.coarse_links_np(cdims, nb, 4)
+    v = syn.coarse_vector_np(cdims, nb, nrhs, 4)
+    want = oracle.coarse_apply(cdims, A, v)
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=1)
+    err_tc = rel_l2_per_rhs(gpu_coarse(c, v), want)
+    assert err_tc.max() < TOL, err_tc
+    c.close()
+    # the two math modes agree with each other far inside the tolerance
+    c0 = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=0)
+    err_fma = rel_l2_per_rhs(gpu_coarse(c0, v), want)
+    c0.close()
+    assert err_tc.max() < 20 * max(err_fma.max(), 1e-7), (err_tc.max(), err_fma.max())
+
+
+@pytest.mark.parametrize("nrhs", [12, 64])
+def test_config3_tensor_core(nrhs):
+    cdims, nb = [8, 8, 8, 8], 24
+    A = syn.coarse_links_np(cdims, nb, 3)
+    v = syn.coarse_vector_np(cdims, nb, nrhs, 3)
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=1)
+    err = rel_l2_per_rhs(gpu_coarse(c, v), oracle.coarse_apply(cdims, A, v))
+    assert err.max() < TOL, err
+    c.close()
+
+
+def test_coarse_tensor_core_rejects_odd_nrhs():
+    cdims, nb = [2, 2, 2, 2], 24
+    A = dev(syn.coarse_links_np(cdims, nb, 3))
+    with pytest.raises(mrhs.MrhsError) as e:
+        mrhs.Coarse(cdims, nb, 1, A, math_mode=1)
+    assert e.value.status == mrhs.ERR_UNSUPPORTED
+
+
 def test_coarse_errors():
     cdims, nb = [2, 2, 2, 2], 24
     A = dev(syn.coarse_links_np(cdims, nb, 3))
