@@ -13,6 +13,7 @@ N_rhs = 12):
     M_ooee (full lattice)                                  row a4
     Schur sequence M_eooe, M_ooee, M_eooe                  row a7
     coarse 9-point apply, FP32 FMA                         row a5
+    coarse 9-point apply, tensor cores (3xTF32, tcgen05)    row a6
 
 All fields are resident in HBM in the library's native layout when the timed region starts; the
 working set of every launch (>= 0.85 GB) is far larger than the 126 MB L2, so no flush is needed
@@ -89,6 +90,7 @@ def step_work(fdims, cdims, nb, N):
         ("schur_mooee_oo", clv_h_f, clv_h_b),
         ("schur_meooe_eo", hop_f, hop_b),
         ("coarse_fma", coarse_flops(nb) * Vc * N, bytes_coarse(Vc, nb, N)),
+        ("coarse_tc", coarse_flops(nb) * Vc * N, bytes_coarse(Vc, nb, N)),
     ]
 
 
@@ -226,7 +228,7 @@ def run_reference(args):
 
 def workload_config():
     return {"workload": "config 5 (48^4 fine, N_rhs=12, mass -0.05, c_sw 1.5: D_hop, M_eooe x2, M_ooee, Schur sequence) "
-                        "+ config 4 (6^3x32 coarse, nbasis 40, N_rhs=12: 9-point apply, FP32 FMA)",
+                        "+ config 4 (6^3x32 coarse, nbasis 40, N_rhs=12: 9-point apply, FP32 FMA and tensor-core variants)",
             "fine_dims": FINE_DIMS, "coarse_dims": COARSE_DIMS, "nbasis": NBASIS, "n_rhs": NRHS,
             "precision": "complex64 fields, fp32 FMA",
             "l2": "every launch touches >= 0.85 GB, far above the 126 MB L2; no flush between iterations",
@@ -270,6 +272,7 @@ class Workload:
         self.t0, self.t1 = self.w.empty(mrhs.ODD), self.w.empty(mrhs.ODD)
         A = syn.coarse_links_torch(cdims, nb, 4, device)
         self.c = mrhs.Coarse(cdims, nb, N, A, stream=stream)
+        self.c_tc = mrhs.Coarse(cdims, nb, N, A, math_mode=mrhs.COARSE_TENSOR, stream=stream)
         del A
         v = syn.spinor_torch(vol(cdims), N, 4, device, ncomp=(nb,))
         self.v = self.c.import_field(v)
@@ -285,6 +288,7 @@ class Workload:
             ("mooee", lambda: w.mooee(self.psi, self.out_full, m.FULL)),
             ("schur", lambda: w.schur_sequence(self.in_e, self.t0, self.t1, self.out_e)),
             ("coarse_fma", lambda: c.apply(self.v, self.v_out)),
+            ("coarse_tc", lambda: self.c_tc.apply(self.v, self.v_out)),
         ]
 
 
@@ -396,7 +400,7 @@ def run_gpu(args):
         "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": cfg, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
-        "gpu_launches": 8 * K, "kernels": kernels, "wall_ms_per_step": t_wall * 1e3 / K,
+        "gpu_launches": len(work) * K, "kernels": kernels, "wall_ms_per_step": t_wall * 1e3 / K,
     }
     print(json.dumps(line))
     if dist is not None:

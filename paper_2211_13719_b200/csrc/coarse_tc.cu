@@ -20,6 +20,7 @@
 // back on an mbarrier via tcgen05.commit.  Several CTAs share an SM, so one CTA's operand conversion
 // overlaps another's MMAs.
 #include "coarse.cuh"
+#include <cstdlib>
 
 namespace mrhs {
 
@@ -316,10 +317,21 @@ template <int NB, int N>
 mrhs_status_t tc_prepare_t(int *ctas_per_sm) {
     typedef TcCfg<NB, N> C;
     MRHS_CUDA(cudaFuncSetAttribute(coarse_tc_kernel<NB, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-    int occ = 0;
-    MRHS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, coarse_tc_kernel<NB, N>, C::THREADS, C::SMEM_BYTES));
-    const int tmem_cap = 512 / C::TMEM_COLS;   // TMEM columns are not part of the occupancy calculation
-    if (occ > tmem_cap) occ = tmem_cap;
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_tc_kernel<NB, N>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    // Resident CTAs per SM from the resources themselves (the occupancy API reports 1 for a kernel that
+    // allocates tensor memory): shared memory (+1 KB reserved per CTA), registers, threads, TMEM columns.
+    cudaFuncAttributes fa;
+    MRHS_CUDA(cudaFuncGetAttributes(&fa, coarse_tc_kernel<NB, N>));
+    int dev = 0, smem_sm = 0, regs_sm = 0;
+    MRHS_CUDA(cudaGetDevice(&dev));
+    MRHS_CUDA(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
+    MRHS_CUDA(cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev));
+    int occ = smem_sm / (C::SMEM_BYTES + (int)fa.sharedSizeBytes + 1024);
+    const int regs_cta = ((fa.numRegs + 7) / 8 * 8) * C::THREADS;
+    if (regs_cta > 0 && occ > regs_sm / regs_cta) occ = regs_sm / regs_cta;
+    if (occ > 2048 / C::THREADS) occ = 2048 / C::THREADS;
+    if (occ > 512 / C::TMEM_COLS) occ = 512 / C::TMEM_COLS;
+    if (occ > 8) occ = 8;
     if (occ < 1) { set_error("coarse tensor-core kernel does not fit an SM (nbasis=%d nrhs=%d)", NB, N); return MRHS_ERR_UNSUPPORTED; }
     *ctas_per_sm = occ;
     return MRHS_OK;
@@ -361,6 +373,7 @@ mrhs_status_t coarse_tc_prepare(const CoarseGeom &g, int *grid) {
     }
     long long want = (long long)per_sm * sms;
     *grid = (int)(want < g.nsites ? want : g.nsites);
+    if (getenv("MRHS_DEBUG")) fprintf(stderr, "[mrhs] coarse tensor-core kernel nb=%d N=%d: %d CTAs/SM x %d SMs, grid %d\n", g.nb, g.N, per_sm, sms, *grid);
     return MRHS_OK;
 }
 
