@@ -131,6 +131,23 @@ mrhs_status_t mrhs_wilson_get_tiling(mrhs_wilson_t *h, int which, int tile[3], i
  * set_tiling resets it to the default (296 tiles: half of the tiles resident on 148 SMs at four per SM). */
 mrhs_status_t mrhs_wilson_set_prefetch(mrhs_wilson_t *h, int which, int distance_tiles);
 
+
+/* The hopping term has two kernels computing the same map:
+ *   MRHS_HOP_GATHER  every thread gathers its eight neighbours from global memory through L1/L2
+ *                    (any N_rhs; the only kernel for odd N_rhs);
+ *   MRHS_HOP_SWEEP   a thread block sweeps a t-segment of an XB x 2 x 2 tile with the current slice,
+ *                    its halo and the links staged in shared memory by TMA bulk copies (even N_rhs;
+ *                    the default where supported).
+ * which: 0 = D_hop, 1 = M_eooe.  UNSUPPORTED if the sweep kernel is asked for with odd N_rhs.
+ * set_sweep: lt = t-slices one thread block sweeps (divides T); chunk = {cy, cz}: tiles (of 2 x 2
+ * sites in y,z) per concurrently scheduled patch; INVALID_ARG if they do not divide the lattice. */
+#define MRHS_HOP_GATHER 0
+#define MRHS_HOP_SWEEP 1
+mrhs_status_t mrhs_wilson_set_hop_kernel(mrhs_wilson_t *h, int which, int kernel);
+mrhs_status_t mrhs_wilson_get_hop_kernel(mrhs_wilson_t *h, int which, int *kernel);
+mrhs_status_t mrhs_wilson_set_sweep(mrhs_wilson_t *h, int which, int lt, const int chunk[2]);
+mrhs_status_t mrhs_wilson_get_sweep(mrhs_wilson_t *h, int which, int *lt, int chunk[2]);
+
 mrhs_status_t mrhs_wilson_destroy(mrhs_wilson_t *h);
 
 /* ---------------------------------------------------------------- coarse level */

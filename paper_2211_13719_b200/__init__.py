@@ -23,6 +23,7 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA = 0, 1, 2, 3, 4
 EVEN, ODD, FULL = 0, 1, 2
 OP_DHOP, OP_MEOOE, OP_MOOEE, OP_SCHUR = 0, 1, 2, 3
 COARSE_FMA, COARSE_TENSOR = 0, 1
+HOP_GATHER, HOP_SWEEP = 0, 1
 COARSE_MODES = (COARSE_FMA, COARSE_TENSOR)
 
 _vp = ctypes.c_void_p
@@ -40,6 +41,10 @@ _SIGNATURES = {
     "mrhs_wilson_set_tiling": (ctypes.c_int, [_vp, ctypes.c_int, _int3, _int2]),
     "mrhs_wilson_get_tiling": (ctypes.c_int, [_vp, ctypes.c_int, _int3, _int2]),
     "mrhs_wilson_set_prefetch": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
+    "mrhs_wilson_set_hop_kernel": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
+    "mrhs_wilson_get_hop_kernel": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]),
+    "mrhs_wilson_set_sweep": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _int2]),
+    "mrhs_wilson_get_sweep": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int), _int2]),
     "mrhs_wilson_destroy": (ctypes.c_int, [_vp]),
     "mrhs_coarse_create": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, ctypes.c_int, ctypes.c_int, _vp, ctypes.c_int, _vp]),
     "mrhs_coarse_apply": (ctypes.c_int, [_vp, _vp, _vp]),
@@ -197,6 +202,26 @@ def wilson_get_tiling(h, which):
 
 def wilson_set_prefetch(h, which, distance_tiles):
     _check(lib().mrhs_wilson_set_prefetch(h, int(which), int(distance_tiles)))
+
+
+def wilson_set_hop_kernel(h, which, kernel):
+    _check(lib().mrhs_wilson_set_hop_kernel(h, int(which), int(kernel)))
+
+
+def wilson_get_hop_kernel(h, which):
+    k = ctypes.c_int()
+    _check(lib().mrhs_wilson_get_hop_kernel(h, int(which), ctypes.byref(k)))
+    return k.value
+
+
+def wilson_set_sweep(h, which, lt, chunk):
+    _check(lib().mrhs_wilson_set_sweep(h, int(which), int(lt), _int2(*[int(v) for v in chunk])))
+
+
+def wilson_get_sweep(h, which):
+    lt, chunk = ctypes.c_int(), _int2()
+    _check(lib().mrhs_wilson_get_sweep(h, int(which), ctypes.byref(lt), chunk))
+    return lt.value, list(chunk)
 
 
 def wilson_apply_host(h, op, parity, h_in, h_out):

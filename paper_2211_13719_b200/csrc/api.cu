@@ -5,6 +5,7 @@
 #include <new>
 
 #include "coarse.cuh"
+#include "fine_sweep.cuh"
 #include "fine_hop.cuh"
 
 namespace mrhs {
@@ -38,6 +39,9 @@ struct mrhs_wilson {
     float4 *gauge_full, *gauge_cb[2];
     float4 *clov_full, *clov_cb[2];
     HopParams hp_full, hp_cb[2];   // hp_cb[p]: output parity p
+    SweepParams sp_full, sp_cb[2]; // the slice-sweep kernel's launch description (fine_sweep.cuh)
+    int kern[2];                   // which kernel runs D_hop [0] / M_eooe [1]: MRHS_HOP_GATHER or MRHS_HOP_SWEEP
+    int num_sms;
     size_t l2_bytes;
     // staging for the host-buffer entry
     void *st_canon, *st_in, *st_out;
@@ -112,6 +116,19 @@ mrhs_status_t wilson_set_default_tiling(mrhs_wilson *h) {
         h->hp_cb[p].gauge_out = h->gauge_cb[p];
         h->hp_cb[p].gauge_in = h->gauge_cb[1 - p];
     }
+    // slice-sweep kernel where the geometry allows it (even N_rhs); the gather kernel otherwise
+    h->kern[0] = h->kern[1] = MRHS_HOP_GATHER;
+    if (sweep_supported(h->gfull) && sweep_supported(h->gcb[0])) {
+        mrhs_status_t s = sweep_prepare();
+        if (s != MRHS_OK) return s;
+        bool ok = build_sweep_params(h->gfull, 0, default_sweep_tiling(h->gfull, h->num_sms), h->sp_full);
+        for (int p = 0; p < 2; p++) ok = ok && build_sweep_params(h->gcb[p], p, default_sweep_tiling(h->gcb[p], h->num_sms), h->sp_cb[p]);
+        if (ok) {
+            h->sp_full.gauge_out = h->sp_full.gauge_in = h->gauge_full;
+            for (int p = 0; p < 2; p++) { h->sp_cb[p].gauge_out = h->gauge_cb[p]; h->sp_cb[p].gauge_in = h->gauge_cb[1 - p]; }
+            h->kern[0] = h->kern[1] = MRHS_HOP_SWEEP;
+        }
+    }
     return MRHS_OK;
 }
 
@@ -160,6 +177,7 @@ mrhs_status_t mrhs_wilson_create(mrhs_wilson_t **out, const int dims[4], int nrh
     int dev = 0, l2 = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) { wilson_free(h); return cuda_fail(e, "device query", __FILE__, __LINE__); }
     h->l2_bytes = (size_t)l2;
     mrhs_status_t s = wilson_build(h, d_gauge, d_clover);
@@ -173,6 +191,7 @@ mrhs_status_t mrhs_dhop(mrhs_wilson_t *h, const void *d_in, void *d_out) {
     MRHS_REQUIRE(h && d_in && d_out, "dhop: NULL argument");
     MRHS_REQUIRE(d_in != d_out, "dhop: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "dhop: buffers must be 16-byte aligned");
+    if (h->kern[0] == MRHS_HOP_SWEEP) return launch_sweep(h->sp_full, d_in, d_out, h->st);
     return launch_hop(h->hp_full, h->nrhs, d_in, d_out, h->st);
 }
 
@@ -181,6 +200,7 @@ mrhs_status_t mrhs_meooe(mrhs_wilson_t *h, const void *d_in, void *d_out, int ou
     MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "meooe: out_parity must be 0 or 1");
     MRHS_REQUIRE(d_in != d_out, "meooe: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "meooe: buffers must be 16-byte aligned");
+    if (h->kern[1] == MRHS_HOP_SWEEP) return launch_sweep(h->sp_cb[out_parity], d_in, d_out, h->st);
     return launch_hop(h->hp_cb[out_parity], h->nrhs, d_in, d_out, h->st);
 }
 
@@ -245,6 +265,55 @@ mrhs_status_t mrhs_wilson_set_prefetch(mrhs_wilson_t *h, int which, int distance
     MRHS_REQUIRE(distance_tiles >= 0, "set prefetch: distance must be >= 0 (0 = off)");
     if (which == 0) h->hp_full.pf_dist = (unsigned)distance_tiles;
     else h->hp_cb[0].pf_dist = h->hp_cb[1].pf_dist = (unsigned)distance_tiles;
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_wilson_set_hop_kernel(mrhs_wilson_t *h, int which, int kernel) {
+    MRHS_REQUIRE(h, "set hop kernel: NULL handle");
+    MRHS_REQUIRE(which == 0 || which == 1, "set hop kernel: which must be 0 (D_hop) or 1 (M_eooe)");
+    MRHS_REQUIRE(kernel == MRHS_HOP_GATHER || kernel == MRHS_HOP_SWEEP, "set hop kernel: kernel must be MRHS_HOP_GATHER or MRHS_HOP_SWEEP");
+    if (kernel == MRHS_HOP_SWEEP && !(sweep_supported(h->gfull) && sweep_supported(h->gcb[0]) && h->sp_full.grid)) {
+        set_error("set hop kernel: the slice-sweep kernel needs an even N_rhs (have %d)", h->nrhs);
+        return MRHS_ERR_UNSUPPORTED;
+    }
+    h->kern[which] = kernel;
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_wilson_get_hop_kernel(mrhs_wilson_t *h, int which, int *kernel) {
+    MRHS_REQUIRE(h && kernel, "get hop kernel: NULL argument");
+    MRHS_REQUIRE(which == 0 || which == 1, "get hop kernel: which must be 0 (D_hop) or 1 (M_eooe)");
+    *kernel = h->kern[which];
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_wilson_set_sweep(mrhs_wilson_t *h, int which, int lt, const int chunk[2]) {
+    MRHS_REQUIRE(h && chunk, "set sweep: NULL argument");
+    MRHS_REQUIRE(which == 0 || which == 1, "set sweep: which must be 0 (D_hop) or 1 (M_eooe)");
+    SweepTiling t = {lt, chunk[0], chunk[1]};
+    if (which == 0) {
+        SweepParams p;
+        MRHS_REQUIRE(build_sweep_params(h->gfull, 0, t, p), "set sweep: segment / chunk does not fit the full lattice (or odd N_rhs)");
+        p.gauge_out = p.gauge_in = h->gauge_full;
+        h->sp_full = p;
+    } else {
+        SweepParams p[2];
+        for (int q = 0; q < 2; q++) {
+            MRHS_REQUIRE(build_sweep_params(h->gcb[q], q, t, p[q]), "set sweep: segment / chunk does not fit the checkerboarded lattice (or odd N_rhs)");
+            p[q].gauge_out = h->gauge_cb[q];
+            p[q].gauge_in = h->gauge_cb[1 - q];
+        }
+        h->sp_cb[0] = p[0];
+        h->sp_cb[1] = p[1];
+    }
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_wilson_get_sweep(mrhs_wilson_t *h, int which, int *lt, int chunk[2]) {
+    MRHS_REQUIRE(h && lt && chunk, "get sweep: NULL argument");
+    MRHS_REQUIRE(which == 0 || which == 1, "get sweep: which must be 0 (D_hop) or 1 (M_eooe)");
+    const SweepParams &p = which == 0 ? h->sp_full : h->sp_cb[0];
+    *lt = p.lt; chunk[0] = p.cy; chunk[1] = p.cz;
     return MRHS_OK;
 }
 

@@ -1,0 +1,41 @@
+// fine_sweep.cuh -- host-side description of the slice-sweep variant of the fine-level hopping kernel
+// (readings S3, S4).  Same operator and same native
+// layouts as fine_hop.cuh; what differs is how the operands reach the SM:
+// a thread block owns a tile of XB x 2 x 2 sites in (x,y,z) and sweeps a segment of t, holding the
+// current t-slice of the tile, its y/z/x halo and the links in shared memory (TMA bulk copies from a
+// producer warp), so every input spinor crosses the L2 -> SM path about 3x instead of 7x.
+#pragma once
+#include "fine_hop.cuh"
+
+namespace mrhs {
+
+constexpr int kSweepBY = 2, kSweepBZ = 2;        // tile extent in y and z (sites)
+constexpr int kSweepRows = kSweepBY * kSweepBZ;
+
+struct SweepTiling {
+    int lt;          // t-slices one thread block sweeps (divides T)
+    int cy, cz;      // tiles per concurrently scheduled chunk in y and z
+};
+
+struct SweepParams {
+    int Y, Z, T;
+    int XB, nxb, NP;              // layout block, blocks per x-line, threads per site (= RHS pairs)
+    int cb, out_parity;
+    int lt, ntseg;                // slices per segment, segments per t-line
+    int pf;                       // L2 prefetch distance of the producer, in slices (0 = off)
+    int cy, cz;
+    FastDiv d_nxb, d_cy, d_cz, d_ntseg, d_ncy;   // block index -> (x-block, tile in chunk, segment, chunk)
+    const float4 *gauge_out;      // links on the sites of the output field, [block][18][xin] float4
+    const float4 *gauge_in;       // links on the sites of the input field
+    unsigned grid, threads, consumers;
+    unsigned smem_bytes;
+};
+
+// true if the sweep kernel can run this geometry (even N_rhs, shared memory fits)
+bool sweep_supported(const FieldGeom &g);
+SweepTiling default_sweep_tiling(const FieldGeom &g, int num_sms);
+bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t, SweepParams &p);
+mrhs_status_t sweep_prepare();    // opt in to large dynamic shared memory for every instantiation
+mrhs_status_t launch_sweep(const SweepParams &p, const void *d_in, void *d_out, cudaStream_t st);
+
+}  // namespace mrhs
