@@ -104,7 +104,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     const SweepSmem L(XB, NP);
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + L.off_bar);
-    uint64_t *fullI = bars, *freeI = bars + 2;
+    uint64_t *fullI = bars, *freeI = bars + 2, *freeG = bars + 4;
 
     const int tid = threadIdx.x;
     const int NC = ROWS * cs, NCpad = (NC + 31) & ~31;
@@ -122,6 +122,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     if (tid == 0) {
         bar_init(&fullI[0], 1); bar_init(&fullI[1], 1);
         bar_init(&freeI[0], NC); bar_init(&freeI[1], NC);
+        bar_init(&freeG[0], NC); bar_init(&freeG[1], NC);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -135,7 +136,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
         // ------------------------------------------------------------------ producer warp
         // slice j of the segment (j = -1 .. lt): the tile rows; for 0 <= j < lt also the links; for j = -1 the t-links
         const int lane = tid - NCpad;
-        auto issue = [&](int j) {
+        auto issue_rows = [&](int j) {
             const int t = tw(j);
             const uint32_t b = (uint32_t)(j + 1) & 1u;
             const bool mid = j >= 0 && j < lt;
@@ -147,11 +148,25 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
                 bar_expect_tx(&fullI[b], bytes);
             }
             __syncwarp();
-            unsigned char *Ib = smem + b * L.I_BYTES, *Gb = smem + L.off_G + b * L.G_BYTES;
+            unsigned char *Ib = smem + b * L.I_BYTES;
             if (lane < ROWS) {
                 const int ty = lane % BY, tz = lane / BY;
                 bulk_g2s(Ib + lane * L.RB, in + blk(xb, y0 + ty, z0 + tz, t) * 12 * cs, L.RB, &fullI[b]);
             }
+            // ask for the rows of a later slice to be brought into L2 now, so that their copy hits L2
+            const int jp = j + p.pf;
+            if (p.pf > 0 && jp <= lt && lane < 2 * ROWS) {
+                const int r = lane % ROWS, tp = tw(jp);
+                const size_t bb = blk(xb, y0 + r % BY, z0 + r / BY, tp);
+                if (lane < ROWS) bulk_prefetch_l2(in + bb * 12 * cs, L.RB);
+                else if (jp < lt) bulk_prefetch_l2(p.gauge_out + bb * kSiteF4 * XB, L.GO);
+            }
+        };
+        auto issue_links = [&](int j) {
+            const int t = tw(j);
+            const uint32_t b = (uint32_t)(j + 1) & 1u;
+            const bool mid = j >= 0 && j < lt;
+            unsigned char *Gb = smem + L.off_G + b * L.G_BYTES;
             if (mid || j == -1) {
                 for (int idx = lane; idx < ROWS * 6; idx += 32) {
                     const int r = idx / 6, w = idx - r * 6;
@@ -172,20 +187,15 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
                     bulk_g2s(dst, src, bytes, &fullI[b]);
                 }
             }
-            // ask for the rows of a later slice to be brought into L2 now, so that their copy hits L2
-            const int jp = j + p.pf;
-            if (p.pf > 0 && jp <= lt && lane < 2 * ROWS) {
-                const int r = lane % ROWS, tp = tw(jp);
-                const size_t bb = blk(xb, y0 + r % BY, z0 + r / BY, tp);
-                if (lane < ROWS) bulk_prefetch_l2(in + bb * 12 * cs, L.RB);
-                else if (jp < lt) bulk_prefetch_l2(p.gauge_out + bb * kSiteF4 * XB, L.GO);
-            }
         };
-        issue(-1);
-        issue(0);
+        issue_rows(-1); issue_links(-1);
+        issue_rows(0); issue_links(0);
         for (int k = -1; k + 2 <= lt; k++) {
-            bar_wait(&freeI[(k + 1) & 1], ((uint32_t)(k + 1) >> 1) & 1u);   // the consumers are done with slice k
-            issue(k + 2);
+            const uint32_t par = ((uint32_t)(k + 1) >> 1) & 1u;
+            bar_wait(&freeI[(k + 1) & 1], par);   // the consumers are done with the rows of slice k (after its x hops)
+            issue_rows(k + 2);
+            bar_wait(&freeG[(k + 1) & 1], par);   // ... and with its links (end of the step)
+            issue_links(k + 2);
         }
         return;
     }
@@ -243,7 +253,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     const int g_bt = CB ? Gr + 38 * XB - 13 * XB + xin : g_own;
 
     CVec<2> acc[12];
-    zero_acc(acc);
+    CVec<2> carry[6];      // (1 + gamma_t) U_t^+ psi of the slice before, as a half spinor
     HopOperands<2> A, B;
 
     // slice 0's halo neighbours: three groups in the order they are waited for (y, z, x)
@@ -259,8 +269,18 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
         const int t = tw(k);
         const uint32_t b = (uint32_t)(k + 1) & 1u;
         bar_wait(&fullI[b], ((uint32_t)(k + 1) >> 1) & 1u);
+        const float4 *G = S + b * G4;
         if (k >= 0) {
-            const float4 *G = S + b * G4;
+            zero_acc(acc);
+            hop_recon<2, 3, false>(carry, acc);
+        }
+        if (k + 1 < lt) {
+            // -t hop of the next slice, first thing, so that the rows of this slice can be released after the x hops:
+            // (1 + gamma_t) U_t(x, t)^+ psi(x, t), both at this thread's own position of slice k
+            hop_load_s<3>(B, S + own.o + b * own.bs, own.cs, G + g_bt, XB);
+            hop_half<2, 3, false>(B, carry);
+        }
+        if (k >= 0) {
             const int tn = tw(k + 1);
             const bool more = k + 1 < lt;
             // x neighbours of this step (checkerboarded lines alternate with t)
@@ -288,21 +308,18 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
             hop_load_s<0>(B, S + xm.o + b * xm.bs, xm.cs, G + g_bx, XB);
             hop_compute<2, 0, true >(A, acc);
             refill_x(tn, more);
+            hop_compute<2, 0, false>(B, acc);
+            bar_arrive(&freeI[b]);             // rows of slice k are no longer read: slice k+2 may land
             bar_wait(&fullI[b ^ 1u], ((uint32_t)(k + 2) >> 1) & 1u);   // slice k+1
             hop_load_s<3>(A, S + own.o + (b ^ 1u) * own.bs, own.cs, G + g_own, XB);
-            hop_compute<2, 0, false>(B, acc);
             hop_compute<2, 3, true >(A, acc);
             float4 *o = out + (blk(xb, y, z, t) * 12 * XB + xin) * NP + pair;
 #pragma unroll
             for (int c = 0; c < 12; c++) o[(size_t)c * cs] = from_cvec(acc[c]);
+        } else {
+            bar_arrive(&freeI[b]);
         }
-        if (k + 1 < lt) {
-            // -t hop of the next slice: (1 + gamma_t) U_t(x, t)^+ psi(x, t), both at this thread's own position of slice k
-            zero_acc(acc);
-            hop_load_s<3>(B, S + own.o + b * own.bs, own.cs, S + b * G4 + g_bt, XB);
-            hop_compute<2, 3, false>(B, acc);
-        }
-        bar_arrive(&freeI[b]);
+        bar_arrive(&freeG[b]);
     }
     cp_wait<0>();
 }

@@ -91,9 +91,11 @@ __device__ __forceinline__ void hop_load_s(HopOperands<2> &o, const float4 *nb, 
     load_link_s<MU>(g, XB, o.u);
 }
 
-// One of the eight hops.  FWD: (1 - gamma_MU) U_MU(x) psi(x+MU); else (1 + gamma_MU) U_MU(x-MU)^+ psi(x-MU).
+// One of the eight hops in two stages.  FWD: (1 - gamma_MU) U_MU(x) psi(x+MU); else (1 + gamma_MU) U_MU(x-MU)^+ psi(x-MU).
+// hop_half: spin projection to a half spinor and colour multiply, r = U h or U^+ h (6 complex numbers);
+// hop_recon: acc += the four spin components rebuilt from r.  hop_compute does both.
 template <int R, int MU, bool FWD>
-__device__ __forceinline__ void hop_compute(const HopOperands<R> &o, CVec<R> (&acc)[12]) {
+__device__ __forceinline__ void hop_half(const HopOperands<R> &o, CVec<R> (&r)[6]) {
     CVec<R> psi[12];
 #pragma unroll
     for (int c = 0; c < 12; c++) psi[c] = to_cvec(o.psi[c]);
@@ -119,7 +121,6 @@ __device__ __forceinline__ void hop_compute(const HopOperands<R> &o, CVec<R> (&a
     }
 
     // colour multiply: r = U h (FWD) or U^+ h
-    CVec<R> r[6];
 #pragma unroll
     for (int s = 0; s < 2; s++) {
 #pragma unroll
@@ -136,6 +137,10 @@ __device__ __forceinline__ void hop_compute(const HopOperands<R> &o, CVec<R> (&a
         }
     }
 
+}
+
+template <int R, int MU, bool FWD>
+__device__ __forceinline__ void hop_recon(const CVec<R> (&r)[6], CVec<R> (&acc)[12]) {
     // reconstruction: upper components get r, lower ones -S i sigma_MU r (spatial) or -S r (time)
 #pragma unroll
     for (int c = 0; c < 3; c++) {
@@ -155,6 +160,13 @@ __device__ __forceinline__ void hop_compute(const HopOperands<R> &o, CVec<R> (&a
             acc[9 + c] = FWD ? csub(acc[9 + c], r[3 + c]) : cadd(acc[9 + c], r[3 + c]);
         }
     }
+}
+
+template <int R, int MU, bool FWD>
+__device__ __forceinline__ void hop_compute(const HopOperands<R> &o, CVec<R> (&acc)[12]) {
+    CVec<R> r[6];
+    hop_half<R, MU, FWD>(o, r);
+    hop_recon<R, MU, FWD>(r, acc);
 }
 
 }  // namespace
