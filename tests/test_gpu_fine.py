@@ -121,6 +121,65 @@ def test_tilings_give_identical_results():
     w.close()
 
 
+# ---- the two hop kernels (gather, slice sweep) compute the same map: both against the oracle, and the sweep
+# kernel under several segment lengths / chunk shapes (prologue slice, wrap in t, partly filled warps, x-blocks
+# of 2..16 sites, checkerboarded half lines of 6 sites, extent-2 directions)
+KERNEL_CASES = [
+    ([4, 4, 4, 4], 4, 40),
+    ([2, 2, 2, 2], 2, 41),
+    ([12, 6, 4, 10], 12, 42),
+    ([48, 4, 2, 4], 12, 43),
+    ([24, 4, 4, 6], 12, 44),
+    ([16, 8, 2, 4], 24, 45),
+    ([8, 4, 4, 4], 96, 46),
+    ([16, 4, 6, 8], 48, 47),
+    ([32, 2, 4, 6], 4, 48),
+]
+
+
+@pytest.mark.parametrize("dims,nrhs,seed", KERNEL_CASES)
+def test_gather_and_sweep_kernels_match_oracle(dims, nrhs, seed):
+    U, psi = _fine_case(dims, nrhs, seed, -0.05, 1.5)
+    w = make_wilson(dims, nrhs, -0.05, 1.5, U)
+    assert mrhs.wilson_get_hop_kernel(w.h, 0) == mrhs.HOP_SWEEP      # the default for even N_rhs
+    want = oracle.dhop(dims, U, psi)
+    pe, po = oracle.cb_split(dims, psi)
+    want_cb = [oracle.meooe(dims, U, po, 0), oracle.meooe(dims, U, pe, 1)]
+    T = dims[3]
+    settings = [(mrhs.HOP_GATHER, None), (mrhs.HOP_SWEEP, None), (mrhs.HOP_SWEEP, (T, [1, 1])),
+                (mrhs.HOP_SWEEP, (2, [dims[1] // 2, 1])), (mrhs.HOP_SWEEP, (1, [1, dims[2] // 2]))]
+    results = []
+    for kern, sweep in settings:
+        for which in (0, 1):
+            mrhs.wilson_set_hop_kernel(w.h, which, kern)
+            if sweep is not None:
+                mrhs.wilson_set_sweep(w.h, which, sweep[0], sweep[1])
+                assert mrhs.wilson_get_sweep(w.h, which) == (sweep[0], sweep[1])
+        got = gpu_dhop(w, psi)
+        assert rel_l2_per_rhs(got, want).max() < TOL, ("dhop", kern, sweep)
+        for out_parity, src in ((0, po), (1, pe)):
+            g = gpu_meooe(w, src, out_parity)
+            assert rel_l2_per_rhs(g, want_cb[out_parity]).max() < TOL, ("meooe", out_parity, kern, sweep)
+        results.append(got)
+    # every sweep setting adds the eight hops in the same order: bit-identical results
+    for r in results[2:]:
+        assert np.array_equal(r, results[1])
+    with pytest.raises(mrhs.MrhsError):
+        mrhs.wilson_set_sweep(w.h, 0, 3 if T % 3 else T + 1, [1, 1])     # does not divide T
+    w.close()
+
+
+def test_sweep_kernel_needs_even_nrhs():
+    dims = [4, 4, 4, 4]
+    U, psi = _fine_case(dims, 3, 50, 0.0, 1.0)
+    w = make_wilson(dims, 3, 0.0, 1.0, U)
+    assert mrhs.wilson_get_hop_kernel(w.h, 0) == mrhs.HOP_GATHER
+    with pytest.raises(mrhs.MrhsError) as e:
+        mrhs.wilson_set_hop_kernel(w.h, 0, mrhs.HOP_SWEEP)
+    assert e.value.status == mrhs.ERR_UNSUPPORTED
+    w.close()
+
+
 def test_argument_errors():
     dims, nrhs = [4, 4, 4, 4], 4
     U, psi = _fine_case(dims, nrhs, 41, 0.0, 1.0)

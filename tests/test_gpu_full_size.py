@@ -75,8 +75,13 @@ def config5():
     w.close()
 
 
-def test_config5_dhop_sampled_sites(config5):
+KERNELS = [mrhs.HOP_SWEEP, mrhs.HOP_GATHER]   # the library default (bench.py's configuration) first
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config5_dhop_sampled_sites(config5, kernel):
     U, psi, w = config5
+    mrhs.wilson_set_hop_kernel(w.h, 0, kernel)
     lex = _sample_sites(DIMS, NSAMPLE, 1)
     d_in = w.import_field(psi, mrhs.FULL)
     d_out = w.empty(mrhs.FULL)
@@ -90,9 +95,11 @@ def test_config5_dhop_sampled_sites(config5):
     assert err.max() < TOL, err
 
 
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("out_parity", [0, 1])
-def test_config5_meooe_sampled_sites(config5, out_parity):
+def test_config5_meooe_sampled_sites(config5, out_parity, kernel):
     U, psi, w = config5
+    mrhs.wilson_set_hop_kernel(w.h, 1, kernel)
     X, Y, Z, T = DIMS
     lex_all = torch.arange(syn.volume(DIMS), device="cuda")
     par = (lex_all % X + (lex_all // X) % Y + (lex_all // (X * Y)) % Z + lex_all // (X * Y * Z)) % 2
