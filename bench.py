@@ -327,8 +327,13 @@ def run_gpu(args):
             mrhs.wilson_set_tiling(wl.w.h, which, t[:3], t[3:5])
         if args.hop_prefetch is not None:
             mrhs.wilson_set_prefetch(wl.w.h, which, args.hop_prefetch)
-    if args.hop_tiling or args.hop_prefetch is not None:
-        tiling_note = "override: tiling %s prefetch %s" % (args.hop_tiling, args.hop_prefetch)
+        if args.hop_kernel is not None:
+            mrhs.wilson_set_hop_kernel(wl.w.h, which, {"gather": mrhs.HOP_GATHER, "sweep": mrhs.HOP_SWEEP}[args.hop_kernel])
+        if args.hop_sweep:
+            t = [int(x) for x in args.hop_sweep.split(",")]
+            mrhs.wilson_set_sweep(wl.w.h, which, t[0], t[1:3])
+    if args.hop_tiling or args.hop_prefetch is not None or args.hop_kernel or args.hop_sweep:
+        tiling_note = "override: kernel %s tiling %s prefetch %s sweep %s" % (args.hop_kernel, args.hop_tiling, args.hop_prefetch, args.hop_sweep)
     launches = wl.launches()
     work = step_work(fdims, cdims, nb, N)
     flops_step = sum(w[1] for w in work)
@@ -382,7 +387,8 @@ def run_gpu(args):
         kernels[name] = {"ms": ms, "gflops": fl / (ms * 1e-3) / 1e9, "gbs": gbs, "hbm_frac": gbs / peak,
                          "share_of_step": ms / sum(seg_ms)}
     d = kernels["dhop"]
-    roofline = {"kernel": "hop_kernel (D_hop, full lattice %dx%dx%dx%d, N_rhs=%d)" % (*fdims, N), "bound": "hbm",
+    kname = {mrhs.HOP_GATHER: "hop_kernel (gather)", mrhs.HOP_SWEEP: "hop_sweep_kernel (slice sweep)"}
+    roofline = {"kernel": "%s: D_hop, full lattice %dx%dx%dx%d, N_rhs=%d" % (kname[mrhs.wilson_get_hop_kernel(wl.w.h, 0)], *fdims, N), "bound": "hbm",
                 "achieved": d["gbs"], "peak": peak, "unit": "GB/s", "frac": d["gbs"] / peak,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_dhop(V, N),
                 "avg_launch_ms": d["ms"], "traffic": ncu_traffic("dhop_48x48x48x48_n12") if not args.small else None}
@@ -391,7 +397,14 @@ def run_gpu(args):
         gf, ms, cores = time_oracle(args.cpu_steps, 1)
         cpu = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": CPU_SAMPLE, "ms_per_sample_step": ms}
     cfg = workload_config()
-    cfg["hop_tiling"] = {"dhop": mrhs.wilson_get_tiling(wl.w.h, 0), "meooe": mrhs.wilson_get_tiling(wl.w.h, 1), "source": tiling_note}
+    def hop_cfg(which):
+        k = mrhs.wilson_get_hop_kernel(wl.w.h, which)
+        if k == mrhs.HOP_SWEEP:
+            lt, chunk = mrhs.wilson_get_sweep(wl.w.h, which)
+            return {"kernel": "sweep", "tile_yz": [2, 2], "segment_t": lt, "chunk_tiles_yz": chunk}
+        tile, chunk = mrhs.wilson_get_tiling(wl.w.h, which)
+        return {"kernel": "gather", "tile_yzt": tile, "chunk_tiles_yz": chunk}
+    cfg["hop_tiling"] = {"dhop": hop_cfg(0), "meooe": hop_cfg(1), "source": tiling_note}
     if args.small:
         cfg["workload"] = "SMALL smoke workload (16^4 fine, 4^4 coarse) -- not the benchmark configuration"
         cfg["fine_dims"], cfg["coarse_dims"] = fdims, cdims
@@ -571,6 +584,8 @@ def main():
     ap.add_argument("--sweep-ops", default="fine,coarse", help="which operator families the sweep covers")
     ap.add_argument("--hop-tiling", default=None, help="by,bz,bt,cy,cz for D_hop and M_eooe instead of the library default")
     ap.add_argument("--hop-prefetch", type=int, default=None, help="L2 prefetch distance in tiles (0 = off)")
+    ap.add_argument("--hop-kernel", default=None, choices=["gather", "sweep"], help="hop kernel instead of the library default")
+    ap.add_argument("--hop-sweep", default=None, help="lt,cy,cz for the sweep kernel instead of the library default")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours" and not args.sweep:
         args.warmup = 3   # timing rule: at least 3 warm-up steps
