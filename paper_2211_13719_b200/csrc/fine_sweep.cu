@@ -104,7 +104,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     const SweepSmem L(XB, NP);
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + L.off_bar);
-    uint64_t *fullI = bars, *freeI = bars + 2, *freeG = bars + 4;
+    uint64_t *fullI = bars, *freeI = bars + 2, *freeG = bars + 4, *fullG = bars + 6;
 
     const int tid = threadIdx.x;
     const int NC = ROWS * cs, NCpad = (NC + 31) & ~31;
@@ -123,6 +123,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
         bar_init(&fullI[0], 1); bar_init(&fullI[1], 1);
         bar_init(&freeI[0], NC); bar_init(&freeI[1], NC);
         bar_init(&freeG[0], NC); bar_init(&freeG[1], NC);
+        bar_init(&fullG[0], 1); bar_init(&fullG[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -140,13 +141,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
             const int t = tw(j);
             const uint32_t b = (uint32_t)(j + 1) & 1u;
             const bool mid = j >= 0 && j < lt;
-            constexpr int NG = CB ? 6 : 4;   // link copies per row: on the full lattice U_x and U_t of the input row are the own links
-            if (lane == 0) {
-                uint32_t bytes = L.I_BYTES;
-                if (mid) bytes += ROWS * (L.GO + (NG - 1) * L.GW);
-                if (j == -1) bytes += ROWS * (CB ? L.GW : L.GO);
-                bar_expect_tx(&fullI[b], bytes);
-            }
+            if (lane == 0) bar_expect_tx(&fullI[b], L.I_BYTES);
             __syncwarp();
             unsigned char *Ib = smem + b * L.I_BYTES;
             if (lane < ROWS) {
@@ -166,8 +161,11 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
             const int t = tw(j);
             const uint32_t b = (uint32_t)(j + 1) & 1u;
             const bool mid = j >= 0 && j < lt;
+            constexpr int NG = CB ? 6 : 4;   // link copies per row: on the full lattice U_x and U_t of the input row are the own links
             unsigned char *Gb = smem + L.off_G + b * L.G_BYTES;
             if (mid || j == -1) {
+                if (lane == 0) bar_expect_tx(&fullG[b], mid ? ROWS * (L.GO + (NG - 1) * L.GW) : ROWS * (CB ? L.GW : L.GO));
+                __syncwarp();
                 for (int idx = lane; idx < ROWS * 6; idx += 32) {
                     const int r = idx / 6, w = idx - r * 6;
                     if (!CB && (w == 1 || w == 5)) continue;
@@ -184,7 +182,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
                         case 4: src = p.gauge_in + (blk(xb, y, wrap(z - 1, Z), t) * kSiteF4 + 9) * XB; dst += L.GO + 3 * L.GW; break;   // U_z at z-1
                         default: src = p.gauge_in + (blk(xb, y, z, t) * kSiteF4 + 13) * XB; dst += L.GO + 4 * L.GW; break;     // U_t of the input row (carry)
                     }
-                    bulk_g2s(dst, src, bytes, &fullI[b]);
+                    bulk_g2s(dst, src, bytes, &fullG[b]);
                 }
             }
         };
@@ -269,6 +267,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
         const int t = tw(k);
         const uint32_t b = (uint32_t)(k + 1) & 1u;
         bar_wait(&fullI[b], ((uint32_t)(k + 1) >> 1) & 1u);
+        bar_wait(&fullG[b], ((uint32_t)(k + 1) >> 1) & 1u);   // links of slice k, on their own barrier: the +t hop below waits for rows only
         const float4 *G = S + b * G4;
         if (k >= 0) {
             zero_acc(acc);
