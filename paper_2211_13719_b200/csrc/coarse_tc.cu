@@ -8,10 +8,10 @@
 // Per coarse site the complex contraction is written as ONE real GEMM accumulated over the nine
 // stencil points and the nb columns:
 //   D[128 x NT] += Aop[128 x nb] * Bop[nb x NT]
-//   Aop rows 0..nb-1      = Re A_p,   rows 64..64+nb-1 = Im A_p            (other rows unused)
+//   Aop rows 0..nb-1      = Re A_p,   rows nb..2nb-1   = Im A_p            (rows 2nb..127: whatever follows in shared memory; their D lanes are never read)
 //   Bop cols 0..N-1       = Re v,     cols N..2N-1     = Im v              (NT = 2N rounded up to 16)
 // so D holds Re A Re v, Re A Im v, Im A Re v, Im A Im v and the epilogue forms
-//   Re out = D[i][n] - D[64+i][N+n],   Im out = D[i][N+n] + D[64+i][n].
+//   Re out = D[i][n] - D[nb+i][N+n],   Im out = D[i][N+n] + D[nb+i][n].
 // Every matrix entry read from HBM serves all N_rhs columns (PAPER.md:23 (i)).
 //
 // Data path: fp32 links and vectors go global -> registers (coalesced 128-bit loads) -> hi/lo split
@@ -125,7 +125,7 @@ struct TcCfg {
     static constexpr int KC = NB / 4;                         // 16-byte K chunks per stencil point
     static constexpr int KS = NB / 8;                         // MMA K steps per stencil point
     static constexpr int THREADS = NT <= 64 ? 128 : 256;
-    static constexpr int A_LBO = 128 * 16;                    // bytes between K chunks of the A operand
+    static constexpr int A_LBO = 2 * NB * 16;                 // bytes between K chunks of the A operand: only the 2 nb used rows are stored
     static constexpr int B_LBO = NT * 16;
     static constexpr int A_BYTES = KC * A_LBO;                // one of hi / lo
     static constexpr int B_BYTES = KC * B_LBO;
@@ -220,7 +220,7 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, const float4 *__r
                     const int kc = r / NB, row = r - kc * NB;
                     float4 hi, lo;
                     split4(ra[it], hi, lo);
-                    const int off = kc * C::A_LBO + (part * 64 + row) * 16;
+                    const int off = kc * C::A_LBO + (part * NB + row) * 16;
                     *reinterpret_cast<float4 *>(a_hi + off) = hi;
                     *reinterpret_cast<float4 *>(a_lo + off) = lo;
                 }
@@ -284,10 +284,10 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, const float4 *__r
             const int i = idx / C::NP, q = idx - i * C::NP;
             const int n0 = 2 * q, n1 = 2 * q + 1;
             float4 o;
-            o.x = S[n0 * C::S_PITCH + i] - S[(N + n0) * C::S_PITCH + 64 + i];
-            o.y = S[n1 * C::S_PITCH + i] - S[(N + n1) * C::S_PITCH + 64 + i];
-            o.z = S[(N + n0) * C::S_PITCH + i] + S[n0 * C::S_PITCH + 64 + i];
-            o.w = S[(N + n1) * C::S_PITCH + i] + S[n1 * C::S_PITCH + 64 + i];
+            o.x = S[n0 * C::S_PITCH + i] - S[(N + n0) * C::S_PITCH + NB + i];
+            o.y = S[n1 * C::S_PITCH + i] - S[(N + n1) * C::S_PITCH + NB + i];
+            o.z = S[(N + n0) * C::S_PITCH + i] + S[n0 * C::S_PITCH + NB + i];
+            o.w = S[(N + n1) * C::S_PITCH + i] + S[n1 * C::S_PITCH + NB + i];
             out[((size_t)site * NB + i) * C::NP + q] = o;
         }
         __syncthreads();   // S (aliasing the operand buffer) is free for the next site
