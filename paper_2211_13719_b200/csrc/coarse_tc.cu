@@ -172,44 +172,50 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, const float4 *__r
     constexpr uint32_t idesc = instr_desc_tf32(128, C::NT);
 
     uint32_t nstage = 0;   // operand stages handed to the tensor core so far (same in every thread)
-    for (long long site = blockIdx.x; site < nsites; site += gridDim.x) {
-        int c[4];
-        {
+    // raw fp32 operands of one stage (stencil point p of a site) in registers; loaded one stage ahead, right after
+    // the previous stage has been handed to the tensor core, so the load latency overlaps its MMAs and the next wait
+    float4 ra[A_IT];
+    float4 rb[B_IT][4];
+    auto load_stage = [&](long long site, int p) {
+        // neighbour of stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
+        long long nbr = site;
+        if (p > 0) {
             long long s = site;
-            c[0] = (int)(s % X); s /= X;
-            c[1] = (int)(s % Y); s /= Y;
-            c[2] = (int)(s % Z);
-            c[3] = (int)(s / Z);
+            int c0 = (int)(s % X); s /= X;
+            int c1 = (int)(s % Y); s /= Y;
+            int c2 = (int)(s % Z);
+            int c3 = (int)(s / Z);
+            const int mu = (p - 1) & 3, d = p <= 4 ? 1 : -1;
+            if (mu == 0) c0 = (c0 + d + X) % X;
+            else if (mu == 1) c1 = (c1 + d + Y) % Y;
+            else if (mu == 2) c2 = (c2 + d + Z) % Z;
+            else c3 = (c3 + d + T) % T;
+            nbr = c0 + (long long)X * (c1 + (long long)Y * (c2 + (long long)Z * c3));
         }
-        const int ext[4] = {X, Y, Z, T};
+        const float4 *lp = links + ((size_t)site * 9 + p) * C::A_UNITS;
+        const float4 *vp = in + (size_t)nbr * NB * C::NP;
+#pragma unroll
+        for (int it = 0; it < A_IT; it++) {
+            const int u = tid + it * C::THREADS;
+            if (u < C::A_UNITS) ra[it] = __ldg(lp + u);
+        }
+#pragma unroll
+        for (int it = 0; it < B_IT; it++) {
+            const int w = tid + it * C::THREADS;
+            if (w < C::B_UNITS) {
+                const int kc = w / C::NP, q = w - kc * C::NP;
+#pragma unroll
+                for (int e = 0; e < 4; e++) rb[it][e] = __ldg(vp + (size_t)(4 * kc + e) * C::NP + q);
+            }
+        }
+    };
+    // For wide operands (two blocks per SM) the load runs one stage ahead; for narrow ones the extra live registers
+    // would cost resident blocks, which hide the latency better, so the load sits at the top of its own stage.
+    constexpr bool AHEAD = C::NT > 96;
+    if (AHEAD && (long long)blockIdx.x < nsites) load_stage(blockIdx.x, 0);
+    for (long long site = blockIdx.x; site < nsites; site += gridDim.x) {
         for (int p = 0; p < 9; p++) {
-            // neighbour of stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
-            long long nbr = site;
-            if (p > 0) {
-                const int mu = (p - 1) & 3, d = p <= 4 ? 1 : -1;
-                int cc[4] = {c[0], c[1], c[2], c[3]};
-                cc[mu] = (cc[mu] + d + ext[mu]) % ext[mu];
-                nbr = cc[0] + (long long)X * (cc[1] + (long long)Y * (cc[2] + (long long)Z * cc[3]));
-            }
-            // raw fp32 operands into registers while the previous stage's MMAs still run
-            const float4 *lp = links + ((size_t)site * 9 + p) * C::A_UNITS;
-            const float4 *vp = in + (size_t)nbr * NB * C::NP;
-            float4 ra[A_IT];
-            float4 rb[B_IT][4];
-#pragma unroll
-            for (int it = 0; it < A_IT; it++) {
-                const int u = tid + it * C::THREADS;
-                if (u < C::A_UNITS) ra[it] = __ldg(lp + u);
-            }
-#pragma unroll
-            for (int it = 0; it < B_IT; it++) {
-                const int w = tid + it * C::THREADS;
-                if (w < C::B_UNITS) {
-                    const int kc = w / C::NP, q = w - kc * C::NP;
-#pragma unroll
-                    for (int e = 0; e < 4; e++) rb[it][e] = __ldg(vp + (size_t)(4 * kc + e) * C::NP + q);
-                }
-            }
+            if (!AHEAD) load_stage(site, p);
             // the single operand buffer is free once the previous stage's MMAs have completed
             if (nstage > 0) mbar_wait(bar, (nstage - 1) & 1);
 #pragma unroll
@@ -265,6 +271,10 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, const float4 *__r
                 mma_commit(bar);
             }
             nstage++;
+            if (AHEAD) {
+                if (p < 8) load_stage(site, p + 1);
+                else if (site + gridDim.x < nsites) load_stage(site + gridDim.x, 0);
+            }
         }
         // all nine points accumulated: TMEM -> shared scratch S[col][lane] -> combine -> global
         mbar_wait(bar, (nstage - 1) & 1);
