@@ -11,7 +11,7 @@ N_rhs = 12):
     D_hop (full lattice)                                   row a2
     M_eooe (odd <- even) and M_eooe (even <- odd)          row a3
     M_ooee (full lattice)                                  row a4
-    Schur sequence M_eooe, M_ooee, M_eooe                  row a7
+    Schur sequence M_eooe, M_ooee, M_eooe                  row a7 (M_ooee fused into the first hop: 2 launches)
     coarse 9-point apply, FP32 FMA                         row a5
     coarse 9-point apply, tensor cores (3xTF32, tcgen05)    row a6
 
@@ -413,7 +413,7 @@ def run_gpu(args):
         "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": cfg, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
-        "gpu_launches": len(work) * K, "kernels": kernels, "wall_ms_per_step": t_wall * 1e3 / K,
+        "gpu_launches": (len(work) - (1 if mrhs.wilson_get_hop_kernel(wl.w.h, 1) == mrhs.HOP_SWEEP else 0)) * K, "kernels": kernels, "wall_ms_per_step": t_wall * 1e3 / K,
     }
     print(json.dumps(line))
     if dist is not None:

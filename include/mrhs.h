@@ -107,9 +107,19 @@ mrhs_status_t mrhs_meooe(mrhs_wilson_t *h, const void *d_in, void *d_out, int ou
  * parity 0/1: checkerboarded fields of that parity; 2: full-lattice fields. */
 mrhs_status_t mrhs_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity);
 
-/* Schur-style sequence of config 5, three launches
- * back to back on the handle's stream with no host synchronisation:
+/* Fused out = M_ooee(out_parity) M_eooe(in): the hopping term onto parity out_parity followed by
+ * the clover term of those sites (the first two steps of the Schur
+ * sequence below).  With the sweep kernel (even N_rhs) this is ONE
+ * launch: the clover blocks are applied to the hop result in registers before it is stored, so the
+ * intermediate field never goes through HBM.  With the gather kernel it is two launches.
+ * d_in: native field of parity 1 - out_parity; d_out: native field of parity out_parity. */
+mrhs_status_t mrhs_meooe_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity);
+
+/* Schur-style sequence of config 5, back to back on the handle's
+ * stream with no host synchronisation:
  *   tmp_o = M_eooe(in_e -> odd); tmp2_o = M_ooee(tmp_o); out_e = M_eooe(tmp2_o -> even).
+ * With the sweep kernel the first two steps are one fused launch (mrhs_meooe_mooee) that writes
+ * tmp2_o into d_tmp1 and leaves d_tmp0 untouched; with the gather kernel three launches.
  * d_in, d_out: even checkerboarded native fields; d_tmp0, d_tmp1: odd ones. */
 mrhs_status_t mrhs_schur_sequence(mrhs_wilson_t *h, const void *d_in, void *d_tmp0,
                                   void *d_tmp1, void *d_out);

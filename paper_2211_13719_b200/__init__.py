@@ -37,6 +37,7 @@ _SIGNATURES = {
     "mrhs_meooe": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_mooee": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_schur_sequence": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "mrhs_meooe_mooee": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_wilson_export_clover": (ctypes.c_int, [_vp, _vp]),
     "mrhs_wilson_set_tiling": (ctypes.c_int, [_vp, ctypes.c_int, _int3, _int2]),
     "mrhs_wilson_get_tiling": (ctypes.c_int, [_vp, ctypes.c_int, _int3, _int2]),
@@ -182,6 +183,10 @@ def mooee(h, d_in, d_out, parity):
     _check(lib().mrhs_mooee(h, _ptr(d_in), _ptr(d_out), int(parity)))
 
 
+def meooe_mooee(h, d_in, d_out, out_parity):
+    _check(lib().mrhs_meooe_mooee(h, _ptr(d_in), _ptr(d_out), int(out_parity)))
+
+
 def schur_sequence(h, d_in, d_tmp0, d_tmp1, d_out):
     _check(lib().mrhs_schur_sequence(h, _ptr(d_in), _ptr(d_tmp0), _ptr(d_tmp1), _ptr(d_out)))
 
@@ -293,6 +298,9 @@ class Wilson:
 
     def mooee(self, d_in, d_out, parity):
         mooee(self.h, d_in, d_out, parity)
+
+    def meooe_mooee(self, d_in, d_out, out_parity):
+        meooe_mooee(self.h, d_in, d_out, out_parity)
 
     def schur_sequence(self, d_in, d_tmp0, d_tmp1, d_out):
         schur_sequence(self.h, d_in, d_tmp0, d_tmp1, d_out)

@@ -213,12 +213,35 @@ mrhs_status_t mrhs_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int pa
     return launch_mooee(h->gcb[parity], h->clov_cb[parity], d_in, d_out, h->st);
 }
 
+mrhs_status_t mrhs_meooe_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity) {
+    MRHS_REQUIRE(h && d_in && d_out, "meooe_mooee: NULL argument");
+    MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "meooe_mooee: out_parity must be 0 or 1");
+    MRHS_REQUIRE(d_in != d_out, "meooe_mooee: in and out must not alias");
+    MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "meooe_mooee: buffers must be 16-byte aligned");
+    if (h->kern[1] == MRHS_HOP_SWEEP) {
+        // one launch: the clover blocks of the output sites are applied to the hop result before it is stored
+        SweepParams p = h->sp_cb[out_parity];
+        p.clover = h->clov_cb[out_parity];
+        return launch_sweep(p, d_in, d_out, h->st);
+    }
+    // gather kernel: two launches; the site-diagonal term reads each site's twelve components before it writes them
+    mrhs_status_t s = launch_hop(h->hp_cb[out_parity], h->nrhs, d_in, d_out, h->st);
+    if (s == MRHS_OK) s = launch_mooee(h->gcb[out_parity], h->clov_cb[out_parity], d_out, d_out, h->st);
+    return s;
+}
+
 mrhs_status_t mrhs_schur_sequence(mrhs_wilson_t *h, const void *d_in, void *d_tmp0, void *d_tmp1, void *d_out) {
     MRHS_REQUIRE(h && d_in && d_tmp0 && d_tmp1 && d_out, "schur sequence: NULL argument");
     MRHS_REQUIRE(d_in != d_out && d_tmp0 != d_tmp1 && d_in != d_tmp0 && d_in != d_tmp1 && d_out != d_tmp0 && d_out != d_tmp1,
                  "schur sequence: the four buffers must be distinct");
-    mrhs_status_t s = mrhs_meooe(h, d_in, d_tmp0, MRHS_ODD);
-    if (s == MRHS_OK) s = mrhs_mooee(h, d_tmp0, d_tmp1, MRHS_ODD);
+    mrhs_status_t s;
+    if (h->kern[1] == MRHS_HOP_SWEEP) {
+        // M_ooee rides in the epilogue of the first hop: two launches, d_tmp0 is not touched
+        s = mrhs_meooe_mooee(h, d_in, d_tmp1, MRHS_ODD);
+    } else {
+        s = mrhs_meooe(h, d_in, d_tmp0, MRHS_ODD);
+        if (s == MRHS_OK) s = mrhs_mooee(h, d_tmp0, d_tmp1, MRHS_ODD);
+    }
     if (s == MRHS_OK) s = mrhs_meooe(h, d_tmp1, d_out, MRHS_EVEN);
     return s;
 }

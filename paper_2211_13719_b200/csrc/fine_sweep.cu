@@ -71,7 +71,8 @@ struct SweepSmem {
     uint32_t RB, GO, GW, GROW;              // tile row, own links of a row, one link window, all links of one row
     uint32_t I_BYTES, G_BYTES;              // per buffer (two buffers each)
     uint32_t H_BYTES, XH_BYTES;             // thread-private halo slots: y and z (every thread), x (edge threads)
-    uint32_t off_G, off_H, off_XH, off_bar, total;
+    uint32_t C_BYTES;                       // packed clover blocks of the tile rows (fused M_ooee epilogue), per buffer
+    uint32_t off_G, off_H, off_XH, off_C, off_bar, total;
     __host__ __device__ SweepSmem(int XB, int NP) {
         RB = 12u * XB * NP * 16u;
         GO = 18u * XB * 16u;
@@ -84,7 +85,9 @@ struct SweepSmem {
         off_G = 2u * I_BYTES;
         off_H = off_G + 2u * G_BYTES;
         off_XH = off_H + H_BYTES;
-        off_bar = off_XH + XH_BYTES;
+        C_BYTES = ROWS * GO;
+        off_C = off_XH + XH_BYTES;
+        off_bar = off_C + 2u * C_BYTES;
         total = off_bar + 64u;
     }
 };
@@ -95,7 +98,9 @@ struct Nbr {
     int o, bs, cs;
 };
 
-template <int XB_, int NP_, bool CB>
+// CLOV: the clover term of the output parity is applied to the result before it is stored, out = M_ooee M_eooe in
+// (the first two steps of the Schur sequence, without the round trip through HBM)
+template <int XB_, int NP_, bool CB, bool CLOV>
 __global__ void __launch_bounds__(224, 1)
 hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__restrict__ out) {
     const int XB = XB_ ? XB_ : p.XB;
@@ -164,7 +169,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
             constexpr int NG = CB ? 6 : 4;   // link copies per row: on the full lattice U_x and U_t of the input row are the own links
             unsigned char *Gb = smem + L.off_G + b * L.G_BYTES;
             if (mid || j == -1) {
-                if (lane == 0) bar_expect_tx(&fullG[b], mid ? ROWS * (L.GO + (NG - 1) * L.GW) : ROWS * (CB ? L.GW : L.GO));
+                if (lane == 0) bar_expect_tx(&fullG[b], mid ? ROWS * (L.GO + (NG - 1) * L.GW + (CLOV ? L.GO : 0u)) : ROWS * (CB ? L.GW : L.GO));
                 __syncwarp();
                 for (int idx = lane; idx < ROWS * 6; idx += 32) {
                     const int r = idx / 6, w = idx - r * 6;
@@ -183,6 +188,10 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
                         default: src = p.gauge_in + (blk(xb, y, z, t) * kSiteF4 + 13) * XB; dst += L.GO + 4 * L.GW; break;     // U_t of the input row (carry)
                     }
                     bulk_g2s(dst, src, bytes, &fullG[b]);
+                }
+                if (CLOV && mid && lane >= 32 - ROWS) {
+                    const int r = lane - (32 - ROWS);
+                    bulk_g2s(smem + L.off_C + b * L.C_BYTES + r * L.GO, p.clover + blk(xb, y0 + r % BY, z0 + r / BY, t) * kSiteF4 * XB, L.GO, &fullG[b]);
                 }
             }
         };
@@ -313,8 +322,33 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
             hop_load_s<3>(A, S + own.o + (b ^ 1u) * own.bs, own.cs, G + g_own, XB);
             hop_compute<2, 3, true >(A, acc);
             float4 *o = out + (blk(xb, y, z, t) * 12 * XB + xin) * NP + pair;
+            if constexpr (CLOV) {
+                // out = M_ooee acc: two 6x6 Hermitian blocks (6 real diagonals + 15 complex lower-triangle entries each,
+                // reading S7), one chirality at a time; the 72 packed floats of the site are broadcast reads
+                const float4 *pc = S + L.off_C / 16 + b * (L.C_BYTES / 16) + r * (18 * XB) + xin;
 #pragma unroll
-            for (int c = 0; c < 12; c++) o[(size_t)c * cs] = from_cvec(acc[c]);
+                for (int ch = 0; ch < 2; ch++) {
+                    float a[36];
+#pragma unroll
+                    for (int j = 0; j < 9; j++) {
+                        const float4 v = pc[(9 * ch + j) * XB];
+                        a[4 * j] = v.x; a[4 * j + 1] = v.y; a[4 * j + 2] = v.z; a[4 * j + 3] = v.w;
+                    }
+#pragma unroll
+                    for (int i = 0; i < 6; i++) {
+                        CVec<2> v = rmul(a[i], acc[6 * ch + i]);
+#pragma unroll
+                        for (int j = 0; j < 6; j++) {
+                            if (j < i) v = cfma(a[6 + 2 * (i * (i - 1) / 2 + j)], a[6 + 2 * (i * (i - 1) / 2 + j) + 1], acc[6 * ch + j], v);
+                            else if (j > i) v = cfma_conj(a[6 + 2 * (j * (j - 1) / 2 + i)], a[6 + 2 * (j * (j - 1) / 2 + i) + 1], acc[6 * ch + j], v);
+                        }
+                        o[(size_t)(6 * ch + i) * cs] = from_cvec(v);
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int c = 0; c < 12; c++) o[(size_t)c * cs] = from_cvec(acc[c]);
+            }
         } else {
             bar_arrive(&freeI[b]);
         }
@@ -389,6 +423,7 @@ bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t
     ok &= make_fastdiv(nty / t.cy, grid, p.d_ncy);
     if (!ok) return false;
     p.gauge_out = p.gauge_in = nullptr;
+    p.clover = nullptr;
     p.pf = 2;
     if (const char *e = getenv("MRHS_SWEEP_PF")) p.pf = atoi(e);
     p.consumers = (unsigned)(ROWS * g.XB * np);
@@ -403,8 +438,9 @@ bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t
 mrhs_status_t sweep_prepare() {
     const int max_smem = 227 * 1024;
 #define MRHS_CASE(XB, NP)                                                                                                     \
-    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem)); \
-    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem)); \
+    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));  \
+    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
     MRHS_SWEEP_LIST(MRHS_CASE)
 #undef MRHS_CASE
     return MRHS_OK;
@@ -413,8 +449,9 @@ mrhs_status_t sweep_prepare() {
 namespace {
 template <int XB, int NP>
 void launch_sweep_t(const SweepParams &p, const void *d_in, void *d_out, cudaStream_t st) {
-    if (p.cb) hop_sweep_kernel<XB, NP, true><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
-    else      hop_sweep_kernel<XB, NP, false><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    if (p.cb && p.clover) hop_sweep_kernel<XB, NP, true, true><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    else if (p.cb)        hop_sweep_kernel<XB, NP, true, false><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    else                  hop_sweep_kernel<XB, NP, false, false><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
 }
 }  // namespace
 

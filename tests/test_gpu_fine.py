@@ -225,6 +225,41 @@ def test_schur_sequence_and_host_entry():
     w.close()
 
 
+FUSED_CASES = [([8, 8, 4, 4], 12, 60), ([4, 4, 4, 4], 4, 61), ([24, 4, 2, 6], 12, 62), ([16, 2, 4, 4], 24, 63),
+               ([8, 4, 6, 2], 3, 64), ([4, 4, 4, 4], 1, 65)]
+
+
+@pytest.mark.parametrize("dims,nrhs,seed", FUSED_CASES)
+def test_fused_meooe_mooee_and_schur_sequence(dims, nrhs, seed):
+    """out = M_ooee M_eooe in (one launch with the sweep kernel, two with the gather kernel; odd N_rhs takes
+    the gather path) and the Schur sequence built on it, both parities, both kernels, against the oracle."""
+    mass, csw = -0.05, 1.5
+    U, psi = _fine_case(dims, nrhs, seed, mass, csw)
+    w = make_wilson(dims, nrhs, mass, csw, U)
+    C, _ = oracle.clover_blocks(dims, U, mass, csw)
+    Cp = oracle.cb_split(dims, C)
+    src = oracle.cb_split(dims, psi)
+    kernels = [mrhs.HOP_GATHER] + ([mrhs.HOP_SWEEP] if nrhs % 2 == 0 else [])
+    for kern in kernels:
+        mrhs.wilson_set_hop_kernel(w.h, 1, kern)
+        for out_parity in (0, 1):
+            want = oracle.mooee(Cp[out_parity], oracle.meooe(dims, U, src[1 - out_parity], out_parity))
+            d_in = w.import_field(dev(src[1 - out_parity]), 1 - out_parity)
+            d_out = w.empty(out_parity)
+            w.meooe_mooee(d_in, d_out, out_parity)
+            torch.cuda.synchronize()
+            err = rel_l2_per_rhs(host(w.export_field(d_out, out_parity)), want)
+            assert err.max() < TOL, ("fused", kern, out_parity, err)
+        want = oracle.meooe(dims, U, oracle.mooee(Cp[1], oracle.meooe(dims, U, src[0], 1)), 0)
+        d_in = w.import_field(dev(src[0]), mrhs.EVEN)
+        t0, t1, d_out = w.empty(mrhs.ODD), w.empty(mrhs.ODD), w.empty(mrhs.EVEN)
+        w.schur_sequence(d_in, t0, t1, d_out)
+        torch.cuda.synchronize()
+        err = rel_l2_per_rhs(host(w.export_field(d_out, mrhs.EVEN)), want)
+        assert err.max() < TOL, ("schur", kern, err)
+    w.close()
+
+
 @pytest.mark.parametrize("nrhs", [1, 12])
 def test_config2_24x24_full_field(nrhs):
     """Config 2 (24^4, mass -0.05, c_sw 1.5): full-field parity for D_hop, M_eooe and M_ooee."""
