@@ -562,6 +562,10 @@ def run_sweep(args):
                 m, mn = timeit(lambda: c.apply(v, vo))
                 emit(cfg, "coarse_mode%d" % mode, dims, N, coarse_flops(nb) * V * N, bytes_coarse(V, nb, N), m, mn, base,
                      {"nbasis": nb, "fp32_fma_peak_frac": coarse_flops(nb) * V * N / (m * 1e-3) / 74.4e12})
+                # the 8-point coarse hopping term alone (what the paper's coarse-level figure measures, reading S12)
+                m, mn = timeit(lambda: c.apply(v, vo, mrhs.COARSE_HOP))
+                emit(cfg, "coarse_hop8_mode%d" % mode, dims, N, 64 * nb * nb * V * N, V * (64 * nb * nb + 16 * nb * N), m, mn, base,
+                     {"nbasis": nb})
                 c.close()
         del A
     out.close()

@@ -174,6 +174,17 @@ mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nb
  * 72 nb^2 flops per site per RHS.  d_in, d_out: native coarse vectors. */
 mrhs_status_t mrhs_coarse_apply(mrhs_coarse_t *h, const void *d_in, void *d_out);
 
+/* The same apply restricted to a subset of the nine stencil points (
+ * PAPER.md:75 benchmarks the coarse hopping term without the self term, reading S12):
+ *   out(x) = sum over p with bit p of point_mask set of A_p(x) in(x + delta_p),
+ * p = 0 self, 1..4 = +x..+t, 5..8 = -x..-t.  MRHS_COARSE_SELF is the stand-alone coarse clover
+ * (self) term, MRHS_COARSE_HOP the 8-point coarse hopping term (M_eooe + M_oeeo on full-lattice
+ * fields), MRHS_COARSE_ALL the 9-point operator.  Both math modes.  INVALID_ARG for an empty mask. */
+#define MRHS_COARSE_SELF 0x001
+#define MRHS_COARSE_HOP 0x1FE
+#define MRHS_COARSE_ALL 0x1FF
+mrhs_status_t mrhs_coarse_apply_points(mrhs_coarse_t *h, const void *d_in, void *d_out, int point_mask);
+
 mrhs_status_t mrhs_coarse_destroy(mrhs_coarse_t *h);
 
 /* ------------------------------------------------- layout helpers (untimed) */

@@ -24,6 +24,7 @@ EVEN, ODD, FULL = 0, 1, 2
 OP_DHOP, OP_MEOOE, OP_MOOEE, OP_SCHUR = 0, 1, 2, 3
 COARSE_FMA, COARSE_TENSOR = 0, 1
 HOP_GATHER, HOP_SWEEP = 0, 1
+COARSE_SELF, COARSE_HOP, COARSE_ALL = 0x001, 0x1FE, 0x1FF
 COARSE_MODES = (COARSE_FMA, COARSE_TENSOR)
 
 _vp = ctypes.c_void_p
@@ -49,6 +50,7 @@ _SIGNATURES = {
     "mrhs_wilson_destroy": (ctypes.c_int, [_vp]),
     "mrhs_coarse_create": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, ctypes.c_int, ctypes.c_int, _vp, ctypes.c_int, _vp]),
     "mrhs_coarse_apply": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_coarse_apply_points": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_coarse_destroy": (ctypes.c_int, [_vp]),
     "mrhs_xblock": (ctypes.c_int, [ctypes.c_int, ctypes.c_int]),
     "mrhs_field_bytes": (ctypes.c_size_t, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
@@ -251,6 +253,10 @@ def coarse_apply(h, d_in, d_out):
     _check(lib().mrhs_coarse_apply(h, _ptr(d_in), _ptr(d_out)))
 
 
+def coarse_apply_points(h, d_in, d_out, point_mask):
+    _check(lib().mrhs_coarse_apply_points(h, _ptr(d_in), _ptr(d_out), int(point_mask)))
+
+
 def coarse_apply_host(h, h_in, h_out):
     _check(lib().mrhs_coarse_apply_host(h, _ptr(h_in), _ptr(h_out)))
 
@@ -335,5 +341,8 @@ class Coarse:
     def export_field(self, native):
         return field_export(self.cdims, self.nbasis, self.nrhs, FULL, native)
 
-    def apply(self, d_in, d_out):
-        coarse_apply(self.h, d_in, d_out)
+    def apply(self, d_in, d_out, point_mask=None):
+        if point_mask is None:
+            coarse_apply(self.h, d_in, d_out)
+        else:
+            coarse_apply_points(self.h, d_in, d_out, point_mask)

@@ -435,12 +435,17 @@ mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nb
     return MRHS_OK;
 }
 
-mrhs_status_t mrhs_coarse_apply(mrhs_coarse_t *h, const void *d_in, void *d_out) {
+mrhs_status_t mrhs_coarse_apply_points(mrhs_coarse_t *h, const void *d_in, void *d_out, int point_mask) {
     MRHS_REQUIRE(h && d_in && d_out, "coarse apply: NULL argument");
     MRHS_REQUIRE(d_in != d_out, "coarse apply: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "coarse apply: buffers must be 16-byte aligned");
-    if (h->mode == 1) return launch_coarse_tc(h->g, h->tc_grid, (const float *)h->links, d_in, d_out, h->st);
-    return launch_coarse_fma(h->g, h->links, d_in, d_out, h->st);
+    MRHS_REQUIRE(point_mask > 0 && point_mask <= 0x1FF, "coarse apply: point_mask must select at least one of the nine stencil points");
+    if (h->mode == 1) return launch_coarse_tc(h->g, h->tc_grid, (unsigned)point_mask, (const float *)h->links, d_in, d_out, h->st);
+    return launch_coarse_fma(h->g, (unsigned)point_mask, h->links, d_in, d_out, h->st);
+}
+
+mrhs_status_t mrhs_coarse_apply(mrhs_coarse_t *h, const void *d_in, void *d_out) {
+    return mrhs_coarse_apply_points(h, d_in, d_out, MRHS_COARSE_ALL);
 }
 
 mrhs_status_t mrhs_coarse_destroy(mrhs_coarse_t *h) {

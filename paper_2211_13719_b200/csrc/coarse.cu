@@ -75,7 +75,7 @@ struct CoarseCfg {
 
 template <int NB, int N>
 __global__ void __launch_bounds__(CoarseCfg<NB, N>::THREADS)
-coarse_fma_kernel(int X, int Y, int Z, int T, const float2 *__restrict__ links,
+coarse_fma_kernel(int X, int Y, int Z, int T, unsigned mask, const float2 *__restrict__ links,
                   const typename Elem<CoarseCfg<NB, N>::R>::type *__restrict__ in,
                   typename Elem<CoarseCfg<NB, N>::R>::type *__restrict__ out) {
     typedef CoarseCfg<NB, N> C;
@@ -105,8 +105,12 @@ coarse_fma_kernel(int X, int Y, int Z, int T, const float2 *__restrict__ links,
         c[mu] = (c[mu] + d + ext[mu]) % ext[mu];
         return c[0] + (long long)X * (c[1] + (long long)Y * (c[2] + (long long)Z * c[3]));
     };
-    auto issue = [&](int p) {
-        const int slot = p % C::NSTAGE;
+    // the stencil points of this apply: bit p of mask (all nine for the full operator, bit 0 = self term alone,
+    // bits 1..8 = the 8-point hopping term); stage s handles the s-th set bit
+    const int npts = __popc(mask);
+    auto issue = [&](int s) {
+        const int p = (int)__fns(mask, 0, s + 1);
+        const int slot = s % C::NSTAGE;
         unsigned char *dst = smem + (size_t)slot * C::STAGE_BYTES;
         mbar_expect_tx(&full[slot], C::STAGE_BYTES);
         bulk_g2s(dst, links + ((size_t)site * 9 + p) * NB * NB, C::A_BYTES, &full[slot]);
@@ -119,7 +123,7 @@ coarse_fma_kernel(int X, int Y, int Z, int T, const float2 *__restrict__ links,
     }
     __syncthreads();
     if (tid == 0)
-        for (int p = 0; p < C::NSTAGE && p < 9; p++) issue(p);
+        for (int s = 0; s < C::NSTAGE && s < npts; s++) issue(s);
 
     CVec<R> acc[TI][TP];
 #pragma unroll
@@ -127,7 +131,7 @@ coarse_fma_kernel(int X, int Y, int Z, int T, const float2 *__restrict__ links,
 #pragma unroll
         for (int b = 0; b < TP; b++) acc[a][b] = czero_c<R>();
 
-    for (int p = 0; p < 9; p++) {
+    for (int p = 0; p < npts; p++) {
         const int slot = p % C::NSTAGE;
         mbar_wait(&full[slot], (p / C::NSTAGE) & 1);
         const float2 *As = reinterpret_cast<const float2 *>(smem + (size_t)slot * C::STAGE_BYTES);   // [col][row]
@@ -152,7 +156,7 @@ coarse_fma_kernel(int X, int Y, int Z, int T, const float2 *__restrict__ links,
                 for (int b = 0; b < TP; b++) acc[i][b] = cfma(a[i].x, a[i].y, v[b], acc[i][b]);
         }
         __syncthreads();   // every thread is done with this slot
-        if (tid == 0 && p + C::NSTAGE < 9) issue(p + C::NSTAGE);
+        if (tid == 0 && p + C::NSTAGE < npts) issue(p + C::NSTAGE);
     }
 
     // sum the column slices (the stage ring is free: the last __syncthreads above covers it)
@@ -196,10 +200,10 @@ __global__ void pack_links_kernel(int nb, const float2 *__restrict__ src, float2
 }
 
 template <int NB, int N>
-mrhs_status_t launch_t(const CoarseGeom &g, const float2 *links, const void *in, void *out, cudaStream_t st) {
+mrhs_status_t launch_t(const CoarseGeom &g, unsigned mask, const float2 *links, const void *in, void *out, cudaStream_t st) {
     typedef CoarseCfg<NB, N> C;
     typedef typename Elem<C::R>::type E;
-    coarse_fma_kernel<NB, N><<<(unsigned)g.nsites, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, links, (const E *)in, (E *)out);
+    coarse_fma_kernel<NB, N><<<(unsigned)g.nsites, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, mask, links, (const E *)in, (E *)out);
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
 }
@@ -232,8 +236,8 @@ mrhs_status_t coarse_fma_prepare(const CoarseGeom &g) {
     return MRHS_ERR_UNSUPPORTED;
 }
 
-mrhs_status_t launch_coarse_fma(const CoarseGeom &g, const float2 *d_links, const void *d_in, void *d_out, cudaStream_t st) {
-#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return launch_t<NB, NN>(g, d_links, d_in, d_out, st);
+mrhs_status_t launch_coarse_fma(const CoarseGeom &g, unsigned mask, const float2 *d_links, const void *d_in, void *d_out, cudaStream_t st) {
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return launch_t<NB, NN>(g, mask, d_links, d_in, d_out, st);
     MRHS_COARSE_N_LIST(MRHS_CASE, 24)
     MRHS_COARSE_N_LIST(MRHS_CASE, 40)
 #undef MRHS_CASE

@@ -18,7 +18,8 @@ mrhs_status_t pack_coarse_links(const CoarseGeom &g, const float2 *d_canonical, 
 // true if an FP32-FMA specialisation for (nbasis, nrhs) is compiled
 bool coarse_fma_supported(int nb, int nrhs);
 mrhs_status_t coarse_fma_prepare(const CoarseGeom &g);   // opt in to large dynamic shared memory
-mrhs_status_t launch_coarse_fma(const CoarseGeom &g, const float2 *d_links, const void *d_in, void *d_out, cudaStream_t st);
+// mask: bit p set = stencil point p is applied (0 self, 1..4 = +x..+t, 5..8 = -x..-t); 0x1FF = the 9-point operator
+mrhs_status_t launch_coarse_fma(const CoarseGeom &g, unsigned mask, const float2 *d_links, const void *d_in, void *d_out, cudaStream_t st);
 
 // ---- tensor-core variant (row a6): tcgen05 kind::tf32 with hi/lo split operands (3 MMAs per K step)
 // true if a tensor-core specialisation for (nbasis, nrhs) is compiled (even nrhs only)
@@ -28,6 +29,6 @@ bool coarse_tc_supported(int nb, int nrhs);
 mrhs_status_t pack_coarse_links_tc(const CoarseGeom &g, const float2 *d_canonical, float *d_native, cudaStream_t st);
 // opt in to large dynamic shared memory and size the persistent grid (CTAs per SM limited by shared memory and TMEM)
 mrhs_status_t coarse_tc_prepare(const CoarseGeom &g, int *grid);
-mrhs_status_t launch_coarse_tc(const CoarseGeom &g, int grid, const float *d_links, const void *d_in, void *d_out, cudaStream_t st);
+mrhs_status_t launch_coarse_tc(const CoarseGeom &g, int grid, unsigned mask, const float *d_links, const void *d_in, void *d_out, cudaStream_t st);
 
 }  // namespace mrhs

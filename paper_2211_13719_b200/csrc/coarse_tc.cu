@@ -144,7 +144,7 @@ struct TcCfg {
 // in/out: coarse vectors [site][component][RHS pair] float4 = (re0 re1 im0 im1), as in the FMA variant
 template <int NB, int N>
 __global__ void __launch_bounds__(TcCfg<NB, N>::THREADS)
-coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, const float4 *__restrict__ links,
+coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, const float4 *__restrict__ links,
                  const float4 *__restrict__ in, float4 *__restrict__ out) {
     typedef TcCfg<NB, N> C;
     constexpr int A_IT = (C::A_UNITS + C::THREADS - 1) / C::THREADS;
@@ -212,9 +212,13 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, const float4 *__r
     // For wide operands (two blocks per SM) the load runs one stage ahead; for narrow ones the extra live registers
     // would cost resident blocks, which hide the latency better, so the load sits at the top of its own stage.
     constexpr bool AHEAD = C::NT > 96;
-    if (AHEAD && (long long)blockIdx.x < nsites) load_stage(blockIdx.x, 0);
+    // the stencil points of this apply: bit p of mask; stage s of a site handles the s-th set bit
+    const int npts = __popc(mask);
+    auto point = [&](int s) { return (int)__fns(mask, 0, s + 1); };
+    if (AHEAD && (long long)blockIdx.x < nsites) load_stage(blockIdx.x, point(0));
     for (long long site = blockIdx.x; site < nsites; site += gridDim.x) {
-        for (int p = 0; p < 9; p++) {
+        for (int sp = 0; sp < npts; sp++) {
+            const int p = point(sp);
             if (!AHEAD) load_stage(site, p);
             // the single operand buffer is free once the previous stage's MMAs have completed
             if (nstage > 0) mbar_wait(bar, (nstage - 1) & 1);
@@ -264,7 +268,7 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, const float4 *__r
                     const uint64_t dal = smem_desc(al + ks * 2 * C::A_LBO, C::A_LBO, 128);
                     const uint64_t dbh = smem_desc(bh + ks * 2 * C::B_LBO, C::B_LBO, 128);
                     const uint64_t dbl = smem_desc(bl + ks * 2 * C::B_LBO, C::B_LBO, 128);
-                    mma_tf32(tmem, dal, dbh, idesc, (p | ks) != 0);
+                    mma_tf32(tmem, dal, dbh, idesc, (sp | ks) != 0);
                     mma_tf32(tmem, dah, dbl, idesc, 1);
                     mma_tf32(tmem, dah, dbh, idesc, 1);
                 }
@@ -272,8 +276,8 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, const float4 *__r
             }
             nstage++;
             if (AHEAD) {
-                if (p < 8) load_stage(site, p + 1);
-                else if (site + gridDim.x < nsites) load_stage(site + gridDim.x, 0);
+                if (sp + 1 < npts) load_stage(site, point(sp + 1));
+                else if (site + gridDim.x < nsites) load_stage(site + gridDim.x, point(0));
             }
         }
         // all nine points accumulated: TMEM -> shared scratch S[col][lane] -> combine -> global
@@ -347,9 +351,9 @@ mrhs_status_t tc_prepare_t(int *ctas_per_sm) {
     return MRHS_OK;
 }
 template <int NB, int N>
-mrhs_status_t tc_launch_t(const CoarseGeom &g, int grid, const float *links, const void *in, void *out, cudaStream_t st) {
+mrhs_status_t tc_launch_t(const CoarseGeom &g, int grid, unsigned mask, const float *links, const void *in, void *out, cudaStream_t st) {
     typedef TcCfg<NB, N> C;
-    coarse_tc_kernel<NB, N><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, g.nsites, (const float4 *)links,
+    coarse_tc_kernel<NB, N><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, g.nsites, mask, (const float4 *)links,
                                                                       (const float4 *)in, (float4 *)out);
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
@@ -387,8 +391,8 @@ mrhs_status_t coarse_tc_prepare(const CoarseGeom &g, int *grid) {
     return MRHS_OK;
 }
 
-mrhs_status_t launch_coarse_tc(const CoarseGeom &g, int grid, const float *d_links, const void *d_in, void *d_out, cudaStream_t st) {
-#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return tc_launch_t<NB, NN>(g, grid, d_links, d_in, d_out, st);
+mrhs_status_t launch_coarse_tc(const CoarseGeom &g, int grid, unsigned mask, const float *d_links, const void *d_in, void *d_out, cudaStream_t st) {
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return tc_launch_t<NB, NN>(g, grid, mask, d_links, d_in, d_out, st);
     MRHS_TC_N_LIST(MRHS_CASE, 24)
     MRHS_TC_N_LIST(MRHS_CASE, 40)
 #undef MRHS_CASE

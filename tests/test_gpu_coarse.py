@@ -17,10 +17,10 @@ import paper_2211_13719_b200 as mrhs   # noqa: E402
 from gpu_common import TOL, dev, host   # noqa: E402
 
 
-def gpu_coarse(c, v):
+def gpu_coarse(c, v, point_mask=None):
     d_in = c.import_field(dev(v))
     d_out = c.empty()
-    c.apply(d_in, d_out)
+    c.apply(d_in, d_out, point_mask)
     torch.cuda.synchronize()
     return host(c.export_field(d_out))
 
@@ -122,6 +122,22 @@ def test_coarse_tensor_core_rejects_odd_nrhs():
     with pytest.raises(mrhs.MrhsError) as e:
         mrhs.Coarse(cdims, nb, 1, A, math_mode=1)
     assert e.value.status == mrhs.ERR_UNSUPPORTED
+
+
+# ---- subsets of the stencil (NEXT-1): stand-alone self term, 8-point hopping term, single points; both math modes
+@pytest.mark.parametrize("mode", [mrhs.COARSE_FMA, mrhs.COARSE_TENSOR])
+@pytest.mark.parametrize("cdims,nb,nrhs", [([4, 2, 6, 2], 24, 12), ([3, 4, 2, 5], 40, 24), ([2, 2, 2, 2], 40, 96)])
+def test_coarse_point_subsets_match_oracle(cdims, nb, nrhs, mode):
+    A = syn.coarse_links_np(cdims, nb, 7)
+    v = syn.coarse_vector_np(cdims, nb, nrhs, 7)
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=mode)
+    for mask in (mrhs.COARSE_SELF, mrhs.COARSE_HOP, mrhs.COARSE_ALL, 1 << 3, 1 << 8, 0x0AA, 0x155):
+        want = oracle.coarse_apply(cdims, A, v, pmask=mask)
+        err = rel_l2_per_rhs(gpu_coarse(c, v, mask), want)
+        assert err.max() < TOL, (hex(mask), err)
+    with pytest.raises(mrhs.MrhsError):
+        c.apply(c.empty(), c.empty(), 0)
+    c.close()
 
 
 def test_coarse_errors():

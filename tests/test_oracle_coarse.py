@@ -30,6 +30,21 @@ def test_coarse_apply_is_per_site_matmul(cdims, nb, N):
                          np.matmul(A[:, 7], v[shift_index(cdims, 2, -1)]))) < 1e-13
 
 
+def test_coarse_point_masks_are_the_single_point_matmuls():
+    """Every single stencil point against numpy, and subsets add up: self + 8-point hop = 9-point (S12)."""
+    cdims, nb, N = (2, 4, 2, 6), 5, 2
+    A = si.coarse_links_np(cdims, nb, 37).astype(np.complex128)
+    v = si.coarse_vector_np(cdims, nb, N, 38).astype(np.complex128)
+    single = [np.matmul(A[:, 0], v)]
+    single += [np.matmul(A[:, 1 + mu], v[shift_index(cdims, mu, +1)]) for mu in range(4)]
+    single += [np.matmul(A[:, 5 + mu], v[shift_index(cdims, mu, -1)]) for mu in range(4)]
+    for p in range(9):
+        assert np.max(np.abs(oracle.coarse_apply(cdims, A, v, pmask=1 << p) - single[p])) < 1e-13
+    hop = oracle.coarse_apply(cdims, A, v, pmask=0x1FE)
+    assert np.max(np.abs(hop - sum(single[1:]))) < 1e-12
+    assert np.max(np.abs(oracle.coarse_apply(cdims, A, v, pmask=0x001) + hop - oracle.coarse_apply(cdims, A, v))) < 1e-12
+
+
 def test_coarse_sites_entry_matches_full():
     cdims, nb, N = (4, 2, 2, 4), 6, 2
     A = si.coarse_links_np(cdims, nb, 33).astype(np.complex128)
