@@ -73,7 +73,8 @@ struct CoarseCfg {
     static_assert(A_BYTES % 16 == 0 && V_BYTES % 16 == 0, "bulk copies need 16-byte multiples");
 };
 
-template <int NB, int N>
+// ALL: the nine-point operator (mask ignored; the stage loop has a compile-time trip count)
+template <int NB, int N, bool ALL>
 __global__ void __launch_bounds__(CoarseCfg<NB, N>::THREADS)
 coarse_fma_kernel(int X, int Y, int Z, int T, unsigned mask, const float2 *__restrict__ links,
                   const typename Elem<CoarseCfg<NB, N>::R>::type *__restrict__ in,
@@ -107,9 +108,9 @@ coarse_fma_kernel(int X, int Y, int Z, int T, unsigned mask, const float2 *__res
     };
     // the stencil points of this apply: bit p of mask (all nine for the full operator, bit 0 = self term alone,
     // bits 1..8 = the 8-point hopping term); stage s handles the s-th set bit
-    const int npts = __popc(mask);
+    const int npts = ALL ? 9 : __popc(mask);
     auto issue = [&](int s) {
-        const int p = (int)__fns(mask, 0, s + 1);
+        const int p = ALL ? s : (int)__fns(mask, 0, s + 1);
         const int slot = s % C::NSTAGE;
         unsigned char *dst = smem + (size_t)slot * C::STAGE_BYTES;
         mbar_expect_tx(&full[slot], C::STAGE_BYTES);
@@ -203,14 +204,16 @@ template <int NB, int N>
 mrhs_status_t launch_t(const CoarseGeom &g, unsigned mask, const float2 *links, const void *in, void *out, cudaStream_t st) {
     typedef CoarseCfg<NB, N> C;
     typedef typename Elem<C::R>::type E;
-    coarse_fma_kernel<NB, N><<<(unsigned)g.nsites, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, mask, links, (const E *)in, (E *)out);
+    if (mask == 0x1FFu) coarse_fma_kernel<NB, N, true><<<(unsigned)g.nsites, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, mask, links, (const E *)in, (E *)out);
+    else coarse_fma_kernel<NB, N, false><<<(unsigned)g.nsites, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, mask, links, (const E *)in, (E *)out);
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
 }
 template <int NB, int N>
 mrhs_status_t prepare_t() {
     typedef CoarseCfg<NB, N> C;
-    MRHS_CUDA(cudaFuncSetAttribute(coarse_fma_kernel<NB, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_fma_kernel<NB, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_fma_kernel<NB, N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
     return MRHS_OK;
 }
 

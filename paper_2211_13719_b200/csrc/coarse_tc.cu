@@ -142,7 +142,8 @@ struct TcCfg {
 
 // links: native tensor-core layout [site][p][part Re/Im][K chunk][row][4 columns] fp32 (pack_coarse_links_tc)
 // in/out: coarse vectors [site][component][RHS pair] float4 = (re0 re1 im0 im1), as in the FMA variant
-template <int NB, int N>
+// ALL: the nine-point operator (mask ignored; compile-time stage count)
+template <int NB, int N, bool ALL>
 __global__ void __launch_bounds__(TcCfg<NB, N>::THREADS)
 coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, const float4 *__restrict__ links,
                  const float4 *__restrict__ in, float4 *__restrict__ out) {
@@ -213,8 +214,8 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, co
     // would cost resident blocks, which hide the latency better, so the load sits at the top of its own stage.
     constexpr bool AHEAD = C::NT > 96;
     // the stencil points of this apply: bit p of mask; stage s of a site handles the s-th set bit
-    const int npts = __popc(mask);
-    auto point = [&](int s) { return (int)__fns(mask, 0, s + 1); };
+    const int npts = ALL ? 9 : __popc(mask);
+    auto point = [&](int s) { return ALL ? s : (int)__fns(mask, 0, s + 1); };
     if (AHEAD && (long long)blockIdx.x < nsites) load_stage(blockIdx.x, point(0));
     for (long long site = blockIdx.x; site < nsites; site += gridDim.x) {
         for (int sp = 0; sp < npts; sp++) {
@@ -330,12 +331,14 @@ __global__ void pack_links_tc_kernel(int nb, const float2 *__restrict__ src, flo
 template <int NB, int N>
 mrhs_status_t tc_prepare_t(int *ctas_per_sm) {
     typedef TcCfg<NB, N> C;
-    MRHS_CUDA(cudaFuncSetAttribute(coarse_tc_kernel<NB, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-    MRHS_CUDA(cudaFuncSetAttribute(coarse_tc_kernel<NB, N>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_tc_kernel<NB, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_tc_kernel<NB, N, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_tc_kernel<NB, N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_tc_kernel<NB, N, false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     // Resident CTAs per SM from the resources themselves (the occupancy API reports 1 for a kernel that
     // allocates tensor memory): shared memory (+1 KB reserved per CTA), registers, threads, TMEM columns.
     cudaFuncAttributes fa;
-    MRHS_CUDA(cudaFuncGetAttributes(&fa, coarse_tc_kernel<NB, N>));
+    MRHS_CUDA(cudaFuncGetAttributes(&fa, coarse_tc_kernel<NB, N, false>));
     int dev = 0, smem_sm = 0, regs_sm = 0;
     MRHS_CUDA(cudaGetDevice(&dev));
     MRHS_CUDA(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
@@ -353,8 +356,12 @@ mrhs_status_t tc_prepare_t(int *ctas_per_sm) {
 template <int NB, int N>
 mrhs_status_t tc_launch_t(const CoarseGeom &g, int grid, unsigned mask, const float *links, const void *in, void *out, cudaStream_t st) {
     typedef TcCfg<NB, N> C;
-    coarse_tc_kernel<NB, N><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, g.nsites, mask, (const float4 *)links,
-                                                                      (const float4 *)in, (float4 *)out);
+    if (mask == 0x1FFu)
+        coarse_tc_kernel<NB, N, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, g.nsites, mask, (const float4 *)links,
+                                                                               (const float4 *)in, (float4 *)out);
+    else
+        coarse_tc_kernel<NB, N, false><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, g.nsites, mask, (const float4 *)links,
+                                                                                (const float4 *)in, (float4 *)out);
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
 }
