@@ -386,12 +386,13 @@ SweepTiling default_sweep_tiling(const FieldGeom &g, int num_sms) {
             if (n > best_n || (n == best_n && shape < best_shape)) { best_n = n; best_shape = shape; t.cy = cy; t.cz = cz; }
         }
     }
-    // segment length: the whole t-line if that still gives eight waves of blocks, else shorter segments
+    // segment length: the whole t-line as long as that leaves two blocks per SM to balance the tail (every segment
+    // pays two extra slice loads, measured slower whenever the line fits); shorter segments only for small lattices
     const long long tiles = (long long)g.nxb * nty * ntz;
     int pick = 0;
     for (int lt = g.T; lt >= 1; lt--) {
         if (g.T % lt) continue;
-        if (tiles * (g.T / lt) >= 8ll * num_sms) { pick = lt; break; }
+        if (tiles * (g.T / lt) >= 2ll * num_sms) { pick = lt; break; }
     }
     if (pick < 4) {
         pick = g.T;

@@ -141,7 +141,7 @@ KERNEL_CASES = [
 def test_gather_and_sweep_kernels_match_oracle(dims, nrhs, seed):
     U, psi = _fine_case(dims, nrhs, seed, -0.05, 1.5)
     w = make_wilson(dims, nrhs, -0.05, 1.5, U)
-    assert mrhs.wilson_get_hop_kernel(w.h, 0) == mrhs.HOP_SWEEP      # the default for even N_rhs
+    assert mrhs.wilson_get_hop_kernel(w.h, 0) == mrhs.HOP_GATHER     # the default on small lattices (sweep from 32^4, N_rhs >= 12)
     want = oracle.dhop(dims, U, psi)
     pe, po = oracle.cb_split(dims, psi)
     want_cb = [oracle.meooe(dims, U, po, 0), oracle.meooe(dims, U, pe, 1)]

@@ -71,6 +71,7 @@ def config5():
     U = syn.gauge_torch(DIMS, SEED, dev)
     psi = syn.spinor_torch(syn.volume(DIMS), NRHS, SEED, dev)
     w = mrhs.Wilson(DIMS, NRHS, MASS, CSW, U)
+    assert mrhs.wilson_get_hop_kernel(w.h, 0) == mrhs.HOP_SWEEP and mrhs.wilson_get_hop_kernel(w.h, 1) == mrhs.HOP_SWEEP
     yield U, psi, w
     w.close()
 
