@@ -107,6 +107,12 @@ mrhs_status_t mrhs_meooe(mrhs_wilson_t *h, const void *d_in, void *d_out, int ou
  * parity 0/1: checkerboarded fields of that parity; 2: full-lattice fields. */
 mrhs_status_t mrhs_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity);
 
+/* M_ooee^-1 ("precomputed"): out(x) = C(x)^-1 in(x).  The inverse
+ * blocks are computed once at create (fp64 Gauss-Jordan per 6x6 block, stored fp32 in the same packed
+ * Hermitian form), so the apply is the same kernel with the same cost as mrhs_mooee.  A singular
+ * user-supplied block gives non-finite entries in its inverse (not checked). */
+mrhs_status_t mrhs_mooee_inv(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity);
+
 /* Fused out = M_ooee(out_parity) M_eooe(in): the hopping term onto parity out_parity followed by
  * the clover term of those sites (the first two steps of the Schur
  * sequence below).  With the sweep kernel (even N_rhs) this is ONE
@@ -114,6 +120,9 @@ mrhs_status_t mrhs_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int pa
  * intermediate field never goes through HBM.  With the gather kernel it is two launches.
  * d_in: native field of parity 1 - out_parity; d_out: native field of parity out_parity. */
 mrhs_status_t mrhs_meooe_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity);
+/* The same with the inverse blocks: out = M_ooee(out_parity)^-1 M_eooe(in), the inner part of the
+ * even-odd (Schur) preconditioned operator. */
+mrhs_status_t mrhs_meooe_mooee_inv(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity);
 
 /* Schur-style sequence of config 5, back to back on the handle's
  * stream with no host synchronisation:

@@ -168,6 +168,12 @@ def clover_blocks(dims, U, mass, csw):
     return C, off.value
 
 
+def clover_inverse(C):
+    """Inverse clover blocks: the matrix inverse of every 6x6 block,
+    by the library routine (numpy.linalg.inv, fp64).  C [n][2][6][6] -> same shape."""
+    return np.linalg.inv(_c128(C))
+
+
 def mooee(C, psi):
     """M_ooee apply.  C [n][2][6][6], psi [n][4][3][N] -> same shape."""
     C = _c128(C); psi = _c128(psi)

@@ -39,6 +39,8 @@ _SIGNATURES = {
     "mrhs_mooee": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_schur_sequence": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "mrhs_meooe_mooee": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
+    "mrhs_meooe_mooee_inv": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
+    "mrhs_mooee_inv": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_wilson_export_clover": (ctypes.c_int, [_vp, _vp]),
     "mrhs_wilson_set_tiling": (ctypes.c_int, [_vp, ctypes.c_int, _int3, _int2]),
     "mrhs_wilson_get_tiling": (ctypes.c_int, [_vp, ctypes.c_int, _int3, _int2]),
@@ -189,6 +191,14 @@ def meooe_mooee(h, d_in, d_out, out_parity):
     _check(lib().mrhs_meooe_mooee(h, _ptr(d_in), _ptr(d_out), int(out_parity)))
 
 
+def meooe_mooee_inv(h, d_in, d_out, out_parity):
+    _check(lib().mrhs_meooe_mooee_inv(h, _ptr(d_in), _ptr(d_out), int(out_parity)))
+
+
+def mooee_inv(h, d_in, d_out, parity):
+    _check(lib().mrhs_mooee_inv(h, _ptr(d_in), _ptr(d_out), int(parity)))
+
+
 def schur_sequence(h, d_in, d_tmp0, d_tmp1, d_out):
     _check(lib().mrhs_schur_sequence(h, _ptr(d_in), _ptr(d_tmp0), _ptr(d_tmp1), _ptr(d_out)))
 
@@ -307,6 +317,12 @@ class Wilson:
 
     def meooe_mooee(self, d_in, d_out, out_parity):
         meooe_mooee(self.h, d_in, d_out, out_parity)
+
+    def meooe_mooee_inv(self, d_in, d_out, out_parity):
+        meooe_mooee_inv(self.h, d_in, d_out, out_parity)
+
+    def mooee_inv(self, d_in, d_out, parity):
+        mooee_inv(self.h, d_in, d_out, parity)
 
     def schur_sequence(self, d_in, d_tmp0, d_tmp1, d_out):
         schur_sequence(self.h, d_in, d_tmp0, d_tmp1, d_out)

@@ -38,6 +38,7 @@ struct mrhs_wilson {
     FieldGeom gfull, gcb[2];
     float4 *gauge_full, *gauge_cb[2];
     float4 *clov_full, *clov_cb[2];
+    float4 *cinv_full, *cinv_cb[2];   // inverse clover blocks, same packing and layouts
     HopParams hp_full, hp_cb[2];   // hp_cb[p]: output parity p
     SweepParams sp_full, sp_cb[2]; // the slice-sweep kernel's launch description (fine_sweep.cuh)
     int kern[2];                   // which kernel runs D_hop [0] / M_eooe [1]: MRHS_HOP_GATHER or MRHS_HOP_SWEEP
@@ -66,6 +67,7 @@ mrhs_status_t wilson_free(mrhs_wilson *h) {
     if (!h) return MRHS_OK;
     cudaFree(h->gauge_full); cudaFree(h->gauge_cb[0]); cudaFree(h->gauge_cb[1]);
     cudaFree(h->clov_full); cudaFree(h->clov_cb[0]); cudaFree(h->clov_cb[1]);
+    cudaFree(h->cinv_full); cudaFree(h->cinv_cb[0]); cudaFree(h->cinv_cb[1]);
     cudaFree(h->st_canon); cudaFree(h->st_in); cudaFree(h->st_out);
     cudaFree(h->st_tmp[0]); cudaFree(h->st_tmp[1]);
     delete h;
@@ -77,9 +79,11 @@ mrhs_status_t wilson_build(mrhs_wilson *h, const void *d_gauge, const void *d_cl
     const size_t V = (size_t)h->gfull.nsites;
     MRHS_CUDA(cudaMalloc(&h->gauge_full, V * site_bytes));
     MRHS_CUDA(cudaMalloc(&h->clov_full, V * site_bytes));
+    MRHS_CUDA(cudaMalloc(&h->cinv_full, V * site_bytes));
     for (int p = 0; p < 2; p++) {
         MRHS_CUDA(cudaMalloc(&h->gauge_cb[p], V / 2 * site_bytes));
         MRHS_CUDA(cudaMalloc(&h->clov_cb[p], V / 2 * site_bytes));
+        MRHS_CUDA(cudaMalloc(&h->cinv_cb[p], V / 2 * site_bytes));
     }
     // the canonical gauge field already is [lex][72 floats]
     mrhs_status_t s;
@@ -92,6 +96,10 @@ mrhs_status_t wilson_build(mrhs_wilson *h, const void *d_gauge, const void *d_cl
     else s = build_clover(h->dims, h->mass, h->csw, (const float2 *)d_gauge, tmp, h->st);
     if (s == MRHS_OK) s = pack_site_data(h->gfull, tmp, h->clov_full, h->st);
     for (int p = 0; p < 2 && s == MRHS_OK; p++) s = pack_site_data(h->gcb[p], tmp, h->clov_cb[p], h->st);
+    // inverse blocks, in place in tmp (pack_site_data above has been enqueued on the same stream)
+    if (s == MRHS_OK) s = invert_clover_blocks((long long)V, tmp, tmp, h->st);
+    if (s == MRHS_OK) s = pack_site_data(h->gfull, tmp, h->cinv_full, h->st);
+    for (int p = 0; p < 2 && s == MRHS_OK; p++) s = pack_site_data(h->gcb[p], tmp, h->cinv_cb[p], h->st);
     cudaError_t e = cudaStreamSynchronize(h->st);
     cudaFree(tmp);
     if (s != MRHS_OK) return s;
@@ -206,16 +214,22 @@ mrhs_status_t mrhs_meooe(mrhs_wilson_t *h, const void *d_in, void *d_out, int ou
     return launch_hop(h->hp_cb[out_parity], h->nrhs, d_in, d_out, h->st);
 }
 
-mrhs_status_t mrhs_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity) {
+static mrhs_status_t mooee_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity, bool inverse);
+mrhs_status_t mrhs_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity) { return mooee_impl(h, d_in, d_out, parity, false); }
+mrhs_status_t mrhs_mooee_inv(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity) { return mooee_impl(h, d_in, d_out, parity, true); }
+static mrhs_status_t mooee_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity, bool inverse) {
     MRHS_REQUIRE(h && d_in && d_out, "mooee: NULL argument");
     MRHS_REQUIRE(parity >= 0 && parity <= 2, "mooee: parity must be 0, 1 or 2");
     MRHS_REQUIRE(d_in != d_out, "mooee: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "mooee: buffers must be 16-byte aligned");
-    if (parity == MRHS_FULL) return launch_mooee(h->gfull, h->clov_full, d_in, d_out, h->st);
-    return launch_mooee(h->gcb[parity], h->clov_cb[parity], d_in, d_out, h->st);
+    if (parity == MRHS_FULL) return launch_mooee(h->gfull, inverse ? h->cinv_full : h->clov_full, d_in, d_out, h->st);
+    return launch_mooee(h->gcb[parity], inverse ? h->cinv_cb[parity] : h->clov_cb[parity], d_in, d_out, h->st);
 }
 
-mrhs_status_t mrhs_meooe_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity) {
+static mrhs_status_t meooe_mooee_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity, bool inverse);
+mrhs_status_t mrhs_meooe_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity) { return meooe_mooee_impl(h, d_in, d_out, out_parity, false); }
+mrhs_status_t mrhs_meooe_mooee_inv(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity) { return meooe_mooee_impl(h, d_in, d_out, out_parity, true); }
+static mrhs_status_t meooe_mooee_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity, bool inverse) {
     MRHS_REQUIRE(h && d_in && d_out, "meooe_mooee: NULL argument");
     MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "meooe_mooee: out_parity must be 0 or 1");
     MRHS_REQUIRE(d_in != d_out, "meooe_mooee: in and out must not alias");
@@ -223,12 +237,12 @@ mrhs_status_t mrhs_meooe_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, 
     if (h->kern[1] == MRHS_HOP_SWEEP) {
         // one launch: the clover blocks of the output sites are applied to the hop result before it is stored
         SweepParams p = h->sp_cb[out_parity];
-        p.clover = h->clov_cb[out_parity];
+        p.clover = inverse ? h->cinv_cb[out_parity] : h->clov_cb[out_parity];
         return launch_sweep(p, d_in, d_out, h->st);
     }
     // gather kernel: two launches; the site-diagonal term reads each site's twelve components before it writes them
     mrhs_status_t s = launch_hop(h->hp_cb[out_parity], h->nrhs, d_in, d_out, h->st);
-    if (s == MRHS_OK) s = launch_mooee(h->gcb[out_parity], h->clov_cb[out_parity], d_out, d_out, h->st);
+    if (s == MRHS_OK) s = launch_mooee(h->gcb[out_parity], inverse ? h->cinv_cb[out_parity] : h->clov_cb[out_parity], d_out, d_out, h->st);
     return s;
 }
 

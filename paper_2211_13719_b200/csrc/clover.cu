@@ -157,6 +157,58 @@ __global__ void unpack_blocks_kernel(const float *__restrict__ packed, float2 *_
         }
 }
 
+// packed Hermitian 6x6 blocks -> packed inverse blocks (the inverse of a Hermitian matrix is Hermitian, so the same
+// packing holds it).  One thread per (site, chirality); Gauss-Jordan with partial pivoting in fp64.  Setup, untimed.
+__global__ void invert_blocks_kernel(const float *__restrict__ packed, float *__restrict__ inv, long long n2) {
+    long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= n2) return;
+    const float *o = packed + g * 36;
+    double ar[6][12], ai[6][12];   // [A | 1] -> [1 | A^-1]
+    for (int i = 0; i < 6; i++)
+        for (int j = 0; j < 12; j++) { ar[i][j] = (j == 6 + i) ? 1.0 : 0.0; ai[i][j] = 0.0; }
+    for (int i = 0; i < 6; i++) ar[i][i] = o[i];
+    for (int i = 1; i < 6; i++)
+        for (int j = 0; j < i; j++) {
+            const int idx = i * (i - 1) / 2 + j;
+            ar[i][j] = o[6 + 2 * idx]; ai[i][j] = o[6 + 2 * idx + 1];
+            ar[j][i] = o[6 + 2 * idx]; ai[j][i] = -(double)o[6 + 2 * idx + 1];
+        }
+    for (int c = 0; c < 6; c++) {
+        int piv = c;
+        double best = ar[c][c] * ar[c][c] + ai[c][c] * ai[c][c];
+        for (int r = c + 1; r < 6; r++) {
+            const double m = ar[r][c] * ar[r][c] + ai[r][c] * ai[r][c];
+            if (m > best) { best = m; piv = r; }
+        }
+        if (piv != c)
+            for (int j = 0; j < 12; j++) {
+                double t = ar[c][j]; ar[c][j] = ar[piv][j]; ar[piv][j] = t;
+                t = ai[c][j]; ai[c][j] = ai[piv][j]; ai[piv][j] = t;
+            }
+        const double pr = ar[c][c] / best, pi = -ai[c][c] / best;   // 1 / pivot
+        for (int j = 0; j < 12; j++) {
+            const double xr = ar[c][j], xi = ai[c][j];
+            ar[c][j] = xr * pr - xi * pi; ai[c][j] = xr * pi + xi * pr;
+        }
+        for (int r = 0; r < 6; r++) {
+            if (r == c) continue;
+            const double fr = ar[r][c], fi = ai[r][c];
+            for (int j = 0; j < 12; j++) {
+                ar[r][j] -= fr * ar[c][j] - fi * ai[c][j];
+                ai[r][j] -= fr * ai[c][j] + fi * ar[c][j];
+            }
+        }
+    }
+    float *q = inv + g * 36;
+    for (int i = 0; i < 6; i++) q[i] = (float)ar[i][6 + i];
+    for (int i = 1; i < 6; i++)
+        for (int j = 0; j < i; j++) {
+            const int idx = i * (i - 1) / 2 + j;   // Hermitian part of the computed inverse
+            q[6 + 2 * idx] = (float)(0.5 * (ar[i][6 + j] + ar[j][6 + i]));
+            q[6 + 2 * idx + 1] = (float)(0.5 * (ai[i][6 + j] - ai[j][6 + i]));
+        }
+}
+
 // ------------------------------------------------------------------ M_ooee apply
 // One thread = one site and R right-hand sides; the 72 packed floats of the site are fetched
 // once and reused by every RHS.  One chirality at a time keeps the live set at 6 + 6 elements.
@@ -217,6 +269,13 @@ mrhs_status_t build_clover(const int dims[4], float mass, float csw, const float
 mrhs_status_t pack_clover_blocks(long long nsites, const float2 *d_blocks, float *d_packed, cudaStream_t st) {
     long long n2 = nsites * 2, blocks = (n2 + 127) / 128;
     pack_blocks_kernel<<<(unsigned)blocks, 128, 0, st>>>(d_blocks, d_packed, n2);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+mrhs_status_t invert_clover_blocks(long long nsites, const float *d_packed, float *d_packed_inv, cudaStream_t st) {
+    long long n2 = nsites * 2, blocks = (n2 + 63) / 64;
+    invert_blocks_kernel<<<(unsigned)blocks, 64, 0, st>>>(d_packed, d_packed_inv, n2);
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
 }

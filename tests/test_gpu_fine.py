@@ -260,6 +260,44 @@ def test_fused_meooe_mooee_and_schur_sequence(dims, nrhs, seed):
     w.close()
 
 
+@pytest.mark.parametrize("dims,nrhs,seed", [([8, 4, 4, 6], 12, 70), ([4, 4, 4, 4], 3, 71), ([24, 2, 4, 2], 24, 72)])
+def test_inverse_clover_blocks(dims, nrhs, seed):
+    """M_ooee^-1 (inverse blocks built on the device at create) on full / even / odd fields, M_ooee^-1 M_ooee = 1,
+    and the fused M_ooee^-1 M_eooe with both hop kernels, against the oracle (inverse by numpy.linalg.inv)."""
+    mass, csw = -0.05, 1.5
+    U, psi = _fine_case(dims, nrhs, seed, mass, csw)
+    w = make_wilson(dims, nrhs, mass, csw, U)
+    C, _ = oracle.clover_blocks(dims, U, mass, csw)
+    Ci = oracle.clover_inverse(C)
+    Cip = oracle.cb_split(dims, Ci)
+    src = oracle.cb_split(dims, psi)
+
+    def apply_inv(field, parity):
+        d_in = w.import_field(dev(field), parity)
+        d_out = w.empty(parity)
+        w.mooee_inv(d_in, d_out, parity)
+        torch.cuda.synchronize()
+        return host(w.export_field(d_out, parity))
+
+    assert rel_l2_per_rhs(apply_inv(psi, mrhs.FULL), oracle.mooee(Ci, psi)).max() < TOL
+    for parity in (0, 1):
+        assert rel_l2_per_rhs(apply_inv(src[parity], parity), oracle.mooee(Cip[parity], src[parity])).max() < TOL
+    back = apply_inv(gpu_mooee(w, psi, mrhs.FULL), mrhs.FULL)
+    assert rel_l2_per_rhs(back, psi.astype(np.complex128)).max() < TOL
+    kernels = [mrhs.HOP_GATHER] + ([mrhs.HOP_SWEEP] if nrhs % 2 == 0 else [])
+    for kern in kernels:
+        mrhs.wilson_set_hop_kernel(w.h, 1, kern)
+        for out_parity in (0, 1):
+            want = oracle.mooee(Cip[out_parity], oracle.meooe(dims, U, src[1 - out_parity], out_parity))
+            d_in = w.import_field(dev(src[1 - out_parity]), 1 - out_parity)
+            d_out = w.empty(out_parity)
+            w.meooe_mooee_inv(d_in, d_out, out_parity)
+            torch.cuda.synchronize()
+            err = rel_l2_per_rhs(host(w.export_field(d_out, out_parity)), want)
+            assert err.max() < TOL, ("fused inverse", kern, out_parity, err)
+    w.close()
+
+
 @pytest.mark.parametrize("nrhs", [1, 12])
 def test_config2_24x24_full_field(nrhs):
     """Config 2 (24^4, mass -0.05, c_sw 1.5): full-field parity for D_hop, M_eooe and M_ooee."""

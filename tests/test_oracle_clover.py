@@ -131,3 +131,20 @@ def test_full_matrix_gamma5_hermiticity():
     lhs = np.vdot(chi, M(psi))
     rhs = np.vdot(g5 * M(g5 * chi), psi)
     assert abs(lhs - rhs) < 1e-10 * abs(lhs)
+
+
+def test_clover_inverse_blocks():
+    """Inverse blocks: C C^-1 = 1, Hermitian, and (4 + m)^-1 on a pure-gauge field (closed form)."""
+    dims, mass, csw = (4, 4, 2, 4), -0.1, 1.3
+    U = si.gauge_np(dims, 61)
+    C, _ = oracle.clover_blocks(dims, U, mass, csw)
+    Ci = oracle.clover_inverse(C)
+    eye = np.broadcast_to(np.eye(6), C.shape)
+    assert np.max(np.abs(np.matmul(C, Ci) - eye)) < 1e-12
+    assert np.max(np.abs(Ci - np.conj(np.swapaxes(Ci, 2, 3)))) < 1e-12
+    g = si.gauge_transform_np(dims, 63)
+    Upg = np.empty((si.volume(dims), 4, 3, 3), dtype=np.complex128)
+    for mu in range(4):
+        Upg[:, mu] = np.einsum("xab,xcb->xac", g, g[shift_index(dims, mu, +1)].conj())   # U_mu(x) = g(x) g(x+mu)^+
+    Cpg, _ = oracle.clover_blocks(dims, Upg, mass, csw)
+    assert np.max(np.abs(oracle.clover_inverse(Cpg) - eye / (4 + mass))) < 1e-12
