@@ -9,7 +9,8 @@
 // stencil points and the nb columns:
 //   D[128 x NT] += Aop[128 x nb] * Bop[nb x NT]
 //   Aop rows 0..nb-1      = Re A_p,   rows nb..2nb-1   = Im A_p            (rows 2nb..127: whatever follows in shared memory; their D lanes are never read)
-//   Bop cols 0..N-1       = Re v,     cols N..2N-1     = Im v              (NT = 2N rounded up to 16)
+//   Bop cols 0..N-1       = Re v,     cols N..2N-1     = Im v              (NT = 2N rounded up to 16; inside each half the
+//                                                                        even RHS come first, then the odd ones)
 // so D holds Re A Re v, Re A Im v, Im A Re v, Im A Im v and the epilogue forms
 //   Re out = D[i][n] - D[nb+i][N+n],   Im out = D[i][N+n] + D[nb+i][n].
 // Every matrix entry read from HBM serves all N_rhs columns (PAPER.md:23 (i)).
@@ -245,17 +246,17 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, co
                     float4 hi, lo;
                     const int base = kc * C::B_LBO;
                     split4(make_float4(x0.x, x1.x, x2.x, x3.x), hi, lo);        // Re, RHS 2q
-                    *reinterpret_cast<float4 *>(b_hi + base + (2 * q) * 16) = hi;
-                    *reinterpret_cast<float4 *>(b_lo + base + (2 * q) * 16) = lo;
+                    *reinterpret_cast<float4 *>(b_hi + base + (q) * 16) = hi;
+                    *reinterpret_cast<float4 *>(b_lo + base + (q) * 16) = lo;
                     split4(make_float4(x0.y, x1.y, x2.y, x3.y), hi, lo);        // Re, RHS 2q+1
-                    *reinterpret_cast<float4 *>(b_hi + base + (2 * q + 1) * 16) = hi;
-                    *reinterpret_cast<float4 *>(b_lo + base + (2 * q + 1) * 16) = lo;
+                    *reinterpret_cast<float4 *>(b_hi + base + (C::NP + q) * 16) = hi;
+                    *reinterpret_cast<float4 *>(b_lo + base + (C::NP + q) * 16) = lo;
                     split4(make_float4(x0.z, x1.z, x2.z, x3.z), hi, lo);        // Im, RHS 2q
-                    *reinterpret_cast<float4 *>(b_hi + base + (N + 2 * q) * 16) = hi;
-                    *reinterpret_cast<float4 *>(b_lo + base + (N + 2 * q) * 16) = lo;
+                    *reinterpret_cast<float4 *>(b_hi + base + (N + q) * 16) = hi;
+                    *reinterpret_cast<float4 *>(b_lo + base + (N + q) * 16) = lo;
                     split4(make_float4(x0.w, x1.w, x2.w, x3.w), hi, lo);        // Im, RHS 2q+1
-                    *reinterpret_cast<float4 *>(b_hi + base + (N + 2 * q + 1) * 16) = hi;
-                    *reinterpret_cast<float4 *>(b_lo + base + (N + 2 * q + 1) * 16) = lo;
+                    *reinterpret_cast<float4 *>(b_hi + base + (N + C::NP + q) * 16) = hi;
+                    *reinterpret_cast<float4 *>(b_lo + base + (N + C::NP + q) * 16) = lo;
                 }
             }
             fence_async_smem();
@@ -297,7 +298,7 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, co
         __syncthreads();
         for (int idx = tid; idx < NB * C::NP; idx += C::THREADS) {
             const int i = idx / C::NP, q = idx - i * C::NP;
-            const int n0 = 2 * q, n1 = 2 * q + 1;
+            const int n0 = q, n1 = C::NP + q;   // column order of D: Re even RHS | Re odd RHS | Im even | Im odd (conflict-free operand stores)
             float4 o;
             o.x = S[n0 * C::S_PITCH + i] - S[(N + n0) * C::S_PITCH + NB + i];
             o.y = S[n1 * C::S_PITCH + i] - S[(N + n1) * C::S_PITCH + NB + i];
