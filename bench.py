@@ -541,6 +541,10 @@ def run_sweep(args):
             m, mn = timeit(lambda: w.schur_sequence(ie, oo, t0, oe))
             emit(cfg, "schur_seq", dims, N, (2 * FLOPS_HOP + FLOPS_CLOVER) * V / 2 * N,
                  2 * bytes_meooe(V, N) + bytes_mooee(V / 2, N), m, mn, base)
+            # simultaneous inner products <psi_r, out_r> (NEXT-4): two fields read once, 8 flops per complex element
+            res = torch.empty(N, dtype=torch.complex128, device=device)
+            m, mn = timeit(lambda: mrhs.inner_products(dims, 12, N, mrhs.FULL, psi, o_full, res, stream=stream))
+            emit(cfg, "inner_products", dims, N, 8.0 * 12 * V * N, 2.0 * 96 * V * N, m, mn, base)
             w.close()
             del psi, o_full, ie, io, oe, oo, t0
         del U

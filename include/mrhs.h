@@ -219,6 +219,17 @@ mrhs_status_t mrhs_cb_split(const int dims[4], int ncomp, int nrhs, const void *
 mrhs_status_t mrhs_cb_merge(const int dims[4], int ncomp, int nrhs, const void *d_even,
                             const void *d_odd, void *d_full, void *cuda_stream);
 
+/* ------------------------------------------- block reductions over the RHS index */
+
+/* Simultaneous inner products:
+ *   result[r] = sum over sites and components of conj(x[..., r]) y[..., r],   r = 0 .. nrhs-1.
+ * d_x, d_y: two fields of the same geometry in NATIVE layout (fine: ncomp = 12, coarse: ncomp =
+ * nbasis; parity 0/1 checkerboarded, 2 full).  d_result: device, nrhs complex128 (re, im doubles),
+ * 16-byte aligned.  One pass over both fields, products and sums in fp64, fixed summation order
+ * (bit-reproducible).  Asynchronous on cuda_stream (scratch is allocated stream-ordered). */
+mrhs_status_t mrhs_inner_products(const int dims[4], int ncomp, int nrhs, int parity,
+                                  const void *d_x, const void *d_y, void *d_result, void *cuda_stream);
+
 /* ------------------------------------------- host-buffer (end-to-end) entries */
 
 /* One operator apply with HOST buffers in CANONICAL layout: host->device copy,

@@ -168,6 +168,18 @@ def clover_blocks(dims, U, mass, csw):
     return C, off.value
 
 
+def inner_products(x, y):
+    """Simultaneous inner products: result[r] = sum conj(x[..., r]) y[..., r]
+    over every index but the last (the RHS index), in fp64.  x, y: canonical fields [...][N]."""
+    x = _c128(x); y = _c128(y)
+    assert x.shape == y.shape
+    N = x.shape[-1]
+    out = np.zeros(N, dtype=np.complex128)
+    for r in range(N):
+        out[r] = np.sum(np.conj(x[..., r]) * y[..., r])
+    return out
+
+
 def clover_inverse(C):
     """Inverse clover blocks: the matrix inverse of every 6x6 block,
     by the library routine (numpy.linalg.inv, fp64).  C [n][2][6][6] -> same shape."""

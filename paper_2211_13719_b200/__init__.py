@@ -54,6 +54,7 @@ _SIGNATURES = {
     "mrhs_coarse_apply": (ctypes.c_int, [_vp, _vp, _vp]),
     "mrhs_coarse_apply_points": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_coarse_destroy": (ctypes.c_int, [_vp]),
+    "mrhs_inner_products": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
     "mrhs_xblock": (ctypes.c_int, [ctypes.c_int, ctypes.c_int]),
     "mrhs_field_bytes": (ctypes.c_size_t, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
     "mrhs_field_import": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]),
@@ -144,6 +145,15 @@ def field_import(dims, ncomp, nrhs, parity, canonical, native=None, stream=None)
         native = empty_field(dims, ncomp, nrhs, parity, canonical.device)
     _check(lib().mrhs_field_import(_dims(dims), ncomp, nrhs, parity, _ptr(canonical), _ptr(native), _stream_ptr(stream)))
     return native
+
+
+def inner_products(dims, ncomp, nrhs, parity, x, y, result=None, stream=None):
+    """result[r] = <x_r, y_r> for two native fields of the same geometry; complex128 device tensor [nrhs]."""
+    import torch
+    if result is None:
+        result = torch.empty(nrhs, dtype=torch.complex128, device=x.device)
+    _check(lib().mrhs_inner_products(_dims(dims), ncomp, nrhs, parity, _ptr(x), _ptr(y), _ptr(result), _stream_ptr(stream)))
+    return result
 
 
 def field_export(dims, ncomp, nrhs, parity, native, canonical=None, stream=None):

@@ -6,6 +6,7 @@
 
 #include "coarse.cuh"
 #include "fine_sweep.cuh"
+#include "blas.cuh"
 #include "fine_hop.cuh"
 
 namespace mrhs {
@@ -485,6 +486,28 @@ mrhs_status_t mrhs_coarse_apply_host(mrhs_coarse_t *h, const void *h_in, void *h
     if (s != MRHS_OK) return s;
     MRHS_CUDA(cudaMemcpyAsync(h_out, h->st_canon, bytes, cudaMemcpyDeviceToHost, h->st));
     MRHS_CUDA(cudaStreamSynchronize(h->st));
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_inner_products(const int dims[4], int ncomp, int nrhs, int parity, const void *d_x, const void *d_y,
+                                  void *d_result, void *cuda_stream) {
+    MRHS_REQUIRE(dims && d_x && d_y && d_result, "inner products: NULL argument");
+    MRHS_REQUIRE(parity >= 0 && parity <= 2, "inner products: parity must be 0, 1 or 2");
+    MRHS_REQUIRE(nrhs >= 1 && nrhs <= 256, "inner products: nrhs must be 1..256");
+    MRHS_REQUIRE(aligned16(d_x) && aligned16(d_y) && aligned16(d_result), "inner products: buffers must be 16-byte aligned");
+    const size_t bytes = mrhs_field_bytes(dims, ncomp, nrhs, parity != MRHS_FULL);
+    MRHS_REQUIRE(bytes > 0, "inner products: invalid lattice (extents >= 2, even for checkerboarded fields)");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    MRHS_CUDA(cudaGetDevice(&dev));
+    MRHS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int grid = inner_grid(sms);
+    double2 *partial = nullptr;
+    MRHS_CUDA(cudaMallocAsync(&partial, (size_t)grid * nrhs * sizeof(double2), st));
+    mrhs_status_t s = launch_inner_products((long long)(bytes / 4), nrhs, d_x, d_y, partial, grid, (double2 *)d_result, st);
+    cudaError_t e = cudaFreeAsync(partial, st);
+    if (s != MRHS_OK) return s;
+    MRHS_CUDA(e);
     return MRHS_OK;
 }
 

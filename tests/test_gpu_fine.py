@@ -298,6 +298,26 @@ def test_inverse_clover_blocks(dims, nrhs, seed):
     w.close()
 
 
+@pytest.mark.parametrize("dims,ncomp,nrhs,parity", [([8, 4, 6, 4], 12, 12, mrhs.FULL), ([8, 4, 6, 4], 12, 12, mrhs.ODD),
+                                                    ([4, 4, 4, 4], 12, 3, mrhs.FULL), ([16, 2, 4, 6], 12, 48, mrhs.EVEN),
+                                                    ([3, 5, 2, 7], 40, 24, mrhs.FULL), ([2, 2, 2, 2], 24, 1, mrhs.FULL)])
+def test_inner_products_match_oracle(dims, ncomp, nrhs, parity):
+    """<x_r, y_r> for all RHS at once on native fields (fine full / checkerboarded, coarse), fp64 sums, reproducible."""
+    V = syn.volume(dims) // (1 if parity == mrhs.FULL else 2)
+    shape = (ncomp,) if ncomp != 12 else (4, 3)
+    rng = np.random.default_rng([91, nrhs])
+    x = (rng.standard_normal((V,) + shape + (nrhs,)) + 1j * rng.standard_normal((V,) + shape + (nrhs,))).astype(np.complex64)
+    y = (rng.standard_normal((V,) + shape + (nrhs,)) + 1j * rng.standard_normal((V,) + shape + (nrhs,))).astype(np.complex64)
+    dx = mrhs.field_import(dims, ncomp, nrhs, parity, dev(x))
+    dy = mrhs.field_import(dims, ncomp, nrhs, parity, dev(y))
+    got = host(mrhs.inner_products(dims, ncomp, nrhs, parity, dx, dy))
+    want = oracle.inner_products(x, y)
+    assert np.max(np.abs(got - want) / np.abs(want)) < 1e-10, (got, want)
+    assert np.array_equal(host(mrhs.inner_products(dims, ncomp, nrhs, parity, dx, dy)), got)
+    nrm = host(mrhs.inner_products(dims, ncomp, nrhs, parity, dx, dx))
+    assert np.max(np.abs(nrm.imag)) == 0.0 and np.all(nrm.real > 0)
+
+
 @pytest.mark.parametrize("nrhs", [1, 12])
 def test_config2_24x24_full_field(nrhs):
     """Config 2 (24^4, mass -0.05, c_sw 1.5): full-field parity for D_hop, M_eooe and M_ooee."""
