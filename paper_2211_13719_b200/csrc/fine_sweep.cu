@@ -342,12 +342,12 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
                             if (j < i) v = cfma(a[6 + 2 * (i * (i - 1) / 2 + j)], a[6 + 2 * (i * (i - 1) / 2 + j) + 1], acc[6 * ch + j], v);
                             else if (j > i) v = cfma_conj(a[6 + 2 * (j * (j - 1) / 2 + i)], a[6 + 2 * (j * (j - 1) / 2 + i) + 1], acc[6 * ch + j], v);
                         }
-                        o[(size_t)(6 * ch + i) * cs] = from_cvec(v);
+                        __stcs(&o[(size_t)(6 * ch + i) * cs], from_cvec(v));
                     }
                 }
             } else {
 #pragma unroll
-                for (int c = 0; c < 12; c++) o[(size_t)c * cs] = from_cvec(acc[c]);
+                for (int c = 0; c < 12; c++) __stcs(&o[(size_t)c * cs], from_cvec(acc[c]));
             }
         } else {
             bar_arrive(&freeI[b]);
