@@ -541,6 +541,9 @@ def run_sweep(args):
             m, mn = timeit(lambda: w.schur_sequence(ie, oo, t0, oe))
             emit(cfg, "schur_seq", dims, N, (2 * FLOPS_HOP + FLOPS_CLOVER) * V / 2 * N,
                  2 * bytes_meooe(V, N) + bytes_mooee(V / 2, N), m, mn, base)
+            # the full Wilson-clover matrix M = M_ooee - D_hop / 2 in one fused launch (NEXT-2): gauge + clover + one field in, one out
+            m, mn = timeit(lambda: w.apply(psi, o_full))
+            emit(cfg, "wilson_M", dims, N, (FLOPS_HOP + FLOPS_CLOVER + 48) * V * N, V * (576.0 + 192.0 * N), m, mn, base)
             # simultaneous inner products <psi_r, out_r> (NEXT-4): two fields read once, 8 flops per complex element
             res = torch.empty(N, dtype=torch.complex128, device=device)
             m, mn = timeit(lambda: mrhs.inner_products(dims, 12, N, mrhs.FULL, psi, o_full, res, stream=stream))

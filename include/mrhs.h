@@ -113,6 +113,13 @@ mrhs_status_t mrhs_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int pa
  * user-supplied block gives non-finite entries in its inverse (not checked). */
 mrhs_status_t mrhs_mooee_inv(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity);
 
+/* The full Wilson-clover matrix on full-lattice fields (reading S6):
+ *   out = M in = M_ooee in - (1/2) D_hop in.
+ * With the sweep kernel ONE launch (the clover term of in(x) is formed from the slice in shared
+ * memory and the eight hops are added to it: no intermediate field, no separate axpy); with the
+ * gather kernel two launches (D_hop, then out = C in - out / 2). */
+mrhs_status_t mrhs_wilson_apply(mrhs_wilson_t *h, const void *d_in, void *d_out);
+
 /* Fused out = M_ooee(out_parity) M_eooe(in): the hopping term onto parity out_parity followed by
  * the clover term of those sites (the first two steps of the Schur
  * sequence below).  With the sweep kernel (even N_rhs) this is ONE

@@ -38,6 +38,7 @@ _SIGNATURES = {
     "mrhs_meooe": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_mooee": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_schur_sequence": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "mrhs_wilson_apply": (ctypes.c_int, [_vp, _vp, _vp]),
     "mrhs_meooe_mooee": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_meooe_mooee_inv": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_mooee_inv": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
@@ -197,6 +198,10 @@ def mooee(h, d_in, d_out, parity):
     _check(lib().mrhs_mooee(h, _ptr(d_in), _ptr(d_out), int(parity)))
 
 
+def wilson_apply(h, d_in, d_out):
+    _check(lib().mrhs_wilson_apply(h, _ptr(d_in), _ptr(d_out)))
+
+
 def meooe_mooee(h, d_in, d_out, out_parity):
     _check(lib().mrhs_meooe_mooee(h, _ptr(d_in), _ptr(d_out), int(out_parity)))
 
@@ -324,6 +329,10 @@ class Wilson:
 
     def mooee(self, d_in, d_out, parity):
         mooee(self.h, d_in, d_out, parity)
+
+    def apply(self, d_in, d_out):
+        """out = M in, the full Wilson-clover matrix on full-lattice fields."""
+        wilson_apply(self.h, d_in, d_out)
 
     def meooe_mooee(self, d_in, d_out, out_parity):
         meooe_mooee(self.h, d_in, d_out, out_parity)

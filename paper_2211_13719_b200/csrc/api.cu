@@ -215,6 +215,21 @@ mrhs_status_t mrhs_meooe(mrhs_wilson_t *h, const void *d_in, void *d_out, int ou
     return launch_hop(h->hp_cb[out_parity], h->nrhs, d_in, d_out, h->st);
 }
 
+mrhs_status_t mrhs_wilson_apply(mrhs_wilson_t *h, const void *d_in, void *d_out) {
+    MRHS_REQUIRE(h && d_in && d_out, "wilson apply: NULL argument");
+    MRHS_REQUIRE(d_in != d_out, "wilson apply: in and out must not alias");
+    MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "wilson apply: buffers must be 16-byte aligned");
+    if (h->kern[0] == MRHS_HOP_SWEEP) {
+        // one launch: C in(x) is formed from the centre slice in shared memory, the eight hops add to it
+        SweepParams p = h->sp_full;
+        p.clover = h->clov_full;
+        return launch_sweep(p, d_in, d_out, h->st);
+    }
+    mrhs_status_t s = launch_hop(h->hp_full, h->nrhs, d_in, d_out, h->st);
+    if (s == MRHS_OK) s = launch_mooee(h->gfull, h->clov_full, d_in, d_out, h->st, true);
+    return s;
+}
+
 static mrhs_status_t mooee_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity, bool inverse);
 mrhs_status_t mrhs_mooee(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity) { return mooee_impl(h, d_in, d_out, parity, false); }
 mrhs_status_t mrhs_mooee_inv(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity) { return mooee_impl(h, d_in, d_out, parity, true); }

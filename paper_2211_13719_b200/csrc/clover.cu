@@ -212,7 +212,8 @@ __global__ void invert_blocks_kernel(const float *__restrict__ packed, float *__
 // ------------------------------------------------------------------ M_ooee apply
 // One thread = one site and R right-hand sides; the 72 packed floats of the site are fetched
 // once and reused by every RHS.  One chirality at a time keeps the live set at 6 + 6 elements.
-template <int R>
+// AXPY: out = C in - out / 2 (out holds the hopping sum: the full Wilson-clover matrix of reading S6, gather-kernel path)
+template <int R, bool AXPY>
 __global__ void __launch_bounds__(256)
 mooee_kernel(int XB, int NP, long long nthreads, const float4 *__restrict__ clov,
              const typename Elem<R>::type *__restrict__ in, typename Elem<R>::type *__restrict__ out) {
@@ -250,6 +251,7 @@ mooee_kernel(int XB, int NP, long long nthreads, const float4 *__restrict__ clov
                     r = cfma_conj(a[6 + 2 * idx], a[6 + 2 * idx + 1], psi[j], r);
                 }
             }
+            if constexpr (AXPY) r = rfma(-0.5f, to_cvec(po[(size_t)(6 * ch + i) * CS]), r);
             po[(size_t)(6 * ch + i) * CS] = from_cvec(r);
         }
     }
@@ -287,14 +289,17 @@ mrhs_status_t unpack_clover_blocks(long long nsites, const float *d_packed, floa
     return MRHS_OK;
 }
 
-mrhs_status_t launch_mooee(const FieldGeom &g, const float4 *d_clover, const void *d_in, void *d_out, cudaStream_t st) {
+mrhs_status_t launch_mooee(const FieldGeom &g, const float4 *d_clover, const void *d_in, void *d_out, cudaStream_t st, bool axpy) {
     const int np = threads_per_site(g.N);
     const long long nthreads = g.nsites * np;
     const long long blocks = (nthreads + 255) / 256;
-    if (g.N & 1)
-        mooee_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(g.XB, np, nthreads, d_clover, (const float2 *)d_in, (float2 *)d_out);
-    else
-        mooee_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(g.XB, np, nthreads, d_clover, (const float4 *)d_in, (float4 *)d_out);
+    if (g.N & 1) {
+        if (axpy) mooee_kernel<1, true><<<(unsigned)blocks, 256, 0, st>>>(g.XB, np, nthreads, d_clover, (const float2 *)d_in, (float2 *)d_out);
+        else      mooee_kernel<1, false><<<(unsigned)blocks, 256, 0, st>>>(g.XB, np, nthreads, d_clover, (const float2 *)d_in, (float2 *)d_out);
+    } else {
+        if (axpy) mooee_kernel<2, true><<<(unsigned)blocks, 256, 0, st>>>(g.XB, np, nthreads, d_clover, (const float4 *)d_in, (float4 *)d_out);
+        else      mooee_kernel<2, false><<<(unsigned)blocks, 256, 0, st>>>(g.XB, np, nthreads, d_clover, (const float4 *)d_in, (float4 *)d_out);
+    }
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
 }

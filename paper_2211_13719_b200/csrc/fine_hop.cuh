@@ -55,6 +55,7 @@ mrhs_status_t pack_clover_blocks(long long nsites, const float2 *d_blocks, float
 // packed blocks [lex][72] -> packed inverse blocks (fp64 Gauss-Jordan per 6x6 block)
 mrhs_status_t invert_clover_blocks(long long nsites, const float *d_packed, float *d_packed_inv, cudaStream_t st);
 mrhs_status_t unpack_clover_blocks(long long nsites, const float *d_packed, float2 *d_blocks, cudaStream_t st);
-mrhs_status_t launch_mooee(const FieldGeom &g, const float4 *d_clover, const void *d_in, void *d_out, cudaStream_t st);
+// axpy: out = C in - out / 2 instead of out = C in
+mrhs_status_t launch_mooee(const FieldGeom &g, const float4 *d_clover, const void *d_in, void *d_out, cudaStream_t st, bool axpy = false);
 
 }  // namespace mrhs

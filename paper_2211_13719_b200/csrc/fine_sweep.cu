@@ -98,9 +98,36 @@ struct Nbr {
     int o, bs, cs;
 };
 
-// CLOV: the clover term of the output parity is applied to the result before it is stored, out = M_ooee M_eooe in
-// (the first two steps of the Schur sequence, without the round trip through HBM)
-template <int XB_, int NP_, bool CB, bool CLOV>
+// out = C in for the two packed Hermitian 6x6 blocks of one site (6 real diagonals + 15 complex lower-triangle entries
+// each, reading S7); pc: float4 0 of the site's 72 packed floats (stride XB), broadcast reads from shared memory
+__device__ __forceinline__ void clover_mul(const float4 *pc, int XB, const CVec<2> (&in)[12], CVec<2> (&out)[12]) {
+#pragma unroll
+    for (int ch = 0; ch < 2; ch++) {
+        float a[36];
+#pragma unroll
+        for (int j = 0; j < 9; j++) {
+            const float4 v = pc[(9 * ch + j) * XB];
+            a[4 * j] = v.x; a[4 * j + 1] = v.y; a[4 * j + 2] = v.z; a[4 * j + 3] = v.w;
+        }
+#pragma unroll
+        for (int i = 0; i < 6; i++) {
+            CVec<2> v = rmul(a[i], in[6 * ch + i]);
+#pragma unroll
+            for (int j = 0; j < 6; j++) {
+                if (j < i) v = cfma(a[6 + 2 * (i * (i - 1) / 2 + j)], a[6 + 2 * (i * (i - 1) / 2 + j) + 1], in[6 * ch + j], v);
+                else if (j > i) v = cfma_conj(a[6 + 2 * (j * (j - 1) / 2 + i)], a[6 + 2 * (j * (j - 1) / 2 + i) + 1], in[6 * ch + j], v);
+            }
+            out[6 * ch + i] = v;
+        }
+    }
+}
+
+// EPI, what happens to the hopping sum H before it is stored (the clover blocks of the output sites come in with the links):
+//   0: out = H                                  D_hop, M_eooe
+//   1: out = C H                                 M_ooee M_eooe, the first two steps of the Schur sequence (row a7), checkerboarded
+//   2: out = C in - H / 2                        the full Wilson-clover matrix M (reading S6), full lattice: the centre
+//                                                slice holds in(x) itself, so C in(x) is formed first and the hops add to it
+template <int XB_, int NP_, bool CB, int EPI>
 __global__ void __launch_bounds__(224, 1)
 hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__restrict__ out) {
     const int XB = XB_ ? XB_ : p.XB;
@@ -111,6 +138,8 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + L.off_bar);
     uint64_t *fullI = bars, *freeI = bars + 2, *freeG = bars + 4, *fullG = bars + 6;
 
+    constexpr bool CLOV = EPI != 0;
+    static_assert(EPI == 0 || (EPI == 1 && CB) || (EPI == 2 && !CB), "fused epilogues: C H on checkerboarded fields, C in - H/2 on the full lattice");
     const int tid = threadIdx.x;
     const int NC = ROWS * cs, NCpad = (NC + 31) & ~31;
     const int Y = p.Y, Z = p.Z, T = p.T, nxb = p.nxb, lt = p.lt;
@@ -278,8 +307,19 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
         bar_wait(&fullI[b], ((uint32_t)(k + 1) >> 1) & 1u);
         bar_wait(&fullG[b], ((uint32_t)(k + 1) >> 1) & 1u);   // links of slice k, on their own barrier: the +t hop below waits for rows only
         const float4 *G = S + b * G4;
+        const float4 *pc = S + L.off_C / 16 + b * (L.C_BYTES / 16) + r * (18 * XB) + xin;   // this site's clover blocks
         if (k >= 0) {
-            zero_acc(acc);
+            if constexpr (EPI == 2) {
+                // acc = -2 C in(x): the hops below add H, and the store scales by -1/2
+                CVec<2> own_psi[12], cpsi[12];
+#pragma unroll
+                for (int c = 0; c < 12; c++) own_psi[c] = to_cvec(S[own.o + b * own.bs + c * own.cs]);
+                clover_mul(pc, XB, own_psi, cpsi);
+#pragma unroll
+                for (int c = 0; c < 12; c++) acc[c] = rmul(-2.f, cpsi[c]);
+            } else {
+                zero_acc(acc);
+            }
             hop_recon<2, 3, false>(carry, acc);
         }
         if (k + 1 < lt) {
@@ -322,29 +362,14 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
             hop_load_s<3>(A, S + own.o + (b ^ 1u) * own.bs, own.cs, G + g_own, XB);
             hop_compute<2, 3, true >(A, acc);
             float4 *o = out + (blk(xb, y, z, t) * 12 * XB + xin) * NP + pair;
-            if constexpr (CLOV) {
-                // out = M_ooee acc: two 6x6 Hermitian blocks (6 real diagonals + 15 complex lower-triangle entries each,
-                // reading S7), one chirality at a time; the 72 packed floats of the site are broadcast reads
-                const float4 *pc = S + L.off_C / 16 + b * (L.C_BYTES / 16) + r * (18 * XB) + xin;
+            if constexpr (EPI == 1) {
+                CVec<2> res[12];
+                clover_mul(pc, XB, acc, res);
 #pragma unroll
-                for (int ch = 0; ch < 2; ch++) {
-                    float a[36];
+                for (int c = 0; c < 12; c++) __stcs(&o[(size_t)c * cs], from_cvec(res[c]));
+            } else if constexpr (EPI == 2) {
 #pragma unroll
-                    for (int j = 0; j < 9; j++) {
-                        const float4 v = pc[(9 * ch + j) * XB];
-                        a[4 * j] = v.x; a[4 * j + 1] = v.y; a[4 * j + 2] = v.z; a[4 * j + 3] = v.w;
-                    }
-#pragma unroll
-                    for (int i = 0; i < 6; i++) {
-                        CVec<2> v = rmul(a[i], acc[6 * ch + i]);
-#pragma unroll
-                        for (int j = 0; j < 6; j++) {
-                            if (j < i) v = cfma(a[6 + 2 * (i * (i - 1) / 2 + j)], a[6 + 2 * (i * (i - 1) / 2 + j) + 1], acc[6 * ch + j], v);
-                            else if (j > i) v = cfma_conj(a[6 + 2 * (j * (j - 1) / 2 + i)], a[6 + 2 * (j * (j - 1) / 2 + i) + 1], acc[6 * ch + j], v);
-                        }
-                        __stcs(&o[(size_t)(6 * ch + i) * cs], from_cvec(v));
-                    }
-                }
+                for (int c = 0; c < 12; c++) __stcs(&o[(size_t)c * cs], from_cvec(rmul(-0.5f, acc[c])));
             } else {
 #pragma unroll
                 for (int c = 0; c < 12; c++) __stcs(&o[(size_t)c * cs], from_cvec(acc[c]));
@@ -439,9 +464,10 @@ bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t
 mrhs_status_t sweep_prepare() {
     const int max_smem = 227 * 1024;
 #define MRHS_CASE(XB, NP)                                                                                                     \
-    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem)); \
-    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));  \
-    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem)); \
+    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));  \
+    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));  \
+    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
     MRHS_SWEEP_LIST(MRHS_CASE)
 #undef MRHS_CASE
     return MRHS_OK;
@@ -450,9 +476,10 @@ mrhs_status_t sweep_prepare() {
 namespace {
 template <int XB, int NP>
 void launch_sweep_t(const SweepParams &p, const void *d_in, void *d_out, cudaStream_t st) {
-    if (p.cb && p.clover) hop_sweep_kernel<XB, NP, true, true><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
-    else if (p.cb)        hop_sweep_kernel<XB, NP, true, false><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
-    else                  hop_sweep_kernel<XB, NP, false, false><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    if (p.cb && p.clover) hop_sweep_kernel<XB, NP, true, 1><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    else if (p.cb)        hop_sweep_kernel<XB, NP, true, 0><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    else if (p.clover)    hop_sweep_kernel<XB, NP, false, 2><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    else                  hop_sweep_kernel<XB, NP, false, 0><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
 }
 }  // namespace
 

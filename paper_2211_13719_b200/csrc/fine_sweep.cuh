@@ -27,7 +27,7 @@ struct SweepParams {
     FastDiv d_nxb, d_cy, d_cz, d_ntseg, d_ncy;   // block index -> (x-block, tile in chunk, segment, chunk)
     const float4 *gauge_out;      // links on the sites of the output field, [block][18][xin] float4
     const float4 *gauge_in;       // links on the sites of the input field
-    const float4 *clover;         // packed clover blocks on the sites of the output field: non-null => out = M_ooee M_eooe in
+    const float4 *clover;         // packed clover blocks on the sites of the output field: non-null => out = C H (checkerboarded) or C in - H/2 (full lattice)
     unsigned grid, threads, consumers;
     unsigned smem_bytes;
 };

@@ -318,6 +318,26 @@ def test_inner_products_match_oracle(dims, ncomp, nrhs, parity):
     assert np.max(np.abs(nrm.imag)) == 0.0 and np.all(nrm.real > 0)
 
 
+@pytest.mark.parametrize("dims,nrhs,seed", [([8, 4, 4, 6], 12, 75), ([4, 4, 4, 4], 3, 76), ([16, 2, 4, 4], 24, 77), ([2, 2, 2, 2], 4, 78)])
+def test_full_wilson_clover_matrix(dims, nrhs, seed):
+    """out = M in = M_ooee in - D_hop in / 2 (reading S6): one fused launch with the sweep kernel, two with the gather kernel."""
+    from oracle import galerkin
+    mass, csw = -0.05, 1.5
+    U, psi = _fine_case(dims, nrhs, seed, mass, csw)
+    w = make_wilson(dims, nrhs, mass, csw, U)
+    want = galerkin.wilson_clover_apply(dims, U.astype(np.complex128), mass, csw, psi.astype(np.complex128))
+    kernels = [mrhs.HOP_GATHER] + ([mrhs.HOP_SWEEP] if nrhs % 2 == 0 else [])
+    for kern in kernels:
+        mrhs.wilson_set_hop_kernel(w.h, 0, kern)
+        d_in = w.import_field(dev(psi), mrhs.FULL)
+        d_out = w.empty(mrhs.FULL)
+        w.apply(d_in, d_out)
+        torch.cuda.synchronize()
+        err = rel_l2_per_rhs(host(w.export_field(d_out, mrhs.FULL)), want)
+        assert err.max() < TOL, (kern, err)
+    w.close()
+
+
 @pytest.mark.parametrize("nrhs", [1, 12])
 def test_config2_24x24_full_field(nrhs):
     """Config 2 (24^4, mass -0.05, c_sw 1.5): full-field parity for D_hop, M_eooe and M_ooee."""
