@@ -154,7 +154,10 @@ mrhs_status_t mrhs_wilson_set_tiling(mrhs_wilson_t *h, int which, const int tile
 mrhs_status_t mrhs_wilson_get_tiling(mrhs_wilson_t *h, int which, int tile[3], int chunk[2]);
 /* L2 prefetch distance of the hopping kernel, in thread-block tiles of its sweep order: a tile
  * asks the copy engine to bring the rows of the tile distance_tiles later into L2 (0 = off).
- * set_tiling resets it to the default (296 tiles: half of the tiles resident on 148 SMs at four per SM). */
+ * set_tiling resets it to the default (296 tiles: half of the tiles resident on 148 SMs at four per SM).
+ * While the sweep kernel is selected for `which`, the call sets ITS prefetch distance instead, in t-slices
+ * (default 2; set_sweep resets it).  The environment variable MRHS_DEBUG=1 makes create calls print
+ * their launch geometry to stderr; nothing else in the library reads the environment. */
 mrhs_status_t mrhs_wilson_set_prefetch(mrhs_wilson_t *h, int which, int distance_tiles);
 
 

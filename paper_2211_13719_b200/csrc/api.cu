@@ -318,7 +318,11 @@ mrhs_status_t mrhs_wilson_set_prefetch(mrhs_wilson_t *h, int which, int distance
     MRHS_REQUIRE(h, "set prefetch: NULL handle");
     MRHS_REQUIRE(which == 0 || which == 1, "set prefetch: which must be 0 (D_hop) or 1 (M_eooe)");
     MRHS_REQUIRE(distance_tiles >= 0, "set prefetch: distance must be >= 0 (0 = off)");
-    if (which == 0) h->hp_full.pf_dist = (unsigned)distance_tiles;
+    if (h->kern[which] == MRHS_HOP_SWEEP) {
+        // sweep kernel: the producer warp asks for the tile rows this many t-slices ahead
+        if (which == 0) h->sp_full.pf = distance_tiles;
+        else h->sp_cb[0].pf = h->sp_cb[1].pf = distance_tiles;
+    } else if (which == 0) h->hp_full.pf_dist = (unsigned)distance_tiles;
     else h->hp_cb[0].pf_dist = h->hp_cb[1].pf_dist = (unsigned)distance_tiles;
     return MRHS_OK;
 }

@@ -160,7 +160,7 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, co
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
-    // one-time setup: barrier, zeroed operand area (pad rows / columns), TMEM accumulator
+    // one-time setup: barrier, zeroed operand area (so that the unused MMA rows / columns never see NaN patterns), TMEM accumulator
     if (tid == 0) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");

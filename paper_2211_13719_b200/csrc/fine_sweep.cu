@@ -18,7 +18,6 @@
 // One thread still owns one output site and one RHS pair (FFMA2 lanes); links are broadcast reads.
 #include "fine_sweep.cuh"
 #include "hop_math.cuh"
-#include <cstdlib>
 
 namespace mrhs {
 
@@ -451,7 +450,6 @@ bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t
     p.gauge_out = p.gauge_in = nullptr;
     p.clover = nullptr;
     p.pf = 2;
-    if (const char *e = getenv("MRHS_SWEEP_PF")) p.pf = atoi(e);
     p.consumers = (unsigned)(ROWS * g.XB * np);
     p.threads = ((p.consumers + 31u) & ~31u) + 32u;
     p.grid = (unsigned)grid;
