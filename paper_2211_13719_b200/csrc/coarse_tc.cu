@@ -178,8 +178,8 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, co
     // the previous stage has been handed to the tensor core, so the load latency overlaps its MMAs and the next wait
     float4 ra[A_IT];
     float4 rb[B_IT][4];
-    auto load_stage = [&](long long site, int p) {
-        // neighbour of stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
+    // neighbour of stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
+    auto neighbour = [&](long long site, int p) -> long long {
         long long nbr = site;
         if (p > 0) {
             long long s = site;
@@ -194,8 +194,17 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, co
             else c3 = (c3 + d + T) % T;
             nbr = c0 + (long long)X * (c1 + (long long)Y * (c2 + (long long)Z * c3));
         }
+        return nbr;
+    };
+    // one thread asks the copy engine to bring a later stage's matrix and neighbour vector into L2 (each is one
+    // contiguous block), so that the register loads of that stage find them there
+    auto prefetch_stage = [&](long long site, int p) {
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(links + ((size_t)site * 9 + p) * C::A_UNITS), "r"(C::A_UNITS * 16) : "memory");
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(in + (size_t)neighbour(site, p) * NB * C::NP), "r"(NB * C::NP * 16) : "memory");
+    };
+    auto load_stage = [&](long long site, int p) {
         const float4 *lp = links + ((size_t)site * 9 + p) * C::A_UNITS;
-        const float4 *vp = in + (size_t)nbr * NB * C::NP;
+        const float4 *vp = in + (size_t)neighbour(site, p) * NB * C::NP;
 #pragma unroll
         for (int it = 0; it < A_IT; it++) {
             const int u = tid + it * C::THREADS;
@@ -214,6 +223,7 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, co
     // For wide operands (two blocks per SM) the load runs one stage ahead; for narrow ones the extra live registers
     // would cost resident blocks, which hide the latency better, so the load sits at the top of its own stage.
     constexpr bool AHEAD = C::NT > 96;
+    constexpr int kPfAhead = AHEAD ? 3 : 2;
     // the stencil points of this apply: bit p of mask; stage s of a site handles the s-th set bit
     const int npts = ALL ? 9 : __popc(mask);
     auto point = [&](int s) { return ALL ? s : (int)__fns(mask, 0, s + 1); };
@@ -275,6 +285,11 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, co
                     mma_tf32(tmem, dah, dbh, idesc, 1);
                 }
                 mma_commit(bar);
+                // L2 prefetch kPfAhead stages ahead (possibly into the next site of this block)
+                int sp2 = sp + kPfAhead;
+                long long site2 = site;
+                while (sp2 >= npts) { sp2 -= npts; site2 += gridDim.x; }
+                if (site2 < nsites) prefetch_stage(site2, point(sp2));
             }
             nstage++;
             if (AHEAD) {
