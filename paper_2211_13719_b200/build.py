@@ -45,7 +45,7 @@ def build(force=False, verbose=False):
         if verbose:
             sys.stdout.write(out)
         objs.append(obj)
-    subprocess.run(["nvcc", "-shared", "-o", LIB] + objs + ["-lcudart"], check=True)
+    subprocess.run(["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs + ["-lcudart"], check=True)
     return LIB
 
 
