@@ -548,6 +548,22 @@ def run_sweep(args):
             res = torch.empty(N, dtype=torch.complex128, device=device)
             m, mn = timeit(lambda: mrhs.inner_products(dims, 12, N, mrhs.FULL, psi, o_full, res, stream=stream))
             emit(cfg, "inner_products", dims, N, 8.0 * 12 * V * N, 2.0 * 96 * V * N, m, mn, base)
+            # intergrid operators (NEXT-3): 4^4 aggregates, 20 basis vectors (nbasis 40); basis 1920 B per site
+            if N in (12, 24) and cfg == "config5":
+                nvec, bd = 20, [4, 4, 4, 4]
+                cd = [d // b for d, b in zip(dims, bd)]
+                basis = syn.spinor_torch(V * nvec, 1, seed + 1, device).reshape(nvec, V, 4, 3)
+                tr = mrhs.Transfer(dims, bd, nvec, N, basis, stream=stream)
+                del basis
+                vc = mrhs.empty_field(cd, 2 * nvec, N, mrhs.FULL, device)
+                vc.normal_()
+                fl, by = 8.0 * 12 * nvec * V * N, V * (96.0 * nvec + 96.0 * N) + vol(cd) * 16.0 * nvec * N
+                m, mn = timeit(lambda: tr.prolong(vc, o_full))
+                emit(cfg, "prolong", dims, N, fl, by, m, mn, base, {"nvec": nvec, "block": bd})
+                m, mn = timeit(lambda: tr.restrict(psi, vc))
+                emit(cfg, "restrict", dims, N, fl, by, m, mn, base, {"nvec": nvec, "block": bd})
+                tr.close()
+                del vc
             w.close()
             del psi, o_full, ie, io, oe, oo, t0
         del U

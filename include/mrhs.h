@@ -59,7 +59,8 @@ extern "C" {
 #endif
 
 typedef struct mrhs_wilson mrhs_wilson_t;   /* opaque: owns packed gauge + clover  */
-typedef struct mrhs_coarse mrhs_coarse_t;   /* opaque: owns packed coarse links    */
+typedef struct mrhs_coarse mrhs_coarse_t;
+typedef struct mrhs_transfer mrhs_transfer_t;   /* opaque, owns the repacked multigrid basis vectors */   /* opaque: owns packed coarse links    */
 
 typedef enum {
     MRHS_OK = 0,
@@ -228,6 +229,25 @@ mrhs_status_t mrhs_cb_split(const int dims[4], int ncomp, int nrhs, const void *
                             void *d_even, void *d_odd, void *cuda_stream);
 mrhs_status_t mrhs_cb_merge(const int dims[4], int ncomp, int nrhs, const void *d_even,
                             const void *d_odd, void *d_full, void *cuda_stream);
+
+/* ------------------------------------------- intergrid operators (projection / promotion) */
+
+/* MRHS prolongation and restriction between the fine level and its first coarse level (SURVEY.md
+ * Sec. 8(f) NEXT-3; reading S9).  n_vec basis vectors phi_k, nbasis = 2 n_vec, chirality
+ * chi = 0 for spins {0,1}, 1 for spins {2,3}, coarse index j = chi n_vec + k, blocks of bdims fine sites:
+ *   prolong:   fine(x)[s][c][r]  = sum_k phi_k(x)[s][c] coarse(B(x))[chi(s) n_vec + k][r]
+ *   restrict:  coarse(B)[chi n_vec + k][r] = sum_{x in B, s in chi, c} conj(phi_k(x)[s][c]) fine(x)[s][c][r]
+ * (restrict is the adjoint of prolong; the basis is used as given, orthonormalising it is the setup's job).
+ * create: dims fine extents, bdims block extents (each divides the fine extent, coarse extent >= 2);
+ *   d_basis: device, canonical [n_vec][site][4][3] complex64, copied and repacked (caller may free it).
+ * prolong: d_coarse_in native coarse vector (ncomp = 2 n_vec) of the coarse lattice dims / bdims,
+ *   d_fine_out native full-lattice fine field; restrict the other way.  Asynchronous on the stream.
+ * UNSUPPORTED: aggregates whose index table does not fit 48 KB of shared memory (> ~2000 sites). */
+mrhs_status_t mrhs_transfer_create(mrhs_transfer_t **out, const int dims[4], const int bdims[4], int nvec,
+                                   int nrhs, const void *d_basis, void *cuda_stream);
+mrhs_status_t mrhs_prolong(mrhs_transfer_t *h, const void *d_coarse_in, void *d_fine_out);
+mrhs_status_t mrhs_restrict(mrhs_transfer_t *h, const void *d_fine_in, void *d_coarse_out);
+mrhs_status_t mrhs_transfer_destroy(mrhs_transfer_t *h);
 
 /* ------------------------------------------- block reductions over the RHS index */
 

@@ -55,6 +55,10 @@ _SIGNATURES = {
     "mrhs_coarse_apply": (ctypes.c_int, [_vp, _vp, _vp]),
     "mrhs_coarse_apply_points": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_coarse_destroy": (ctypes.c_int, [_vp]),
+    "mrhs_transfer_create": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, _int4, ctypes.c_int, ctypes.c_int, _vp, _vp]),
+    "mrhs_prolong": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_restrict": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_transfer_destroy": (ctypes.c_int, [_vp]),
     "mrhs_inner_products": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
     "mrhs_xblock": (ctypes.c_int, [ctypes.c_int, ctypes.c_int]),
     "mrhs_field_bytes": (ctypes.c_size_t, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
@@ -146,6 +150,29 @@ def field_import(dims, ncomp, nrhs, parity, canonical, native=None, stream=None)
         native = empty_field(dims, ncomp, nrhs, parity, canonical.device)
     _check(lib().mrhs_field_import(_dims(dims), ncomp, nrhs, parity, _ptr(canonical), _ptr(native), _stream_ptr(stream)))
     return native
+
+
+class Transfer:
+    """MRHS prolongation / restriction between the fine level and its first coarse level (handle owner)."""
+
+    def __init__(self, dims, bdims, nvec, nrhs, basis, stream=None):
+        self.dims, self.bdims, self.nvec, self.nrhs = [int(d) for d in dims], [int(b) for b in bdims], int(nvec), int(nrhs)
+        self.cdims = [d // b for d, b in zip(self.dims, self.bdims)]
+        h = _vp()
+        _check(lib().mrhs_transfer_create(ctypes.byref(h), _dims(self.dims), _dims(self.bdims), self.nvec, self.nrhs,
+                                          _ptr(basis), _stream_ptr(stream)))
+        self.h = h
+
+    def prolong(self, d_coarse, d_fine):
+        _check(lib().mrhs_prolong(self.h, _ptr(d_coarse), _ptr(d_fine)))
+
+    def restrict(self, d_fine, d_coarse):
+        _check(lib().mrhs_restrict(self.h, _ptr(d_fine), _ptr(d_coarse)))
+
+    def close(self):
+        if self.h:
+            _check(lib().mrhs_transfer_destroy(self.h))
+            self.h = None
 
 
 def inner_products(dims, ncomp, nrhs, parity, x, y, result=None, stream=None):

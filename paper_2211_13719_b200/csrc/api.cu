@@ -7,6 +7,7 @@
 #include "coarse.cuh"
 #include "fine_sweep.cuh"
 #include "blas.cuh"
+#include "transfer.cuh"
 #include "fine_hop.cuh"
 
 namespace mrhs {
@@ -50,6 +51,12 @@ struct mrhs_wilson {
     size_t st_bytes;
     void *st_tmp[2];               // odd-parity temporaries of the Schur sequence
     size_t st_tmp_bytes;
+};
+
+struct mrhs_transfer {
+    TransferGeom g;
+    cudaStream_t st;
+    float2 *basis;   // native [site][k][12]
 };
 
 struct mrhs_coarse {
@@ -505,6 +512,60 @@ mrhs_status_t mrhs_coarse_apply_host(mrhs_coarse_t *h, const void *h_in, void *h
     if (s != MRHS_OK) return s;
     MRHS_CUDA(cudaMemcpyAsync(h_out, h->st_canon, bytes, cudaMemcpyDeviceToHost, h->st));
     MRHS_CUDA(cudaStreamSynchronize(h->st));
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_transfer_create(mrhs_transfer_t **out, const int dims[4], const int bdims[4], int nvec, int nrhs,
+                                   const void *d_basis, void *cuda_stream) {
+    MRHS_REQUIRE(out, "transfer create: out is NULL");
+    *out = nullptr;
+    MRHS_REQUIRE(dims && bdims && d_basis, "transfer create: NULL argument");
+    MRHS_REQUIRE(nvec >= 1 && nvec <= 256 && nrhs >= 1 && nrhs <= 128, "transfer create: nvec must be 1..256 and nrhs 1..128");
+    MRHS_REQUIRE(aligned16(d_basis), "transfer create: basis must be 16-byte aligned");
+    for (int i = 0; i < 4; i++)
+        MRHS_REQUIRE(dims[i] >= 2 && bdims[i] >= 1 && dims[i] % bdims[i] == 0 && dims[i] / bdims[i] >= 2,
+                     "transfer create: every block extent must divide the lattice extent and leave a coarse extent >= 2");
+    mrhs_transfer *h = new (std::nothrow) mrhs_transfer();
+    if (!h) { set_error("transfer create: host allocation failed"); return MRHS_ERR_ALLOC; }
+    memset(h, 0, sizeof(*h));
+    TransferGeom &g = h->g;
+    g.X = dims[0]; g.Y = dims[1]; g.Z = dims[2]; g.T = dims[3];
+    g.bx = bdims[0]; g.by = bdims[1]; g.bz = bdims[2]; g.bt = bdims[3];
+    g.cX = g.X / g.bx; g.cY = g.Y / g.by; g.cZ = g.Z / g.bz; g.cT = g.T / g.bt;
+    g.nvec = nvec; g.N = nrhs;
+    const FieldGeom fg = make_geom(dims, 12, nrhs, MRHS_FULL);
+    g.XB = fg.XB; g.nxb = fg.nxb;
+    g.nsites = fg.nsites;
+    g.ncoarse = (long long)g.cX * g.cY * g.cZ * g.cT;
+    h->st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaMalloc(&h->basis, (size_t)g.nsites * nvec * 12 * sizeof(float2));
+    if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaMalloc(basis)", __FILE__, __LINE__); }
+    mrhs_status_t s = pack_basis(g, (const float2 *)d_basis, h->basis, h->st);
+    if (s == MRHS_OK) {
+        e = cudaStreamSynchronize(h->st);
+        if (e != cudaSuccess) s = cuda_fail(e, "cudaStreamSynchronize", __FILE__, __LINE__);
+    }
+    if (s != MRHS_OK) { cudaFree(h->basis); delete h; return s; }
+    *out = h;
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_prolong(mrhs_transfer_t *h, const void *d_coarse_in, void *d_fine_out) {
+    MRHS_REQUIRE(h && d_coarse_in && d_fine_out, "prolong: NULL argument");
+    MRHS_REQUIRE(aligned16(d_coarse_in) && aligned16(d_fine_out), "prolong: buffers must be 16-byte aligned");
+    return launch_prolong(h->g, h->basis, d_coarse_in, d_fine_out, h->st);
+}
+
+mrhs_status_t mrhs_restrict(mrhs_transfer_t *h, const void *d_fine_in, void *d_coarse_out) {
+    MRHS_REQUIRE(h && d_fine_in && d_coarse_out, "restrict: NULL argument");
+    MRHS_REQUIRE(aligned16(d_fine_in) && aligned16(d_coarse_out), "restrict: buffers must be 16-byte aligned");
+    return launch_restrict(h->g, h->basis, d_fine_in, d_coarse_out, h->st);
+}
+
+mrhs_status_t mrhs_transfer_destroy(mrhs_transfer_t *h) {
+    if (!h) return MRHS_OK;
+    cudaFree(h->basis);
+    delete h;
     return MRHS_OK;
 }
 

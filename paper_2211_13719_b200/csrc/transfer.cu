@@ -1,0 +1,167 @@
+// transfer.cu -- prolongation and restriction between the fine level and the first coarse level for N_rhs
+// right-hand sides at once (reading S9).  First correct version:
+// FP32 FMA (FFMA2 over RHS pairs), operands through L1/L2; fields in the library's native layouts.
+#include "transfer.cuh"
+
+namespace mrhs {
+
+namespace {
+
+template <int R> __device__ __forceinline__ CVec<R> czero_t();
+template <> __device__ __forceinline__ CVec<1> czero_t<1>() { return {{0.f}, {0.f}}; }
+template <> __device__ __forceinline__ CVec<2> czero_t<2>() { return {{0ull}, {0ull}}; }
+
+__global__ void pack_basis_kernel(int nvec, long long V, const float2 *__restrict__ src, float2 *__restrict__ dst, long long total) {
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // native order [lex][k][12]
+    if (idx >= total) return;
+    const int c = (int)(idx % 12);
+    long long q = idx / 12;
+    const int k = (int)(q % nvec);
+    const long long lex = q / nvec;
+    dst[idx] = src[((long long)k * V + lex) * 12 + c];
+}
+
+// One thread = one fine site and R right-hand sides (the thread order of the fine native layout, as in M_ooee):
+// the 2 nvec coarse coefficients of the site's block are read once per k and serve all twelve components.
+template <int R>
+__global__ void __launch_bounds__(256)
+prolong_kernel(TransferGeom g, int NP, long long nthreads, const float4 *__restrict__ basis,
+               const typename Elem<R>::type *__restrict__ coarse, typename Elem<R>::type *__restrict__ fine) {
+    typedef typename Elem<R>::type E;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= nthreads) return;
+    const int CS = g.XB * NP;
+    long long b = gid / CS;
+    const int rem = (int)(gid - b * CS);
+    const int xin = rem / NP, pair = rem - xin * NP;
+    E *po = fine + (size_t)b * 12 * CS + rem;
+    const int xb = (int)(b % g.nxb); b /= g.nxb;
+    const int y = (int)(b % g.Y); b /= g.Y;
+    const int z = (int)(b % g.Z);
+    const int t = (int)(b / g.Z);
+    const int x = xb * g.XB + xin;
+    const long long lex = x + (long long)g.X * (y + (long long)g.Y * (z + (long long)g.Z * t));
+    const long long B = (x / g.bx) + (long long)g.cX * ((y / g.by) + (long long)g.cY * ((z / g.bz) + (long long)g.cZ * (t / g.bt)));
+    const E *vc = coarse + (size_t)B * 2 * g.nvec * NP + pair;
+    const float4 *ph = basis + (size_t)lex * g.nvec * 6;
+    CVec<R> acc[12];
+#pragma unroll
+    for (int c = 0; c < 12; c++) acc[c] = czero_t<R>();
+    for (int k = 0; k < g.nvec; k++) {
+        const CVec<R> v0 = to_cvec(__ldg(vc + (size_t)k * NP)), v1 = to_cvec(__ldg(vc + (size_t)(g.nvec + k) * NP));
+#pragma unroll
+        for (int j = 0; j < 6; j++) {
+            const float4 a = __ldg(ph + k * 6 + j);   // components 2j, 2j+1
+            const CVec<R> &v = j < 3 ? v0 : v1;
+            acc[2 * j] = cfma(a.x, a.y, v, acc[2 * j]);
+            acc[2 * j + 1] = cfma(a.z, a.w, v, acc[2 * j + 1]);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 12; c++) po[(size_t)c * CS] = from_cvec(acc[c]);
+}
+
+// One thread block = one aggregate and a chunk of PC RHS lanes; a thread owns one (slice, k, lane) and sums its slice of
+// the aggregate's sites into the two chiral coefficients; slices are added through shared memory in a fixed order.
+template <int R>
+__global__ void __launch_bounds__(256)
+restrict_kernel(TransferGeom g, int NP, int PC, int S, const float4 *__restrict__ basis,
+                const typename Elem<R>::type *__restrict__ fine, typename Elem<R>::type *__restrict__ coarse) {
+    typedef typename Elem<R>::type E;
+    extern __shared__ __align__(16) unsigned char sm[];
+    const int nagg = g.bx * g.by * g.bz * g.bt;
+    long long *s_lex = reinterpret_cast<long long *>(sm);                 // [nagg] canonical site index (basis)
+    long long *s_off = s_lex + nagg;                                      // [nagg] native element offset of component 0, lane 0
+    E *red = reinterpret_cast<E *>(s_off + nagg);                         // [S-1][items][2]
+    const int CS = g.XB * NP;
+    const long long B = blockIdx.x;
+    const int c0x = (int)(B % g.cX), c0y = (int)((B / g.cX) % g.cY), c0z = (int)((B / ((long long)g.cX * g.cY)) % g.cZ);
+    const int c0t = (int)(B / ((long long)g.cX * g.cY * g.cZ));
+    for (int i = threadIdx.x; i < nagg; i += blockDim.x) {
+        int q = i;
+        const int ix = q % g.bx; q /= g.bx;
+        const int iy = q % g.by; q /= g.by;
+        const int iz = q % g.bz;
+        const int it = q / g.bz;
+        const int x = c0x * g.bx + ix, y = c0y * g.by + iy, z = c0z * g.bz + iz, t = c0t * g.bt + it;
+        s_lex[i] = x + (long long)g.X * (y + (long long)g.Y * (z + (long long)g.Z * t));
+        const long long b = (x / g.XB) + (long long)g.nxb * (y + (long long)g.Y * (z + (long long)g.Z * t));
+        s_off[i] = b * 12 * CS + (long long)(x % g.XB) * NP;
+    }
+    __syncthreads();
+    const int items = g.nvec * PC;
+    const int tid = threadIdx.x;
+    const int s = tid / items, item = tid - s * items;
+    const int k = item / PC, lane = blockIdx.y * PC + (item - k * PC);
+    const bool active = s < S && lane < NP;
+    CVec<R> a0 = czero_t<R>(), a1 = czero_t<R>();
+    if (active) {
+        for (int i = s; i < nagg; i += S) {
+            const float4 *ph = basis + ((size_t)s_lex[i] * g.nvec + k) * 6;
+            const E *pf = fine + s_off[i] + lane;
+#pragma unroll
+            for (int j = 0; j < 6; j++) {
+                const float4 a = __ldg(ph + j);
+                const CVec<R> f0 = to_cvec(__ldg(pf + (size_t)(2 * j) * CS)), f1 = to_cvec(__ldg(pf + (size_t)(2 * j + 1) * CS));
+                if (j < 3) { a0 = cfma_conj(a.x, a.y, f0, a0); a0 = cfma_conj(a.z, a.w, f1, a0); }
+                else       { a1 = cfma_conj(a.x, a.y, f0, a1); a1 = cfma_conj(a.z, a.w, f1, a1); }
+            }
+        }
+        if (s > 0) {
+            red[((size_t)(s - 1) * items + item) * 2] = from_cvec(a0);
+            red[((size_t)(s - 1) * items + item) * 2 + 1] = from_cvec(a1);
+        }
+    }
+    __syncthreads();
+    if (active && s == 0) {
+        for (int q = 1; q < S; q++) {
+            a0 = cadd(a0, to_cvec(red[((size_t)(q - 1) * items + item) * 2]));
+            a1 = cadd(a1, to_cvec(red[((size_t)(q - 1) * items + item) * 2 + 1]));
+        }
+        E *po = coarse + (size_t)B * 2 * g.nvec * NP + lane;
+        po[(size_t)k * NP] = from_cvec(a0);
+        po[(size_t)(g.nvec + k) * NP] = from_cvec(a1);
+    }
+}
+
+}  // namespace
+
+mrhs_status_t pack_basis(const TransferGeom &g, const float2 *d_canonical, float2 *d_native, cudaStream_t st) {
+    const long long total = g.nsites * g.nvec * 12;
+    pack_basis_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(g.nvec, g.nsites, d_canonical, d_native, total);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+mrhs_status_t launch_prolong(const TransferGeom &g, const float2 *d_basis, const void *d_coarse, void *d_fine, cudaStream_t st) {
+    const int np = threads_per_site(g.N);
+    const long long nthreads = g.nsites * np;
+    const unsigned blocks = (unsigned)((nthreads + 255) / 256);
+    if (g.N & 1) prolong_kernel<1><<<blocks, 256, 0, st>>>(g, np, nthreads, (const float4 *)d_basis, (const float2 *)d_coarse, (float2 *)d_fine);
+    else         prolong_kernel<2><<<blocks, 256, 0, st>>>(g, np, nthreads, (const float4 *)d_basis, (const float4 *)d_coarse, (float4 *)d_fine);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+mrhs_status_t launch_restrict(const TransferGeom &g, const float2 *d_basis, const void *d_fine, void *d_coarse, cudaStream_t st) {
+    const int np = threads_per_site(g.N);
+    if (g.nvec > 256) { set_error("restrict: nvec = %d exceeds 256", g.nvec); return MRHS_ERR_UNSUPPORTED; }
+    int pc = 256 / g.nvec;
+    if (pc > np) pc = np;
+    const int items = g.nvec * pc;
+    const int nagg = g.bx * g.by * g.bz * g.bt;
+    int S = 256 / items;
+    if (S > nagg) S = nagg;
+    if (S < 1) S = 1;
+    const int threads = S * items;
+    const int esz = (g.N & 1) ? 8 : 16;
+    const size_t smem = (size_t)nagg * 16 + (size_t)(S - 1) * items * 2 * esz;
+    if (smem > 48 * 1024) { set_error("restrict: aggregate of %d sites needs %zu bytes of shared memory (max 48 KB)", nagg, smem); return MRHS_ERR_UNSUPPORTED; }
+    dim3 grid((unsigned)g.ncoarse, (unsigned)((np + pc - 1) / pc));
+    if (g.N & 1) restrict_kernel<1><<<grid, threads, smem, st>>>(g, np, pc, S, (const float4 *)d_basis, (const float2 *)d_fine, (float2 *)d_coarse);
+    else         restrict_kernel<2><<<grid, threads, smem, st>>>(g, np, pc, S, (const float4 *)d_basis, (const float4 *)d_fine, (float4 *)d_coarse);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+}  // namespace mrhs
