@@ -47,6 +47,7 @@ prolong_kernel(TransferGeom g, int NP, long long nthreads, const float4 *__restr
     CVec<R> acc[12];
 #pragma unroll
     for (int c = 0; c < 12; c++) acc[c] = czero_t<R>();
+#pragma unroll 4
     for (int k = 0; k < g.nvec; k++) {
         const CVec<R> v0 = to_cvec(__ldg(vc + (size_t)k * NP)), v1 = to_cvec(__ldg(vc + (size_t)(g.nvec + k) * NP));
 #pragma unroll
@@ -96,6 +97,7 @@ restrict_kernel(TransferGeom g, int NP, int PC, int S, const float4 *__restrict_
     const bool active = s < S && lane < NP;
     CVec<R> a0 = czero_t<R>(), a1 = czero_t<R>();
     if (active) {
+#pragma unroll 2
         for (int i = s; i < nagg; i += S) {
             const float4 *ph = basis + ((size_t)s_lex[i] * g.nvec + k) * 6;
             const E *pf = fine + s_off[i] + lane;
