@@ -62,6 +62,92 @@ prolong_kernel(TransferGeom g, int NP, long long nthreads, const float4 *__restr
     for (int c = 0; c < 12; c++) po[(size_t)c * CS] = from_cvec(acc[c]);
 }
 
+// The same map with the basis staged in shared memory: a thread block owns ROWS consecutive block rows of the fine
+// native layout (XB sites each, ROWS XB NP threads); the basis of a row is one contiguous run of XB nvec 96 bytes, brought
+// in by one bulk async copy per row (completion on an mbarrier), so the HBM stream of the basis has tens of KB in flight
+// per SM instead of one 16-byte load per thread.  Sites read their k in a staggered order to spread shared-memory banks.
+template <int R>
+__global__ void __launch_bounds__(256)
+prolong_smem_kernel(TransferGeom g, int NP, int rows, long long nblk, const float4 *__restrict__ basis,
+                    const typename Elem<R>::type *__restrict__ coarse, typename Elem<R>::type *__restrict__ fine) {
+    typedef typename Elem<R>::type E;
+    extern __shared__ __align__(128) unsigned char sm[];
+    __shared__ uint64_t bar;
+    const float4 *sb = reinterpret_cast<const float4 *>(sm);
+    const int CS = g.XB * NP;
+    const int tid = threadIdx.x;
+    const long long b0 = (long long)blockIdx.x * rows;
+    const uint32_t row_bytes = (uint32_t)g.XB * g.nvec * 96u;
+    auto row_lex0 = [&](long long b) {
+        const int xb = (int)(b % g.nxb); b /= g.nxb;
+        const int y = (int)(b % g.Y); b /= g.Y;
+        const int z = (int)(b % g.Z);
+        const int t = (int)(b / g.Z);
+        return (long long)xb * g.XB + (long long)g.X * (y + (long long)g.Y * (z + (long long)g.Z * t));
+    };
+    if (tid == 0) {
+        const uint32_t bs = (uint32_t)__cvta_generic_to_shared(&bar);
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bs) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        int nrow = 0;
+        for (int r = 0; r < rows; r++) nrow += b0 + r < nblk;
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bs), "r"(nrow * row_bytes) : "memory");
+        for (int r = 0; r < nrow; r++) {
+            const float4 *src = basis + (size_t)row_lex0(b0 + r) * g.nvec * 6;
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                             (uint32_t)__cvta_generic_to_shared(sm + (size_t)r * row_bytes)),
+                         "l"(src), "r"(row_bytes), "r"(bs)
+                         : "memory");
+        }
+    }
+    __syncthreads();
+    const int row = tid / CS, rem = tid - row * CS;
+    const long long b = b0 + row;
+    const bool active = row < rows && b < nblk;
+    const int xin = rem / NP, pair = rem - xin * NP;
+    const E *vc = coarse;
+    int x = 0, y = 0, z = 0, t = 0;
+    if (active) {
+        long long q = b;
+        const int xb = (int)(q % g.nxb); q /= g.nxb;
+        y = (int)(q % g.Y); q /= g.Y;
+        z = (int)(q % g.Z);
+        t = (int)(q / g.Z);
+        x = xb * g.XB + xin;
+        const long long B = (x / g.bx) + (long long)g.cX * ((y / g.by) + (long long)g.cY * ((z / g.bz) + (long long)g.cZ * (t / g.bt)));
+        vc = coarse + (size_t)B * 2 * g.nvec * NP + pair;
+    }
+    {   // wait for the basis rows
+        const uint32_t bs = (uint32_t)__cvta_generic_to_shared(&bar);
+        uint32_t ok;
+        do {
+            asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}" : "=r"(ok) : "r"(bs), "r"(0u) : "memory");
+        } while (!ok);
+    }
+    if (!active) return;
+    const int site = row * g.XB + xin;
+    const float4 *ph = sb + (size_t)site * g.nvec * 6;
+    CVec<R> acc[12];
+#pragma unroll
+    for (int c = 0; c < 12; c++) acc[c] = czero_t<R>();
+    int k = site % g.nvec;
+#pragma unroll 2
+    for (int i = 0; i < g.nvec; i++) {
+        const CVec<R> v0 = to_cvec(__ldg(vc + (size_t)k * NP)), v1 = to_cvec(__ldg(vc + (size_t)(g.nvec + k) * NP));
+#pragma unroll
+        for (int j = 0; j < 6; j++) {
+            const float4 a = ph[k * 6 + j];
+            const CVec<R> &v = j < 3 ? v0 : v1;
+            acc[2 * j] = cfma(a.x, a.y, v, acc[2 * j]);
+            acc[2 * j + 1] = cfma(a.z, a.w, v, acc[2 * j + 1]);
+        }
+        k = k + 1 == g.nvec ? 0 : k + 1;
+    }
+    E *po = fine + (size_t)b * 12 * CS + rem;
+#pragma unroll
+    for (int c = 0; c < 12; c++) po[(size_t)c * CS] = from_cvec(acc[c]);
+}
+
 // One thread block = one aggregate and a chunk of PC RHS lanes; a thread owns one (slice, k, lane) and sums its slice of
 // the aggregate's sites into the two chiral coefficients; slices are added through shared memory in a fixed order.
 template <int R>
@@ -138,6 +224,24 @@ mrhs_status_t pack_basis(const TransferGeom &g, const float2 *d_canonical, float
 mrhs_status_t launch_prolong(const TransferGeom &g, const float2 *d_basis, const void *d_coarse, void *d_fine, cudaStream_t st) {
     const int np = threads_per_site(g.N);
     const long long nthreads = g.nsites * np;
+    // shared-memory staging when at least two blocks fit an SM; the plain kernel otherwise
+    const int cs = g.XB * np;
+    const int rows = cs <= 256 ? 256 / cs : 0;
+    const size_t smem = (size_t)rows * g.XB * g.nvec * 96;
+    if (rows >= 1 && smem <= 100 * 1024) {
+        const long long nblk = (long long)g.nxb * g.Y * g.Z * g.T;
+        const unsigned grid = (unsigned)((nblk + rows - 1) / rows);
+        const int threads = rows * cs;
+        if (g.N & 1) {
+            MRHS_CUDA(cudaFuncSetAttribute(prolong_smem_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            prolong_smem_kernel<1><<<grid, threads, smem, st>>>(g, np, rows, nblk, (const float4 *)d_basis, (const float2 *)d_coarse, (float2 *)d_fine);
+        } else {
+            MRHS_CUDA(cudaFuncSetAttribute(prolong_smem_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            prolong_smem_kernel<2><<<grid, threads, smem, st>>>(g, np, rows, nblk, (const float4 *)d_basis, (const float4 *)d_coarse, (float4 *)d_fine);
+        }
+        MRHS_CUDA(cudaGetLastError());
+        return MRHS_OK;
+    }
     const unsigned blocks = (unsigned)((nthreads + 255) / 256);
     if (g.N & 1) prolong_kernel<1><<<blocks, 256, 0, st>>>(g, np, nthreads, (const float4 *)d_basis, (const float2 *)d_coarse, (float2 *)d_fine);
     else         prolong_kernel<2><<<blocks, 256, 0, st>>>(g, np, nthreads, (const float4 *)d_basis, (const float4 *)d_coarse, (float4 *)d_fine);
