@@ -226,7 +226,7 @@ mrhs_status_t launch_prolong(const TransferGeom &g, const float2 *d_basis, const
     const long long nthreads = g.nsites * np;
     // shared-memory staging when at least two blocks fit an SM; the plain kernel otherwise
     const int cs = g.XB * np;
-    const int rows = cs <= 256 ? 256 / cs : 0;
+    const int rows = cs <= 256 ? (256 / cs < 2 ? 256 / cs : 2) : 0;   // two rows (96 threads at XB NP = 48) measured best: many small blocks per SM
     const size_t smem = (size_t)rows * g.XB * g.nvec * 96;
     if (rows >= 1 && smem <= 100 * 1024) {
         const long long nblk = (long long)g.nxb * g.Y * g.Z * g.T;
