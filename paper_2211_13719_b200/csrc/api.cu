@@ -582,6 +582,15 @@ mrhs_status_t mrhs_inner_products(const int dims[4], int ncomp, int nrhs, int pa
     MRHS_CUDA(cudaGetDevice(&dev));
     MRHS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     const int grid = inner_grid(sms);
+    // the scratch comes from the device's stream-ordered pool; keep freed blocks in the pool so that the
+    // allocation does not go back to the driver on every call
+    static bool pool_ready = false;
+    if (!pool_ready) {
+        cudaMemPool_t pool;
+        unsigned long long keep = ~0ull;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        pool_ready = true;
+    }
     double2 *partial = nullptr;
     MRHS_CUDA(cudaMallocAsync(&partial, (size_t)grid * nrhs * sizeof(double2), st));
     mrhs_status_t s = launch_inner_products((long long)(bytes / 4), nrhs, d_x, d_y, partial, grid, (double2 *)d_result, st);
