@@ -133,7 +133,7 @@ prolong_smem_kernel(TransferGeom g, int NP, int rows, long long nblk, const floa
 #pragma unroll
     for (int c = 0; c < 12; c++) acc[c] = czero_t<R>();
     int k = site % g.nvec;
-#pragma unroll 2
+#pragma unroll 10
     for (int i = 0; i < g.nvec; i++) {
         const CVec<R> v0 = to_cvec(__ldg(vc + (size_t)k * NP)), v1 = to_cvec(__ldg(vc + (size_t)(g.nvec + k) * NP));
 #pragma unroll
