@@ -242,7 +242,7 @@ mrhs_status_t mrhs_cb_merge(const int dims[4], int ncomp, int nrhs, const void *
  *   d_basis: device, canonical [n_vec][site][4][3] complex64, copied and repacked (caller may free it).
  * prolong: d_coarse_in native coarse vector (ncomp = 2 n_vec) of the coarse lattice dims / bdims,
  *   d_fine_out native full-lattice fine field; restrict the other way.  Asynchronous on the stream.
- * UNSUPPORTED: aggregates whose index table does not fit 48 KB of shared memory (> ~2000 sites). */
+ * UNSUPPORTED: aggregates whose index table and reduction scratch do not fit 100 KB of shared memory (> ~2000 sites). */
 mrhs_status_t mrhs_transfer_create(mrhs_transfer_t **out, const int dims[4], const int bdims[4], int nvec,
                                    int nrhs, const void *d_basis, void *cuda_stream);
 mrhs_status_t mrhs_prolong(mrhs_transfer_t *h, const void *d_coarse_in, void *d_fine_out);

@@ -150,10 +150,11 @@ prolong_smem_kernel(TransferGeom g, int NP, int rows, long long nblk, const floa
     for (int c = 0; c < 12; c++) po[(size_t)c * CS] = from_cvec(acc[c]);
 }
 
-// One thread block = one aggregate and a chunk of PC RHS lanes; a thread owns one (slice, group of KT basis vectors, lane)
-// and sums its slice of the aggregate's sites into the 2 KT chiral coefficients (each field element loaded serves KT
-// basis vectors from registers); slices are added through shared memory in a fixed order.
-template <int R, int KT>
+// One thread block = one aggregate and a chunk of PC x LT RHS lanes; a thread owns one (slice, group of KT basis vectors,
+// group of LT lanes) and sums its slice of the aggregate's sites into the 2 KT LT chiral coefficients: every field element
+// loaded serves KT basis vectors and every basis entry LT lanes from registers.  Slices are added through shared memory in
+// a fixed order (bit-reproducible).
+template <int R, int KT, int LT>
 __global__ void __launch_bounds__(256)
 restrict_kernel(TransferGeom g, int NP, int PC, int S, const float4 *__restrict__ basis,
                 const typename Elem<R>::type *__restrict__ fine, typename Elem<R>::type *__restrict__ coarse) {
@@ -162,7 +163,7 @@ restrict_kernel(TransferGeom g, int NP, int PC, int S, const float4 *__restrict_
     const int nagg = g.bx * g.by * g.bz * g.bt;
     long long *s_lex = reinterpret_cast<long long *>(sm);                 // [nagg] canonical site index (basis)
     long long *s_off = s_lex + nagg;                                      // [nagg] native element offset of component 0, lane 0
-    E *red = reinterpret_cast<E *>(s_off + nagg);                         // [S-1][items][2 KT]
+    E *red = reinterpret_cast<E *>(s_off + nagg);                         // [S-1][items][2 KT LT]
     const int CS = g.XB * NP;
     const long long B = blockIdx.x;
     const int c0x = (int)(B % g.cX), c0y = (int)((B / g.cX) % g.cY), c0z = (int)((B / ((long long)g.cX * g.cY)) % g.cZ);
@@ -182,55 +183,74 @@ restrict_kernel(TransferGeom g, int NP, int PC, int S, const float4 *__restrict_
     const int items = (g.nvec / KT) * PC;
     const int tid = threadIdx.x;
     const int s = tid / items, item = tid - s * items;
-    const int k0 = (item / PC) * KT, lane = blockIdx.y * PC + (item - (item / PC) * PC);
-    const bool active = s < S && lane < NP;
-    CVec<R> a0[KT], a1[KT];
+    const int k0 = (item / PC) * KT, lane = (blockIdx.y * PC + (item - (item / PC) * PC)) * LT;
+    const bool active = s < S && lane < NP;   // NP is a multiple of LT
+    CVec<R> a0[KT][LT], a1[KT][LT];
 #pragma unroll
-    for (int kk = 0; kk < KT; kk++) { a0[kk] = czero_t<R>(); a1[kk] = czero_t<R>(); }
+    for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+        for (int l = 0; l < LT; l++) { a0[kk][l] = czero_t<R>(); a1[kk][l] = czero_t<R>(); }
     if (active) {
         for (int i = s; i < nagg; i += S) {
-            // a few threads per slice ask for the lines of a site some iterations ahead (L2 prefetch), so that the loads
+            // the threads of a slice ask for the lines of the site some iterations ahead (L2 prefetch), so that the loads
             // below pay L2 instead of HBM latency: the basis of the site and the 12 component runs of the field
             const int ip = i + kRestrictAhead * S;
             if (ip < nagg) {
                 if (item * 128 < g.nvec * 96) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(basis + (size_t)s_lex[ip] * g.nvec * 6) + item * 128));
-                else if (item >= 16 && item < 28) asm volatile("prefetch.global.L2 [%0];" ::"l"(fine + s_off[ip] + (size_t)(item - 16) * CS + blockIdx.y * PC));
+                if (item < 12) asm volatile("prefetch.global.L2 [%0];" ::"l"(fine + s_off[ip] + (size_t)item * CS + blockIdx.y * PC * LT));
             }
             const float4 *ph = basis + ((size_t)s_lex[i] * g.nvec + k0) * 6;
             const E *pf = fine + s_off[i] + lane;
 #pragma unroll
             for (int j = 0; j < 6; j++) {
-                const CVec<R> f0 = to_cvec(__ldg(pf + (size_t)(2 * j) * CS)), f1 = to_cvec(__ldg(pf + (size_t)(2 * j + 1) * CS));
+                CVec<R> f0[LT], f1[LT];
+#pragma unroll
+                for (int l = 0; l < LT; l++) {
+                    f0[l] = to_cvec(__ldg(pf + (size_t)(2 * j) * CS + l));
+                    f1[l] = to_cvec(__ldg(pf + (size_t)(2 * j + 1) * CS + l));
+                }
 #pragma unroll
                 for (int kk = 0; kk < KT; kk++) {
                     const float4 a = __ldg(ph + kk * 6 + j);
-                    if (j < 3) { a0[kk] = cfma_conj(a.x, a.y, f0, a0[kk]); a0[kk] = cfma_conj(a.z, a.w, f1, a0[kk]); }
-                    else       { a1[kk] = cfma_conj(a.x, a.y, f0, a1[kk]); a1[kk] = cfma_conj(a.z, a.w, f1, a1[kk]); }
+#pragma unroll
+                    for (int l = 0; l < LT; l++) {
+                        if (j < 3) { a0[kk][l] = cfma_conj(a.x, a.y, f0[l], a0[kk][l]); a0[kk][l] = cfma_conj(a.z, a.w, f1[l], a0[kk][l]); }
+                        else       { a1[kk][l] = cfma_conj(a.x, a.y, f0[l], a1[kk][l]); a1[kk][l] = cfma_conj(a.z, a.w, f1[l], a1[kk][l]); }
+                    }
                 }
             }
         }
         if (s > 0) {
+            E *rp = red + ((size_t)(s - 1) * items + item) * 2 * KT * LT;
 #pragma unroll
-            for (int kk = 0; kk < KT; kk++) {
-                red[((size_t)(s - 1) * items + item) * 2 * KT + 2 * kk] = from_cvec(a0[kk]);
-                red[((size_t)(s - 1) * items + item) * 2 * KT + 2 * kk + 1] = from_cvec(a1[kk]);
-            }
+            for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+                for (int l = 0; l < LT; l++) {
+                    rp[2 * (kk * LT + l)] = from_cvec(a0[kk][l]);
+                    rp[2 * (kk * LT + l) + 1] = from_cvec(a1[kk][l]);
+                }
         }
     }
     __syncthreads();
     if (active && s == 0) {
-        for (int q = 1; q < S; q++)
+        for (int q = 1; q < S; q++) {
+            const E *rp = red + ((size_t)(q - 1) * items + item) * 2 * KT * LT;
 #pragma unroll
-            for (int kk = 0; kk < KT; kk++) {
-                a0[kk] = cadd(a0[kk], to_cvec(red[((size_t)(q - 1) * items + item) * 2 * KT + 2 * kk]));
-                a1[kk] = cadd(a1[kk], to_cvec(red[((size_t)(q - 1) * items + item) * 2 * KT + 2 * kk + 1]));
-            }
+            for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+                for (int l = 0; l < LT; l++) {
+                    a0[kk][l] = cadd(a0[kk][l], to_cvec(rp[2 * (kk * LT + l)]));
+                    a1[kk][l] = cadd(a1[kk][l], to_cvec(rp[2 * (kk * LT + l) + 1]));
+                }
+        }
         E *po = coarse + (size_t)B * 2 * g.nvec * NP + lane;
 #pragma unroll
-        for (int kk = 0; kk < KT; kk++) {
-            po[(size_t)(k0 + kk) * NP] = from_cvec(a0[kk]);
-            po[(size_t)(g.nvec + k0 + kk) * NP] = from_cvec(a1[kk]);
-        }
+        for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+            for (int l = 0; l < LT; l++) {
+                po[(size_t)(k0 + kk) * NP + l] = from_cvec(a0[kk][l]);
+                po[(size_t)(g.nvec + k0 + kk) * NP + l] = from_cvec(a1[kk][l]);
+            }
     }
 }
 
@@ -275,9 +295,10 @@ mrhs_status_t launch_restrict(const TransferGeom &g, const float2 *d_basis, cons
     const int np = threads_per_site(g.N);
     if (g.nvec > 256) { set_error("restrict: nvec = %d exceeds 256", g.nvec); return MRHS_ERR_UNSUPPORTED; }
     const int kt = g.nvec % 4 == 0 ? 4 : (g.nvec % 2 == 0 ? 2 : 1);   // basis vectors per thread
-    const int groups = g.nvec / kt;
-    int pc = 256 / groups;
-    if (pc > np) pc = np;
+    const int lt = np % 2 == 0 ? 2 : 1;                              // RHS lanes per thread
+    const int groups = g.nvec / kt, lgroups = np / lt;
+    int pc = 256 / groups;                                           // lane groups per thread block
+    if (pc > lgroups) pc = lgroups;
     const int items = groups * pc;
     const int nagg = g.bx * g.by * g.bz * g.bt;
     int S = 256 / items;
@@ -285,15 +306,18 @@ mrhs_status_t launch_restrict(const TransferGeom &g, const float2 *d_basis, cons
     if (S < 1) S = 1;
     const int threads = S * items;
     const int esz = (g.N & 1) ? 8 : 16;
-    const size_t smem = (size_t)nagg * 16 + (size_t)(S - 1) * items * 2 * kt * esz;
-    if (smem > 48 * 1024) { set_error("restrict: aggregate of %d sites needs %zu bytes of shared memory (max 48 KB)", nagg, smem); return MRHS_ERR_UNSUPPORTED; }
-    dim3 grid((unsigned)g.ncoarse, (unsigned)((np + pc - 1) / pc));
-#define MRHS_RESTRICT(RR, KT, ET) restrict_kernel<RR, KT><<<grid, threads, smem, st>>>(g, np, pc, S, (const float4 *)d_basis, (const ET *)d_fine, (ET *)d_coarse)
+    const size_t smem = (size_t)nagg * 16 + (size_t)(S - 1) * items * 2 * kt * lt * esz;
+    if (smem > 100 * 1024) { set_error("restrict: aggregate of %d sites needs %zu bytes of shared memory (max 100 KB)", nagg, smem); return MRHS_ERR_UNSUPPORTED; }
+    dim3 grid((unsigned)g.ncoarse, (unsigned)((lgroups + pc - 1) / pc));
+#define MRHS_RESTRICT(RR, KT, LT, ET) MRHS_CUDA(cudaFuncSetAttribute(restrict_kernel<RR, KT, LT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)); \
+    restrict_kernel<RR, KT, LT><<<grid, threads, smem, st>>>(g, np, pc, S, (const float4 *)d_basis, (const ET *)d_fine, (ET *)d_coarse)
+#define MRHS_RESTRICT_KT(RR, LT, ET) do { if (kt == 4) { MRHS_RESTRICT(RR, 4, LT, ET); } else if (kt == 2) { MRHS_RESTRICT(RR, 2, LT, ET); } else { MRHS_RESTRICT(RR, 1, LT, ET); } } while (0)
     if (g.N & 1) {
-        if (kt == 4) MRHS_RESTRICT(1, 4, float2); else if (kt == 2) MRHS_RESTRICT(1, 2, float2); else MRHS_RESTRICT(1, 1, float2);
+        if (lt == 2) MRHS_RESTRICT_KT(1, 2, float2); else MRHS_RESTRICT_KT(1, 1, float2);
     } else {
-        if (kt == 4) MRHS_RESTRICT(2, 4, float4); else if (kt == 2) MRHS_RESTRICT(2, 2, float4); else MRHS_RESTRICT(2, 1, float4);
+        if (lt == 2) MRHS_RESTRICT_KT(2, 2, float4); else MRHS_RESTRICT_KT(2, 1, float4);
     }
+#undef MRHS_RESTRICT_KT
 #undef MRHS_RESTRICT
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
