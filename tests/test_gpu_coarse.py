@@ -51,7 +51,7 @@ def test_config3_intermediate_level(nrhs):
     c.close()
 
 
-@pytest.mark.parametrize("nrhs", [12, 96])
+@pytest.mark.parametrize("nrhs", [12, 24, 48, 96])
 def test_config4_coarsest_level(nrhs):
     cdims, nb = [6, 6, 6, 32], 40
     A = syn.coarse_links_np(cdims, nb, 4)
@@ -102,6 +102,7 @@ def test_config4_tensor_core(nrhs):
     c0 = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=0)
     err_fma = rel_l2_per_rhs(gpu_coarse(c0, v), want)
     c0.close()
+    assert err_fma.max() < TOL, err_fma
     assert err_tc.max() < 20 * max(err_fma.max(), 1e-7), (err_tc.max(), err_fma.max())
 
 

@@ -56,7 +56,7 @@ def test_dhop_meooe_mooee_match_oracle(dims, nrhs, seed, mass, csw):
         assert err.max() < TOL, ("meooe", out_parity, err)
     # clover construction on the device (row a0) and M_ooee on full / even / odd fields (row a4)
     C, _ = oracle.clover_blocks(dims, U, mass, csw)
-    Cg = torch.empty((syn.volume(dims), 2, 6, 6), dtype=torch.complex64, device="cuda")
+    Cg = torch.full((syn.volume(dims), 2, 6, 6), float("nan"), dtype=torch.complex64, device="cuda")
     mrhs.wilson_export_clover(w.h, Cg)
     cerr = np.linalg.norm(host(Cg) - C) / np.linalg.norm(C)
     assert cerr < 1e-6, cerr
@@ -134,6 +134,8 @@ KERNEL_CASES = [
     ([8, 4, 4, 4], 96, 46),
     ([16, 4, 6, 8], 48, 47),
     ([32, 2, 4, 6], 4, 48),
+    ([16, 4, 4, 4], 12, 49),      # checkerboarded half line of 8 sites at N_rhs = 12: the instantiation config 5 runs
+    ([32, 4, 2, 6], 12, 50),
 ]
 
 
@@ -225,8 +227,11 @@ def test_schur_sequence_and_host_entry():
     w.close()
 
 
+# [16, 4, 4, 4] and [32, 2, 4, 4] at N_rhs = 12 have checkerboarded half lines cut in x-blocks of 8 sites: the
+# hop_sweep_kernel<8, 6, .., ..> instantiations that config 5 (48^4) and bench.py run
 FUSED_CASES = [([8, 8, 4, 4], 12, 60), ([4, 4, 4, 4], 4, 61), ([24, 4, 2, 6], 12, 62), ([16, 2, 4, 4], 24, 63),
-               ([8, 4, 6, 2], 3, 64), ([4, 4, 4, 4], 1, 65)]
+               ([8, 4, 6, 2], 3, 64), ([4, 4, 4, 4], 1, 65), ([16, 4, 4, 4], 12, 66), ([32, 2, 4, 4], 12, 67),
+               ([48, 2, 2, 4], 12, 68)]
 
 
 @pytest.mark.parametrize("dims,nrhs,seed", FUSED_CASES)
@@ -260,7 +265,7 @@ def test_fused_meooe_mooee_and_schur_sequence(dims, nrhs, seed):
     w.close()
 
 
-@pytest.mark.parametrize("dims,nrhs,seed", [([8, 4, 4, 6], 12, 70), ([4, 4, 4, 4], 3, 71), ([24, 2, 4, 2], 24, 72)])
+@pytest.mark.parametrize("dims,nrhs,seed", [([8, 4, 4, 6], 12, 70), ([4, 4, 4, 4], 3, 71), ([24, 2, 4, 2], 24, 72), ([16, 4, 2, 4], 12, 73)])
 def test_inverse_clover_blocks(dims, nrhs, seed):
     """M_ooee^-1 (inverse blocks built on the device at create) on full / even / odd fields, M_ooee^-1 M_ooee = 1,
     and the fused M_ooee^-1 M_eooe with both hop kernels, against the oracle (inverse by numpy.linalg.inv)."""
@@ -318,7 +323,8 @@ def test_inner_products_match_oracle(dims, ncomp, nrhs, parity):
     assert np.max(np.abs(nrm.imag)) == 0.0 and np.all(nrm.real > 0)
 
 
-@pytest.mark.parametrize("dims,nrhs,seed", [([8, 4, 4, 6], 12, 75), ([4, 4, 4, 4], 3, 76), ([16, 2, 4, 4], 24, 77), ([2, 2, 2, 2], 4, 78)])
+@pytest.mark.parametrize("dims,nrhs,seed", [([8, 4, 4, 6], 12, 75), ([4, 4, 4, 4], 3, 76), ([16, 2, 4, 4], 24, 77), ([2, 2, 2, 2], 4, 78),
+                                            ([16, 4, 4, 4], 12, 79), ([48, 2, 4, 2], 12, 80)])
 def test_full_wilson_clover_matrix(dims, nrhs, seed):
     """out = M in = M_ooee in - D_hop in / 2 (reading S6): one fused launch with the sweep kernel, two with the gather kernel."""
     from oracle import galerkin
@@ -338,17 +344,26 @@ def test_full_wilson_clover_matrix(dims, nrhs, seed):
     w.close()
 
 
-@pytest.mark.parametrize("nrhs", [1, 12])
+@pytest.mark.parametrize("nrhs", [1, 4, 12, 24, 48])
 def test_config2_24x24_full_field(nrhs):
-    """Config 2 (24^4, mass -0.05, c_sw 1.5): full-field parity for D_hop, M_eooe and M_ooee."""
+    """Config 2 (24^4, mass -0.05, c_sw 1.5, every N_rhs of the config): full-field parity for D_hop, M_eooe (both
+    parities) and M_ooee with the library's default kernels, and for the sweep kernel where N_rhs allows it."""
     dims, mass, csw = [24, 24, 24, 24], -0.05, 1.5
     U, psi = _fine_case(dims, nrhs, 2, mass, csw)
     w = make_wilson(dims, nrhs, mass, csw, U)
-    err = rel_l2_per_rhs(gpu_dhop(w, psi), oracle.dhop(dims, U, psi))
-    assert err.max() < TOL, err
+    want = oracle.dhop(dims, U, psi)
     pe, po = oracle.cb_split(dims, psi)
-    err = rel_l2_per_rhs(gpu_meooe(w, pe, 1), oracle.meooe(dims, U, pe, 1))
-    assert err.max() < TOL, err
+    want_cb = [oracle.meooe(dims, U, po, 0), oracle.meooe(dims, U, pe, 1)]
+    kernels = [None] + ([mrhs.HOP_SWEEP] if nrhs % 2 == 0 else [])
+    for kern in kernels:
+        if kern is not None:
+            mrhs.wilson_set_hop_kernel(w.h, 0, kern)
+            mrhs.wilson_set_hop_kernel(w.h, 1, kern)
+        err = rel_l2_per_rhs(gpu_dhop(w, psi), want)
+        assert err.max() < TOL, (kern, err)
+        for out_parity, src in ((0, po), (1, pe)):
+            err = rel_l2_per_rhs(gpu_meooe(w, src, out_parity), want_cb[out_parity])
+            assert err.max() < TOL, (kern, out_parity, err)
     C, _ = oracle.clover_blocks(dims, U, mass, csw)
     err = rel_l2_per_rhs(gpu_mooee(w, psi, mrhs.FULL), oracle.mooee(C, psi))
     assert err.max() < TOL, err

@@ -1,8 +1,11 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (library
 default tiling), on sampled output sites the oracle computes one by one (SURVEY.md Sec. 8(d)
-"Parity at 48^4"): config 5 (48^4, N_rhs = 12) for D_hop, M_eooe and M_ooee, and config 4
-(6^3x32, nb = 40) full-field is in test_gpu_coarse.py.  The stencils are local, so the oracle needs
-only the sampled sites' neighbours and links, gathered from the device inputs (never from outputs)."""
+"Parity at 48^4"): config 5 (48^4, N_rhs in {1, 12, 24}) for D_hop, M_eooe, M_ooee, the fused
+M_ooee M_eooe launch, the Schur-style sequence (row a7) and the full matrix; config 4 (6^3x32,
+nb = 40) full-field is in test_gpu_coarse.py.  N_rhs = 24 is the one shape whose fields pass 2^31
+floats (64-bit indexing); N_rhs = 1 runs the scalar gather kernel at full size.  The stencils are
+local, so the oracle needs only the sampled sites' neighbours and links, gathered from the device
+inputs (never from outputs)."""
 import numpy as np
 import pytest
 
@@ -19,7 +22,7 @@ import oracle                      # noqa: E402
 import paper_2211_13719_b200 as mrhs   # noqa: E402
 from gpu_common import TOL   # noqa: E402
 
-DIMS, NRHS, MASS, CSW, SEED = [48, 48, 48, 48], 12, -0.05, 1.5, 5
+DIMS, MASS, CSW, SEED = [48, 48, 48, 48], -0.05, 1.5, 5
 NSAMPLE = 4096
 
 
@@ -65,24 +68,54 @@ def _gather_hop_inputs(dims, U_dev, psi_dev, lex, cb):
     return links, nbrs
 
 
-@pytest.fixture(scope="module")
-def config5():
+@pytest.fixture(scope="module", params=[12, 1, 24], ids=lambda n: "N%d" % n)
+def config5(request):
+    nrhs = request.param
     dev = torch.device("cuda", 0)
     U = syn.gauge_torch(DIMS, SEED, dev)
-    psi = syn.spinor_torch(syn.volume(DIMS), NRHS, SEED, dev)
-    w = mrhs.Wilson(DIMS, NRHS, MASS, CSW, U)
-    assert mrhs.wilson_get_hop_kernel(w.h, 0) == mrhs.HOP_SWEEP and mrhs.wilson_get_hop_kernel(w.h, 1) == mrhs.HOP_SWEEP
+    psi = syn.spinor_torch(syn.volume(DIMS), nrhs, SEED, dev)
+    w = mrhs.Wilson(DIMS, nrhs, MASS, CSW, U)
+    # the library default is what bench.py times: the sweep kernel from N_rhs = 12, the gather kernel for N_rhs = 1
+    want = mrhs.HOP_SWEEP if nrhs >= 12 else mrhs.HOP_GATHER
+    assert mrhs.wilson_get_hop_kernel(w.h, 0) == want and mrhs.wilson_get_hop_kernel(w.h, 1) == want
     yield U, psi, w
     w.close()
+    del U, psi, w
+    torch.cuda.empty_cache()
 
 
 KERNELS = [mrhs.HOP_SWEEP, mrhs.HOP_GATHER]   # the library default (bench.py's configuration) first
 
 
+def _set_kernel(w, which, kernel):
+    if kernel == mrhs.HOP_SWEEP and w.nrhs % 2:
+        pytest.skip("the sweep kernel needs an even N_rhs")
+    mrhs.wilson_set_hop_kernel(w.h, which, kernel)
+
+
+def _parity_of(lex):
+    X, Y, Z, T = DIMS
+    return (lex % X + (lex // X) % Y + (lex // (X * Y)) % Z + lex // (X * Y * Z)) % 2
+
+
+def _cb_input(psi, parity):
+    """canonical checkerboarded field (index lex >> 1) of the sites of one parity"""
+    lex_all = torch.arange(syn.volume(DIMS), device="cuda")
+    return psi[_parity_of(lex_all) == parity].contiguous()
+
+
+def _clover_at(U_host, lex):
+    C = np.empty((lex.size, 2, 6, 6), dtype=np.complex128)
+    for i, x in enumerate(lex):
+        M = oracle.clover_site_matrix(DIMS, U_host, MASS, CSW, int(x))     # 12x12, index 3*spin + colour
+        C[i, 0], C[i, 1] = M[0:6, 0:6], M[6:12, 6:12]
+    return C
+
+
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_config5_dhop_sampled_sites(config5, kernel):
     U, psi, w = config5
-    mrhs.wilson_set_hop_kernel(w.h, 0, kernel)
+    _set_kernel(w, 0, kernel)
     lex = _sample_sites(DIMS, NSAMPLE, 1)
     d_in = w.import_field(psi, mrhs.FULL)
     d_out = w.empty(mrhs.FULL)
@@ -100,15 +133,10 @@ def test_config5_dhop_sampled_sites(config5, kernel):
 @pytest.mark.parametrize("out_parity", [0, 1])
 def test_config5_meooe_sampled_sites(config5, out_parity, kernel):
     U, psi, w = config5
-    mrhs.wilson_set_hop_kernel(w.h, 1, kernel)
-    X, Y, Z, T = DIMS
-    lex_all = torch.arange(syn.volume(DIMS), device="cuda")
-    par = (lex_all % X + (lex_all // X) % Y + (lex_all // (X * Y)) % Z + lex_all // (X * Y * Z)) % 2
-    psi_in = psi[par == (1 - out_parity)].contiguous()          # canonical checkerboarded input, index lex >> 1
-    del lex_all, par
+    _set_kernel(w, 1, kernel)
+    psi_in = _cb_input(psi, 1 - out_parity)
     lex = _sample_sites(DIMS, NSAMPLE, 2 + out_parity)
-    c = [lex % X, (lex // X) % Y, (lex // (X * Y)) % Z, lex // (X * Y * Z)]
-    lex = lex[(c[0] + c[1] + c[2] + c[3]) % 2 == out_parity]
+    lex = lex[_parity_of(lex) == out_parity]
     d_in = w.import_field(psi_in, 1 - out_parity)
     d_out = w.empty(out_parity)
     w.meooe(d_in, d_out, out_parity)
@@ -131,11 +159,81 @@ def test_config5_mooee_sampled_sites(config5):
     t_lex = torch.from_numpy(lex).cuda()
     got = w.export_field(d_out, mrhs.FULL)[t_lex].cpu().numpy()
     del d_in, d_out
-    Uh = U.cpu().numpy().astype(np.complex128)
-    C = np.empty((lex.size, 2, 6, 6), dtype=np.complex128)
-    for i, x in enumerate(lex):
-        M = oracle.clover_site_matrix(DIMS, Uh, MASS, CSW, int(x))     # 12x12, index 3*spin + colour
-        C[i, 0], C[i, 1] = M[0:6, 0:6], M[6:12, 6:12]
+    C = _clover_at(U.cpu().numpy().astype(np.complex128), lex)
     want = oracle.mooee(C, psi[t_lex].cpu().numpy())
+    err = rel_l2_per_rhs(got, want)
+    assert err.max() < TOL, err
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config5_fused_meooe_mooee_sampled_sites(config5, kernel):
+    """The fused M_ooee M_eooe launch (first launch of the Schur-style sequence, the sweep kernel's clover
+    epilogue) at full size: out(y) = C(y) H(y) on sampled odd sites, H from the oracle's site-wise hop."""
+    U, psi, w = config5
+    _set_kernel(w, 1, kernel)
+    out_parity = 1
+    psi_in = _cb_input(psi, 1 - out_parity)
+    lex = _sample_sites(DIMS, 512, 6)
+    lex = lex[_parity_of(lex) == out_parity]
+    d_in = w.import_field(psi_in, 1 - out_parity)
+    d_out = w.empty(out_parity)
+    w.meooe_mooee(d_in, d_out, out_parity)
+    torch.cuda.synchronize()
+    got = w.export_field(d_out, out_parity)[torch.from_numpy(lex >> 1).cuda()].cpu().numpy()
+    del d_in, d_out
+    links, nbrs = _gather_hop_inputs(DIMS, U, psi_in, lex, cb=True)
+    C = _clover_at(U.cpu().numpy().astype(np.complex128), lex)
+    want = oracle.mooee(C, oracle.dhop_sites(links, nbrs))
+    err = rel_l2_per_rhs(got, want)
+    assert err.max() < TOL, err
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config5_schur_sequence_sampled_sites(config5, kernel):
+    """Row a7 at full size: chi_e = M_eooe M_ooee M_eooe psi_e on sampled even sites.  The oracle evaluates the
+    inner two operators on the eight odd neighbours of every sample site (each from its own eight neighbours)."""
+    U, psi, w = config5
+    _set_kernel(w, 1, kernel)
+    psi_e = _cb_input(psi, 0)
+    lex = _sample_sites(DIMS, 64, 7)
+    lex = lex[_parity_of(lex) == 0][:48]
+    d_in = w.import_field(psi_e, mrhs.EVEN)
+    t0, t1, d_out = w.empty(mrhs.ODD), w.empty(mrhs.ODD), w.empty(mrhs.EVEN)
+    w.schur_sequence(d_in, t0, t1, d_out)
+    torch.cuda.synchronize()
+    got = w.export_field(d_out, mrhs.EVEN)[torch.from_numpy(lex >> 1).cuda()].cpu().numpy()
+    del d_in, t0, t1, d_out
+    # the odd neighbours y of the sample sites, psi(x+mu) first, then psi(x-mu): t(y) = C(y) (M_eooe psi_e)(y)
+    nb_lex = np.stack([_nbr_lex(DIMS, lex, mu, sgn) for sgn in (+1, -1) for mu in range(4)], axis=1)      # [n][8]
+    flat = nb_lex.reshape(-1)
+    links_y, nbrs_y = _gather_hop_inputs(DIMS, U, psi_e, flat, cb=True)
+    Uh = U.cpu().numpy().astype(np.complex128)
+    t_y = oracle.mooee(_clover_at(Uh, flat), oracle.dhop_sites(links_y, nbrs_y))
+    links = np.empty((lex.size, 8, 3, 3), dtype=np.complex64)
+    t_lex = torch.from_numpy(lex).cuda()
+    links[:, 0:4] = U[t_lex].cpu().numpy()
+    for mu in range(4):
+        links[:, 4 + mu] = U[torch.from_numpy(nb_lex[:, 4 + mu]).cuda(), mu].cpu().numpy()
+    want = oracle.dhop_sites(links, t_y.reshape(lex.size, 8, 4, 3, -1))
+    err = rel_l2_per_rhs(got, want)
+    assert err.max() < TOL, err
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config5_full_matrix_sampled_sites(config5, kernel):
+    """mrhs_wilson_apply at full size: out = M_ooee in - D_hop in / 2 (reading S6) on sampled sites."""
+    U, psi, w = config5
+    _set_kernel(w, 0, kernel)
+    lex = _sample_sites(DIMS, 512, 8)
+    d_in = w.import_field(psi, mrhs.FULL)
+    d_out = w.empty(mrhs.FULL)
+    w.apply(d_in, d_out)
+    torch.cuda.synchronize()
+    t_lex = torch.from_numpy(lex).cuda()
+    got = w.export_field(d_out, mrhs.FULL)[t_lex].cpu().numpy()
+    del d_in, d_out
+    links, nbrs = _gather_hop_inputs(DIMS, U, psi, lex, cb=False)
+    C = _clover_at(U.cpu().numpy().astype(np.complex128), lex)
+    want = oracle.mooee(C, psi[t_lex].cpu().numpy()) - 0.5 * oracle.dhop_sites(links, nbrs)
     err = rel_l2_per_rhs(got, want)
     assert err.max() < TOL, err
