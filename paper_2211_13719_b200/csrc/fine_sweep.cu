@@ -1,22 +1,32 @@
-// fine_sweep.cu -- slice-sweep variant of the fine-level hopping kernel:
+// fine_sweep.cu -- slice-sweep kernel of the fine-level hopping term:
 //   out(x) = sum_mu (1-gamma_mu) U_mu(x) in(x+mu) + (1+gamma_mu) U_mu(x-mu)^+ in(x-mu)
 // (reading S3) for N_rhs right-hand sides at once, D_hop and M_eooe from one body with
 // different index maps ("different site ordering").
 //
-// Why a second kernel: ncu shows the gather kernel of fine_hop.cu at the L2 -> SM crossbar limit
-// (12.2 TB/s), not at the HBM limit: every neighbour spinor is fetched from L2 again by each of its
-// eight users.  Here a thread block owns a tile of XB x 2 x 2 sites in (x,y,z) and sweeps a segment
-// of t, and every operand of a step is staged in shared memory once:
-//   * tile rows of the current slice and the links: cp.async.bulk by a producer warp, double buffered,
-//     completion on mbarriers (the only block-wide synchronisation of a step);
-//   * the +t hop reads the next slice, which is resident already because it is the next centre slice;
-//   * the -t hop of slice s+1 is computed while slice s is the centre and carried in registers (it is
-//     the initial value of the next accumulator), so no slice is loaded twice along t;
-//   * y, z and x halo neighbours: every thread owns a private shared-memory slot per direction and
-//     refills it itself with 16-byte cp.async right after reading it, for the next slice; only that
-//     thread ever touches the slot, so cp.async.wait_group is all the synchronisation it needs.
-// One thread still owns one output site and one RHS pair (FFMA2 lanes); links are broadcast reads.
+// A thread block owns a tile of XB x 2 x 2 sites in (x,y,z) and sweeps a segment of t.  Every operand of a
+// step (one t-slice of the tile) is staged in shared memory once, by a producer warp, with TMA bulk copies that
+// complete on mbarriers:
+//   * the four tile rows (double buffered: the +t hop reads the next slice, which is the next centre slice);
+//   * the eight halo rows in y and z (the rows of the neighbouring tiles; single buffered, released right after
+//     the y / z hops so that they are refilled while the rest of the step runs);
+//   * the links of the output sites and 640-byte windows of the backward links (double buffered), and for the
+//     fused epilogues the packed clover blocks;
+//   * only the x halo (one site on each side of the x-block) is fetched by the threads themselves, with 16-byte
+//     cp.async into slots that only the fetching thread reads.
+// The -t hop of slice s+1 is computed while slice s is the centre and carried in registers as a half spinor,
+// so no slice is loaded twice along t.
+//
+// Work split: a "unit" is one site and one pair of right-hand sides (the two lanes of FFMA2 / FADD2, links are
+// the broadcast scalar operand).  The two half-warps of a warp split a unit by the spin row of the projected
+// half spinor: lanes 0-15 own h_0, lanes 16-31 own h_1 of the same sixteen units.  Each computes its row of
+// (1 -+ gamma_mu) psi, the SU(3) product on it and its share of the reconstruction (9 complex accumulators instead
+// of 12), and the halves meet in warp shuffles before the store.  The code is the same for both halves: which
+// spin rows a lane reads is an address offset, and the two sign flips that depend on the spin row are the
+// scalar operand e = +-1 of an FFMA2 that replaces an FADD2.  Twelve consumer warps per block (three per SM
+// sub-partition) instead of six with twice the registers: balanced sub-partitions and enough warps to cover
+// shared-memory latency without register double buffering.
 #include "fine_sweep.cuh"
+#include "async_copy.cuh"
 #include "hop_math.cuh"
 
 namespace mrhs {
@@ -24,100 +34,136 @@ namespace mrhs {
 namespace {
 
 constexpr int BY = kSweepBY, BZ = kSweepBZ, ROWS = kSweepRows;
-static_assert(BY == 2 && BZ == 2, "every thread has exactly one halo neighbour in y and one in z");
-
-__device__ __forceinline__ uint32_t s_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void bar_init(uint64_t *bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(s_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void bar_expect_tx(uint64_t *bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(s_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bar_arrive(uint64_t *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void bar_wait(uint64_t *bar, unsigned parity) {
-    uint32_t ok;
-    do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(ok)
-                     : "r"(s_u32(bar)), "r"(parity)
-                     : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(s_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(s_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_prefetch_l2(const void *src, unsigned bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
-}
-// 16 bytes global -> shared, asynchronously, bypassing L1 (no reuse on this SM)
-__device__ __forceinline__ void cp16(const float4 *dst_smem, const float4 *src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s_u32(dst_smem)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-__device__ __forceinline__ void zero_acc(CVec<2> (&acc)[12]) {
-#pragma unroll
-    for (int c = 0; c < 12; c++) acc[c] = czero<2>();
-}
+static_assert(BY == 2 && BZ == 2, "every tile row has exactly one halo row in y and one in z");
 
 // Byte sizes of the shared-memory regions for a layout block of XB sites and NP RHS pairs.
 struct SweepSmem {
     uint32_t RB, GO, GW, GROW;              // tile row, own links of a row, one link window, all links of one row
     uint32_t I_BYTES, G_BYTES;              // per buffer (two buffers each)
-    uint32_t H_BYTES, XH_BYTES;             // thread-private halo slots: y and z (every thread), x (edge threads)
-    uint32_t C_BYTES;                       // packed clover blocks of the tile rows (fused M_ooee epilogue), per buffer
+    uint32_t H_BYTES, XH_BYTES;             // halo rows in y and z (ROWS each); x halo slots [side][row][component][pair]
+    uint32_t C_BYTES;                       // packed clover blocks of the tile rows (fused epilogues), per buffer
     uint32_t off_G, off_H, off_XH, off_C, off_bar, total;
-    __host__ __device__ SweepSmem(int XB, int NP) {
+    __host__ __device__ SweepSmem(int XB, int NP, bool clov) {
         RB = 12u * XB * NP * 16u;
         GO = 18u * XB * 16u;
         GW = 5u * XB * 16u;
         GROW = GO + 5u * GW;
         I_BYTES = ROWS * RB;
         G_BYTES = ROWS * GROW;
-        H_BYTES = 2u * ROWS * RB;           // 2 slots x 12 components x (ROWS XB NP) threads x 16 bytes
+        H_BYTES = 2u * ROWS * RB;
         XH_BYTES = 2u * ROWS * 12u * NP * 16u;
         off_G = 2u * I_BYTES;
         off_H = off_G + 2u * G_BYTES;
         off_XH = off_H + H_BYTES;
-        C_BYTES = ROWS * GO;
+        C_BYTES = clov ? ROWS * GO : 0u;
         off_C = off_XH + XH_BYTES;
         off_bar = off_C + 2u * C_BYTES;
-        total = off_bar + 64u;
+        total = off_bar + 128u;
     }
 };
 
-// A neighbour's position in shared memory, in float4 units: component 0 of this thread's element, what to add
-// for buffer 1, and the component stride.
-struct Nbr {
-    int o, bs, cs;
+__device__ __forceinline__ CVec<2> shfl_half(CVec<2> v) {
+    CVec<2> r;
+    r.re.v = __shfl_xor_sync(0xffffffffu, v.re.v, 16);
+    r.im.v = __shfl_xor_sync(0xffffffffu, v.im.v, 16);
+    return r;
+}
+__device__ __forceinline__ CVec<2> csel(bool take_a, CVec<2> a, CVec<2> b) {
+    CVec<2> r;
+    r.re.v = take_a ? a.re.v : b.re.v;
+    r.im.v = take_a ? a.im.v : b.im.v;
+    return r;
+}
+
+// Operands of one hop for this lane: its own spin row of the neighbour (ps), the partner row the projector
+// combines it with (pp), and the link.
+struct SplitOperands {
+    float4 ps[3], pp[3];
+    float u[18];
 };
 
-// out = C in for the two packed Hermitian 6x6 blocks of one site (6 real diagonals + 15 complex lower-triangle entries
-// each, reading S7); pc: float4 0 of the site's 72 packed floats (stride XB), broadcast reads from shared memory
-__device__ __forceinline__ void clover_mul(const float4 *pc, int XB, const CVec<2> (&in)[12], CVec<2> (&out)[12]) {
+// nbs / nbp: float4 index of colour 0 of the two spin rows; st: component stride; g: float4 0 of the link's site data
+template <int MU>
+__device__ __forceinline__ void split_load(SplitOperands &o, const float4 *S, int nbs, int nbp, int st, const float4 *g, int XB) {
 #pragma unroll
-    for (int ch = 0; ch < 2; ch++) {
-        float a[36];
+    for (int c = 0; c < 3; c++) {
+        o.ps[c] = S[nbs + c * st];
+        o.pp[c] = S[nbp + c * st];
+    }
+    load_link_s<MU>(g, XB, o.u);
+}
+
+// This lane's row of the projected half spinor and of r = U h (FWD) or U^+ h.  Spin row s (e = +1 for s = 0, -1 for s = 1):
+//   x: h_s = psi_s + S i psi_{3-s}     y: h_s = psi_s + e S psi_{3-s}     z: h_s = psi_s + e S i psi_{2+s}     t: h_s = psi_s - S psi_{2+s}
+// with S = +1 for the forward hop (reading S2/S3, the rows of hop_half in hop_math.cuh).
+template <int MU, bool FWD>
+__device__ __forceinline__ void split_half(const SplitOperands &o, float e, CVec<2> (&r)[3]) {
+    const float sg = FWD ? e : -e;
+    CVec<2> h[3];
 #pragma unroll
-        for (int j = 0; j < 9; j++) {
-            const float4 v = pc[(9 * ch + j) * XB];
-            a[4 * j] = v.x; a[4 * j + 1] = v.y; a[4 * j + 2] = v.z; a[4 * j + 3] = v.w;
+    for (int c = 0; c < 3; c++) {
+        const CVec<2> a = to_cvec(o.ps[c]), b = to_cvec(o.pp[c]);
+        if constexpr (MU == 0) h[c] = FWD ? cadd_i(a, b) : csub_i(a, b);
+        else if constexpr (MU == 1) h[c] = rfma(sg, b, a);
+        else if constexpr (MU == 2) { h[c].re = sfnma(sg, b.im, a.re); h[c].im = sfma(sg, b.re, a.im); }
+        else h[c] = FWD ? csub(a, b) : cadd(a, b);
+    }
+    const float (&u)[18] = o.u;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        if constexpr (FWD) {
+            CVec<2> t = cmul(u[2 * (3 * c + 0)], u[2 * (3 * c + 0) + 1], h[0]);
+            t = cfma(u[2 * (3 * c + 1)], u[2 * (3 * c + 1) + 1], h[1], t);
+            r[c] = cfma(u[2 * (3 * c + 2)], u[2 * (3 * c + 2) + 1], h[2], t);
+        } else {
+            CVec<2> t = cmul_conj(u[2 * (0 + c)], u[2 * (0 + c) + 1], h[0]);
+            t = cfma_conj(u[2 * (3 + c)], u[2 * (3 + c) + 1], h[1], t);
+            r[c] = cfma_conj(u[2 * (6 + c)], u[2 * (6 + c) + 1], h[2], t);
         }
+    }
+}
+
+// This lane's share of the reconstruction: up (output spin row s) += r; the lower rows get
+//   x: out_{3-s} -= S i r     y: out_{3-s} += e S r     (accumulated in la)
+//   z: out_{2+s} -= e S i r   t: out_{2+s} -= S r       (accumulated in lb)
+template <int MU, bool FWD>
+__device__ __forceinline__ void split_recon(const CVec<2> (&r)[3], float e, CVec<2> (&up)[3], CVec<2> (&la)[3], CVec<2> (&lb)[3]) {
+    const float sg = FWD ? e : -e;
 #pragma unroll
-        for (int i = 0; i < 6; i++) {
-            CVec<2> v = rmul(a[i], in[6 * ch + i]);
+    for (int c = 0; c < 3; c++) {
+        up[c] = cadd(up[c], r[c]);
+        if constexpr (MU == 0) la[c] = FWD ? csub_i(la[c], r[c]) : cadd_i(la[c], r[c]);
+        else if constexpr (MU == 1) la[c] = rfma(sg, r[c], la[c]);
+        else if constexpr (MU == 2) { lb[c].re = sfma(sg, r[c].im, lb[c].re); lb[c].im = sfnma(sg, r[c].re, lb[c].im); }
+        else lb[c] = FWD ? csub(lb[c], r[c]) : cadd(lb[c], r[c]);
+    }
+}
+
+template <int MU, bool FWD>
+__device__ __forceinline__ void split_hop(const SplitOperands &o, float e, CVec<2> (&up)[3], CVec<2> (&la)[3], CVec<2> (&lb)[3]) {
+    CVec<2> r[3];
+    split_half<MU, FWD>(o, e, r);
+    split_recon<MU, FWD>(r, e, up, la, lb);
+}
+
+// out = C v for ONE packed Hermitian 6x6 block (6 real diagonals + 15 complex lower-triangle entries, reading S7);
+// pc: float4 0 of the block for this site (stride XB), broadcast reads from shared memory
+__device__ __forceinline__ void clover_block_mul(const float4 *pc, int XB, const CVec<2> (&v)[6], CVec<2> (&out)[6]) {
+    float a[36];
 #pragma unroll
-            for (int j = 0; j < 6; j++) {
-                if (j < i) v = cfma(a[6 + 2 * (i * (i - 1) / 2 + j)], a[6 + 2 * (i * (i - 1) / 2 + j) + 1], in[6 * ch + j], v);
-                else if (j > i) v = cfma_conj(a[6 + 2 * (j * (j - 1) / 2 + i)], a[6 + 2 * (j * (j - 1) / 2 + i) + 1], in[6 * ch + j], v);
-            }
-            out[6 * ch + i] = v;
+    for (int j = 0; j < 9; j++) {
+        const float4 w = pc[j * XB];
+        a[4 * j] = w.x; a[4 * j + 1] = w.y; a[4 * j + 2] = w.z; a[4 * j + 3] = w.w;
+    }
+#pragma unroll
+    for (int i = 0; i < 6; i++) {
+        CVec<2> t = rmul(a[i], v[i]);
+#pragma unroll
+        for (int j = 0; j < 6; j++) {
+            if (j < i) t = cfma(a[6 + 2 * (i * (i - 1) / 2 + j)], a[6 + 2 * (i * (i - 1) / 2 + j) + 1], v[j], t);
+            else if (j > i) t = cfma_conj(a[6 + 2 * (j * (j - 1) / 2 + i)], a[6 + 2 * (j * (j - 1) / 2 + i) + 1], v[j], t);
         }
+        out[i] = t;
     }
 }
 
@@ -125,22 +171,23 @@ __device__ __forceinline__ void clover_mul(const float4 *pc, int XB, const CVec<
 //   0: out = H                                  D_hop, M_eooe
 //   1: out = C H                                 M_ooee M_eooe, the first two steps of the Schur sequence (row a7), checkerboarded
 //   2: out = C in - H / 2                        the full Wilson-clover matrix M (reading S6), full lattice: the centre
-//                                                slice holds in(x) itself, so C in(x) is formed first and the hops add to it
+//                                                slice in shared memory holds in(x) itself
 template <int XB_, int NP_, bool CB, int EPI>
-__global__ void __launch_bounds__(224, 1)
+__global__ void __launch_bounds__(kSweepMaxThreads, 1)
 hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__restrict__ out) {
-    const int XB = XB_ ? XB_ : p.XB;
-    const int NP = NP_ ? NP_ : p.NP;
-    const int cs = XB * NP;
-    const SweepSmem L(XB, NP);
-    extern __shared__ __align__(128) unsigned char smem[];
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + L.off_bar);
-    uint64_t *fullI = bars, *freeI = bars + 2, *freeG = bars + 4, *fullG = bars + 6;
-
     constexpr bool CLOV = EPI != 0;
     static_assert(EPI == 0 || (EPI == 1 && CB) || (EPI == 2 && !CB), "fused epilogues: C H on checkerboarded fields, C in - H/2 on the full lattice");
-    const int tid = threadIdx.x;
-    const int NC = ROWS * cs, NCpad = (NC + 31) & ~31;
+    const int XB = XB_ ? XB_ : p.XB;
+    const int NP = NP_ ? NP_ : p.NP;
+    const int cs = XB * NP;                       // units (site, RHS pair) per tile row = elements of one row component
+    const int WPR = (cs + 15) >> 4;               // consumer warps per tile row: sixteen units x two spin rows each
+    const int NWC = ROWS * WPR;
+    const SweepSmem L(XB, NP, CLOV);
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + L.off_bar);
+    uint64_t *fullI = bars, *freeI = bars + 2, *fullG = bars + 4, *freeG = bars + 6, *fullH = bars + 8, *freeH = bars + 10;
+
+    const int tid = threadIdx.x, wid = tid >> 5, lane = tid & 31;
     const int Y = p.Y, Z = p.Z, T = p.T, nxb = p.nxb, lt = p.lt;
 
     // block -> (x-block, tile, t-segment): x-blocks fastest, then the tiles of a chunk, then segments, then chunks
@@ -153,11 +200,12 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     const int y0 = (int)(chy * p.cy + yc) * BY, z0 = (int)(chz * p.cz + zc) * BZ, t0 = (int)seg * lt;
 
     if (tid == 0) {
-        bar_init(&fullI[0], 1); bar_init(&fullI[1], 1);
-        bar_init(&freeI[0], NC); bar_init(&freeI[1], NC);
-        bar_init(&freeG[0], NC); bar_init(&freeG[1], NC);
-        bar_init(&fullG[0], 1); bar_init(&fullG[1], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        for (int i = 0; i < 2; i++) {
+            mbar_init(&fullI[i], 1); mbar_init(&freeI[i], NWC);
+            mbar_init(&fullG[i], 2); mbar_init(&freeG[i], NWC);
+            mbar_init(&fullH[i], 1); mbar_init(&freeH[i], NWC);
+        }
+        mbar_fence_init();
     }
     __syncthreads();
 
@@ -166,117 +214,167 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     auto wrap = [](int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); };
     const int xbm = xb == 0 ? nxb - 1 : (int)xb - 1, xbp = (int)xb + 1 == nxb ? 0 : (int)xb + 1;
 
-    if (tid >= NCpad) {
-        // ------------------------------------------------------------------ producer warp
-        // slice j of the segment (j = -1 .. lt): the tile rows; for 0 <= j < lt also the links; for j = -1 the t-links
-        const int lane = tid - NCpad;
-        auto issue_rows = [&](int j) {
-            const int t = tw(j);
-            const uint32_t b = (uint32_t)(j + 1) & 1u;
-            const bool mid = j >= 0 && j < lt;
-            if (lane == 0) bar_expect_tx(&fullI[b], L.I_BYTES);
-            __syncwarp();
-            unsigned char *Ib = smem + b * L.I_BYTES;
-            if (lane < ROWS) {
-                const int ty = lane % BY, tz = lane / BY;
-                bulk_g2s(Ib + lane * L.RB, in + blk(xb, y0 + ty, z0 + tz, t) * 12 * cs, L.RB, &fullI[b]);
-            }
-            // ask for the rows of a later slice to be brought into L2 now, so that their copy hits L2
-            const int jp = j + p.pf;
-            if (p.pf > 0 && jp <= lt && lane < 2 * ROWS) {
-                const int r = lane % ROWS, tp = tw(jp);
-                const size_t bb = blk(xb, y0 + r % BY, z0 + r / BY, tp);
-                if (lane < ROWS) bulk_prefetch_l2(in + bb * 12 * cs, L.RB);
-                else if (jp < lt) bulk_prefetch_l2(p.gauge_out + bb * kSiteF4 * XB, L.GO);
-            }
+    if (wid >= NWC) {
+        // ------------------------------------------------------------------ producer warps
+        warpgroup_reg_dec<kSweepProducerRegs>();
+        // Four warps, each with its own wait / issue loop so that a late release of one region never delays the copies
+        // into another: warp NWC the tile rows, NWC + 1 the halo rows, NWC + 2 and NWC + 3 the links of two tile rows each.
+        // slice j of the segment (j = -1 .. lt): the tile rows; for 0 <= j < lt also the halo rows and the links; for j = -1 the t-links
+        const int role = wid - NWC;
+        auto halo_yz = [&](int h, int &yy, int &zz) {      // h < ROWS: y halo of tile row h; else z halo of tile row h - ROWS
+            const int r = h % ROWS, ty = r % BY, tz = r / BY;
+            yy = y0 + ty; zz = z0 + tz;
+            if (h < ROWS) yy = ty == 0 ? wrap(y0 - 1, Y) : wrap(y0 + BY, Y);
+            else zz = tz == 0 ? wrap(z0 - 1, Z) : wrap(z0 + BZ, Z);
         };
-        auto issue_links = [&](int j) {
-            const int t = tw(j);
-            const uint32_t b = (uint32_t)(j + 1) & 1u;
-            const bool mid = j >= 0 && j < lt;
-            constexpr int NG = CB ? 6 : 4;   // link copies per row: on the full lattice U_x and U_t of the input row are the own links
-            unsigned char *Gb = smem + L.off_G + b * L.G_BYTES;
-            if (mid || j == -1) {
-                if (lane == 0) bar_expect_tx(&fullG[b], mid ? ROWS * (L.GO + (NG - 1) * L.GW + (CLOV ? L.GO : 0u)) : ROWS * (CB ? L.GW : L.GO));
+        if (role == 0) {
+            auto issue_rows = [&](int j) {
+                const int t = tw(j);
+                const uint32_t b = (uint32_t)(j + 1) & 1u;
+                if (lane == 0) mbar_expect_tx(&fullI[b], L.I_BYTES);
                 __syncwarp();
-                for (int idx = lane; idx < ROWS * 6; idx += 32) {
-                    const int r = idx / 6, w = idx - r * 6;
-                    if (!CB && (w == 1 || w == 5)) continue;
-                    if (j == -1 && w != (CB ? 5 : 0)) continue;
-                    const int y = y0 + r % BY, z = z0 + r / BY;
-                    unsigned char *dst = Gb + r * L.GROW;
-                    const float4 *src;
-                    uint32_t bytes = L.GW;
-                    switch (w) {
-                        case 0: src = p.gauge_out + blk(xb, y, z, t) * kSiteF4 * XB; bytes = L.GO; break;                       // own links
-                        case 1: src = p.gauge_in + blk(xb, y, z, t) * kSiteF4 * XB; dst += L.GO; break;                        // U_x at the -x neighbours in this x-block
-                        case 2: src = p.gauge_in + blk(xbm, y, z, t) * kSiteF4 * XB; dst += L.GO + L.GW; break;                // ... and in the x-block before it
-                        case 3: src = p.gauge_in + (blk(xb, wrap(y - 1, Y), z, t) * kSiteF4 + 4) * XB; dst += L.GO + 2 * L.GW; break;   // U_y at y-1
-                        case 4: src = p.gauge_in + (blk(xb, y, wrap(z - 1, Z), t) * kSiteF4 + 9) * XB; dst += L.GO + 3 * L.GW; break;   // U_z at z-1
-                        default: src = p.gauge_in + (blk(xb, y, z, t) * kSiteF4 + 13) * XB; dst += L.GO + 4 * L.GW; break;     // U_t of the input row (carry)
+                if (lane < ROWS) bulk_g2s(smem + b * L.I_BYTES + lane * L.RB, in + blk(xb, y0 + lane % BY, z0 + lane / BY, t) * 12 * cs, L.RB, &fullI[b]);
+                // ask for the rows and links of a later slice to be brought into L2 now, so that their copy hits L2
+                const int jp = j + p.pf;
+                if (p.pf > 0 && jp <= lt && lane >= ROWS && lane < 3 * ROWS) {
+                    const int q = lane - ROWS, rr = q % ROWS, tp = tw(jp);
+                    const size_t bb = blk(xb, y0 + rr % BY, z0 + rr / BY, tp);
+                    if (q < ROWS) bulk_prefetch_l2(in + bb * 12 * cs, L.RB);
+                    else if (jp < lt) {
+                        bulk_prefetch_l2(p.gauge_out + bb * kSiteF4 * XB, L.GO);
+                        if (CB) bulk_prefetch_l2(p.gauge_in + bb * kSiteF4 * XB, L.GO);      // the backward links live on the input sites
                     }
-                    bulk_g2s(dst, src, bytes, &fullG[b]);
                 }
-                if (CLOV && mid && lane >= 32 - ROWS) {
-                    const int r = lane - (32 - ROWS);
-                    bulk_g2s(smem + L.off_C + b * L.C_BYTES + r * L.GO, p.clover + blk(xb, y0 + r % BY, z0 + r / BY, t) * kSiteF4 * XB, L.GO, &fullG[b]);
-                }
+            };
+            issue_rows(-1);
+            issue_rows(0);
+            for (int k = -1; k + 2 <= lt; k++) {
+                mbar_wait(&freeI[(k + 1) & 1], ((uint32_t)(k + 1) >> 1) & 1u);   // the consumers are done with the rows of slice k
+                issue_rows(k + 2);
             }
-        };
-        issue_rows(-1); issue_links(-1);
-        issue_rows(0); issue_links(0);
-        for (int k = -1; k + 2 <= lt; k++) {
-            const uint32_t par = ((uint32_t)(k + 1) >> 1) & 1u;
-            bar_wait(&freeI[(k + 1) & 1], par);   // the consumers are done with the rows of slice k (after its x hops)
-            issue_rows(k + 2);
-            bar_wait(&freeG[(k + 1) & 1], par);   // ... and with its links (end of the step)
-            issue_links(k + 2);
+        } else if (role == 1) {
+            auto issue_halo = [&](int j, int d) {     // d = 0: the y halo rows of slice j, d = 1: the z halo rows
+                const int t = tw(j);
+                if (lane == 0) mbar_expect_tx(&fullH[d], ROWS * L.RB);
+                __syncwarp();
+                if (lane < ROWS) {
+                    int yy, zz;
+                    halo_yz(d * ROWS + lane, yy, zz);
+                    bulk_g2s(smem + L.off_H + (d * ROWS + lane) * L.RB, in + blk(xb, yy, zz, t) * 12 * cs, L.RB, &fullH[d]);
+                }
+                const int jp = j + p.pf;
+                if (p.pf > 0 && jp < lt && lane >= ROWS && lane < 2 * ROWS) {
+                    int yy, zz;
+                    halo_yz(d * ROWS + lane - ROWS, yy, zz);
+                    bulk_prefetch_l2(in + blk(xb, yy, zz, tw(jp)) * 12 * cs, L.RB);
+                }
+            };
+            issue_halo(0, 0);
+            issue_halo(0, 1);
+            for (int k = 0; k + 1 < lt; k++) {
+                mbar_wait(&freeH[0], (uint32_t)k & 1u); issue_halo(k + 1, 0);   // the consumers are done with the y hops of slice k
+                mbar_wait(&freeH[1], (uint32_t)k & 1u); issue_halo(k + 1, 1);   // ... and with its z hops
+            }
+        } else {
+            // two link warps, tile rows [0, ROWS/2) and [ROWS/2, ROWS): each announces its own bytes on the common barrier
+            const int r_lo = (role - 2) * (ROWS / 2);
+            auto issue_links = [&](int j) {
+                const int t = tw(j);
+                const uint32_t b = (uint32_t)(j + 1) & 1u;
+                const bool mid = j >= 0 && j < lt;
+                // link copies per row: on the full lattice U_x and U_t of the input row are the own links
+                constexpr int NG = CB ? 6 : 4;
+                unsigned char *Gb = smem + L.off_G + b * L.G_BYTES;
+                if (mid || j == -1) {
+                    if (lane == 0) mbar_expect_tx(&fullG[b], mid ? (ROWS / 2) * (L.GO + (NG - 1) * L.GW + (CLOV ? L.GO : 0u)) : (ROWS / 2) * (CB ? L.GW : L.GO));
+                    __syncwarp();
+                    for (int idx = lane; idx < (ROWS / 2) * 6; idx += 32) {
+                        const int r = r_lo + idx / 6, w = idx % 6;
+                        if (!CB && (w == 1 || w == 5)) continue;
+                        if (j == -1 && w != (CB ? 5 : 0)) continue;
+                        const int y = y0 + r % BY, z = z0 + r / BY;
+                        unsigned char *dst = Gb + r * L.GROW;
+                        const float4 *src;
+                        uint32_t bytes = L.GW;
+                        switch (w) {
+                            case 0: src = p.gauge_out + blk(xb, y, z, t) * kSiteF4 * XB; bytes = L.GO; break;                       // own links
+                            case 1: src = p.gauge_in + blk(xb, y, z, t) * kSiteF4 * XB; dst += L.GO; break;                        // U_x at the -x neighbours in this x-block
+                            case 2: src = p.gauge_in + blk(xbm, y, z, t) * kSiteF4 * XB; dst += L.GO + L.GW; break;                // ... and in the x-block before it
+                            case 3: src = p.gauge_in + (blk(xb, wrap(y - 1, Y), z, t) * kSiteF4 + 4) * XB; dst += L.GO + 2 * L.GW; break;   // U_y at y-1
+                            case 4: src = p.gauge_in + (blk(xb, y, wrap(z - 1, Z), t) * kSiteF4 + 9) * XB; dst += L.GO + 3 * L.GW; break;   // U_z at z-1
+                            default: src = p.gauge_in + (blk(xb, y, z, t) * kSiteF4 + 13) * XB; dst += L.GO + 4 * L.GW; break;     // U_t of the input row (carry)
+                        }
+                        bulk_g2s(dst, src, bytes, &fullG[b]);
+                    }
+                    if (CLOV && mid && lane >= 32 - ROWS / 2) {
+                        const int r = r_lo + lane - (32 - ROWS / 2);
+                        bulk_g2s(smem + L.off_C + b * L.C_BYTES + r * L.GO, p.clover + blk(xb, y0 + r % BY, z0 + r / BY, t) * kSiteF4 * XB, L.GO, &fullG[b]);
+                    }
+                }
+            };
+            issue_links(-1);
+            issue_links(0);
+            for (int k = -1; k + 2 < lt; k++) {
+                mbar_wait(&freeG[(k + 1) & 1], ((uint32_t)(k + 1) >> 1) & 1u);   // the consumers are done with the links of slice k (end of the step)
+                issue_links(k + 2);
+            }
         }
         return;
     }
-    if (tid >= NC) return;
 
     // ---------------------------------------------------------------------- consumers
-    int q = tid / NP;
-    const int pair = tid - q * NP;
-    const int r = q / XB, xin = q - r * XB;
+    warpgroup_reg_inc<kSweepConsumerRegs>();
+    const int s = lane >> 4;                          // spin row of the half spinor this lane owns
+    const float e = s ? -1.f : 1.f;
+    const int r = wid / WPR;                          // tile row
+    const int u0 = (wid - r * WPR) * 16 + (lane & 15);
+    const bool live = u0 < cs;                        // lanes past the end of a row repeat unit 0 and store nothing
+    const int u = live ? u0 : 0;                      // unit = element inside a row component
+    const int xin = u / NP, pair = u - xin * NP;
     const int ty = r % BY, tz = r / BY;
     const int y = y0 + ty, z = z0 + tz;
     const float4 *S = reinterpret_cast<const float4 *>(smem);
     const int IB4 = L.I_BYTES / 16, G4 = L.G_BYTES / 16;
-    const int oH = L.off_H / 16, oXH = L.off_XH / 16;
-    const int e = xin * NP + pair;                    // this thread's element inside a row component
     const int rowlen = 12 * cs;
-    // private halo slots: [y | z][component][thread], and for the edge sites of a row [side][row][component][pair]
-    const Nbr hy = {oH + tid, 0, NC}, hz = {oH + 12 * NC + tid, 0, NC};
-    const Nbr hxp = {oXH + ((ROWS + r) * 12) * NP + pair, 0, NP}, hxm = {oXH + (r * 12) * NP + pair, 0, NP};
+    const int oHy = (int)(L.off_H / 16) + r * rowlen + u, oHz = oHy + ROWS * rowlen;
+    const int oXH = L.off_XH / 16;
+    // spin rows this lane reads: its own (s) and the partner row of the projector: 3 - s for x and y, 2 + s for z and t
+    const int rs = 3 * s, ra = 3 * (3 - s), rb = 3 * (2 + s);     // component index of colour 0 of those rows
+    const int os = rs * cs, oa = ra * cs, ob = rb * cs;            // ... and its offset inside a tile row
+    // neighbour positions, float4 index of component 0 of this unit: o for buffer 0, bs to add for buffer 1
+    const int own = r * rowlen + u;
+    const int yp_o = ty == 0 ? own + rowlen : oHy, yp_bs = ty == 0 ? IB4 : 0;
+    const int ym_o = ty == 0 ? oHy : own - rowlen, ym_bs = ty == 0 ? 0 : IB4;
+    const int zp_o = tz == 0 ? own + BY * rowlen : oHz, zp_bs = tz == 0 ? IB4 : 0;
+    const int zm_o = tz == 0 ? oHz : own - BY * rowlen, zm_bs = tz == 0 ? 0 : IB4;
     const bool edge_p = xin + 1 == XB, edge_m = xin == 0;
-    const Nbr own = {r * rowlen + e, IB4, cs};
-    const Nbr yp = ty + 1 < BY ? Nbr{(r + 1) * rowlen + e, IB4, cs} : hy;
-    const Nbr ym = ty > 0 ? Nbr{(r - 1) * rowlen + e, IB4, cs} : hy;
-    const Nbr zp = tz + 1 < BZ ? Nbr{(r + BY) * rowlen + e, IB4, cs} : hz;
-    const Nbr zm = tz > 0 ? Nbr{(r - BY) * rowlen + e, IB4, cs} : hz;
-    const Nbr xps = edge_p ? hxp : Nbr{r * rowlen + e + NP, IB4, cs};
-    const Nbr xms = edge_m ? hxm : Nbr{r * rowlen + e - NP, IB4, cs};
-    // where the halo neighbours live in global memory (slice 0; one slice further is st elements on)
+    const int hxp = oXH + ((ROWS + r) * 12) * NP + pair, hxm = oXH + (r * 12) * NP + pair;
+    // where the x halo lives in global memory (slice 0; one slice further is st elements on)
     const size_t st = (size_t)nxb * Y * Z * 12 * cs;
-    const float4 *gy = in + blk(xb, ty == 0 ? wrap(y - 1, Y) : wrap(y + 1, Y), z, 0) * 12 * cs + e;
-    const float4 *gz = in + blk(xb, y, tz == 0 ? wrap(z - 1, Z) : wrap(z + 1, Z), 0) * 12 * cs + e;
     const float4 *gxp = in + blk(xbp, y, z, 0) * 12 * cs + pair;                      // site 0 of the next x-block
     const float4 *gxm = in + blk(xbm, y, z, 0) * 12 * cs + (XB - 1) * NP + pair;      // last site of the previous one
-    // refill of a private slot for slice tn (every thread for itself)
-    auto refill = [&](const Nbr &slot, const float4 *g, int tn, bool on) {
-        if (on) {
-            const float4 *src = g + st * tn;
-#pragma unroll
-            for (int c = 0; c < 12; c++) cp16(S + slot.o + c * slot.cs, src + (size_t)c * cs);
-        }
-    };
+    // refill of this lane's part of the x halo slots for slice tn: the two spin rows the x hops read
     auto refill_x = [&](int tn, bool active) {
-        const int s = (p.out_parity + y + z + tn) & 1;
-        refill(hxp, gxp, tn, active && edge_p && (!CB || s == 1));
-        refill(hxm, gxm, tn, active && edge_m && (!CB || s == 0));
-        cp_commit();
+        const int sn = (p.out_parity + y + z + tn) & 1;
+        if (active && live) {
+            if (edge_p && (!CB || sn == 1)) {
+                const float4 *src = gxp + st * tn;
+#pragma unroll
+                for (int c = 0; c < 3; c++) {
+                    cp_async16(S + hxp + (rs + c) * NP, src + (size_t)(rs + c) * cs);
+                    cp_async16(S + hxp + (ra + c) * NP, src + (size_t)(ra + c) * cs);
+                }
+            }
+            if (edge_m && (!CB || sn == 0)) {
+                const float4 *src = gxm + st * tn;
+#pragma unroll
+                for (int c = 0; c < 3; c++) {
+                    cp_async16(S + hxm + (rs + c) * NP, src + (size_t)(rs + c) * cs);
+                    cp_async16(S + hxm + (ra + c) * NP, src + (size_t)(ra + c) * cs);
+                }
+            }
+        }
+        cp_async_commit();
     };
     // links (float4 units): row r of the link buffer; windows are addressed through the base of a virtual 18-row site
     const int Gr = (int)(L.off_G / 16) + r * (int)(L.GROW / 16);
@@ -287,98 +385,118 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     const int g_bz = Gr + 33 * XB - 9 * XB + xin;
     const int g_bt = CB ? Gr + 38 * XB - 13 * XB + xin : g_own;
 
-    CVec<2> acc[12];
-    CVec<2> carry[6];      // (1 + gamma_t) U_t^+ psi of the slice before, as a half spinor
-    HopOperands<2> A, B;
+    CVec<2> up[3], la[3], lb[3];   // output spin row s; rows 3 - s (from the x and y hops) and 2 + s (from the z and t hops)
+    CVec<2> carry[3];              // this lane's row of U_t^+ (1 + gamma_t) psi of the slice before
+    SplitOperands A;
 
-    // slice 0's halo neighbours: three groups in the order they are waited for (y, z, x)
-    {
-        const int tn = tw(0);
-        refill(hy, gy, tn, true); cp_commit();
-        refill(hz, gz, tn, true); cp_commit();
-        refill_x(tn, true);
-    }
+    refill_x(tw(0), true);
 
 #pragma unroll 1
     for (int k = -1; k < lt; k++) {
         const int t = tw(k);
         const uint32_t b = (uint32_t)(k + 1) & 1u;
-        bar_wait(&fullI[b], ((uint32_t)(k + 1) >> 1) & 1u);
-        bar_wait(&fullG[b], ((uint32_t)(k + 1) >> 1) & 1u);   // links of slice k, on their own barrier: the +t hop below waits for rows only
+        const int bo = b ? IB4 : 0;
+        mbar_wait(&fullI[b], ((uint32_t)(k + 1) >> 1) & 1u);
+        mbar_wait(&fullG[b], ((uint32_t)(k + 1) >> 1) & 1u);
         const float4 *G = S + b * G4;
-        const float4 *pc = S + L.off_C / 16 + b * (L.C_BYTES / 16) + r * (18 * XB) + xin;   // this site's clover blocks
         if (k >= 0) {
-            if constexpr (EPI == 2) {
-                // acc = -2 C in(x): the hops below add H, and the store scales by -1/2
-                CVec<2> own_psi[12], cpsi[12];
 #pragma unroll
-                for (int c = 0; c < 12; c++) own_psi[c] = to_cvec(S[own.o + b * own.bs + c * own.cs]);
-                clover_mul(pc, XB, own_psi, cpsi);
-#pragma unroll
-                for (int c = 0; c < 12; c++) acc[c] = rmul(-2.f, cpsi[c]);
-            } else {
-                zero_acc(acc);
-            }
-            hop_recon<2, 3, false>(carry, acc);
+            for (int c = 0; c < 3; c++) { up[c] = carry[c]; lb[c] = carry[c]; la[c] = czero<2>(); }    // the -t hop (S = -1): up += r, out_{2+s} += r
         }
         if (k + 1 < lt) {
-            // -t hop of the next slice, first thing, so that the rows of this slice can be released after the x hops:
-            // (1 + gamma_t) U_t(x, t)^+ psi(x, t), both at this thread's own position of slice k
-            hop_load_s<3>(B, S + own.o + b * own.bs, own.cs, G + g_bt, XB);
-            hop_half<2, 3, false>(B, carry);
+            // -t hop of the next slice: U_t(x, t)^+ (1 + gamma_t) psi(x, t), both at this unit's own position of slice k
+            split_load<3>(A, S, own + bo + os, own + bo + ob, cs, G + g_bt, XB);
+            split_half<3, false>(A, e, carry);
         }
         if (k >= 0) {
             const int tn = tw(k + 1);
             const bool more = k + 1 < lt;
-            // x neighbours of this step (checkerboarded lines alternate with t)
-            Nbr xp = xps, xm = xms;
+            // y hops
+            mbar_wait(&fullH[0], (uint32_t)k & 1u);
+            split_load<1>(A, S, yp_o + (yp_bs ? bo : 0) + os, yp_o + (yp_bs ? bo : 0) + oa, cs, G + g_own, XB);
+            split_hop<1, true>(A, e, up, la, lb);
+            split_load<1>(A, S, ym_o + (ym_bs ? bo : 0) + os, ym_o + (ym_bs ? bo : 0) + oa, cs, G + g_by, XB);
+            split_hop<1, false>(A, e, up, la, lb);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&freeH[0]);
+            // z hops
+            mbar_wait(&fullH[1], (uint32_t)k & 1u);
+            split_load<2>(A, S, zp_o + (zp_bs ? bo : 0) + os, zp_o + (zp_bs ? bo : 0) + ob, cs, G + g_own, XB);
+            split_hop<2, true>(A, e, up, la, lb);
+            split_load<2>(A, S, zm_o + (zm_bs ? bo : 0) + os, zm_o + (zm_bs ? bo : 0) + ob, cs, G + g_bz, XB);
+            split_hop<2, false>(A, e, up, la, lb);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&freeH[1]);
+            // x hops (checkerboarded lines alternate with t: one neighbour has this unit's own index, the other is one site on)
+            int xp_o = edge_p ? hxp : own + bo + NP, xp_st = edge_p ? NP : cs;
+            int xm_o = edge_m ? hxm : own + bo - NP, xm_st = edge_m ? NP : cs;
             int g_bx = g_bx_step;
             if (CB) {
-                const int s = (p.out_parity + y + z + t) & 1;
-                if (s) { xm = own; g_bx = g_bx_same; }
-                else xp = own;
+                if ((p.out_parity + y + z + t) & 1) { xm_o = own + bo; xm_st = cs; g_bx = g_bx_same; }
+                else { xp_o = own + bo; xp_st = cs; }
             }
-            cp_wait<2>();                      // this thread's y slot holds slice k
-            hop_load_s<1>(A, S + yp.o + b * yp.bs, yp.cs, G + g_own, XB);
-            hop_load_s<1>(B, S + ym.o + b * ym.bs, ym.cs, G + g_by, XB);
-            hop_compute<2, 1, true >(A, acc);
-            refill(hy, gy, tn, more); cp_commit();
-            cp_wait<2>();                      // z slot
-            hop_load_s<2>(A, S + zp.o + b * zp.bs, zp.cs, G + g_own, XB);
-            hop_compute<2, 1, false>(B, acc);
-            hop_load_s<2>(B, S + zm.o + b * zm.bs, zm.cs, G + g_bz, XB);
-            hop_compute<2, 2, true >(A, acc);
-            refill(hz, gz, tn, more); cp_commit();
-            cp_wait<2>();                      // x slot
-            hop_load_s<0>(A, S + xp.o + b * xp.bs, xp.cs, G + g_own, XB);
-            hop_compute<2, 2, false>(B, acc);
-            hop_load_s<0>(B, S + xm.o + b * xm.bs, xm.cs, G + g_bx, XB);
-            hop_compute<2, 0, true >(A, acc);
+            cp_async_wait<0>();                // this lane's x halo slots hold slice k
+            split_load<0>(A, S, xp_o + rs * xp_st, xp_o + ra * xp_st, xp_st, G + g_own, XB);
+            split_hop<0, true>(A, e, up, la, lb);
+            split_load<0>(A, S, xm_o + rs * xm_st, xm_o + ra * xm_st, xm_st, G + g_bx, XB);
+            split_hop<0, false>(A, e, up, la, lb);
             refill_x(tn, more);
-            hop_compute<2, 0, false>(B, acc);
-            bar_arrive(&freeI[b]);             // rows of slice k are no longer read: slice k+2 may land
-            bar_wait(&fullI[b ^ 1u], ((uint32_t)(k + 2) >> 1) & 1u);   // slice k+1
-            hop_load_s<3>(A, S + own.o + (b ^ 1u) * own.bs, own.cs, G + g_own, XB);
-            hop_compute<2, 3, true >(A, acc);
-            float4 *o = out + (blk(xb, y, z, t) * 12 * XB + xin) * NP + pair;
-            if constexpr (EPI == 1) {
-                CVec<2> res[12];
-                clover_mul(pc, XB, acc, res);
+            if constexpr (EPI != 2) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&freeI[b]);       // rows of slice k are no longer read: slice k+2 may land
+            }
+            // +t hop: the next slice at this unit's own position
+            mbar_wait(&fullI[b ^ 1u], ((uint32_t)(k + 2) >> 1) & 1u);
+            split_load<3>(A, S, own + (IB4 - bo) + os, own + (IB4 - bo) + ob, cs, G + g_own, XB);
+            split_hop<3, true>(A, e, up, la, lb);
+            float4 *o = out + blk(xb, y, z, t) * 12 * cs + u;
+            if constexpr (EPI == 0) {
+                // lane s holds out_s (up), its share of out_{3-s} (la) and the partner's missing share of out_{2+s} (lb)
 #pragma unroll
-                for (int c = 0; c < 12; c++) __stcs(&o[(size_t)c * cs], from_cvec(res[c]));
-            } else if constexpr (EPI == 2) {
+                for (int c = 0; c < 3; c++) la[c] = cadd(la[c], shfl_half(lb[c]));
+                if (live) {
 #pragma unroll
-                for (int c = 0; c < 12; c++) __stcs(&o[(size_t)c * cs], from_cvec(rmul(-0.5f, acc[c])));
+                    for (int c = 0; c < 3; c++) {
+                        __stcs(&o[(size_t)(rs + c) * cs], from_cvec(up[c]));
+                        __stcs(&o[(size_t)(ra + c) * cs], from_cvec(la[c]));
+                    }
+                }
             } else {
+                // gather one chirality per lane: lane s gets spin rows 2s and 2s+1 of H
+                CVec<2> H[6];
 #pragma unroll
-                for (int c = 0; c < 12; c++) __stcs(&o[(size_t)c * cs], from_cvec(acc[c]));
+                for (int c = 0; c < 3; c++) {
+                    const CVec<2> pu = shfl_half(up[c]), pla = shfl_half(la[c]), plb = shfl_half(lb[c]);
+                    H[c] = csel(s != 0, cadd(plb, la[c]), up[c]);          // s = 1: out_2 = lb(lane s=0) + la;  s = 0: out_0
+                    H[3 + c] = csel(s != 0, cadd(pla, lb[c]), pu);         // s = 1: out_3 = la(lane s=0) + lb;  s = 0: out_1 (the partner's up)
+                }
+                const float4 *pc = S + L.off_C / 16 + b * (L.C_BYTES / 16) + r * (18 * XB) + 9 * s * XB + xin;   // this site's block of chirality s
+                CVec<2> res[6];
+                if constexpr (EPI == 1) {
+                    clover_block_mul(pc, XB, H, res);
+                } else {
+                    CVec<2> v[6];
+#pragma unroll
+                    for (int i = 0; i < 6; i++) v[i] = to_cvec(S[own + bo + (6 * s + i) * cs]);
+                    clover_block_mul(pc, XB, v, res);
+#pragma unroll
+                    for (int i = 0; i < 6; i++) res[i] = rfma(-0.5f, H[i], res[i]);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&freeI[b]);
+                }
+                if (live) {
+#pragma unroll
+                    for (int i = 0; i < 6; i++) __stcs(&o[(size_t)(6 * s + i) * cs], from_cvec(res[i]));
+                }
             }
         } else {
-            bar_arrive(&freeI[b]);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&freeI[b]);
         }
-        bar_arrive(&freeG[b]);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&freeG[b]);
     }
-    cp_wait<0>();
+    cp_async_wait<0>();
 }
 
 }  // namespace
@@ -388,8 +506,8 @@ bool sweep_supported(const FieldGeom &g) {
     if (g.N & 1) return false;                       // RHS pairs in FFMA2 lanes; bulk copies need 16-byte pieces
     if (g.Y < 2 || g.Z < 2 || (g.Y % BY) || (g.Z % BZ)) return false;
     const int np = threads_per_site(g.N);
-    if (g.XB * np > 48) return false;                // 4 rows of consumers + the producer warp fit 224 threads
-    const SweepSmem L(g.XB, np);
+    if (g.XB * np > 48) return false;                // three consumer warps per tile row, twelve per block, plus the producer warps
+    const SweepSmem L(g.XB, np, true);
     return L.total <= 227u * 1024u;
 }
 
@@ -450,10 +568,11 @@ bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t
     p.gauge_out = p.gauge_in = nullptr;
     p.clover = nullptr;
     p.pf = 2;
-    p.consumers = (unsigned)(ROWS * g.XB * np);
-    p.threads = ((p.consumers + 31u) & ~31u) + 32u;
+    const int wpr = (g.XB * np + 15) / 16;
+    p.threads = (unsigned)(ROWS * wpr + kSweepProducerWarps) * 32u;
     p.grid = (unsigned)grid;
-    p.smem_bytes = SweepSmem(g.XB, np).total;
+    p.smem_bytes = SweepSmem(g.XB, np, false).total;
+    p.smem_bytes_clover = SweepSmem(g.XB, np, true).total;
     return true;
 }
 
@@ -474,9 +593,9 @@ mrhs_status_t sweep_prepare() {
 namespace {
 template <int XB, int NP>
 void launch_sweep_t(const SweepParams &p, const void *d_in, void *d_out, cudaStream_t st) {
-    if (p.cb && p.clover) hop_sweep_kernel<XB, NP, true, 1><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    if (p.cb && p.clover) hop_sweep_kernel<XB, NP, true, 1><<<p.grid, p.threads, p.smem_bytes_clover, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
     else if (p.cb)        hop_sweep_kernel<XB, NP, true, 0><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
-    else if (p.clover)    hop_sweep_kernel<XB, NP, false, 2><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    else if (p.clover)    hop_sweep_kernel<XB, NP, false, 2><<<p.grid, p.threads, p.smem_bytes_clover, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
     else                  hop_sweep_kernel<XB, NP, false, 0><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
 }
 }  // namespace

@@ -3,7 +3,8 @@
 // layouts as fine_hop.cuh; what differs is how the operands reach the SM:
 // a thread block owns a tile of XB x 2 x 2 sites in (x,y,z) and sweeps a segment of t, holding the
 // current t-slice of the tile, its y/z/x halo and the links in shared memory (TMA bulk copies from a
-// producer warp), so every input spinor crosses the L2 -> SM path about 3x instead of 7x.
+// producer warp), so every input spinor crosses the L2 -> SM path about 3x instead of 7x; the two
+// half-warps of a consumer warp split every site by the spin row of the projected half spinor.
 #pragma once
 #include "fine_hop.cuh"
 
@@ -11,6 +12,11 @@ namespace mrhs {
 
 constexpr int kSweepBY = 2, kSweepBZ = 2;        // tile extent in y and z (sites)
 constexpr int kSweepRows = kSweepBY * kSweepBZ;
+constexpr int kSweepProducerWarps = 4;                          // tile rows, halo rows, links (two warps): one warp per stream of bulk copies
+// Four warps per SM sub-partition start with 128 registers; the producer warp group hands most of its share to the three consumer
+// warp groups (3 x 152 + 40 <= 512 per lane of a sub-partition).
+constexpr int kSweepConsumerRegs = 152, kSweepProducerRegs = 40;
+constexpr int kSweepMaxThreads = (kSweepRows * 3 + 4) * 32;   // three consumer warps per tile row, the producer warps, rounded to four warps per SM sub-partition (128 registers)
 
 struct SweepTiling {
     int lt;          // t-slices one thread block sweeps (divides T)
@@ -28,8 +34,8 @@ struct SweepParams {
     const float4 *gauge_out;      // links on the sites of the output field, [block][18][xin] float4
     const float4 *gauge_in;       // links on the sites of the input field
     const float4 *clover;         // packed clover blocks on the sites of the output field: non-null => out = C H (checkerboarded) or C in - H/2 (full lattice)
-    unsigned grid, threads, consumers;
-    unsigned smem_bytes;
+    unsigned grid, threads;
+    unsigned smem_bytes, smem_bytes_clover;   // dynamic shared memory without / with the clover blocks of the fused epilogues
 };
 
 // true if the sweep kernel can run this geometry (even N_rhs, shared memory fits)
