@@ -82,13 +82,14 @@ struct SplitOperands {
     float u[18];
 };
 
-// nbs / nbp: float4 index of colour 0 of the two spin rows; st: component stride; g: float4 0 of the link's site data
+// nb: component 0 of the neighbour's element for this unit; os / op: offsets of colour 0 of the two spin rows; st: component
+// stride; g: float4 0 of the link's site data
 template <int MU>
-__device__ __forceinline__ void split_load(SplitOperands &o, const float4 *S, int nbs, int nbp, int st, const float4 *g, int XB) {
+__device__ __forceinline__ void split_load(SplitOperands &o, const float4 *nb, int os, int op, int st, const float4 *g, int XB) {
 #pragma unroll
     for (int c = 0; c < 3; c++) {
-        o.ps[c] = S[nbs + c * st];
-        o.pp[c] = S[nbp + c * st];
+        o.ps[c] = nb[os + c * st];
+        o.pp[c] = nb[op + c * st];
     }
     load_link_s<MU>(g, XB, o.u);
 }
@@ -349,33 +350,6 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     const int zm_o = tz == 0 ? oHz : own - BY * rowlen, zm_bs = tz == 0 ? 0 : IB4;
     const bool edge_p = xin + 1 == XB, edge_m = xin == 0;
     const int hxp = oXH + ((ROWS + r) * 12) * NP + pair, hxm = oXH + (r * 12) * NP + pair;
-    // where the x halo lives in global memory (slice 0; one slice further is st elements on)
-    const size_t st = (size_t)nxb * Y * Z * 12 * cs;
-    const float4 *gxp = in + blk(xbp, y, z, 0) * 12 * cs + pair;                      // site 0 of the next x-block
-    const float4 *gxm = in + blk(xbm, y, z, 0) * 12 * cs + (XB - 1) * NP + pair;      // last site of the previous one
-    // refill of this lane's part of the x halo slots for slice tn: the two spin rows the x hops read
-    auto refill_x = [&](int tn, bool active) {
-        const int sn = (p.out_parity + y + z + tn) & 1;
-        if (active && live) {
-            if (edge_p && (!CB || sn == 1)) {
-                const float4 *src = gxp + st * tn;
-#pragma unroll
-                for (int c = 0; c < 3; c++) {
-                    cp_async16(S + hxp + (rs + c) * NP, src + (size_t)(rs + c) * cs);
-                    cp_async16(S + hxp + (ra + c) * NP, src + (size_t)(ra + c) * cs);
-                }
-            }
-            if (edge_m && (!CB || sn == 0)) {
-                const float4 *src = gxm + st * tn;
-#pragma unroll
-                for (int c = 0; c < 3; c++) {
-                    cp_async16(S + hxm + (rs + c) * NP, src + (size_t)(rs + c) * cs);
-                    cp_async16(S + hxm + (ra + c) * NP, src + (size_t)(ra + c) * cs);
-                }
-            }
-        }
-        cp_async_commit();
-    };
     // links (float4 units): row r of the link buffer; windows are addressed through the base of a virtual 18-row site
     const int Gr = (int)(L.off_G / 16) + r * (int)(L.GROW / 16);
     const int g_own = Gr + xin;
@@ -386,115 +360,160 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     const int g_bt = CB ? Gr + 38 * XB - 13 * XB + xin : g_own;
 
     CVec<2> up[3], la[3], lb[3];   // output spin row s; rows 3 - s (from the x and y hops) and 2 + s (from the z and t hops)
-    CVec<2> carry[3];              // this lane's row of U_t^+ (1 + gamma_t) psi of the slice before
+    // this lane's row of U_t^+ (1 + gamma_t) psi of the slice before the centre slice.  The own rows of a slice are read from
+    // shared memory ONCE, when the slice is the +t neighbour, and stay in registers until its links have arrived: both t hops
+    CVec<2> c1[3];
     SplitOperands A;
-
-    refill_x(tw(0), true);
-
-#pragma unroll 1
-    for (int k = -1; k < lt; k++) {
-        const int t = tw(k);
-        const uint32_t b = (uint32_t)(k + 1) & 1u;
-        const int bo = b ? IB4 : 0;
-        mbar_wait(&fullI[b], ((uint32_t)(k + 1) >> 1) & 1u);
-        mbar_wait(&fullG[b], ((uint32_t)(k + 1) >> 1) & 1u);
-        const float4 *G = S + b * G4;
-        if (k >= 0) {
-#pragma unroll
-            for (int c = 0; c < 3; c++) { up[c] = carry[c]; lb[c] = carry[c]; la[c] = czero<2>(); }    // the -t hop (S = -1): up += r, out_{2+s} += r
-        }
-        if (k + 1 < lt) {
-            // -t hop of the next slice: U_t(x, t)^+ (1 + gamma_t) psi(x, t), both at this unit's own position of slice k
-            split_load<3>(A, S, own + bo + os, own + bo + ob, cs, G + g_bt, XB);
-            split_half<3, false>(A, e, carry);
-        }
-        if (k >= 0) {
-            const int tn = tw(k + 1);
-            const bool more = k + 1 < lt;
-            // y hops
-            mbar_wait(&fullH[0], (uint32_t)k & 1u);
-            split_load<1>(A, S, yp_o + (yp_bs ? bo : 0) + os, yp_o + (yp_bs ? bo : 0) + oa, cs, G + g_own, XB);
-            split_hop<1, true>(A, e, up, la, lb);
-            split_load<1>(A, S, ym_o + (ym_bs ? bo : 0) + os, ym_o + (ym_bs ? bo : 0) + oa, cs, G + g_by, XB);
-            split_hop<1, false>(A, e, up, la, lb);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&freeH[0]);
-            // z hops
-            mbar_wait(&fullH[1], (uint32_t)k & 1u);
-            split_load<2>(A, S, zp_o + (zp_bs ? bo : 0) + os, zp_o + (zp_bs ? bo : 0) + ob, cs, G + g_own, XB);
-            split_hop<2, true>(A, e, up, la, lb);
-            split_load<2>(A, S, zm_o + (zm_bs ? bo : 0) + os, zm_o + (zm_bs ? bo : 0) + ob, cs, G + g_bz, XB);
-            split_hop<2, false>(A, e, up, la, lb);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&freeH[1]);
-            // x hops (checkerboarded lines alternate with t: one neighbour has this unit's own index, the other is one site on)
-            int xp_o = edge_p ? hxp : own + bo + NP, xp_st = edge_p ? NP : cs;
-            int xm_o = edge_m ? hxm : own + bo - NP, xm_st = edge_m ? NP : cs;
-            int g_bx = g_bx_step;
-            if (CB) {
-                if ((p.out_parity + y + z + t) & 1) { xm_o = own + bo; xm_st = cs; g_bx = g_bx_same; }
-                else { xp_o = own + bo; xp_st = cs; }
-            }
-            cp_async_wait<0>();                // this lane's x halo slots hold slice k
-            split_load<0>(A, S, xp_o + rs * xp_st, xp_o + ra * xp_st, xp_st, G + g_own, XB);
-            split_hop<0, true>(A, e, up, la, lb);
-            split_load<0>(A, S, xm_o + rs * xm_st, xm_o + ra * xm_st, xm_st, G + g_bx, XB);
-            split_hop<0, false>(A, e, up, la, lb);
-            refill_x(tn, more);
-            if constexpr (EPI != 2) {
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&freeI[b]);       // rows of slice k are no longer read: slice k+2 may land
-            }
-            // +t hop: the next slice at this unit's own position
-            mbar_wait(&fullI[b ^ 1u], ((uint32_t)(k + 2) >> 1) & 1u);
-            split_load<3>(A, S, own + (IB4 - bo) + os, own + (IB4 - bo) + ob, cs, G + g_own, XB);
-            split_hop<3, true>(A, e, up, la, lb);
-            float4 *o = out + blk(xb, y, z, t) * 12 * cs + u;
-            if constexpr (EPI == 0) {
-                // lane s holds out_s (up), its share of out_{3-s} (la) and the partner's missing share of out_{2+s} (lb)
-#pragma unroll
-                for (int c = 0; c < 3; c++) la[c] = cadd(la[c], shfl_half(lb[c]));
-                if (live) {
-#pragma unroll
-                    for (int c = 0; c < 3; c++) {
-                        __stcs(&o[(size_t)(rs + c) * cs], from_cvec(up[c]));
-                        __stcs(&o[(size_t)(ra + c) * cs], from_cvec(la[c]));
-                    }
-                }
-            } else {
-                // gather one chirality per lane: lane s gets spin rows 2s and 2s+1 of H
-                CVec<2> H[6];
+    const float4 *Sown = S + own;
+    // this unit's output element and x halo sources of the current slice, advanced slice by slice
+    const int tfirst = tw(0);
+    float4 *o = out + blk(xb, y, z, tfirst) * 12 * cs + u;
+    const float4 *gxp = in + blk(xbp, y, z, tfirst) * 12 * cs + pair;                      // site 0 of the next x-block
+    const float4 *gxm = in + blk(xbm, y, z, tfirst) * 12 * cs + (XB - 1) * NP + pair;      // last site of the previous one
+    const size_t st = (size_t)nxb * Y * Z * 12 * cs;                                       // one slice further
+    int t = tfirst;                                                                        // the centre slice
+    // refill of this lane's part of the x halo slots from slice pointers gp / gm: the two spin rows the x hops read
+    auto refill_x = [&](const float4 *gp, const float4 *gm, int tn, bool active) {
+        const int sn = (p.out_parity + y + z + tn) & 1;
+        if (active && live) {
+            if (edge_p && (!CB || sn == 1)) {
 #pragma unroll
                 for (int c = 0; c < 3; c++) {
-                    const CVec<2> pu = shfl_half(up[c]), pla = shfl_half(la[c]), plb = shfl_half(lb[c]);
-                    H[c] = csel(s != 0, cadd(plb, la[c]), up[c]);          // s = 1: out_2 = lb(lane s=0) + la;  s = 0: out_0
-                    H[3 + c] = csel(s != 0, cadd(pla, lb[c]), pu);         // s = 1: out_3 = la(lane s=0) + lb;  s = 0: out_1 (the partner's up)
+                    cp_async16(S + hxp + (rs + c) * NP, gp + (size_t)(rs + c) * cs);
+                    cp_async16(S + hxp + (ra + c) * NP, gp + (size_t)(ra + c) * cs);
                 }
-                const float4 *pc = S + L.off_C / 16 + b * (L.C_BYTES / 16) + r * (18 * XB) + 9 * s * XB + xin;   // this site's block of chirality s
-                CVec<2> res[6];
-                if constexpr (EPI == 1) {
-                    clover_block_mul(pc, XB, H, res);
-                } else {
-                    CVec<2> v[6];
+            }
+            if (edge_m && (!CB || sn == 0)) {
 #pragma unroll
-                    for (int i = 0; i < 6; i++) v[i] = to_cvec(S[own + bo + (6 * s + i) * cs]);
-                    clover_block_mul(pc, XB, v, res);
-#pragma unroll
-                    for (int i = 0; i < 6; i++) res[i] = rfma(-0.5f, H[i], res[i]);
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(&freeI[b]);
+                for (int c = 0; c < 3; c++) {
+                    cp_async16(S + hxm + (rs + c) * NP, gm + (size_t)(rs + c) * cs);
+                    cp_async16(S + hxm + (ra + c) * NP, gm + (size_t)(ra + c) * cs);
                 }
-                if (live) {
+            }
+        }
+        cp_async_commit();
+    };
+    refill_x(gxp, gxm, t, true);
+
+    // prologue (slice -1 in buffer 0, slice 0 in buffer 1): the carry of the first step, and the own rows of slice 0 in registers
+    mbar_wait(&fullI[0], 0);
+    mbar_wait(&fullG[0], 0);
+    split_load<3>(A, Sown, os, ob, cs, S + g_bt, XB);
+    split_half<3, false>(A, e, c1);
+    __syncwarp();
+    if (lane == 0) { mbar_arrive(&freeI[0]); mbar_arrive(&freeG[0]); }
+    mbar_wait(&fullI[1], 0);
 #pragma unroll
-                    for (int i = 0; i < 6; i++) __stcs(&o[(size_t)(6 * s + i) * cs], from_cvec(res[i]));
+    for (int c = 0; c < 3; c++) { A.ps[c] = Sown[IB4 + os + c * cs]; A.pp[c] = Sown[IB4 + ob + c * cs]; }
+
+#pragma unroll 1
+    for (int k = 0; k < lt; k++) {
+        const uint32_t b = (uint32_t)(k + 1) & 1u;
+        const int bo = b ? IB4 : 0;
+        const bool more = k + 1 < lt;
+        int tn = t + 1;
+        if (tn == T) tn = 0;
+        mbar_wait(&fullG[b], ((uint32_t)(k + 1) >> 1) & 1u);    // the rows of slice k were waited for as the +t slice of the step before
+        const float4 *G = S + b * G4;
+        const float4 *Sb = S + bo;
+#pragma unroll
+        for (int c = 0; c < 3; c++) { up[c] = c1[c]; lb[c] = c1[c]; la[c] = czero<2>(); }    // the -t hop (S = -1): up += r, out_{2+s} += r
+        if (more) {
+            // A still holds the own rows of this slice (loaded as the +t neighbour of the step before): the -t hop of the next slice
+            load_link_s<3>(G + g_bt, XB, A.u);
+            split_half<3, false>(A, e, c1);
+        }
+        // y hops
+        mbar_wait(&fullH[0], (uint32_t)k & 1u);
+        split_load<1>(A, yp_bs ? Sb + yp_o : S + yp_o, os, oa, cs, G + g_own, XB);
+        split_hop<1, true>(A, e, up, la, lb);
+        split_load<1>(A, ym_bs ? Sb + ym_o : S + ym_o, os, oa, cs, G + g_by, XB);
+        split_hop<1, false>(A, e, up, la, lb);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&freeH[0]);
+        // z hops
+        mbar_wait(&fullH[1], (uint32_t)k & 1u);
+        split_load<2>(A, zp_bs ? Sb + zp_o : S + zp_o, os, ob, cs, G + g_own, XB);
+        split_hop<2, true>(A, e, up, la, lb);
+        split_load<2>(A, zm_bs ? Sb + zm_o : S + zm_o, os, ob, cs, G + g_bz, XB);
+        split_hop<2, false>(A, e, up, la, lb);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&freeH[1]);
+        // x hops (checkerboarded lines alternate with t: one neighbour has this unit's own index, the other is one site on)
+        {
+            const float4 *xp = edge_p ? S + hxp : Sb + own + NP, *xm = edge_m ? S + hxm : Sb + own - NP;
+            int xp_st = edge_p ? NP : cs, xm_st = edge_m ? NP : cs;
+            int g_bx = g_bx_step;
+            if (CB) {
+                if ((p.out_parity + y + z + t) & 1) { xm = Sb + own; xm_st = cs; g_bx = g_bx_same; }
+                else { xp = Sb + own; xp_st = cs; }
+            }
+            cp_async_wait<0>();                // this lane's x halo slots hold slice k
+            split_load<0>(A, xp, rs * xp_st, ra * xp_st, xp_st, G + g_own, XB);
+            split_hop<0, true>(A, e, up, la, lb);
+            split_load<0>(A, xm, rs * xm_st, ra * xm_st, xm_st, G + g_bx, XB);
+            split_hop<0, false>(A, e, up, la, lb);
+        }
+        gxp += st; gxm += st;
+        if (tn == 0) { gxp -= st * T; gxm -= st * T; }
+        refill_x(gxp, gxm, tn, more);
+        if constexpr (EPI != 2) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&freeI[b]);       // rows of slice k are no longer read: slice k+2 may land
+        }
+        // the next slice at this unit's own position: the +t hop of this slice and the -t hop of the slice after the next
+        mbar_wait(&fullI[b ^ 1u], ((uint32_t)(k + 2) >> 1) & 1u);
+        {
+            const float4 *Sn = S + (IB4 - bo) + own;
+#pragma unroll
+            for (int c = 0; c < 3; c++) { A.ps[c] = Sn[os + c * cs]; A.pp[c] = Sn[ob + c * cs]; }
+            load_link_s<3>(G + g_own, XB, A.u);
+            split_hop<3, true>(A, e, up, la, lb);      // A.ps / A.pp stay live: the next step's -t carry is made from them
+        }
+        if constexpr (EPI == 0) {
+            // lane s holds out_s (up), its share of out_{3-s} (la) and the partner's missing share of out_{2+s} (lb)
+#pragma unroll
+            for (int c = 0; c < 3; c++) la[c] = cadd(la[c], shfl_half(lb[c]));
+            if (live) {
+#pragma unroll
+                for (int c = 0; c < 3; c++) {
+                    __stcs(&o[(size_t)(rs + c) * cs], from_cvec(up[c]));
+                    __stcs(&o[(size_t)(ra + c) * cs], from_cvec(la[c]));
                 }
             }
         } else {
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&freeI[b]);
+            // gather one chirality per lane: lane s gets spin rows 2s and 2s+1 of H
+            CVec<2> H[6];
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                const CVec<2> pu = shfl_half(up[c]), pla = shfl_half(la[c]), plb = shfl_half(lb[c]);
+                H[c] = csel(s != 0, cadd(plb, la[c]), up[c]);          // s = 1: out_2 = lb(lane s=0) + la;  s = 0: out_0
+                H[3 + c] = csel(s != 0, cadd(pla, lb[c]), pu);         // s = 1: out_3 = la(lane s=0) + lb;  s = 0: out_1 (the partner's up)
+            }
+            const float4 *pc = S + L.off_C / 16 + b * (L.C_BYTES / 16) + r * (18 * XB) + 9 * s * XB + xin;   // this site's block of chirality s
+            CVec<2> res[6];
+            if constexpr (EPI == 1) {
+                clover_block_mul(pc, XB, H, res);
+            } else {
+                CVec<2> v[6];
+#pragma unroll
+                for (int i = 0; i < 6; i++) v[i] = to_cvec(Sb[own + (6 * s + i) * cs]);
+                clover_block_mul(pc, XB, v, res);
+#pragma unroll
+                for (int i = 0; i < 6; i++) res[i] = rfma(-0.5f, H[i], res[i]);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&freeI[b]);
+            }
+            if (live) {
+#pragma unroll
+                for (int i = 0; i < 6; i++) __stcs(&o[(size_t)(6 * s + i) * cs], from_cvec(res[i]));
+            }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&freeG[b]);
+        o += st;
+        if (tn == 0) o -= st * T;
+        t = tn;
     }
     cp_async_wait<0>();
 }
