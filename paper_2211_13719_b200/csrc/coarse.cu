@@ -8,34 +8,13 @@
 // neighbour vector) signalled on mbarriers.  A thread owns a TI x TP register tile of (rows, RHS
 // pairs) and, for small N_rhs, one of KS slices of the column range; slices are summed through
 // shared memory at the end.
+#include "async_copy.cuh"
 #include "coarse.cuh"
 #include "layout.cuh"
 
 namespace mrhs {
 
 namespace {
-
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
-    uint32_t ok;
-    do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(ok)
-                     : "r"(smem_u32(bar)), "r"(parity)
-                     : "memory");
-    } while (!ok);
-}
 
 template <int R> __device__ __forceinline__ CVec<R> czero_c();
 template <> __device__ __forceinline__ CVec<1> czero_c<1>() { return {{0.f}, {0.f}}; }
@@ -48,14 +27,23 @@ constexpr int largest_ks(int nb, int groups) {
     return best;
 }
 
+// Register tile of (rows, RHS lanes) per thread, chosen from measurements at nbasis 24 / 40: up to
+// N_rhs = 24 the small 2 x 1 tile with many column slices keeps more warps busy per site (few lanes to spread over
+// threads); from N_rhs = 32 the 4-row tile with 2 or 3 lanes (per column 2 + TP shared-memory loads of 16 bytes feed
+// 16 TP FFMA2) relieves the shared-memory pipe, as long as the block keeps at least six warps.
+constexpr int pick_ti(int nb, int np, int r) { return np * r >= 32 || nb * np / 2 > 256 ? 4 : 2; }
+constexpr int pick_tp(int nb, int np, int r) {
+    if (np * r < 32) return (nb * np / 2 > 256 && np % 2 == 0) ? 2 : 1;
+    return (np % 3 == 0 && nb / 4 * (np / 3) >= 192) ? 3 : 2;
+}
+
 template <int NB, int N>
 struct CoarseCfg {
     static constexpr int R = (N % 2 == 0) ? 2 : 1;
     static constexpr int NP = N / R;                       // RHS lanes (elements) per component
-    static constexpr int ITEMS = NB * NP;
-    static constexpr int TP = (ITEMS / 2 > 256 && NP % 2 == 0) ? 2 : 1;
-    static constexpr int TI = (ITEMS / (2 * TP) > 256) ? 4 : 2;
-    static constexpr int NPG = NP / TP;                    // pair groups
+    static constexpr int TI = pick_ti(NB, NP, R);
+    static constexpr int TP = pick_tp(NB, NP, R);
+    static constexpr int NPG = NP / TP;                    // lane groups
     static constexpr int NRG = NB / TI;                    // row groups
     static constexpr int GROUPS = NPG * NRG;
     static constexpr int KS = largest_ks(NB, GROUPS);
@@ -65,7 +53,7 @@ struct CoarseCfg {
     static constexpr int V_BYTES = NB * N * 8;
     static constexpr int STAGE_BYTES = A_BYTES + V_BYTES;
     static constexpr int NSTAGE = STAGE_BYTES < 24 * 1024 ? 4 : 3;
-    static constexpr int RED_BYTES = (KS - 1) * GROUPS * TI * TP * R * 8;
+    static constexpr int RED_BYTES = (KS > 1 ? KS : 0) * GROUPS * TI * TP * R * 8;
     static constexpr int DATA_BYTES = NSTAGE * STAGE_BYTES > RED_BYTES ? NSTAGE * STAGE_BYTES : RED_BYTES;
     static constexpr int SMEM_BYTES = DATA_BYTES + 64;     // + mbarriers
     static_assert(NB % TI == 0 && NP % TP == 0, "tile must divide the site");
@@ -120,7 +108,7 @@ coarse_fma_kernel(int X, int Y, int Z, int T, unsigned mask, const float2 *__res
 
     if (tid == 0) {
         for (int s = 0; s < C::NSTAGE; s++) mbar_init(&full[s], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
     }
     __syncthreads();
     if (tid == 0)
@@ -160,28 +148,25 @@ coarse_fma_kernel(int X, int Y, int Z, int T, unsigned mask, const float2 *__res
         if (tid == 0 && p + C::NSTAGE < npts) issue(p + C::NSTAGE);
     }
 
-    // sum the column slices (the stage ring is free: the last __syncthreads above covers it)
+    // sum the column slices (the stage ring is free: the last __syncthreads above covers it): every slice leaves its tile in
+    // shared memory as [slice][group][TI x TP], then thread e adds element e of all slices in a fixed order and stores it
+    constexpr int TILE = TI * TP, ELEMS = C::GROUPS * TILE;
     if (C::KS > 1) {
         E *red = reinterpret_cast<E *>(smem);
-        if (ks > 0) {
-            E *r = red + ((size_t)(ks - 1) * C::GROUPS + (tid % C::GROUPS)) * (TI * TP);
+        E *r = red + ((size_t)ks * C::GROUPS + (tid % C::GROUPS)) * TILE;
 #pragma unroll
-            for (int i = 0; i < TI; i++)
+        for (int i = 0; i < TI; i++)
 #pragma unroll
-                for (int b = 0; b < TP; b++) r[i * TP + b] = from_cvec(acc[i][b]);
-        }
+            for (int b = 0; b < TP; b++) r[i * TP + b] = from_cvec(acc[i][b]);
         __syncthreads();
-        if (ks == 0) {
-            for (int k = 1; k < C::KS; k++) {
-                const E *r = red + ((size_t)(k - 1) * C::GROUPS + tid) * (TI * TP);
-#pragma unroll
-                for (int i = 0; i < TI; i++)
-#pragma unroll
-                    for (int b = 0; b < TP; b++) acc[i][b] = cadd(acc[i][b], to_cvec(r[i * TP + b]));
-            }
+        for (int e = tid; e < ELEMS; e += C::THREADS) {
+            CVec<R> sum = to_cvec(red[e]);
+            for (int k = 1; k < C::KS; k++) sum = cadd(sum, to_cvec(red[(size_t)k * ELEMS + e]));
+            const int grp = e / TILE, w = e - grp * TILE, i = w / TP, b = w - i * TP;
+            const int epg = grp % C::NPG, erg = grp / C::NPG;
+            out[((size_t)site * NB + erg * TI + i) * C::NP + epg * TP + b] = from_cvec(sum);
         }
-    }
-    if (ks == 0) {
+    } else {
         E *o = out + ((size_t)site * NB + rg * TI) * C::NP + pg * TP;
 #pragma unroll
         for (int i = 0; i < TI; i++)
