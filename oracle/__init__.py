@@ -209,6 +209,20 @@ def coarse_apply(cdims, A, v, pmask=0x1FF):
     return out
 
 
+def coarse_meooe(cdims, A, v_cb, out_parity):
+    """Coarse M_eooe: the 8-point hopping term at the coarse sites of parity
+    out_parity from the sites of the other parity.  A [V][9][nb][nb] (full lattice), v_cb [V/2][nb][N] -> [V/2][nb][N]."""
+    V = volume(cdims)
+    assert all(int(d) % 2 == 0 for d in cdims), "checkerboarded coarse fields need even extents"
+    A = _c128(A); v_cb = _c128(v_cb)
+    nb = A.shape[2]
+    assert A.shape == (V, 9, nb, nb) and v_cb.shape[:2] == (V // 2, nb)
+    N = v_cb.shape[2]
+    out = np.empty_like(v_cb)
+    _load().orc_coarse_meooe(_cdims(cdims), ctypes.c_int(nb), ctypes.c_int(N), _ptr(A), _ptr(v_cb), _ptr(out), ctypes.c_int(out_parity))
+    return out
+
+
 def coarse_sites(A, nbrs):
     """Coarse apply at isolated sites: A [n][9][nb][nb], nbrs [n][9][nb][N] -> [n][nb][N]."""
     A = _c128(A); nbrs = _c128(nbrs)

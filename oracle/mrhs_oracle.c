@@ -408,6 +408,27 @@ void orc_coarse_apply(const int cdims[4], int nb, int N, const dc *A, const dc *
     }
 }
 
+/* Coarse M_eooe ("M_eooe" on the coarse levels): the 8-point hopping term of S8 at
+ * the coarse sites x of parity out_parity only, reading v at sites of the other parity:
+ *   out(x) = sum_{p=1..8} A_p(x) v(x + delta_p),   parity(x) = (x+y+z+t) mod 2.
+ * v_cb [V/2][nb][N] holds the sites of parity 1 - out_parity, out [V/2][nb][N] those of parity out_parity, both ordered by
+ * increasing lex (index lex >> 1; all coarse extents even).  A is the full-lattice link field [V][9][nb][nb]. */
+void orc_coarse_meooe(const int cdims[4], int nb, int N, const dc *A, const dc *v_cb, dc *out, int out_parity)
+{
+    long V = (long)cdims[0] * cdims[1] * cdims[2] * cdims[3];
+#pragma omp parallel for schedule(static)
+    for (long x = 0; x < V; x++) {
+        if (parity_of(cdims, x) != out_parity) continue;
+        const dc *nbr[9];
+        nbr[0] = NULL;                               /* the self term is not part of M_eooe */
+        for (int mu = 0; mu < 4; mu++) {
+            nbr[1 + mu] = v_cb + (neighbour(cdims, x, mu, +1) >> 1) * nb * (long)N;
+            nbr[5 + mu] = v_cb + (neighbour(cdims, x, mu, -1) >> 1) * nb * (long)N;
+        }
+        coarse_site(nb, N, A + x * 9 * (long)nb * nb, nbr, 0x1FE, out + (x >> 1) * nb * (long)N);
+    }
+}
+
 /* Packed per-site entry: A[nsites][9][nb][nb], nbrs[nsites][9][nb][N]. */
 void orc_coarse_sites(long nsites, int nb, int N, const dc *A, const dc *nbrs, dc *out)
 {

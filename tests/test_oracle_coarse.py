@@ -85,3 +85,41 @@ def test_coarse_apply_equals_galerkin_rmp(dims, bdims, n_vec):
         rhs = np.einsum("ij,xkj,kl->xil", G5, A[xm, 1 + mu].conj(), G5)
         assert np.max(np.abs(A[:, 5 + mu] - rhs)) < 1e-13
     assert np.max(np.abs(A[:, 0] - np.einsum("ij,xkj,kl->xil", G5, A[:, 0].conj(), G5))) < 1e-13
+
+
+@pytest.mark.parametrize("cdims,nb,N", [((4, 2, 4, 2), 6, 3), ((2, 2, 2, 4), 4, 1), ((6, 4, 2, 2), 5, 2)])
+def test_coarse_meooe_pins(cdims, nb, N):
+    """Coarse M_eooe (NEXT-1).  Pins: (1) the 8-point hopping term on the full lattice equals the merge of
+    the two parities' M_eooe (identity, like D_hop = M_eooe(0) + M_eooe(1)); (2) brute force: every output site from
+    hand-computed integer coordinates and numpy matmuls; (3) RHS columns are independent; (4) the input is read from the
+    other parity only (perturbing the same-parity sites of the full field changes nothing)."""
+    A = si.coarse_links_np(cdims, nb, 41).astype(np.complex128)
+    v = si.coarse_vector_np(cdims, nb, N, 42).astype(np.complex128)
+    ve, vo = oracle.cb_split(cdims, v)
+    got = [oracle.coarse_meooe(cdims, A, vo, 0), oracle.coarse_meooe(cdims, A, ve, 1)]
+    # (1) hop8 = M_eooe(0) + M_eooe(1) after merging parities
+    hop = oracle.coarse_apply(cdims, A, v, pmask=0x1FE)
+    assert np.max(np.abs(oracle.cb_merge(cdims, got[0], got[1]) - hop)) < 1e-12
+    # (2) brute force, one site at a time, coordinates by hand
+    X, Y, Z, T = cdims
+    for out_parity, src in ((0, vo), (1, ve)):
+        for lex in range(X * Y * Z * T):
+            c = [lex % X, (lex // X) % Y, (lex // (X * Y)) % Z, lex // (X * Y * Z)]
+            if sum(c) % 2 != out_parity:
+                continue
+            want = np.zeros((nb, N), dtype=np.complex128)
+            for mu in range(4):
+                for sign, p in ((+1, 1 + mu), (-1, 5 + mu)):
+                    d = list(c)
+                    d[mu] = (d[mu] + sign) % cdims[mu]
+                    nlex = d[0] + X * (d[1] + Y * (d[2] + Z * d[3]))
+                    assert sum(d) % 2 == 1 - out_parity
+                    want += A[lex, p] @ src[nlex >> 1]
+            assert np.max(np.abs(got[out_parity][lex >> 1] - want)) < 1e-12
+    # (3) columns
+    for r in range(N):
+        assert np.array_equal(oracle.coarse_meooe(cdims, A, vo[..., r:r + 1], 0)[..., 0], got[0][..., r])
+    # (4) M_eooe(0) of a field does not depend on its even sites
+    v2 = v.copy()
+    v2[oracle.parity_mask(cdims) == 0] += 1.0
+    assert np.array_equal(oracle.coarse_meooe(cdims, A, oracle.cb_split(cdims, v2)[1], 0), got[0])
