@@ -205,6 +205,15 @@ mrhs_status_t mrhs_coarse_apply(mrhs_coarse_t *h, const void *d_in, void *d_out)
 #define MRHS_COARSE_ALL 0x1FF
 mrhs_status_t mrhs_coarse_apply_points(mrhs_coarse_t *h, const void *d_in, void *d_out, int point_mask);
 
+/* Coarse M_eooe (Sec. 6: "M_eooe" on both coarse levels): the 8-point coarse
+ * hopping term at the coarse sites of parity out_parity, reading a field of the other parity,
+ *   out(x) = sum_{p=1..8} A_p(x) in(x + delta_p),  parity(x) = (x+y+z+t) mod 2 = out_parity.
+ * d_in: native checkerboarded coarse vector of parity 1 - out_parity, d_out: of parity out_parity (V/2 sites each, made by
+ * mrhs_coarse_field_import / mrhs_coarse_cb_split); the link matrices are the handle's full-lattice field.  Both math
+ * modes (same kernels with a parity site map).  64 nb^2 flops per output site per RHS.  INVALID_ARG: odd coarse extent,
+ * bad parity, aliasing. */
+mrhs_status_t mrhs_coarse_meooe(mrhs_coarse_t *h, const void *d_in, void *d_out, int out_parity);
+
 mrhs_status_t mrhs_coarse_destroy(mrhs_coarse_t *h);
 
 /* ------------------------------------------------- layout helpers (untimed) */
@@ -229,6 +238,19 @@ mrhs_status_t mrhs_cb_split(const int dims[4], int ncomp, int nrhs, const void *
                             void *d_even, void *d_odd, void *cuda_stream);
 mrhs_status_t mrhs_cb_merge(const int dims[4], int ncomp, int nrhs, const void *d_even,
                             const void *d_odd, void *d_full, void *cuda_stream);
+
+/* The four calls above choose the layout from ncomp: 12 = fine spinor (x-blocked, Sec. "Native layouts"), anything else =
+ * coarse vector (site-contiguous [site][component][rhs]).  A coarse level whose vectors happen to have 12 components
+ * (n_vec = 6) must say so: these entries always use the COARSE layout.  parity 0/1 = checkerboarded coarse field of that
+ * parity (V/2 sites ordered by lex, index lex >> 1; needs even extents), 2 = full.  (NEXT-1.) */
+mrhs_status_t mrhs_coarse_field_import(const int cdims[4], int nbasis, int nrhs, int parity,
+                                       const void *d_canonical, void *d_native, void *cuda_stream);
+mrhs_status_t mrhs_coarse_field_export(const int cdims[4], int nbasis, int nrhs, int parity,
+                                       const void *d_native, void *d_canonical, void *cuda_stream);
+mrhs_status_t mrhs_coarse_cb_split(const int cdims[4], int nbasis, int nrhs, const void *d_full,
+                                   void *d_even, void *d_odd, void *cuda_stream);
+mrhs_status_t mrhs_coarse_cb_merge(const int cdims[4], int nbasis, int nrhs, const void *d_even,
+                                   const void *d_odd, void *d_full, void *cuda_stream);
 
 /* ------------------------------------------- intergrid operators (projection / promotion) */
 

@@ -54,6 +54,7 @@ _SIGNATURES = {
     "mrhs_coarse_create": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, ctypes.c_int, ctypes.c_int, _vp, ctypes.c_int, _vp]),
     "mrhs_coarse_apply": (ctypes.c_int, [_vp, _vp, _vp]),
     "mrhs_coarse_apply_points": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
+    "mrhs_coarse_meooe": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_coarse_destroy": (ctypes.c_int, [_vp]),
     "mrhs_transfer_create": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, _int4, ctypes.c_int, ctypes.c_int, _vp, _vp]),
     "mrhs_prolong": (ctypes.c_int, [_vp, _vp, _vp]),
@@ -66,6 +67,10 @@ _SIGNATURES = {
     "mrhs_field_export": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]),
     "mrhs_cb_split": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
     "mrhs_cb_merge": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
+    "mrhs_coarse_field_import": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]),
+    "mrhs_coarse_field_export": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]),
+    "mrhs_coarse_cb_split": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
+    "mrhs_coarse_cb_merge": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
     "mrhs_wilson_apply_host": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _vp, _vp]),
     "mrhs_coarse_apply_host": (ctypes.c_int, [_vp, _vp, _vp]),
     "mrhs_last_error": (ctypes.c_char_p, []),
@@ -196,6 +201,31 @@ def field_export(dims, ncomp, nrhs, parity, native, canonical=None, stream=None)
     return canonical
 
 
+def coarse_field_import(cdims, nbasis, nrhs, parity, canonical, native=None, stream=None):
+    """canonical coarse vector [sites][nbasis][nrhs] -> native (coarse layout whatever nbasis is; parity 0/1 = one parity)."""
+    if native is None:
+        native = empty_field(cdims, nbasis, nrhs, parity, canonical.device)
+    _check(lib().mrhs_coarse_field_import(_dims(cdims), nbasis, nrhs, parity, _ptr(canonical), _ptr(native), _stream_ptr(stream)))
+    return native
+
+
+def coarse_field_export(cdims, nbasis, nrhs, parity, native, canonical=None, stream=None):
+    import torch
+    if canonical is None:
+        nsites = int(cdims[0]) * int(cdims[1]) * int(cdims[2]) * int(cdims[3]) // (1 if parity == FULL else 2)
+        canonical = torch.empty((nsites, nbasis, nrhs), dtype=torch.complex64, device=native.device)
+    _check(lib().mrhs_coarse_field_export(_dims(cdims), nbasis, nrhs, parity, _ptr(native), _ptr(canonical), _stream_ptr(stream)))
+    return canonical
+
+
+def coarse_cb_split(cdims, nbasis, nrhs, full, even, odd, stream=None):
+    _check(lib().mrhs_coarse_cb_split(_dims(cdims), nbasis, nrhs, _ptr(full), _ptr(even), _ptr(odd), _stream_ptr(stream)))
+
+
+def coarse_cb_merge(cdims, nbasis, nrhs, even, odd, full, stream=None):
+    _check(lib().mrhs_coarse_cb_merge(_dims(cdims), nbasis, nrhs, _ptr(even), _ptr(odd), _ptr(full), _stream_ptr(stream)))
+
+
 def cb_split(dims, ncomp, nrhs, full, even, odd, stream=None):
     _check(lib().mrhs_cb_split(_dims(dims), ncomp, nrhs, _ptr(full), _ptr(even), _ptr(odd), _stream_ptr(stream)))
 
@@ -309,6 +339,10 @@ def coarse_apply_points(h, d_in, d_out, point_mask):
     _check(lib().mrhs_coarse_apply_points(h, _ptr(d_in), _ptr(d_out), int(point_mask)))
 
 
+def coarse_meooe(h, d_in, d_out, out_parity):
+    _check(lib().mrhs_coarse_meooe(h, _ptr(d_in), _ptr(d_out), int(out_parity)))
+
+
 def coarse_apply_host(h, h_in, h_out):
     _check(lib().mrhs_coarse_apply_host(h, _ptr(h_in), _ptr(h_out)))
 
@@ -394,14 +428,18 @@ class Coarse:
         except Exception:
             pass
 
-    def empty(self, device="cuda"):
-        return empty_field(self.cdims, self.nbasis, self.nrhs, FULL, device)
+    def empty(self, device="cuda", parity=FULL):
+        return empty_field(self.cdims, self.nbasis, self.nrhs, parity, device)
 
-    def import_field(self, canonical):
-        return field_import(self.cdims, self.nbasis, self.nrhs, FULL, canonical)
+    def import_field(self, canonical, parity=FULL):
+        return coarse_field_import(self.cdims, self.nbasis, self.nrhs, parity, canonical)
 
-    def export_field(self, native):
-        return field_export(self.cdims, self.nbasis, self.nrhs, FULL, native)
+    def export_field(self, native, parity=FULL):
+        return coarse_field_export(self.cdims, self.nbasis, self.nrhs, parity, native)
+
+    def meooe(self, d_in, d_out, out_parity):
+        """out = coarse M_eooe in: the 8-point hopping term on the sites of out_parity from the other parity."""
+        coarse_meooe(self.h, d_in, d_out, out_parity)
 
     def apply(self, d_in, d_out, point_mask=None):
         if point_mask is None:

@@ -483,8 +483,21 @@ mrhs_status_t mrhs_coarse_apply_points(mrhs_coarse_t *h, const void *d_in, void 
     MRHS_REQUIRE(d_in != d_out, "coarse apply: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "coarse apply: buffers must be 16-byte aligned");
     MRHS_REQUIRE(point_mask > 0 && point_mask <= 0x1FF, "coarse apply: point_mask must select at least one of the nine stencil points");
-    if (h->mode == 1) return launch_coarse_tc(h->g, h->tc_grid, (unsigned)point_mask, (const float *)h->links, d_in, d_out, h->st);
-    return launch_coarse_fma(h->g, (unsigned)point_mask, h->links, d_in, d_out, h->st);
+    const CoarseSites sites = coarse_sites_full(h->g);
+    if (h->mode == 1) return launch_coarse_tc(h->g, sites, h->tc_grid, (unsigned)point_mask, (const float *)h->links, d_in, d_out, h->st);
+    return launch_coarse_fma(h->g, sites, (unsigned)point_mask, h->links, d_in, d_out, h->st);
+}
+
+mrhs_status_t mrhs_coarse_meooe(mrhs_coarse_t *h, const void *d_in, void *d_out, int out_parity) {
+    MRHS_REQUIRE(h && d_in && d_out, "coarse meooe: NULL argument");
+    MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "coarse meooe: out_parity must be 0 or 1");
+    MRHS_REQUIRE(d_in != d_out, "coarse meooe: in and out must not alias");
+    MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "coarse meooe: buffers must be 16-byte aligned");
+    MRHS_REQUIRE(!((h->g.X | h->g.Y | h->g.Z | h->g.T) & 1), "coarse meooe: checkerboarded coarse fields need even extents");
+    // the 8-point hopping term at the sites of one parity: same kernels, same link field, parity site map
+    const CoarseSites sites = coarse_sites_parity(h->g, out_parity);
+    if (h->mode == 1) return launch_coarse_tc(h->g, sites, h->tc_grid, MRHS_COARSE_HOP, (const float *)h->links, d_in, d_out, h->st);
+    return launch_coarse_fma(h->g, sites, MRHS_COARSE_HOP, h->links, d_in, d_out, h->st);
 }
 
 mrhs_status_t mrhs_coarse_apply(mrhs_coarse_t *h, const void *d_in, void *d_out) {

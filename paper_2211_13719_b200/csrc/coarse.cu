@@ -64,7 +64,7 @@ struct CoarseCfg {
 // ALL: the nine-point operator (mask ignored; the stage loop has a compile-time trip count)
 template <int NB, int N, bool ALL>
 __global__ void __launch_bounds__(CoarseCfg<NB, N>::THREADS)
-coarse_fma_kernel(int X, int Y, int Z, int T, unsigned mask, const float2 *__restrict__ links,
+coarse_fma_kernel(const CoarseSites sites, unsigned mask, const float2 *__restrict__ links,
                   const typename Elem<CoarseCfg<NB, N>::R>::type *__restrict__ in,
                   typename Elem<CoarseCfg<NB, N>::R>::type *__restrict__ out) {
     typedef CoarseCfg<NB, N> C;
@@ -78,21 +78,12 @@ coarse_fma_kernel(int X, int Y, int Z, int T, unsigned mask, const float2 *__res
     const int rg = (tid / C::NPG) % C::NRG;
     const int ks = tid / C::GROUPS;
 
-    const long long site = blockIdx.x;
-    // neighbour sites of the nine stencil points: 0 self, 1..4 = +x..+t, 5..8 = -x..-t
+    const long long osite = blockIdx.x;                       // output site; its links live at lex
+    const long long site = coarse_site_lex(sites, osite);
+    // vector index of the neighbour at stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t
     auto neighbour = [&](int p) -> long long {
-        if (p == 0) return site;
-        int c[4];
-        long long s = site;
-        c[0] = (int)(s % X); s /= X;
-        c[1] = (int)(s % Y); s /= Y;
-        c[2] = (int)(s % Z);
-        c[3] = (int)(s / Z);
-        const int ext[4] = {X, Y, Z, T};
-        const int mu = (p - 1) & 3;
-        const int d = p <= 4 ? 1 : -1;
-        c[mu] = (c[mu] + d + ext[mu]) % ext[mu];
-        return c[0] + (long long)X * (c[1] + (long long)Y * (c[2] + (long long)Z * c[3]));
+        const long long n = coarse_neighbour_lex(sites, site, p);
+        return sites.cb ? n >> 1 : n;
     };
     // the stencil points of this apply: bit p of mask (all nine for the full operator, bit 0 = self term alone,
     // bits 1..8 = the 8-point hopping term); stage s handles the s-th set bit
@@ -164,10 +155,10 @@ coarse_fma_kernel(int X, int Y, int Z, int T, unsigned mask, const float2 *__res
             for (int k = 1; k < C::KS; k++) sum = cadd(sum, to_cvec(red[(size_t)k * ELEMS + e]));
             const int grp = e / TILE, w = e - grp * TILE, i = w / TP, b = w - i * TP;
             const int epg = grp % C::NPG, erg = grp / C::NPG;
-            out[((size_t)site * NB + erg * TI + i) * C::NP + epg * TP + b] = from_cvec(sum);
+            out[((size_t)osite * NB + erg * TI + i) * C::NP + epg * TP + b] = from_cvec(sum);
         }
     } else {
-        E *o = out + ((size_t)site * NB + rg * TI) * C::NP + pg * TP;
+        E *o = out + ((size_t)osite * NB + rg * TI) * C::NP + pg * TP;
 #pragma unroll
         for (int i = 0; i < TI; i++)
 #pragma unroll
@@ -186,11 +177,11 @@ __global__ void pack_links_kernel(int nb, const float2 *__restrict__ src, float2
 }
 
 template <int NB, int N>
-mrhs_status_t launch_t(const CoarseGeom &g, unsigned mask, const float2 *links, const void *in, void *out, cudaStream_t st) {
+mrhs_status_t launch_t(const CoarseSites &sites, unsigned mask, const float2 *links, const void *in, void *out, cudaStream_t st) {
     typedef CoarseCfg<NB, N> C;
     typedef typename Elem<C::R>::type E;
-    if (mask == 0x1FFu) coarse_fma_kernel<NB, N, true><<<(unsigned)g.nsites, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, mask, links, (const E *)in, (E *)out);
-    else coarse_fma_kernel<NB, N, false><<<(unsigned)g.nsites, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, mask, links, (const E *)in, (E *)out);
+    if (mask == 0x1FFu) coarse_fma_kernel<NB, N, true><<<(unsigned)sites.nout, C::THREADS, C::SMEM_BYTES, st>>>(sites, mask, links, (const E *)in, (E *)out);
+    else coarse_fma_kernel<NB, N, false><<<(unsigned)sites.nout, C::THREADS, C::SMEM_BYTES, st>>>(sites, mask, links, (const E *)in, (E *)out);
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
 }
@@ -224,8 +215,8 @@ mrhs_status_t coarse_fma_prepare(const CoarseGeom &g) {
     return MRHS_ERR_UNSUPPORTED;
 }
 
-mrhs_status_t launch_coarse_fma(const CoarseGeom &g, unsigned mask, const float2 *d_links, const void *d_in, void *d_out, cudaStream_t st) {
-#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return launch_t<NB, NN>(g, mask, d_links, d_in, d_out, st);
+mrhs_status_t launch_coarse_fma(const CoarseGeom &g, const CoarseSites &sites, unsigned mask, const float2 *d_links, const void *d_in, void *d_out, cudaStream_t st) {
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return launch_t<NB, NN>(sites, mask, d_links, d_in, d_out, st);
     MRHS_COARSE_N_LIST(MRHS_CASE, 24)
     MRHS_COARSE_N_LIST(MRHS_CASE, 40)
 #undef MRHS_CASE

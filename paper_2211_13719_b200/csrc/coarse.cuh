@@ -11,6 +11,45 @@ struct CoarseGeom {
     long long nsites;
 };
 
+// Which sites an apply runs over (the coarse operators exist on the full lattice and, as M_eooe, on one
+// parity).  cb = 0: all sites, vectors indexed by lex.  cb = 1: the sites of parity `parity`, output indexed by lex >> 1,
+// input vectors (the other parity) also by lex >> 1; the link matrices are always indexed by lex.
+struct CoarseSites {
+    int X, Y, Z, T;
+    int cb, parity;
+    long long nout;     // output sites: V or V / 2
+};
+
+#ifdef __CUDACC__
+// idx-th output site -> lex
+__device__ __forceinline__ long long coarse_site_lex(const CoarseSites &g, long long idx) {
+    if (!g.cb) return idx;
+    long long s = 2 * idx;                 // the pair (2 idx, 2 idx + 1) holds one site of each parity (X even)
+    const int x = (int)(s % g.X); s /= g.X;
+    const int y = (int)(s % g.Y); s /= g.Y;
+    const int z = (int)(s % g.Z);
+    const int t = (int)(s / g.Z);
+    return 2 * idx + (((x + y + z + t) & 1) != g.parity);
+}
+// lex of the neighbour at stencil point p (0 self, 1..4 = +x..+t, 5..8 = -x..-t, periodic)
+__device__ __forceinline__ long long coarse_neighbour_lex(const CoarseSites &g, long long lex, int p) {
+    if (p == 0) return lex;
+    long long s = lex;
+    int c0 = (int)(s % g.X); s /= g.X;
+    int c1 = (int)(s % g.Y); s /= g.Y;
+    int c2 = (int)(s % g.Z);
+    int c3 = (int)(s / g.Z);
+    const int mu = (p - 1) & 3, d = p <= 4 ? 1 : -1;
+    if (mu == 0) c0 = (c0 + d + g.X) % g.X;
+    else if (mu == 1) c1 = (c1 + d + g.Y) % g.Y;
+    else if (mu == 2) c2 = (c2 + d + g.Z) % g.Z;
+    else c3 = (c3 + d + g.T) % g.T;
+    return c0 + (long long)g.X * (c1 + (long long)g.Y * (c2 + (long long)g.Z * c3));
+}
+#endif
+inline CoarseSites coarse_sites_full(const CoarseGeom &g) { return {g.X, g.Y, g.Z, g.T, 0, 0, g.nsites}; }
+inline CoarseSites coarse_sites_parity(const CoarseGeom &g, int parity) { return {g.X, g.Y, g.Z, g.T, 1, parity, g.nsites / 2}; }
+
 // canonical A[site][p][row][col] -> native A[site][p][col][row] (one bulk copy per stencil point
 // lands the matrix so that a thread's TI consecutive rows of one column are contiguous).
 mrhs_status_t pack_coarse_links(const CoarseGeom &g, const float2 *d_canonical, float2 *d_native, cudaStream_t st);
@@ -19,7 +58,7 @@ mrhs_status_t pack_coarse_links(const CoarseGeom &g, const float2 *d_canonical, 
 bool coarse_fma_supported(int nb, int nrhs);
 mrhs_status_t coarse_fma_prepare(const CoarseGeom &g);   // opt in to large dynamic shared memory
 // mask: bit p set = stencil point p is applied (0 self, 1..4 = +x..+t, 5..8 = -x..-t); 0x1FF = the 9-point operator
-mrhs_status_t launch_coarse_fma(const CoarseGeom &g, unsigned mask, const float2 *d_links, const void *d_in, void *d_out, cudaStream_t st);
+mrhs_status_t launch_coarse_fma(const CoarseGeom &g, const CoarseSites &sites, unsigned mask, const float2 *d_links, const void *d_in, void *d_out, cudaStream_t st);
 
 // ---- tensor-core variant (row a6): tcgen05 kind::tf32 with hi/lo split operands (3 MMAs per K step)
 // true if a tensor-core specialisation for (nbasis, nrhs) is compiled (even nrhs only)
@@ -29,6 +68,6 @@ bool coarse_tc_supported(int nb, int nrhs);
 mrhs_status_t pack_coarse_links_tc(const CoarseGeom &g, const float2 *d_canonical, float *d_native, cudaStream_t st);
 // opt in to large dynamic shared memory and size the persistent grid (CTAs per SM limited by shared memory and TMEM)
 mrhs_status_t coarse_tc_prepare(const CoarseGeom &g, int *grid);
-mrhs_status_t launch_coarse_tc(const CoarseGeom &g, int grid, unsigned mask, const float *d_links, const void *d_in, void *d_out, cudaStream_t st);
+mrhs_status_t launch_coarse_tc(const CoarseGeom &g, const CoarseSites &sites, int grid, unsigned mask, const float *d_links, const void *d_in, void *d_out, cudaStream_t st);
 
 }  // namespace mrhs

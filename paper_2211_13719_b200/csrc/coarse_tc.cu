@@ -146,7 +146,7 @@ struct TcCfg {
 // ALL: the nine-point operator (mask ignored; compile-time stage count)
 template <int NB, int N, bool ALL>
 __global__ void __launch_bounds__(TcCfg<NB, N>::THREADS)
-coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, const float4 *__restrict__ links,
+coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restrict__ links,
                  const float4 *__restrict__ in, float4 *__restrict__ out) {
     typedef TcCfg<NB, N> C;
     constexpr int A_IT = (C::A_UNITS + C::THREADS - 1) / C::THREADS;
@@ -178,31 +178,21 @@ coarse_tc_kernel(int X, int Y, int Z, int T, long long nsites, unsigned mask, co
     // the previous stage has been handed to the tensor core, so the load latency overlaps its MMAs and the next wait
     float4 ra[A_IT];
     float4 rb[B_IT][4];
-    // neighbour of stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
-    auto neighbour = [&](long long site, int p) -> long long {
-        long long nbr = site;
-        if (p > 0) {
-            long long s = site;
-            int c0 = (int)(s % X); s /= X;
-            int c1 = (int)(s % Y); s /= Y;
-            int c2 = (int)(s % Z);
-            int c3 = (int)(s / Z);
-            const int mu = (p - 1) & 3, d = p <= 4 ? 1 : -1;
-            if (mu == 0) c0 = (c0 + d + X) % X;
-            else if (mu == 1) c1 = (c1 + d + Y) % Y;
-            else if (mu == 2) c2 = (c2 + d + Z) % Z;
-            else c3 = (c3 + d + T) % T;
-            nbr = c0 + (long long)X * (c1 + (long long)Y * (c2 + (long long)Z * c3));
-        }
-        return nbr;
+    const long long nsites = sites.nout;       // output sites, enumerated by osite; the links of output site osite live at its lex
+    // vector index of the neighbour at stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
+    auto neighbour = [&](long long lex, int p) -> long long {
+        const long long n = coarse_neighbour_lex(sites, lex, p);
+        return sites.cb ? n >> 1 : n;
     };
     // one thread asks the copy engine to bring a later stage's matrix and neighbour vector into L2 (each is one
     // contiguous block), so that the register loads of that stage find them there
-    auto prefetch_stage = [&](long long site, int p) {
+    auto prefetch_stage = [&](long long osite, int p) {
+        const long long site = coarse_site_lex(sites, osite);
         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(links + ((size_t)site * 9 + p) * C::A_UNITS), "r"(C::A_UNITS * 16) : "memory");
         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(in + (size_t)neighbour(site, p) * NB * C::NP), "r"(NB * C::NP * 16) : "memory");
     };
-    auto load_stage = [&](long long site, int p) {
+    auto load_stage = [&](long long osite, int p) {
+        const long long site = coarse_site_lex(sites, osite);
         const float4 *lp = links + ((size_t)site * 9 + p) * C::A_UNITS;
         const float4 *vp = in + (size_t)neighbour(site, p) * NB * C::NP;
 #pragma unroll
@@ -370,14 +360,13 @@ mrhs_status_t tc_prepare_t(int *ctas_per_sm) {
     return MRHS_OK;
 }
 template <int NB, int N>
-mrhs_status_t tc_launch_t(const CoarseGeom &g, int grid, unsigned mask, const float *links, const void *in, void *out, cudaStream_t st) {
+mrhs_status_t tc_launch_t(const CoarseSites &sites, int grid, unsigned mask, const float *links, const void *in, void *out, cudaStream_t st) {
     typedef TcCfg<NB, N> C;
+    if ((long long)grid > sites.nout) grid = (int)sites.nout;
     if (mask == 0x1FFu)
-        coarse_tc_kernel<NB, N, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, g.nsites, mask, (const float4 *)links,
-                                                                               (const float4 *)in, (float4 *)out);
+        coarse_tc_kernel<NB, N, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(sites, mask, (const float4 *)links, (const float4 *)in, (float4 *)out);
     else
-        coarse_tc_kernel<NB, N, false><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(g.X, g.Y, g.Z, g.T, g.nsites, mask, (const float4 *)links,
-                                                                                (const float4 *)in, (float4 *)out);
+        coarse_tc_kernel<NB, N, false><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(sites, mask, (const float4 *)links, (const float4 *)in, (float4 *)out);
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
 }
@@ -414,8 +403,8 @@ mrhs_status_t coarse_tc_prepare(const CoarseGeom &g, int *grid) {
     return MRHS_OK;
 }
 
-mrhs_status_t launch_coarse_tc(const CoarseGeom &g, int grid, unsigned mask, const float *d_links, const void *d_in, void *d_out, cudaStream_t st) {
-#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return tc_launch_t<NB, NN>(g, grid, mask, d_links, d_in, d_out, st);
+mrhs_status_t launch_coarse_tc(const CoarseGeom &g, const CoarseSites &sites, int grid, unsigned mask, const float *d_links, const void *d_in, void *d_out, cudaStream_t st) {
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return tc_launch_t<NB, NN>(sites, grid, mask, d_links, d_in, d_out, st);
     MRHS_TC_N_LIST(MRHS_CASE, 24)
     MRHS_TC_N_LIST(MRHS_CASE, 40)
 #undef MRHS_CASE

@@ -81,6 +81,24 @@ __global__ void cb_kernel(FieldGeom gf, FieldGeom ge, FieldGeom go, float *__res
     else full[idx] = cbp[coff];
 }
 
+// Coarse vectors, full native [lex][nb][2N floats] <-> even/odd native [lex >> 1][nb][2N floats].  One thread per float of the full field.
+template <bool SPLIT>
+__global__ void coarse_cb_kernel(int X, int Y, int Z, long long per_site, float *__restrict__ full, float *__restrict__ even,
+                                 float *__restrict__ odd, long long total) {
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    const long long lex = idx / per_site, e = idx - lex * per_site;
+    long long s = lex;
+    const int x = (int)(s % X); s /= X;
+    const int y = (int)(s % Y); s /= Y;
+    const int z = (int)(s % Z);
+    const int t = (int)(s / Z);
+    float *cbp = ((x + y + z + t) & 1) ? odd : even;
+    const long long coff = (lex >> 1) * per_site + e;
+    if (SPLIT) cbp[coff] = full[idx];
+    else full[idx] = cbp[coff];
+}
+
 bool valid_fine_dims(const int dims[4]) {
     for (int i = 0; i < 4; i++)
         if (dims[i] < 2 || (dims[i] & 1)) return false;
@@ -93,9 +111,10 @@ bool valid_coarse_dims(const int dims[4]) {
 }
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// kind: 0 = decide by ncomp (12 -> fine layout, anything else -> coarse layout), 1 = coarse layout whatever ncomp is
 template <bool IMPORT>
 mrhs_status_t convert(const int dims[4], int ncomp, int nrhs, int parity, const void *src, void *dst,
-                      void *stream) {
+                      void *stream, int kind = 0) {
     MRHS_REQUIRE(dims && src && dst, "field convert: NULL argument");
     MRHS_REQUIRE(nrhs >= 1 && ncomp >= 1, "field convert: nrhs and ncomp must be positive");
     MRHS_REQUIRE(parity >= 0 && parity <= 2, "field convert: parity must be 0, 1 or 2");
@@ -103,7 +122,7 @@ mrhs_status_t convert(const int dims[4], int ncomp, int nrhs, int parity, const 
     MRHS_REQUIRE(src != dst, "field convert: in-place conversion is not supported");
     cudaStream_t st = (cudaStream_t)stream;
     const int threads = 256;
-    if (ncomp == 12) {
+    if (ncomp == 12 && kind == 0) {
         MRHS_REQUIRE(valid_fine_dims(dims), "field convert: fine extents must be even and >= 2");
         FieldGeom g = make_geom(dims, ncomp, nrhs, parity);
         long long total = g.nsites * ncomp * nrhs;
@@ -115,8 +134,9 @@ mrhs_status_t convert(const int dims[4], int ncomp, int nrhs, int parity, const 
             fine_convert_kernel<false><<<(unsigned)blocks, threads, 0, st>>>(g, nullptr, (float *)const_cast<void *>(src), (float2 *)dst, total);
     } else {
         MRHS_REQUIRE(valid_coarse_dims(dims), "field convert: coarse extents must be >= 2");
-        MRHS_REQUIRE(parity == MRHS_FULL, "field convert: coarse fields are full-lattice only");
-        long long total = (long long)dims[0] * dims[1] * dims[2] * dims[3] * ncomp * nrhs;
+        // a checkerboarded coarse field holds the sites of one parity ordered by lex (index lex >> 1): same element order
+        MRHS_REQUIRE(parity == MRHS_FULL || valid_fine_dims(dims), "field convert: checkerboarded coarse fields need even extents");
+        long long total = (long long)dims[0] * dims[1] * dims[2] * dims[3] * ncomp * nrhs / (parity == MRHS_FULL ? 1 : 2);
         long long blocks = (total + threads - 1) / threads;
         MRHS_REQUIRE(blocks < (1ll << 31), "field convert: field too large");
         if (IMPORT)
@@ -129,10 +149,22 @@ mrhs_status_t convert(const int dims[4], int ncomp, int nrhs, int parity, const 
 }
 
 template <bool SPLIT>
-mrhs_status_t cb_convert(const int dims[4], int ncomp, int nrhs, void *full, void *even, void *odd, void *stream) {
+mrhs_status_t cb_convert(const int dims[4], int ncomp, int nrhs, void *full, void *even, void *odd, void *stream, int kind = 0) {
     MRHS_REQUIRE(dims && full && even && odd, "cb split/merge: NULL argument");
-    MRHS_REQUIRE(ncomp == 12, "cb split/merge: only fine fields (ncomp = 12) are checkerboarded");
-    MRHS_REQUIRE(nrhs >= 1, "cb split/merge: nrhs must be positive");
+    MRHS_REQUIRE(nrhs >= 1 && ncomp >= 1, "cb split/merge: nrhs and ncomp must be positive");
+    if (ncomp != 12 || kind == 1) {
+        MRHS_REQUIRE(valid_fine_dims(dims), "cb split/merge: extents must be even and >= 2");
+        MRHS_REQUIRE(aligned16(full) && aligned16(even) && aligned16(odd), "cb split/merge: buffers must be 16-byte aligned");
+        MRHS_REQUIRE(full != even && full != odd && even != odd, "cb split/merge: buffers must be distinct");
+        const long long per_site = 2ll * ncomp * nrhs;
+        const long long total = (long long)dims[0] * dims[1] * dims[2] * dims[3] * per_site;
+        const long long blocks = (total + 255) / 256;
+        MRHS_REQUIRE(blocks < (1ll << 31), "cb split/merge: field too large");
+        coarse_cb_kernel<SPLIT><<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(dims[0], dims[1], dims[2], per_site, (float *)full, (float *)even,
+                                                                                   (float *)odd, total);
+        MRHS_CUDA(cudaGetLastError());
+        return MRHS_OK;
+    }
     MRHS_REQUIRE(valid_fine_dims(dims), "cb split/merge: extents must be even and >= 2");
     MRHS_REQUIRE(aligned16(full) && aligned16(even) && aligned16(odd), "cb split/merge: buffers must be 16-byte aligned");
     MRHS_REQUIRE(full != even && full != odd && even != odd, "cb split/merge: buffers must be distinct");
@@ -181,6 +213,26 @@ mrhs_status_t mrhs_field_import(const int dims[4], int ncomp, int nrhs, int pari
 mrhs_status_t mrhs_field_export(const int dims[4], int ncomp, int nrhs, int parity, const void *d_native,
                                 void *d_canonical, void *cuda_stream) {
     return convert<false>(dims, ncomp, nrhs, parity, d_native, d_canonical, cuda_stream);
+}
+
+mrhs_status_t mrhs_coarse_field_import(const int cdims[4], int nbasis, int nrhs, int parity, const void *d_canonical,
+                                       void *d_native, void *cuda_stream) {
+    return convert<true>(cdims, nbasis, nrhs, parity, d_canonical, d_native, cuda_stream, 1);
+}
+
+mrhs_status_t mrhs_coarse_field_export(const int cdims[4], int nbasis, int nrhs, int parity, const void *d_native,
+                                       void *d_canonical, void *cuda_stream) {
+    return convert<false>(cdims, nbasis, nrhs, parity, d_native, d_canonical, cuda_stream, 1);
+}
+
+mrhs_status_t mrhs_coarse_cb_split(const int cdims[4], int nbasis, int nrhs, const void *d_full, void *d_even, void *d_odd,
+                                   void *cuda_stream) {
+    return cb_convert<true>(cdims, nbasis, nrhs, const_cast<void *>(d_full), d_even, d_odd, cuda_stream, 1);
+}
+
+mrhs_status_t mrhs_coarse_cb_merge(const int cdims[4], int nbasis, int nrhs, const void *d_even, const void *d_odd,
+                                   void *d_full, void *cuda_stream) {
+    return cb_convert<false>(cdims, nbasis, nrhs, d_full, const_cast<void *>(d_even), const_cast<void *>(d_odd), cuda_stream, 1);
 }
 
 mrhs_status_t mrhs_cb_split(const int dims[4], int ncomp, int nrhs, const void *d_full, void *d_even, void *d_odd,

@@ -152,3 +152,62 @@ def test_coarse_errors():
     with pytest.raises(mrhs.MrhsError):
         c.apply(f, f)
     c.close()
+
+
+# ---- NEXT-1: checkerboarded coarse fields and coarse M_eooe, both math modes, both parities
+MEOOE_CASES = [([4, 2, 6, 2], 24, 12), ([2, 4, 2, 6], 40, 24), ([2, 2, 2, 2], 40, 96), ([6, 4, 2, 4], 24, 1), ([8, 4, 4, 6], 40, 12)]
+
+
+@pytest.mark.parametrize("mode", [mrhs.COARSE_FMA, mrhs.COARSE_TENSOR])
+@pytest.mark.parametrize("cdims,nb,nrhs", MEOOE_CASES)
+def test_coarse_meooe_matches_oracle(cdims, nb, nrhs, mode):
+    if mode == mrhs.COARSE_TENSOR and nrhs % 2:
+        pytest.skip("the tensor-core variant needs an even N_rhs")
+    A = syn.coarse_links_np(cdims, nb, 8)
+    v = syn.coarse_vector_np(cdims, nb, nrhs, 8)
+    src = oracle.cb_split(cdims, v)
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=mode)
+    for out_parity in (0, 1):
+        want = oracle.coarse_meooe(cdims, A, src[1 - out_parity], out_parity)
+        d_in = c.import_field(dev(src[1 - out_parity]), 1 - out_parity)
+        d_out = c.empty(parity=out_parity)
+        c.meooe(d_in, d_out, out_parity)
+        torch.cuda.synchronize()
+        err = rel_l2_per_rhs(host(c.export_field(d_out, out_parity)), want)
+        assert err.max() < TOL, (out_parity, err)
+    with pytest.raises(mrhs.MrhsError):
+        c.meooe(c.empty(parity=0), c.empty(parity=1), 2)
+    c.close()
+
+
+def test_coarse_meooe_needs_even_extents():
+    cdims, nb, nrhs = [3, 2, 2, 2], 24, 4
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(syn.coarse_links_np(cdims, nb, 9)))
+    with pytest.raises(mrhs.MrhsError) as e:
+        c.meooe(c.empty(), c.empty(), 0)
+    assert e.value.status == mrhs.ERR_INVALID_ARG
+    c.close()
+
+
+@pytest.mark.parametrize("cdims,nb,nrhs", [([4, 2, 6, 2], 24, 12), ([2, 2, 4, 2], 12, 3), ([2, 4, 2, 2], 12, 4)])
+def test_coarse_layout_round_trips_are_bit_exact(cdims, nb, nrhs):
+    """Checkerboarded coarse fields: import / export and split / merge against the oracle-side canonical split; nb = 12
+    (a coarse level with n_vec = 6) goes through the explicit coarse entries and is NOT packed like a fine spinor."""
+    v = syn.coarse_vector_np(cdims, nb, nrhs, 10)
+    d = dev(v)
+    nat = mrhs.coarse_field_import(cdims, nb, nrhs, mrhs.FULL, d)
+    assert torch.equal(mrhs.coarse_field_export(cdims, nb, nrhs, mrhs.FULL, nat), d)
+    ev = mrhs.empty_field(cdims, nb, nrhs, mrhs.EVEN)
+    od = mrhs.empty_field(cdims, nb, nrhs, mrhs.ODD)
+    mrhs.coarse_cb_split(cdims, nb, nrhs, nat, ev, od)
+    ve, vo = oracle.cb_split(cdims, v)
+    assert np.array_equal(host(mrhs.coarse_field_export(cdims, nb, nrhs, mrhs.EVEN, ev)), ve)
+    assert np.array_equal(host(mrhs.coarse_field_export(cdims, nb, nrhs, mrhs.ODD, od)), vo)
+    assert torch.equal(mrhs.coarse_field_import(cdims, nb, nrhs, mrhs.ODD, dev(vo)), od)
+    full2 = torch.zeros_like(nat)
+    mrhs.coarse_cb_merge(cdims, nb, nrhs, ev, od, full2)
+    assert torch.equal(full2, nat)
+    # the coarse layout is site-contiguous: one site's nb x nrhs block is one run of the native field
+    if nrhs % 2 == 0:
+        site = host(nat).reshape(-1, nb, nrhs // 2, 4)[1]
+        assert np.array_equal(site[:, :, 0] + 1j * site[:, :, 2], v[1][:, 0::2])
