@@ -141,6 +141,22 @@ mrhs_status_t mrhs_meooe_mooee_inv(mrhs_wilson_t *h, const void *d_in, void *d_o
 mrhs_status_t mrhs_schur_sequence(mrhs_wilson_t *h, const void *d_in, void *d_tmp0,
                                   void *d_tmp1, void *d_out);
 
+/* Adjoint operators (reading S3): D_hop^+ = gamma_5 D_hop gamma_5,
+ *   (D_hop^+ in)(x) = sum_mu (1+gamma_mu) U_mu(x) in(x+mu) + (1-gamma_mu) U_mu(x-mu)^+ in(x-mu),
+ * the same links with the projector signs exchanged; M_eooe^+ is the same sum at the sites of out_parity (it maps a field
+ * of parity 1 - out_parity to one of parity out_parity, like mrhs_meooe); M^+ = M_ooee - D_hop^+ / 2 (the clover blocks are
+ * Hermitian).  Same kernels, same cost, same argument rules as the plain calls. */
+mrhs_status_t mrhs_dhop_dag(mrhs_wilson_t *h, const void *d_in, void *d_out);
+mrhs_status_t mrhs_meooe_dag(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity);
+mrhs_status_t mrhs_wilson_apply_dag(mrhs_wilson_t *h, const void *d_in, void *d_out);
+
+/* The even-odd preconditioned operator (Schur complement of M on the even sites; PAPER.md:43,
+ * :53 "precomputed clover term"; reading S6 with M_eo = -M_eooe / 2):
+ *   out = S in,  S = M_ee - M_eo M_oo^-1 M_oe = C_e - M_eooe(e<-o) C_o^-1 M_eooe(o<-e) / 4,    dagger != 0: S^+ (daggered hops).
+ * d_in, d_out: native EVEN fields; d_tmp: native ODD scratch field (overwritten); all three distinct.  Sweep kernel: two
+ * launches (C_o^-1 rides in the first hop's epilogue, C_e in - ... / 4 in the second's); gather kernel: four. */
+mrhs_status_t mrhs_schur_apply(mrhs_wilson_t *h, const void *d_in, void *d_tmp, void *d_out, int dagger);
+
 /* Copy the handle's native clover blocks back in canonical form
  * d_clover_out[lex][2][6][6] complex64 (parity check of the device-side
  * construction, row a0). */

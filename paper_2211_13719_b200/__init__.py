@@ -39,6 +39,10 @@ _SIGNATURES = {
     "mrhs_mooee": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_schur_sequence": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "mrhs_wilson_apply": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_dhop_dag": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_meooe_dag": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
+    "mrhs_wilson_apply_dag": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_schur_apply": (ctypes.c_int, [_vp, _vp, _vp, _vp, ctypes.c_int]),
     "mrhs_meooe_mooee": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_meooe_mooee_inv": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_mooee_inv": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
@@ -259,6 +263,22 @@ def wilson_apply(h, d_in, d_out):
     _check(lib().mrhs_wilson_apply(h, _ptr(d_in), _ptr(d_out)))
 
 
+def dhop_dag(h, d_in, d_out):
+    _check(lib().mrhs_dhop_dag(h, _ptr(d_in), _ptr(d_out)))
+
+
+def meooe_dag(h, d_in, d_out, out_parity):
+    _check(lib().mrhs_meooe_dag(h, _ptr(d_in), _ptr(d_out), int(out_parity)))
+
+
+def wilson_apply_dag(h, d_in, d_out):
+    _check(lib().mrhs_wilson_apply_dag(h, _ptr(d_in), _ptr(d_out)))
+
+
+def schur_apply(h, d_in, d_tmp, d_out, dagger=False):
+    _check(lib().mrhs_schur_apply(h, _ptr(d_in), _ptr(d_tmp), _ptr(d_out), int(bool(dagger))))
+
+
 def meooe_mooee(h, d_in, d_out, out_parity):
     _check(lib().mrhs_meooe_mooee(h, _ptr(d_in), _ptr(d_out), int(out_parity)))
 
@@ -391,9 +411,19 @@ class Wilson:
     def mooee(self, d_in, d_out, parity):
         mooee(self.h, d_in, d_out, parity)
 
-    def apply(self, d_in, d_out):
-        """out = M in, the full Wilson-clover matrix on full-lattice fields."""
-        wilson_apply(self.h, d_in, d_out)
+    def apply(self, d_in, d_out, dagger=False):
+        """out = M in (or M^+ in), the full Wilson-clover matrix on full-lattice fields."""
+        (wilson_apply_dag if dagger else wilson_apply)(self.h, d_in, d_out)
+
+    def dhop_dag(self, d_in, d_out):
+        dhop_dag(self.h, d_in, d_out)
+
+    def meooe_dag(self, d_in, d_out, out_parity):
+        meooe_dag(self.h, d_in, d_out, out_parity)
+
+    def schur_apply(self, d_in, d_tmp, d_out, dagger=False):
+        """out = S in on even fields, S = C_e - H_eo C_o^-1 H_oe / 4 (d_tmp: odd scratch)."""
+        schur_apply(self.h, d_in, d_tmp, d_out, dagger)
 
     def meooe_mooee(self, d_in, d_out, out_parity):
         meooe_mooee(self.h, d_in, d_out, out_parity)

@@ -123,6 +123,7 @@ mrhs_status_t wilson_set_default_tiling(mrhs_wilson *h) {
         return MRHS_ERR_UNSUPPORTED;
     }
     h->hp_full.gauge_out = h->hp_full.gauge_in = h->gauge_full;
+    h->hp_full.pf_dist = 2u * (unsigned)h->num_sms;
     for (int p = 0; p < 2; p++) {
         HopTiling tc = default_tiling(h->gcb[p], budget);
         if (!build_hop_params(h->gcb[p], p, tc, h->hp_cb[p])) {
@@ -131,6 +132,7 @@ mrhs_status_t wilson_set_default_tiling(mrhs_wilson *h) {
         }
         h->hp_cb[p].gauge_out = h->gauge_cb[p];
         h->hp_cb[p].gauge_in = h->gauge_cb[1 - p];
+        h->hp_cb[p].pf_dist = 2u * (unsigned)h->num_sms;
     }
     // slice-sweep kernel where the geometry allows it (even N_rhs); the gather kernel otherwise
     h->kern[0] = h->kern[1] = MRHS_HOP_GATHER;
@@ -205,35 +207,70 @@ mrhs_status_t mrhs_wilson_create(mrhs_wilson_t **out, const int dims[4], int nrh
     return MRHS_OK;
 }
 
-mrhs_status_t mrhs_dhop(mrhs_wilson_t *h, const void *d_in, void *d_out) {
+// The hopping term with its options: parity -1 = D_hop on the full lattice, 0 / 1 = M_eooe with that output parity;
+// dagger = the adjoint; clover / aux = the fused epilogues of the sweep kernel (fine_sweep.cuh), sweep kernel only.
+static mrhs_status_t hop_launch(mrhs_wilson_t *h, int parity, int dagger, const float4 *clover, const void *aux, const void *d_in, void *d_out) {
+    const int which = parity < 0 ? 0 : 1;
+    if (h->kern[which] == MRHS_HOP_SWEEP) {
+        SweepParams p = parity < 0 ? h->sp_full : h->sp_cb[parity];
+        p.dagger = dagger;
+        p.clover = clover;
+        p.aux = (const float4 *)aux;
+        return launch_sweep(p, d_in, d_out, h->st);
+    }
+    HopParams p = parity < 0 ? h->hp_full : h->hp_cb[parity];
+    p.dagger = dagger;
+    return launch_hop(p, h->nrhs, d_in, d_out, h->st);
+}
+
+static mrhs_status_t dhop_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int dagger) {
     MRHS_REQUIRE(h && d_in && d_out, "dhop: NULL argument");
     MRHS_REQUIRE(d_in != d_out, "dhop: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "dhop: buffers must be 16-byte aligned");
-    if (h->kern[0] == MRHS_HOP_SWEEP) return launch_sweep(h->sp_full, d_in, d_out, h->st);
-    return launch_hop(h->hp_full, h->nrhs, d_in, d_out, h->st);
+    return hop_launch(h, -1, dagger, nullptr, nullptr, d_in, d_out);
 }
+mrhs_status_t mrhs_dhop(mrhs_wilson_t *h, const void *d_in, void *d_out) { return dhop_impl(h, d_in, d_out, 0); }
+mrhs_status_t mrhs_dhop_dag(mrhs_wilson_t *h, const void *d_in, void *d_out) { return dhop_impl(h, d_in, d_out, 1); }
 
-mrhs_status_t mrhs_meooe(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity) {
+static mrhs_status_t meooe_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity, int dagger) {
     MRHS_REQUIRE(h && d_in && d_out, "meooe: NULL argument");
     MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "meooe: out_parity must be 0 or 1");
     MRHS_REQUIRE(d_in != d_out, "meooe: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "meooe: buffers must be 16-byte aligned");
-    if (h->kern[1] == MRHS_HOP_SWEEP) return launch_sweep(h->sp_cb[out_parity], d_in, d_out, h->st);
-    return launch_hop(h->hp_cb[out_parity], h->nrhs, d_in, d_out, h->st);
+    return hop_launch(h, out_parity, dagger, nullptr, nullptr, d_in, d_out);
 }
+mrhs_status_t mrhs_meooe(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity) { return meooe_impl(h, d_in, d_out, out_parity, 0); }
+mrhs_status_t mrhs_meooe_dag(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity) { return meooe_impl(h, d_in, d_out, out_parity, 1); }
 
-mrhs_status_t mrhs_wilson_apply(mrhs_wilson_t *h, const void *d_in, void *d_out) {
+static mrhs_status_t wilson_apply_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int dagger) {
     MRHS_REQUIRE(h && d_in && d_out, "wilson apply: NULL argument");
     MRHS_REQUIRE(d_in != d_out, "wilson apply: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "wilson apply: buffers must be 16-byte aligned");
-    if (h->kern[0] == MRHS_HOP_SWEEP) {
-        // one launch: C in(x) is formed from the centre slice in shared memory, the eight hops add to it
-        SweepParams p = h->sp_full;
-        p.clover = h->clov_full;
-        return launch_sweep(p, d_in, d_out, h->st);
+    // sweep kernel: one launch, C in(x) is formed from the centre slice in shared memory and the eight hops are added to it
+    if (h->kern[0] == MRHS_HOP_SWEEP) return hop_launch(h, -1, dagger, h->clov_full, nullptr, d_in, d_out);
+    mrhs_status_t s = hop_launch(h, -1, dagger, nullptr, nullptr, d_in, d_out);
+    if (s == MRHS_OK) s = launch_mooee(h->gfull, h->clov_full, d_in, d_out, h->st, -0.5f);
+    return s;
+}
+mrhs_status_t mrhs_wilson_apply(mrhs_wilson_t *h, const void *d_in, void *d_out) { return wilson_apply_impl(h, d_in, d_out, 0); }
+mrhs_status_t mrhs_wilson_apply_dag(mrhs_wilson_t *h, const void *d_in, void *d_out) { return wilson_apply_impl(h, d_in, d_out, 1); }
+
+mrhs_status_t mrhs_schur_apply(mrhs_wilson_t *h, const void *d_in, void *d_tmp, void *d_out, int dagger) {
+    MRHS_REQUIRE(h && d_in && d_tmp && d_out, "schur apply: NULL argument");
+    MRHS_REQUIRE(dagger == 0 || dagger == 1, "schur apply: dagger must be 0 or 1");
+    MRHS_REQUIRE(d_in != d_out && d_in != d_tmp && d_tmp != d_out, "schur apply: the three buffers must be distinct");
+    MRHS_REQUIRE(aligned16(d_in) && aligned16(d_tmp) && aligned16(d_out), "schur apply: buffers must be 16-byte aligned");
+    // S = C_e - H_eo C_o^-1 H_oe / 4 (the daggered hops for S^+; the clover blocks are Hermitian)
+    if (h->kern[1] == MRHS_HOP_SWEEP) {
+        // two launches: tmp = C_o^-1 H_oe in;  out = C_e in - H_eo tmp / 4 (the input is read again by the second epilogue)
+        mrhs_status_t s = hop_launch(h, MRHS_ODD, dagger, h->cinv_cb[MRHS_ODD], nullptr, d_in, d_tmp);
+        if (s == MRHS_OK) s = hop_launch(h, MRHS_EVEN, dagger, h->clov_cb[MRHS_EVEN], d_in, d_tmp, d_out);
+        return s;
     }
-    mrhs_status_t s = launch_hop(h->hp_full, h->nrhs, d_in, d_out, h->st);
-    if (s == MRHS_OK) s = launch_mooee(h->gfull, h->clov_full, d_in, d_out, h->st, true);
+    mrhs_status_t s = hop_launch(h, MRHS_ODD, dagger, nullptr, nullptr, d_in, d_tmp);
+    if (s == MRHS_OK) s = launch_mooee(h->gcb[MRHS_ODD], h->cinv_cb[MRHS_ODD], d_tmp, d_tmp, h->st);
+    if (s == MRHS_OK) s = hop_launch(h, MRHS_EVEN, dagger, nullptr, nullptr, d_tmp, d_out);
+    if (s == MRHS_OK) s = launch_mooee(h->gcb[MRHS_EVEN], h->clov_cb[MRHS_EVEN], d_in, d_out, h->st, -0.25f);
     return s;
 }
 
@@ -257,15 +294,12 @@ static mrhs_status_t meooe_mooee_impl(mrhs_wilson_t *h, const void *d_in, void *
     MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "meooe_mooee: out_parity must be 0 or 1");
     MRHS_REQUIRE(d_in != d_out, "meooe_mooee: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "meooe_mooee: buffers must be 16-byte aligned");
-    if (h->kern[1] == MRHS_HOP_SWEEP) {
-        // one launch: the clover blocks of the output sites are applied to the hop result before it is stored
-        SweepParams p = h->sp_cb[out_parity];
-        p.clover = inverse ? h->cinv_cb[out_parity] : h->clov_cb[out_parity];
-        return launch_sweep(p, d_in, d_out, h->st);
-    }
-    // gather kernel: two launches; the site-diagonal term reads each site's twelve components before it writes them
-    mrhs_status_t s = launch_hop(h->hp_cb[out_parity], h->nrhs, d_in, d_out, h->st);
-    if (s == MRHS_OK) s = launch_mooee(h->gcb[out_parity], inverse ? h->cinv_cb[out_parity] : h->clov_cb[out_parity], d_out, d_out, h->st);
+    const float4 *blocks = inverse ? h->cinv_cb[out_parity] : h->clov_cb[out_parity];
+    // sweep kernel: one launch, the clover blocks of the output sites are applied to the hop result before it is stored
+    if (h->kern[1] == MRHS_HOP_SWEEP) return hop_launch(h, out_parity, 0, blocks, nullptr, d_in, d_out);
+    // gather kernel: two launches, the second in place
+    mrhs_status_t s = hop_launch(h, out_parity, 0, nullptr, nullptr, d_in, d_out);
+    if (s == MRHS_OK) s = launch_mooee(h->gcb[out_parity], blocks, d_out, d_out, h->st);
     return s;
 }
 
@@ -307,6 +341,7 @@ mrhs_status_t mrhs_wilson_set_tiling(mrhs_wilson_t *h, int which, const int tile
         HopParams p;
         MRHS_REQUIRE(build_hop_params(h->gfull, 0, t, p), "set tiling: tiling does not fit the full lattice");
         p.gauge_out = p.gauge_in = h->gauge_full;
+        p.pf_dist = h->hp_full.pf_dist;
         h->hp_full = p;
     } else {
         HopParams p[2];
@@ -314,6 +349,7 @@ mrhs_status_t mrhs_wilson_set_tiling(mrhs_wilson_t *h, int which, const int tile
             MRHS_REQUIRE(build_hop_params(h->gcb[q], q, t, p[q]), "set tiling: tiling does not fit the checkerboarded lattice");
             p[q].gauge_out = h->gauge_cb[q];
             p[q].gauge_in = h->gauge_cb[1 - q];
+            p[q].pf_dist = h->hp_cb[q].pf_dist;
         }
         h->hp_cb[0] = p[0];
         h->hp_cb[1] = p[1];
@@ -361,6 +397,7 @@ mrhs_status_t mrhs_wilson_set_sweep(mrhs_wilson_t *h, int which, int lt, const i
         SweepParams p;
         MRHS_REQUIRE(build_sweep_params(h->gfull, 0, t, p), "set sweep: segment / chunk does not fit the full lattice (or odd N_rhs)");
         p.gauge_out = p.gauge_in = h->gauge_full;
+        p.pf = h->sp_full.pf;
         h->sp_full = p;
     } else {
         SweepParams p[2];
@@ -368,6 +405,7 @@ mrhs_status_t mrhs_wilson_set_sweep(mrhs_wilson_t *h, int which, int lt, const i
             MRHS_REQUIRE(build_sweep_params(h->gcb[q], q, t, p[q]), "set sweep: segment / chunk does not fit the checkerboarded lattice (or odd N_rhs)");
             p[q].gauge_out = h->gauge_cb[q];
             p[q].gauge_in = h->gauge_cb[1 - q];
+            p[q].pf = h->sp_cb[q].pf;
         }
         h->sp_cb[0] = p[0];
         h->sp_cb[1] = p[1];

@@ -212,11 +212,13 @@ __global__ void invert_blocks_kernel(const float *__restrict__ packed, float *__
 // ------------------------------------------------------------------ M_ooee apply
 // One thread = one site and R right-hand sides; the 72 packed floats of the site are fetched
 // once and reused by every RHS.  One chirality at a time keeps the live set at 6 + 6 elements.
-// AXPY: out = C in - out / 2 (out holds the hopping sum: the full Wilson-clover matrix of reading S6, gather-kernel path)
-template <int R, bool AXPY>
+// MODE 0: out = C in.  MODE 1: out = C in + scale * out (out holds a hopping sum: scale -1/2 gives the full Wilson-clover
+// matrix of reading S6, -1/4 the Schur complement; gather-kernel paths).  MODE 2: out = C out, in place (in is not read; a
+// thread reads the six components of a chirality before it writes them, and no other thread touches them).
+template <int R, int MODE>
 __global__ void __launch_bounds__(256)
-mooee_kernel(int XB, int NP, long long nthreads, const float4 *__restrict__ clov,
-             const typename Elem<R>::type *__restrict__ in, typename Elem<R>::type *__restrict__ out) {
+mooee_kernel(int XB, int NP, long long nthreads, float scale, const float4 *__restrict__ clov,
+             const typename Elem<R>::type *in, typename Elem<R>::type *out) {
     typedef typename Elem<R>::type E;
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= nthreads) return;
@@ -231,7 +233,7 @@ mooee_kernel(int XB, int NP, long long nthreads, const float4 *__restrict__ clov
     for (int ch = 0; ch < 2; ch++) {
         CVec<R> psi[6];
 #pragma unroll
-        for (int c = 0; c < 6; c++) psi[c] = to_cvec(__ldg(pi + (size_t)(6 * ch + c) * CS));
+        for (int c = 0; c < 6; c++) psi[c] = to_cvec(MODE == 2 ? po[(size_t)(6 * ch + c) * CS] : __ldg(pi + (size_t)(6 * ch + c) * CS));
         float a[36];
 #pragma unroll
         for (int j = 0; j < 9; j++) {
@@ -251,7 +253,7 @@ mooee_kernel(int XB, int NP, long long nthreads, const float4 *__restrict__ clov
                     r = cfma_conj(a[6 + 2 * idx], a[6 + 2 * idx + 1], psi[j], r);
                 }
             }
-            if constexpr (AXPY) r = rfma(-0.5f, to_cvec(po[(size_t)(6 * ch + i) * CS]), r);
+            if constexpr (MODE == 1) r = rfma(scale, to_cvec(po[(size_t)(6 * ch + i) * CS]), r);
             po[(size_t)(6 * ch + i) * CS] = from_cvec(r);
         }
     }
@@ -289,17 +291,18 @@ mrhs_status_t unpack_clover_blocks(long long nsites, const float *d_packed, floa
     return MRHS_OK;
 }
 
-mrhs_status_t launch_mooee(const FieldGeom &g, const float4 *d_clover, const void *d_in, void *d_out, cudaStream_t st, bool axpy) {
+mrhs_status_t launch_mooee(const FieldGeom &g, const float4 *d_clover, const void *d_in, void *d_out, cudaStream_t st, float axpy_scale) {
     const int np = threads_per_site(g.N);
     const long long nthreads = g.nsites * np;
-    const long long blocks = (nthreads + 255) / 256;
+    const unsigned blocks = (unsigned)((nthreads + 255) / 256);
+    const int mode = d_in == d_out ? 2 : (axpy_scale != 0.f ? 1 : 0);
+#define MRHS_MOOEE(R, E, MODE) mooee_kernel<R, MODE><<<blocks, 256, 0, st>>>(g.XB, np, nthreads, axpy_scale, d_clover, (const E *)d_in, (E *)d_out)
     if (g.N & 1) {
-        if (axpy) mooee_kernel<1, true><<<(unsigned)blocks, 256, 0, st>>>(g.XB, np, nthreads, d_clover, (const float2 *)d_in, (float2 *)d_out);
-        else      mooee_kernel<1, false><<<(unsigned)blocks, 256, 0, st>>>(g.XB, np, nthreads, d_clover, (const float2 *)d_in, (float2 *)d_out);
+        if (mode == 2) MRHS_MOOEE(1, float2, 2); else if (mode == 1) MRHS_MOOEE(1, float2, 1); else MRHS_MOOEE(1, float2, 0);
     } else {
-        if (axpy) mooee_kernel<2, true><<<(unsigned)blocks, 256, 0, st>>>(g.XB, np, nthreads, d_clover, (const float4 *)d_in, (float4 *)d_out);
-        else      mooee_kernel<2, false><<<(unsigned)blocks, 256, 0, st>>>(g.XB, np, nthreads, d_clover, (const float4 *)d_in, (float4 *)d_out);
+        if (mode == 2) MRHS_MOOEE(2, float4, 2); else if (mode == 1) MRHS_MOOEE(2, float4, 1); else MRHS_MOOEE(2, float4, 0);
     }
+#undef MRHS_MOOEE
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
 }

@@ -14,10 +14,10 @@ namespace {
 
 template <int R, int MU, bool FWD>
 __device__ __forceinline__ void hop_dir(const typename Elem<R>::type *__restrict__ nb, size_t cs,
-                                        const float4 *__restrict__ g, int XB, CVec<R> (&acc)[12]) {
+                                        const float4 *__restrict__ g, int XB, CVec<R> (&acc)[12], float dg) {
     HopOperands<R> o;
     hop_load<R, MU>(o, nb, cs, g, XB);
-    hop_compute<R, MU, FWD>(o, acc);
+    hop_compute<R, MU, FWD>(o, acc, dg);
 }
 
 // blk -> origin of its tile.  Sweep order: x-blocks, then y and z tiles inside a chunk, then t, then chunks.
@@ -114,6 +114,7 @@ hop_kernel(const HopParams p, const typename Elem<R>::type *__restrict__ in, typ
 #pragma unroll
     for (int c = 0; c < 12; c++) acc[c] = czero<R>();
 
+    const float dg = p.dagger ? -1.f : 1.f;      // -1: the adjoint (projector signs exchanged, hop_math.cuh)
     const float4 *gown = MRHS_LINK(p.gauge_out, b, xin);
     const E *n0p = MRHS_ELEM(bxp, xinp), *n0m = MRHS_ELEM(bxm, xinm);
     const E *n1p = MRHS_ELEM(byp, xin), *n1m = MRHS_ELEM(bym, xin);
@@ -126,23 +127,23 @@ hop_kernel(const HopParams p, const typename Elem<R>::type *__restrict__ in, typ
         HopOperands<R> A, B;
         hop_load<R, 0>(A, n0p, cs, gown, XB);
         hop_load<R, 0>(B, n0m, cs, g0m, XB);
-        hop_compute<R, 0, true >(A, acc);  hop_load<R, 1>(A, n1p, cs, gown, XB);
-        hop_compute<R, 0, false>(B, acc);  hop_load<R, 1>(B, n1m, cs, g1m, XB);
-        hop_compute<R, 1, true >(A, acc);  hop_load<R, 2>(A, n2p, cs, gown, XB);
-        hop_compute<R, 1, false>(B, acc);  hop_load<R, 2>(B, n2m, cs, g2m, XB);
-        hop_compute<R, 2, true >(A, acc);  hop_load<R, 3>(A, n3p, cs, gown, XB);
-        hop_compute<R, 2, false>(B, acc);  hop_load<R, 3>(B, n3m, cs, g3m, XB);
-        hop_compute<R, 3, true >(A, acc);
-        hop_compute<R, 3, false>(B, acc);
+        hop_compute<R, 0, true >(A, acc, dg);  hop_load<R, 1>(A, n1p, cs, gown, XB);
+        hop_compute<R, 0, false>(B, acc, dg);  hop_load<R, 1>(B, n1m, cs, g1m, XB);
+        hop_compute<R, 1, true >(A, acc, dg);  hop_load<R, 2>(A, n2p, cs, gown, XB);
+        hop_compute<R, 1, false>(B, acc, dg);  hop_load<R, 2>(B, n2m, cs, g2m, XB);
+        hop_compute<R, 2, true >(A, acc, dg);  hop_load<R, 3>(A, n3p, cs, gown, XB);
+        hop_compute<R, 2, false>(B, acc, dg);  hop_load<R, 3>(B, n3m, cs, g3m, XB);
+        hop_compute<R, 3, true >(A, acc, dg);
+        hop_compute<R, 3, false>(B, acc, dg);
     } else {
-        hop_dir<R, 0, true >(n0p, cs, gown, XB, acc);
-        hop_dir<R, 0, false>(n0m, cs, g0m, XB, acc);
-        hop_dir<R, 1, true >(n1p, cs, gown, XB, acc);
-        hop_dir<R, 1, false>(n1m, cs, g1m, XB, acc);
-        hop_dir<R, 2, true >(n2p, cs, gown, XB, acc);
-        hop_dir<R, 2, false>(n2m, cs, g2m, XB, acc);
-        hop_dir<R, 3, true >(n3p, cs, gown, XB, acc);
-        hop_dir<R, 3, false>(n3m, cs, g3m, XB, acc);
+        hop_dir<R, 0, true >(n0p, cs, gown, XB, acc, dg);
+        hop_dir<R, 0, false>(n0m, cs, g0m, XB, acc, dg);
+        hop_dir<R, 1, true >(n1p, cs, gown, XB, acc, dg);
+        hop_dir<R, 1, false>(n1m, cs, g1m, XB, acc, dg);
+        hop_dir<R, 2, true >(n2p, cs, gown, XB, acc, dg);
+        hop_dir<R, 2, false>(n2m, cs, g2m, XB, acc, dg);
+        hop_dir<R, 3, true >(n3p, cs, gown, XB, acc, dg);
+        hop_dir<R, 3, false>(n3m, cs, g3m, XB, acc, dg);
     }
 
     E *o = out + ((size_t)b * 12 * XB + xin) * NP + lane;
@@ -268,6 +269,7 @@ bool build_hop_params(const FieldGeom &g, int out_parity, const HopTiling &t, Ho
     p.Y = g.Y; p.Z = g.Z; p.T = g.T;
     p.XB = g.XB; p.nxb = g.nxb; p.NP = np;
     p.cb = g.cb; p.out_parity = out_parity;
+    p.dagger = 0;
     p.by = t.by; p.bz = t.bz; p.bt = t.bt; p.cy = t.cy; p.cz = t.cz;
     bool ok = true;
     ok &= make_fastdiv(np, kHopMaxThreads, p.d_np);
@@ -284,7 +286,7 @@ bool build_hop_params(const FieldGeom &g, int out_parity, const HopTiling &t, Ho
     // default prefetch distance: one t-step of the chunk (the t+1 rows a tile reads) plus two waves of tiles
     // default prefetch distance: about half of the tiles resident on the GPU at once (two per SM).  Farther
     // ahead the prefetched rows are evicted again before their tile runs and DRAM reads double (measured).
-    p.pf_dist = 2u * 148u;
+    p.pf_dist = 2u * 148u;      // the handle replaces this with twice its SM count
     p.grid = (unsigned)grid;
     p.threads = (unsigned)threads;
     return true;

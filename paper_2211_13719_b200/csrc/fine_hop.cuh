@@ -20,6 +20,7 @@ struct HopParams {
     int Y, Z, T;              // lattice extents (x enters through Xe, XB, nxb)
     int XB, nxb, NP;          // layout block, blocks per x-line, threads per site
     int cb, out_parity;       // checkerboarded fields? parity of the output field
+    int dagger;               // 1: apply the adjoint D_hop^+ = gamma_5 D_hop gamma_5
     int by, bz, bt;           // tile extents
     int cy, cz;               // chunk extents in tiles
     unsigned pf_dist;         // L2 prefetch distance in tiles of the sweep order (0 = off)
@@ -55,7 +56,7 @@ mrhs_status_t pack_clover_blocks(long long nsites, const float2 *d_blocks, float
 // packed blocks [lex][72] -> packed inverse blocks (fp64 Gauss-Jordan per 6x6 block)
 mrhs_status_t invert_clover_blocks(long long nsites, const float *d_packed, float *d_packed_inv, cudaStream_t st);
 mrhs_status_t unpack_clover_blocks(long long nsites, const float *d_packed, float2 *d_blocks, cudaStream_t st);
-// axpy: out = C in - out / 2 instead of out = C in
-mrhs_status_t launch_mooee(const FieldGeom &g, const float4 *d_clover, const void *d_in, void *d_out, cudaStream_t st, bool axpy = false);
+// axpy_scale != 0: out = C in + axpy_scale * out instead of out = C in (-1/2: full matrix, -1/4: Schur complement)
+mrhs_status_t launch_mooee(const FieldGeom &g, const float4 *d_clover, const void *d_in, void *d_out, cudaStream_t st, float axpy_scale = 0.f);
 
 }  // namespace mrhs

@@ -96,18 +96,19 @@ __device__ __forceinline__ void split_load(SplitOperands &o, const float4 *nb, i
 
 // This lane's row of the projected half spinor and of r = U h (FWD) or U^+ h.  Spin row s (e = +1 for s = 0, -1 for s = 1):
 //   x: h_s = psi_s + S i psi_{3-s}     y: h_s = psi_s + e S psi_{3-s}     z: h_s = psi_s + e S i psi_{2+s}     t: h_s = psi_s - S psi_{2+s}
-// with S = +1 for the forward hop (reading S2/S3, the rows of hop_half in hop_math.cuh).
+// with S = +1 for the forward hop (reading S2/S3, the rows of hop_half in hop_math.cuh).  d = +1: the operator as written;
+// d = -1: its adjoint (gamma_5 D_hop gamma_5: S -> -S in projection and reconstruction, links unchanged); ed = e d.
+// Every sign is the scalar operand of an FFMA2 (a * (+-1) is exact), so both variants cost the same.
 template <int MU, bool FWD>
-__device__ __forceinline__ void split_half(const SplitOperands &o, float e, CVec<2> (&r)[3]) {
-    const float sg = FWD ? e : -e;
+__device__ __forceinline__ void split_half(const SplitOperands &o, float d, float ed, CVec<2> (&r)[3]) {
+    const float sg = (MU == 1 || MU == 2) ? (FWD ? ed : -ed) : (FWD ? d : -d);
     CVec<2> h[3];
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         const CVec<2> a = to_cvec(o.ps[c]), b = to_cvec(o.pp[c]);
-        if constexpr (MU == 0) h[c] = FWD ? cadd_i(a, b) : csub_i(a, b);
+        if constexpr (MU == 0 || MU == 2) { h[c].re = sfnma(sg, b.im, a.re); h[c].im = sfma(sg, b.re, a.im); }
         else if constexpr (MU == 1) h[c] = rfma(sg, b, a);
-        else if constexpr (MU == 2) { h[c].re = sfnma(sg, b.im, a.re); h[c].im = sfma(sg, b.re, a.im); }
-        else h[c] = FWD ? csub(a, b) : cadd(a, b);
+        else h[c] = rfma(-sg, b, a);
     }
     const float (&u)[18] = o.u;
 #pragma unroll
@@ -127,13 +128,15 @@ __device__ __forceinline__ void split_half(const SplitOperands &o, float e, CVec
 // This lane's share of the reconstruction: up (output spin row s) += r; the lower rows get
 //   x: out_{3-s} -= S i r     y: out_{3-s} += e S r     (accumulated in la)
 //   z: out_{2+s} -= e S i r   t: out_{2+s} -= S r       (accumulated in lb)
+// For the adjoint (d = -1) S changes sign.  lb is kept as d times its true value, so that the z and t updates do not depend
+// on d (d d = 1) and the -t carry enters with +1; whoever reads lb multiplies it by d (one FFMA2 in place of an FADD2).
 template <int MU, bool FWD>
-__device__ __forceinline__ void split_recon(const CVec<2> (&r)[3], float e, CVec<2> (&up)[3], CVec<2> (&la)[3], CVec<2> (&lb)[3]) {
-    const float sg = FWD ? e : -e;
+__device__ __forceinline__ void split_recon(const CVec<2> (&r)[3], float d, float e, float ed, CVec<2> (&up)[3], CVec<2> (&la)[3], CVec<2> (&lb)[3]) {
+    const float sg = MU == 1 ? (FWD ? ed : -ed) : MU == 2 ? (FWD ? e : -e) : (FWD ? d : -d);
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         up[c] = cadd(up[c], r[c]);
-        if constexpr (MU == 0) la[c] = FWD ? csub_i(la[c], r[c]) : cadd_i(la[c], r[c]);
+        if constexpr (MU == 0) { la[c].re = sfma(sg, r[c].im, la[c].re); la[c].im = sfnma(sg, r[c].re, la[c].im); }
         else if constexpr (MU == 1) la[c] = rfma(sg, r[c], la[c]);
         else if constexpr (MU == 2) { lb[c].re = sfma(sg, r[c].im, lb[c].re); lb[c].im = sfnma(sg, r[c].re, lb[c].im); }
         else lb[c] = FWD ? csub(lb[c], r[c]) : cadd(lb[c], r[c]);
@@ -141,10 +144,10 @@ __device__ __forceinline__ void split_recon(const CVec<2> (&r)[3], float e, CVec
 }
 
 template <int MU, bool FWD>
-__device__ __forceinline__ void split_hop(const SplitOperands &o, float e, CVec<2> (&up)[3], CVec<2> (&la)[3], CVec<2> (&lb)[3]) {
+__device__ __forceinline__ void split_hop(const SplitOperands &o, float d, float e, float ed, CVec<2> (&up)[3], CVec<2> (&la)[3], CVec<2> (&lb)[3]) {
     CVec<2> r[3];
-    split_half<MU, FWD>(o, e, r);
-    split_recon<MU, FWD>(r, e, up, la, lb);
+    split_half<MU, FWD>(o, d, ed, r);
+    split_recon<MU, FWD>(r, d, e, ed, up, la, lb);
 }
 
 // out = C v for ONE packed Hermitian 6x6 block (6 real diagonals + 15 complex lower-triangle entries, reading S7);
@@ -173,11 +176,14 @@ __device__ __forceinline__ void clover_block_mul(const float4 *pc, int XB, const
 //   1: out = C H                                 M_ooee M_eooe, the first two steps of the Schur sequence (row a7), checkerboarded
 //   2: out = C in - H / 2                        the full Wilson-clover matrix M (reading S6), full lattice: the centre
 //                                                slice in shared memory holds in(x) itself
+//   3: out = C aux - H / 4                       second launch of the even-odd preconditioned (Schur complement) operator
+//                                                C_e - H_eo C_o^-1 H_oe / 4 (NEXT-2): checkerboarded, aux = the operator's
+//                                                input on the output sites, read from global memory
 template <int XB_, int NP_, bool CB, int EPI>
 __global__ void __launch_bounds__(kSweepMaxThreads, 1)
 hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__restrict__ out) {
     constexpr bool CLOV = EPI != 0;
-    static_assert(EPI == 0 || (EPI == 1 && CB) || (EPI == 2 && !CB), "fused epilogues: C H on checkerboarded fields, C in - H/2 on the full lattice");
+    static_assert(EPI == 0 || ((EPI == 1 || EPI == 3) && CB) || (EPI == 2 && !CB), "fused epilogues: C H and C aux - H/4 on checkerboarded fields, C in - H/2 on the full lattice");
     const int XB = XB_ ? XB_ : p.XB;
     const int NP = NP_ ? NP_ : p.NP;
     const int cs = XB * NP;                       // units (site, RHS pair) per tile row = elements of one row component
@@ -326,7 +332,9 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     // ---------------------------------------------------------------------- consumers
     warpgroup_reg_inc<kSweepConsumerRegs>();
     const int s = lane >> 4;                          // spin row of the half spinor this lane owns
-    const float e = s ? -1.f : 1.f;
+    const float d = p.dagger ? -1.f : 1.f;            // -1: the adjoint operator (projector signs exchanged)
+    const float e = s ? -1.f : 1.f;                   // sign of this lane's spin row in the y and z projectors
+    const float ed = e * d;
     const int r = wid / WPR;                          // tile row
     const int u0 = (wid - r * WPR) * 16 + (lane & 15);
     const bool live = u0 < cs;                        // lanes past the end of a row repeat unit 0 and store nothing
@@ -399,7 +407,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     mbar_wait(&fullI[0], 0);
     mbar_wait(&fullG[0], 0);
     split_load<3>(A, Sown, os, ob, cs, S + g_bt, XB);
-    split_half<3, false>(A, e, c1);
+    split_half<3, false>(A, d, ed, c1);
     __syncwarp();
     if (lane == 0) { mbar_arrive(&freeI[0]); mbar_arrive(&freeG[0]); }
     mbar_wait(&fullI[1], 0);
@@ -417,26 +425,26 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
         const float4 *G = S + b * G4;
         const float4 *Sb = S + bo;
 #pragma unroll
-        for (int c = 0; c < 3; c++) { up[c] = c1[c]; lb[c] = c1[c]; la[c] = czero<2>(); }    // the -t hop (S = -1): up += r, out_{2+s} += r
+        for (int c = 0; c < 3; c++) { up[c] = c1[c]; lb[c] = c1[c]; la[c] = czero<2>(); }    // the -t hop (S = -1): up += r, out_{2+s} += d r (lb holds d times its value)
         if (more) {
             // A still holds the own rows of this slice (loaded as the +t neighbour of the step before): the -t hop of the next slice
             load_link_s<3>(G + g_bt, XB, A.u);
-            split_half<3, false>(A, e, c1);
+            split_half<3, false>(A, d, ed, c1);
         }
         // y hops
         mbar_wait(&fullH[0], (uint32_t)k & 1u);
         split_load<1>(A, yp_bs ? Sb + yp_o : S + yp_o, os, oa, cs, G + g_own, XB);
-        split_hop<1, true>(A, e, up, la, lb);
+        split_hop<1, true>(A, d, e, ed, up, la, lb);
         split_load<1>(A, ym_bs ? Sb + ym_o : S + ym_o, os, oa, cs, G + g_by, XB);
-        split_hop<1, false>(A, e, up, la, lb);
+        split_hop<1, false>(A, d, e, ed, up, la, lb);
         __syncwarp();
         if (lane == 0) mbar_arrive(&freeH[0]);
         // z hops
         mbar_wait(&fullH[1], (uint32_t)k & 1u);
         split_load<2>(A, zp_bs ? Sb + zp_o : S + zp_o, os, ob, cs, G + g_own, XB);
-        split_hop<2, true>(A, e, up, la, lb);
+        split_hop<2, true>(A, d, e, ed, up, la, lb);
         split_load<2>(A, zm_bs ? Sb + zm_o : S + zm_o, os, ob, cs, G + g_bz, XB);
-        split_hop<2, false>(A, e, up, la, lb);
+        split_hop<2, false>(A, d, e, ed, up, la, lb);
         __syncwarp();
         if (lane == 0) mbar_arrive(&freeH[1]);
         // x hops (checkerboarded lines alternate with t: one neighbour has this unit's own index, the other is one site on)
@@ -450,9 +458,9 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
             }
             cp_async_wait<0>();                // this lane's x halo slots hold slice k
             split_load<0>(A, xp, rs * xp_st, ra * xp_st, xp_st, G + g_own, XB);
-            split_hop<0, true>(A, e, up, la, lb);
+            split_hop<0, true>(A, d, e, ed, up, la, lb);
             split_load<0>(A, xm, rs * xm_st, ra * xm_st, xm_st, G + g_bx, XB);
-            split_hop<0, false>(A, e, up, la, lb);
+            split_hop<0, false>(A, d, e, ed, up, la, lb);
         }
         gxp += st; gxm += st;
         if (tn == 0) { gxp -= st * T; gxm -= st * T; }
@@ -468,12 +476,12 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
 #pragma unroll
             for (int c = 0; c < 3; c++) { A.ps[c] = Sn[os + c * cs]; A.pp[c] = Sn[ob + c * cs]; }
             load_link_s<3>(G + g_own, XB, A.u);
-            split_hop<3, true>(A, e, up, la, lb);      // A.ps / A.pp stay live: the next step's -t carry is made from them
+            split_hop<3, true>(A, d, e, ed, up, la, lb);      // A.ps / A.pp stay live: the next step's -t carry is made from them
         }
         if constexpr (EPI == 0) {
             // lane s holds out_s (up), its share of out_{3-s} (la) and the partner's missing share of out_{2+s} (lb)
 #pragma unroll
-            for (int c = 0; c < 3; c++) la[c] = cadd(la[c], shfl_half(lb[c]));
+            for (int c = 0; c < 3; c++) la[c] = rfma(d, shfl_half(lb[c]), la[c]);
             if (live) {
 #pragma unroll
                 for (int c = 0; c < 3; c++) {
@@ -487,8 +495,8 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
 #pragma unroll
             for (int c = 0; c < 3; c++) {
                 const CVec<2> pu = shfl_half(up[c]), pla = shfl_half(la[c]), plb = shfl_half(lb[c]);
-                H[c] = csel(s != 0, cadd(plb, la[c]), up[c]);          // s = 1: out_2 = lb(lane s=0) + la;  s = 0: out_0
-                H[3 + c] = csel(s != 0, cadd(pla, lb[c]), pu);         // s = 1: out_3 = la(lane s=0) + lb;  s = 0: out_1 (the partner's up)
+                H[c] = csel(s != 0, rfma(d, plb, la[c]), up[c]);       // s = 1: out_2 = lb(lane s=0) + la;  s = 0: out_0
+                H[3 + c] = csel(s != 0, rfma(d, lb[c], pla), pu);      // s = 1: out_3 = la(lane s=0) + lb;  s = 0: out_1 (the partner's up)
             }
             const float4 *pc = S + L.off_C / 16 + b * (L.C_BYTES / 16) + r * (18 * XB) + 9 * s * XB + xin;   // this site's block of chirality s
             CVec<2> res[6];
@@ -496,13 +504,21 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
                 clover_block_mul(pc, XB, H, res);
             } else {
                 CVec<2> v[6];
+                if constexpr (EPI == 2) {
 #pragma unroll
-                for (int i = 0; i < 6; i++) v[i] = to_cvec(Sb[own + (6 * s + i) * cs]);
+                    for (int i = 0; i < 6; i++) v[i] = to_cvec(Sb[own + (6 * s + i) * cs]);
+                } else {
+                    const float4 *ax = p.aux + (o - out);       // the same element of the auxiliary field
+#pragma unroll
+                    for (int i = 0; i < 6; i++) v[i] = to_cvec(__ldg(ax + (size_t)(6 * s + i) * cs));
+                }
                 clover_block_mul(pc, XB, v, res);
 #pragma unroll
-                for (int i = 0; i < 6; i++) res[i] = rfma(-0.5f, H[i], res[i]);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&freeI[b]);
+                for (int i = 0; i < 6; i++) res[i] = rfma(EPI == 2 ? -0.5f : -0.25f, H[i], res[i]);
+                if constexpr (EPI == 2) {
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&freeI[b]);
+                }
             }
             if (live) {
 #pragma unroll
@@ -589,6 +605,8 @@ bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t
     if (!ok) return false;
     p.gauge_out = p.gauge_in = nullptr;
     p.clover = nullptr;
+    p.aux = nullptr;
+    p.dagger = 0;
     p.pf = 0;   // bulk L2 prefetch of later slices: measured to add DRAM traffic (early lines are evicted before use) and no speed
     const int wpr = (g.XB * np + 15) / 16;
     p.threads = (unsigned)(ROWS * wpr + kSweepProducerWarps) * 32u;
@@ -606,7 +624,8 @@ mrhs_status_t sweep_prepare() {
     MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem)); \
     MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));  \
     MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));  \
-    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem)); \
+    MRHS_CUDA(cudaFuncSetAttribute(hop_sweep_kernel<XB, NP, true, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
     MRHS_SWEEP_LIST(MRHS_CASE)
 #undef MRHS_CASE
     return MRHS_OK;
@@ -615,7 +634,8 @@ mrhs_status_t sweep_prepare() {
 namespace {
 template <int XB, int NP>
 void launch_sweep_t(const SweepParams &p, const void *d_in, void *d_out, cudaStream_t st) {
-    if (p.cb && p.clover) hop_sweep_kernel<XB, NP, true, 1><<<p.grid, p.threads, p.smem_bytes_clover, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    if (p.cb && p.clover && p.aux) hop_sweep_kernel<XB, NP, true, 3><<<p.grid, p.threads, p.smem_bytes_clover, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
+    else if (p.cb && p.clover) hop_sweep_kernel<XB, NP, true, 1><<<p.grid, p.threads, p.smem_bytes_clover, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
     else if (p.cb)        hop_sweep_kernel<XB, NP, true, 0><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
     else if (p.clover)    hop_sweep_kernel<XB, NP, false, 2><<<p.grid, p.threads, p.smem_bytes_clover, st>>>(p, (const float4 *)d_in, (float4 *)d_out);
     else                  hop_sweep_kernel<XB, NP, false, 0><<<p.grid, p.threads, p.smem_bytes, st>>>(p, (const float4 *)d_in, (float4 *)d_out);

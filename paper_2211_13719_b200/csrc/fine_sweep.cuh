@@ -34,6 +34,8 @@ struct SweepParams {
     const float4 *gauge_out;      // links on the sites of the output field, [block][18][xin] float4
     const float4 *gauge_in;       // links on the sites of the input field
     const float4 *clover;         // packed clover blocks on the sites of the output field: non-null => out = C H (checkerboarded) or C in - H/2 (full lattice)
+    const float4 *aux;            // with clover on checkerboarded fields: non-null => out = C aux - H/4 (Schur complement, second launch)
+    int dagger;                   // 1: the adjoint hopping term (gamma_5 D_hop gamma_5)
     unsigned grid, threads;
     unsigned smem_bytes, smem_bytes_clover;   // dynamic shared memory without / with the clover blocks of the fused epilogues
 };

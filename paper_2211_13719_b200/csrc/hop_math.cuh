@@ -94,29 +94,33 @@ __device__ __forceinline__ void hop_load_s(HopOperands<2> &o, const float4 *nb, 
 // One of the eight hops in two stages.  FWD: (1 - gamma_MU) U_MU(x) psi(x+MU); else (1 + gamma_MU) U_MU(x-MU)^+ psi(x-MU).
 // hop_half: spin projection to a half spinor and colour multiply, r = U h or U^+ h (6 complex numbers);
 // hop_recon: acc += the four spin components rebuilt from r.  hop_compute does both.
+// dg = +1: the operator as written; dg = -1: its adjoint D_hop^+ = gamma_5 D_hop gamma_5 (gamma_5 = diag(1,1,-1,-1), reading S2;
+// SURVEY.md Sec. 8(f) NEXT-2), i.e. the same links with the projector signs exchanged.  The sign rides as the scalar operand of
+// an FMA that replaces the add (same instruction count, and a * (+-1) is exact).
 template <int R, int MU, bool FWD>
-__device__ __forceinline__ void hop_half(const HopOperands<R> &o, CVec<R> (&r)[6]) {
+__device__ __forceinline__ void hop_half(const HopOperands<R> &o, CVec<R> (&r)[6], float dg) {
     CVec<R> psi[12];
 #pragma unroll
     for (int c = 0; c < 12; c++) psi[c] = to_cvec(o.psi[c]);
     const float (&u)[18] = o.u;
+    const float sg = FWD ? dg : -dg;      // S of the projector (1 - S gamma_MU)
 
-    // spin projection: h = upper two spin components of (1 -+ gamma_MU) psi  (S = +1 for FWD)
+    // spin projection: h = upper two spin components of (1 - S gamma_MU) psi
     CVec<R> h[6];
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         if constexpr (MU == 0) {          // h0 = psi0 + S i psi3 ; h1 = psi1 + S i psi2
-            h[c]     = FWD ? cadd_i(psi[c], psi[9 + c])     : csub_i(psi[c], psi[9 + c]);
-            h[3 + c] = FWD ? cadd_i(psi[3 + c], psi[6 + c]) : csub_i(psi[3 + c], psi[6 + c]);
+            h[c]     = {sfnma(sg, psi[9 + c].im, psi[c].re),     sfma(sg, psi[9 + c].re, psi[c].im)};
+            h[3 + c] = {sfnma(sg, psi[6 + c].im, psi[3 + c].re), sfma(sg, psi[6 + c].re, psi[3 + c].im)};
         } else if constexpr (MU == 1) {   // h0 = psi0 + S psi3 ; h1 = psi1 - S psi2
-            h[c]     = FWD ? cadd(psi[c], psi[9 + c])     : csub(psi[c], psi[9 + c]);
-            h[3 + c] = FWD ? csub(psi[3 + c], psi[6 + c]) : cadd(psi[3 + c], psi[6 + c]);
+            h[c]     = rfma(sg, psi[9 + c], psi[c]);
+            h[3 + c] = rfma(-sg, psi[6 + c], psi[3 + c]);
         } else if constexpr (MU == 2) {   // h0 = psi0 + S i psi2 ; h1 = psi1 - S i psi3
-            h[c]     = FWD ? cadd_i(psi[c], psi[6 + c])     : csub_i(psi[c], psi[6 + c]);
-            h[3 + c] = FWD ? csub_i(psi[3 + c], psi[9 + c]) : cadd_i(psi[3 + c], psi[9 + c]);
+            h[c]     = {sfnma(sg, psi[6 + c].im, psi[c].re),    sfma(sg, psi[6 + c].re, psi[c].im)};
+            h[3 + c] = {sfma(sg, psi[9 + c].im, psi[3 + c].re), sfnma(sg, psi[9 + c].re, psi[3 + c].im)};
         } else {                          // h0 = psi0 - S psi2 ; h1 = psi1 - S psi3
-            h[c]     = FWD ? csub(psi[c], psi[6 + c])     : cadd(psi[c], psi[6 + c]);
-            h[3 + c] = FWD ? csub(psi[3 + c], psi[9 + c]) : cadd(psi[3 + c], psi[9 + c]);
+            h[c]     = rfma(-sg, psi[6 + c], psi[c]);
+            h[3 + c] = rfma(-sg, psi[9 + c], psi[3 + c]);
         }
     }
 
@@ -140,33 +144,34 @@ __device__ __forceinline__ void hop_half(const HopOperands<R> &o, CVec<R> (&r)[6
 }
 
 template <int R, int MU, bool FWD>
-__device__ __forceinline__ void hop_recon(const CVec<R> (&r)[6], CVec<R> (&acc)[12]) {
+__device__ __forceinline__ void hop_recon(const CVec<R> (&r)[6], CVec<R> (&acc)[12], float dg) {
     // reconstruction: upper components get r, lower ones -S i sigma_MU r (spatial) or -S r (time)
+    const float sg = FWD ? dg : -dg;
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         acc[c] = cadd(acc[c], r[c]);
         acc[3 + c] = cadd(acc[3 + c], r[3 + c]);
         if constexpr (MU == 0) {          // out2 += -S i r1 ; out3 += -S i r0
-            acc[6 + c] = FWD ? csub_i(acc[6 + c], r[3 + c]) : cadd_i(acc[6 + c], r[3 + c]);
-            acc[9 + c] = FWD ? csub_i(acc[9 + c], r[c])     : cadd_i(acc[9 + c], r[c]);
+            acc[6 + c] = {sfma(sg, r[3 + c].im, acc[6 + c].re), sfnma(sg, r[3 + c].re, acc[6 + c].im)};
+            acc[9 + c] = {sfma(sg, r[c].im, acc[9 + c].re),     sfnma(sg, r[c].re, acc[9 + c].im)};
         } else if constexpr (MU == 1) {   // out2 += -S r1 ; out3 += S r0
-            acc[6 + c] = FWD ? csub(acc[6 + c], r[3 + c]) : cadd(acc[6 + c], r[3 + c]);
-            acc[9 + c] = FWD ? cadd(acc[9 + c], r[c])     : csub(acc[9 + c], r[c]);
+            acc[6 + c] = rfma(-sg, r[3 + c], acc[6 + c]);
+            acc[9 + c] = rfma(sg, r[c], acc[9 + c]);
         } else if constexpr (MU == 2) {   // out2 += -S i r0 ; out3 += S i r1
-            acc[6 + c] = FWD ? csub_i(acc[6 + c], r[c])     : cadd_i(acc[6 + c], r[c]);
-            acc[9 + c] = FWD ? cadd_i(acc[9 + c], r[3 + c]) : csub_i(acc[9 + c], r[3 + c]);
+            acc[6 + c] = {sfma(sg, r[c].im, acc[6 + c].re),      sfnma(sg, r[c].re, acc[6 + c].im)};
+            acc[9 + c] = {sfnma(sg, r[3 + c].im, acc[9 + c].re), sfma(sg, r[3 + c].re, acc[9 + c].im)};
         } else {                          // out2 += -S r0 ; out3 += -S r1
-            acc[6 + c] = FWD ? csub(acc[6 + c], r[c])     : cadd(acc[6 + c], r[c]);
-            acc[9 + c] = FWD ? csub(acc[9 + c], r[3 + c]) : cadd(acc[9 + c], r[3 + c]);
+            acc[6 + c] = rfma(-sg, r[c], acc[6 + c]);
+            acc[9 + c] = rfma(-sg, r[3 + c], acc[9 + c]);
         }
     }
 }
 
 template <int R, int MU, bool FWD>
-__device__ __forceinline__ void hop_compute(const HopOperands<R> &o, CVec<R> (&acc)[12]) {
+__device__ __forceinline__ void hop_compute(const HopOperands<R> &o, CVec<R> (&acc)[12], float dg) {
     CVec<R> r[6];
-    hop_half<R, MU, FWD>(o, r);
-    hop_recon<R, MU, FWD>(r, acc);
+    hop_half<R, MU, FWD>(o, r, dg);
+    hop_recon<R, MU, FWD>(r, acc, dg);
 }
 
 }  // namespace

@@ -368,3 +368,51 @@ def test_config2_24x24_full_field(nrhs):
     err = rel_l2_per_rhs(gpu_mooee(w, psi, mrhs.FULL), oracle.mooee(C, psi))
     assert err.max() < TOL, err
     w.close()
+
+
+# ---- NEXT-2: adjoint operators and the even-odd preconditioned (Schur complement) operator, both hop kernels
+DAG_CASES = [([8, 4, 4, 6], 12, 81), ([4, 4, 4, 4], 3, 82), ([16, 4, 4, 4], 12, 83), ([16, 2, 4, 4], 24, 84), ([2, 2, 2, 2], 4, 85),
+             ([48, 2, 2, 4], 12, 86)]
+
+
+@pytest.mark.parametrize("dims,nrhs,seed", DAG_CASES)
+def test_dagger_variants_and_schur_operator(dims, nrhs, seed):
+    from oracle import evenodd
+    mass, csw = -0.05, 1.5
+    U, psi = _fine_case(dims, nrhs, seed, mass, csw)
+    w = make_wilson(dims, nrhs, mass, csw, U)
+    C, _ = oracle.clover_blocks(dims, U, mass, csw)
+    src = oracle.cb_split(dims, psi)
+    want_dd = evenodd.dhop_dag(dims, U, psi)
+    want_md = evenodd.wilson_clover(dims, U, C, psi, dagger=True)
+    kernels = [mrhs.HOP_GATHER] + ([mrhs.HOP_SWEEP] if nrhs % 2 == 0 else [])
+    for kern in kernels:
+        mrhs.wilson_set_hop_kernel(w.h, 0, kern)
+        mrhs.wilson_set_hop_kernel(w.h, 1, kern)
+        d_in = w.import_field(dev(psi), mrhs.FULL)
+        d_out = w.empty(mrhs.FULL)
+        w.dhop_dag(d_in, d_out)
+        torch.cuda.synchronize()
+        assert rel_l2_per_rhs(host(w.export_field(d_out, mrhs.FULL)), want_dd).max() < TOL, ("dhop_dag", kern)
+        d_out = w.empty(mrhs.FULL)
+        w.apply(d_in, d_out, dagger=True)
+        torch.cuda.synchronize()
+        assert rel_l2_per_rhs(host(w.export_field(d_out, mrhs.FULL)), want_md).max() < TOL, ("M^+", kern)
+        for out_parity in (0, 1):
+            c_in = w.import_field(dev(src[1 - out_parity]), 1 - out_parity)
+            c_out = w.empty(out_parity)
+            w.meooe_dag(c_in, c_out, out_parity)
+            torch.cuda.synchronize()
+            want = evenodd.meooe_dag(dims, U, src[1 - out_parity], out_parity)
+            assert rel_l2_per_rhs(host(w.export_field(c_out, out_parity)), want).max() < TOL, ("meooe_dag", kern, out_parity)
+        for dagger in (False, True):
+            e_in = w.import_field(dev(src[0]), mrhs.EVEN)
+            tmp, e_out = w.empty(mrhs.ODD), w.empty(mrhs.EVEN)
+            w.schur_apply(e_in, tmp, e_out, dagger)
+            torch.cuda.synchronize()
+            want = evenodd.schur(dims, U, C, src[0], dagger=dagger)
+            assert rel_l2_per_rhs(host(w.export_field(e_out, mrhs.EVEN)), want).max() < TOL, ("schur", kern, dagger)
+    with pytest.raises(mrhs.MrhsError):
+        f = w.empty(mrhs.EVEN)
+        w.schur_apply(f, w.empty(mrhs.ODD), f)
+    w.close()
