@@ -278,11 +278,23 @@ mrhs_status_t mrhs_coarse_cb_merge(const int cdims[4], int nbasis, int nrhs, con
  * (restrict is the adjoint of prolong; the basis is used as given, orthonormalising it is the setup's job).
  * create: dims fine extents, bdims block extents (each divides the fine extent, coarse extent >= 2);
  *   d_basis: device, canonical [n_vec][site][4][3] complex64, copied and repacked (caller may free it).
- * prolong: d_coarse_in native coarse vector (ncomp = 2 n_vec) of the coarse lattice dims / bdims,
- *   d_fine_out native full-lattice fine field; restrict the other way.  Asynchronous on the stream.
+ * prolong: d_coarse_in native coarse vector (ncomp = 2 n_vec, COARSE layout: mrhs_coarse_field_import, which is what
+ *   mrhs_field_import does for ncomp != 12; with n_vec = 6 the explicit coarse entry is required) of the coarse lattice
+ *   dims / bdims, d_fine_out native full-lattice fine field; restrict the other way.  Asynchronous on the stream.
  * UNSUPPORTED: aggregates whose index table and reduction scratch do not fit 100 KB of shared memory (> ~2000 sites). */
 mrhs_status_t mrhs_transfer_create(mrhs_transfer_t **out, const int dims[4], const int bdims[4], int nvec,
                                    int nrhs, const void *d_basis, void *cuda_stream);
+/* The same pair one level up (the operators between the intermediate and the coarsest level, nbasis 40
+ * -> 60 in the paper's solve, where it reports its largest intergrid gains): the "fine" field is a coarse vector of nf
+ * components per site (nf a multiple of 4; chirality chi(c) = 0 for c < nf / 2, else 1) on the lattice fdims, in the COARSE
+ * native layout (mrhs_coarse_field_import); blocks of bdims of its sites:
+ *   prolong:   out(x)[c][r] = sum_k phi_k(x)[c] coarse(B(x))[chi(c) n_vec + k][r]
+ *   restrict:  coarse(B)[chi n_vec + k][r] = sum_{x in B, c in chi} conj(phi_k(x)[c]) in(x)[c][r]
+ * d_basis: device, canonical [n_vec][site][nf] complex64, copied and repacked.  The handle is used with mrhs_prolong /
+ * mrhs_restrict / mrhs_transfer_destroy like a fine-level one.  UNSUPPORTED (at restrict): more than 256 (chirality, basis
+ * pair, RHS lane group) items per aggregate. */
+mrhs_status_t mrhs_transfer_create_coarse(mrhs_transfer_t **out, const int fdims[4], const int bdims[4], int nf, int nvec,
+                                          int nrhs, const void *d_basis, void *cuda_stream);
 mrhs_status_t mrhs_prolong(mrhs_transfer_t *h, const void *d_coarse_in, void *d_fine_out);
 mrhs_status_t mrhs_restrict(mrhs_transfer_t *h, const void *d_fine_in, void *d_coarse_out);
 mrhs_status_t mrhs_transfer_destroy(mrhs_transfer_t *h);

@@ -61,6 +61,7 @@ _SIGNATURES = {
     "mrhs_coarse_meooe": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
     "mrhs_coarse_destroy": (ctypes.c_int, [_vp]),
     "mrhs_transfer_create": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, _int4, ctypes.c_int, ctypes.c_int, _vp, _vp]),
+    "mrhs_transfer_create_coarse": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, _int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp]),
     "mrhs_prolong": (ctypes.c_int, [_vp, _vp, _vp]),
     "mrhs_restrict": (ctypes.c_int, [_vp, _vp, _vp]),
     "mrhs_transfer_destroy": (ctypes.c_int, [_vp]),
@@ -162,14 +163,20 @@ def field_import(dims, ncomp, nrhs, parity, canonical, native=None, stream=None)
 
 
 class Transfer:
-    """MRHS prolongation / restriction between the fine level and its first coarse level (handle owner)."""
+    """MRHS prolongation / restriction (handle owner): between the fine level and its first coarse level, or, with
+    nf = the finer level's nbasis, between two coarse levels (fields of both levels in the coarse layout)."""
 
-    def __init__(self, dims, bdims, nvec, nrhs, basis, stream=None):
+    def __init__(self, dims, bdims, nvec, nrhs, basis, stream=None, nf=None):
         self.dims, self.bdims, self.nvec, self.nrhs = [int(d) for d in dims], [int(b) for b in bdims], int(nvec), int(nrhs)
         self.cdims = [d // b for d, b in zip(self.dims, self.bdims)]
+        self.nf = nf
         h = _vp()
-        _check(lib().mrhs_transfer_create(ctypes.byref(h), _dims(self.dims), _dims(self.bdims), self.nvec, self.nrhs,
-                                          _ptr(basis), _stream_ptr(stream)))
+        if nf is None:
+            _check(lib().mrhs_transfer_create(ctypes.byref(h), _dims(self.dims), _dims(self.bdims), self.nvec, self.nrhs,
+                                              _ptr(basis), _stream_ptr(stream)))
+        else:
+            _check(lib().mrhs_transfer_create_coarse(ctypes.byref(h), _dims(self.dims), _dims(self.bdims), int(nf), self.nvec,
+                                                     self.nrhs, _ptr(basis), _stream_ptr(stream)))
         self.h = h
 
     def prolong(self, d_coarse, d_fine):

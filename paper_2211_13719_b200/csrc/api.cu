@@ -54,9 +54,11 @@ struct mrhs_wilson {
 };
 
 struct mrhs_transfer {
+    int coarse_level;        // 0: fine spinors (12 components, x-blocked layout) -> first coarse level; 1: coarse -> coarser
     TransferGeom g;
+    CoarseTransferGeom cg;
     cudaStream_t st;
-    float2 *basis;   // native [site][k][12]
+    float2 *basis;           // native [site][k][12] or [site][k][nf]
 };
 
 struct mrhs_coarse {
@@ -601,15 +603,54 @@ mrhs_status_t mrhs_transfer_create(mrhs_transfer_t **out, const int dims[4], con
     return MRHS_OK;
 }
 
+mrhs_status_t mrhs_transfer_create_coarse(mrhs_transfer_t **out, const int fdims[4], const int bdims[4], int nf, int nvec, int nrhs,
+                                          const void *d_basis, void *cuda_stream) {
+    MRHS_REQUIRE(out, "transfer create: out is NULL");
+    *out = nullptr;
+    MRHS_REQUIRE(fdims && bdims && d_basis, "transfer create: NULL argument");
+    MRHS_REQUIRE(nf >= 4 && nf % 4 == 0 && nf <= 512, "transfer create: the finer level's nbasis must be a multiple of 4 (two chiralities of an even number of components)");
+    MRHS_REQUIRE(nvec >= 1 && nvec <= 256 && nrhs >= 1 && nrhs <= 128, "transfer create: nvec must be 1..256 and nrhs 1..128");
+    MRHS_REQUIRE(aligned16(d_basis), "transfer create: basis must be 16-byte aligned");
+    for (int i = 0; i < 4; i++)
+        MRHS_REQUIRE(fdims[i] >= 2 && bdims[i] >= 1 && fdims[i] % bdims[i] == 0 && fdims[i] / bdims[i] >= 2,
+                     "transfer create: every block extent must divide the lattice extent and leave a coarse extent >= 2");
+    mrhs_transfer *h = new (std::nothrow) mrhs_transfer();
+    if (!h) { set_error("transfer create: host allocation failed"); return MRHS_ERR_ALLOC; }
+    memset(h, 0, sizeof(*h));
+    h->coarse_level = 1;
+    CoarseTransferGeom &g = h->cg;
+    g.X = fdims[0]; g.Y = fdims[1]; g.Z = fdims[2]; g.T = fdims[3];
+    g.bx = bdims[0]; g.by = bdims[1]; g.bz = bdims[2]; g.bt = bdims[3];
+    g.cX = g.X / g.bx; g.cY = g.Y / g.by; g.cZ = g.Z / g.bz; g.cT = g.T / g.bt;
+    g.nf = nf; g.nvec = nvec; g.N = nrhs;
+    g.nsites = (long long)g.X * g.Y * g.Z * g.T;
+    g.ncoarse = (long long)g.cX * g.cY * g.cZ * g.cT;
+    h->st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaMalloc(&h->basis, (size_t)g.nsites * nvec * nf * sizeof(float2));
+    if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaMalloc(basis)", __FILE__, __LINE__); }
+    mrhs_status_t s = pack_basis_coarse(g, (const float2 *)d_basis, h->basis, h->st);
+    if (s == MRHS_OK) {
+        e = cudaStreamSynchronize(h->st);
+        if (e != cudaSuccess) s = cuda_fail(e, "cudaStreamSynchronize", __FILE__, __LINE__);
+    }
+    if (s != MRHS_OK) { cudaFree(h->basis); delete h; return s; }
+    *out = h;
+    return MRHS_OK;
+}
+
 mrhs_status_t mrhs_prolong(mrhs_transfer_t *h, const void *d_coarse_in, void *d_fine_out) {
     MRHS_REQUIRE(h && d_coarse_in && d_fine_out, "prolong: NULL argument");
+    MRHS_REQUIRE(d_coarse_in != d_fine_out, "prolong: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_coarse_in) && aligned16(d_fine_out), "prolong: buffers must be 16-byte aligned");
+    if (h->coarse_level) return launch_prolong_coarse(h->cg, h->basis, d_coarse_in, d_fine_out, h->st);
     return launch_prolong(h->g, h->basis, d_coarse_in, d_fine_out, h->st);
 }
 
 mrhs_status_t mrhs_restrict(mrhs_transfer_t *h, const void *d_fine_in, void *d_coarse_out) {
     MRHS_REQUIRE(h && d_fine_in && d_coarse_out, "restrict: NULL argument");
+    MRHS_REQUIRE(d_fine_in != d_coarse_out, "restrict: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_fine_in) && aligned16(d_coarse_out), "restrict: buffers must be 16-byte aligned");
+    if (h->coarse_level) return launch_restrict_coarse(h->cg, h->basis, d_fine_in, d_coarse_out, h->st);
     return launch_restrict(h->g, h->basis, d_fine_in, d_coarse_out, h->st);
 }
 

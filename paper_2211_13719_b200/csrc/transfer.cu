@@ -254,6 +254,129 @@ restrict_kernel(TransferGeom g, int NP, int PC, int S, const float4 *__restrict_
     }
 }
 
+
+// ------------------------------------------------------------------ coarse -> coarser
+__global__ void pack_basis_coarse_kernel(int nvec, int nf, long long V, const float2 *__restrict__ src, float2 *__restrict__ dst, long long total) {
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // native order [x][k][c]
+    if (idx >= total) return;
+    const int c = (int)(idx % nf);
+    long long q = idx / nf;
+    const int k = (int)(q % nvec);
+    const long long x = q / nvec;
+    dst[idx] = src[((long long)k * V + x) * nf + c];
+}
+
+__device__ __forceinline__ long long coarser_block(const CoarseTransferGeom &g, long long x) {
+    const int ix = (int)(x % g.X); x /= g.X;
+    const int iy = (int)(x % g.Y); x /= g.Y;
+    const int iz = (int)(x % g.Z);
+    const int it = (int)(x / g.Z);
+    return (ix / g.bx) + (long long)g.cX * ((iy / g.by) + (long long)g.cY * ((iz / g.bz) + (long long)g.cZ * (it / g.bt)));
+}
+
+// One thread = one finer site, two components (same chirality: nf / 2 is even) and TP RHS lanes; per basis vector k one
+// 16-byte load of phi_k(x)[2 cp .. 2 cp + 1] and TP loads of the block's coarser coefficients feed 2 TP complex FMAs.
+template <int R, int TP>
+__global__ void __launch_bounds__(256)
+prolong_coarse_kernel(CoarseTransferGeom g, int NP, int items, long long nthreads, const float4 *__restrict__ basis,
+                      const typename Elem<R>::type *__restrict__ coarse, typename Elem<R>::type *__restrict__ fine) {
+    typedef typename Elem<R>::type E;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= nthreads) return;
+    const long long x = gid / items;
+    const int item = (int)(gid - x * items);
+    const int lgs = NP / TP, cp = item / lgs, lane = (item - cp * lgs) * TP;
+    const int chi = 2 * cp >= g.nf / 2;
+    const E *vc = coarse + ((size_t)coarser_block(g, x) * 2 * g.nvec + (size_t)chi * g.nvec) * NP + lane;
+    const float4 *ph = basis + ((size_t)x * g.nvec * g.nf) / 2 + cp;          // float4 = two complex components
+    CVec<R> acc[2][TP];
+#pragma unroll
+    for (int l = 0; l < TP; l++) { acc[0][l] = czero_t<R>(); acc[1][l] = czero_t<R>(); }
+#pragma unroll 4
+    for (int k = 0; k < g.nvec; k++) {
+        const float4 a = __ldg(ph + (size_t)k * (g.nf / 2));
+#pragma unroll
+        for (int l = 0; l < TP; l++) {
+            const CVec<R> v = to_cvec(__ldg(vc + (size_t)k * NP + l));
+            acc[0][l] = cfma(a.x, a.y, v, acc[0][l]);
+            acc[1][l] = cfma(a.z, a.w, v, acc[1][l]);
+        }
+    }
+    E *po = fine + ((size_t)x * g.nf + 2 * cp) * NP + lane;
+#pragma unroll
+    for (int l = 0; l < TP; l++) { po[l] = from_cvec(acc[0][l]); po[NP + l] = from_cvec(acc[1][l]); }
+}
+
+// One thread block = one aggregate; a thread owns one (site slice, chirality, KT basis vectors, LT RHS lanes) and sums its slice of
+// the aggregate's sites over the nf / 2 components of its chirality; slices are added through shared memory in a fixed order.
+template <int R, int KT, int LT>
+__global__ void __launch_bounds__(256)
+restrict_coarse_kernel(CoarseTransferGeom g, int NP, int S, const float2 *__restrict__ basis,
+                       const typename Elem<R>::type *__restrict__ fine, typename Elem<R>::type *__restrict__ coarse) {
+    typedef typename Elem<R>::type E;
+    extern __shared__ __align__(16) unsigned char sm[];
+    E *red = reinterpret_cast<E *>(sm);                                   // [S-1][items][KT LT]
+    const int nagg = g.bx * g.by * g.bz * g.bt, h = g.nf / 2;
+    const int kgs = g.nvec / KT, lgs = NP / LT, items = 2 * kgs * lgs;
+    const long long B = blockIdx.x;
+    const int c0x = (int)(B % g.cX) * g.bx, c0y = (int)((B / g.cX) % g.cY) * g.by, c0z = (int)((B / ((long long)g.cX * g.cY)) % g.cZ) * g.bz;
+    const int c0t = (int)(B / ((long long)g.cX * g.cY * g.cZ)) * g.bt;
+    const int tid = threadIdx.x, s = tid / items, item = tid - s * items;
+    const int chi = item / (kgs * lgs), rem = item - chi * (kgs * lgs), k0 = (rem / lgs) * KT, lane = (rem - (rem / lgs) * lgs) * LT;
+    const bool active = s < S;
+    CVec<R> acc[KT][LT];
+#pragma unroll
+    for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+        for (int l = 0; l < LT; l++) acc[kk][l] = czero_t<R>();
+    if (active) {
+        for (int i = s; i < nagg; i += S) {
+            int q = i;
+            const int ix = q % g.bx; q /= g.bx;
+            const int iy = q % g.by; q /= g.by;
+            const int iz = q % g.bz;
+            const int it = q / g.bz;
+            const long long x = (c0x + ix) + (long long)g.X * ((c0y + iy) + (long long)g.Y * ((c0z + iz) + (long long)g.Z * (c0t + it)));
+            const float2 *ph = basis + ((size_t)x * g.nvec + k0) * g.nf + chi * h;
+            const E *pf = fine + ((size_t)x * g.nf + chi * h) * NP + lane;
+#pragma unroll 4
+            for (int c = 0; c < h; c++) {
+                CVec<R> f[LT];
+#pragma unroll
+                for (int l = 0; l < LT; l++) f[l] = to_cvec(__ldg(pf + (size_t)c * NP + l));
+#pragma unroll
+                for (int kk = 0; kk < KT; kk++) {
+                    const float2 a = __ldg(ph + (size_t)kk * g.nf + c);
+#pragma unroll
+                    for (int l = 0; l < LT; l++) acc[kk][l] = cfma_conj(a.x, a.y, f[l], acc[kk][l]);
+                }
+            }
+        }
+        if (s > 0) {
+            E *rp = red + ((size_t)(s - 1) * items + item) * KT * LT;
+#pragma unroll
+            for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+                for (int l = 0; l < LT; l++) rp[kk * LT + l] = from_cvec(acc[kk][l]);
+        }
+    }
+    __syncthreads();
+    if (active && s == 0) {
+        for (int q = 1; q < S; q++) {
+            const E *rp = red + ((size_t)(q - 1) * items + item) * KT * LT;
+#pragma unroll
+            for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+                for (int l = 0; l < LT; l++) acc[kk][l] = cadd(acc[kk][l], to_cvec(rp[kk * LT + l]));
+        }
+        E *po = coarse + ((size_t)B * 2 * g.nvec + (size_t)chi * g.nvec + k0) * NP + lane;
+#pragma unroll
+        for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+            for (int l = 0; l < LT; l++) po[(size_t)kk * NP + l] = from_cvec(acc[kk][l]);
+    }
+}
+
 }  // namespace
 
 mrhs_status_t pack_basis(const TransferGeom &g, const float2 *d_canonical, float2 *d_native, cudaStream_t st) {
@@ -319,6 +442,50 @@ mrhs_status_t launch_restrict(const TransferGeom &g, const float2 *d_basis, cons
     }
 #undef MRHS_RESTRICT_KT
 #undef MRHS_RESTRICT
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+mrhs_status_t pack_basis_coarse(const CoarseTransferGeom &g, const float2 *d_canonical, float2 *d_native, cudaStream_t st) {
+    const long long total = g.nsites * g.nvec * g.nf;
+    pack_basis_coarse_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(g.nvec, g.nf, g.nsites, d_canonical, d_native, total);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+mrhs_status_t launch_prolong_coarse(const CoarseTransferGeom &g, const float2 *d_basis, const void *d_coarse, void *d_fine, cudaStream_t st) {
+    const int np = threads_per_site(g.N);
+    const int tp = np % 3 == 0 ? 3 : (np % 2 == 0 ? 2 : 1);
+    const int items = (g.nf / 2) * (np / tp);
+    const long long nthreads = g.nsites * items;
+    const unsigned blocks = (unsigned)((nthreads + 255) / 256);
+#define MRHS_PC(RR, TP, ET) prolong_coarse_kernel<RR, TP><<<blocks, 256, 0, st>>>(g, np, items, nthreads, (const float4 *)d_basis, (const ET *)d_coarse, (ET *)d_fine)
+    if (g.N & 1) { if (tp == 3) MRHS_PC(1, 3, float2); else if (tp == 2) MRHS_PC(1, 2, float2); else MRHS_PC(1, 1, float2); }
+    else         { if (tp == 3) MRHS_PC(2, 3, float4); else if (tp == 2) MRHS_PC(2, 2, float4); else MRHS_PC(2, 1, float4); }
+#undef MRHS_PC
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
+mrhs_status_t launch_restrict_coarse(const CoarseTransferGeom &g, const float2 *d_basis, const void *d_fine, void *d_coarse, cudaStream_t st) {
+    const int np = threads_per_site(g.N);
+    const int kt = g.nvec % 2 == 0 ? 2 : 1;
+    const int lt = np % 3 == 0 ? 3 : (np % 2 == 0 ? 2 : 1);
+    const int items = 2 * (g.nvec / kt) * (np / lt);
+    if (items > 256) { set_error("restrict (coarse level): %d work items per aggregate exceed one thread block (nvec = %d, nrhs = %d)", items, g.nvec, g.N); return MRHS_ERR_UNSUPPORTED; }
+    const int nagg = g.bx * g.by * g.bz * g.bt;
+    int S = 256 / items;
+    if (S > nagg) S = nagg;
+    const int threads = S * items;
+    const int esz = (g.N & 1) ? 8 : 16;
+    const size_t smem = (size_t)(S - 1) * items * kt * lt * esz;
+    if (smem > 48 * 1024) { set_error("restrict (coarse level): %zu bytes of shared memory needed (max 48 KB)", smem); return MRHS_ERR_UNSUPPORTED; }
+#define MRHS_RC(RR, KT, LT, ET) restrict_coarse_kernel<RR, KT, LT><<<(unsigned)g.ncoarse, threads, smem, st>>>(g, np, S, d_basis, (const ET *)d_fine, (ET *)d_coarse)
+#define MRHS_RC_LT(RR, KT, ET) do { if (lt == 3) MRHS_RC(RR, KT, 3, ET); else if (lt == 2) MRHS_RC(RR, KT, 2, ET); else MRHS_RC(RR, KT, 1, ET); } while (0)
+    if (g.N & 1) { if (kt == 2) MRHS_RC_LT(1, 2, float2); else MRHS_RC_LT(1, 1, float2); }
+    else         { if (kt == 2) MRHS_RC_LT(2, 2, float4); else MRHS_RC_LT(2, 1, float4); }
+#undef MRHS_RC_LT
+#undef MRHS_RC
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
 }

@@ -61,3 +61,59 @@ def test_transfer_argument_errors():
         mrhs.Transfer([4, 4, 4, 4], [3, 2, 2, 2], 2, 4, basis)      # 3 does not divide 4
     with pytest.raises(mrhs.MrhsError):
         mrhs.Transfer([4, 4, 4, 4], [4, 2, 2, 2], 2, 4, basis)      # coarse extent 1
+
+
+# ---- coarse -> coarser (nbasis 40 -> 60 in the paper's solve); both fields in the coarse layout
+COARSE_CASES = [
+    ([4, 4, 4, 4], [2, 2, 2, 2], 8, 3, 4),
+    ([6, 6, 6, 8], [3, 3, 3, 2], 40, 30, 12),      # the paper's intermediate -> coarsest shape: 40 -> 60 components
+    ([4, 4, 2, 6], [2, 2, 1, 3], 24, 20, 24),
+    ([4, 2, 4, 4], [2, 1, 2, 2], 12, 6, 12),       # 12-component "fine" level: must NOT be packed like a fine spinor
+    ([4, 4, 4, 4], [2, 2, 2, 2], 40, 5, 3),        # odd n_vec, odd N_rhs
+    ([2, 4, 4, 4], [1, 2, 2, 2], 24, 12, 96),
+]
+
+
+@pytest.mark.parametrize("fdims,bdims,nf,nvec,nrhs", COARSE_CASES)
+def test_coarse_level_prolong_restrict_match_oracle(fdims, bdims, nf, nvec, nrhs):
+    cdims = [d // b for d, b in zip(fdims, bdims)]
+    Vf, Vc, nb = syn.volume(fdims), syn.volume(cdims), 2 * nvec
+    basis = np.stack([syn.coarse_vector_np(fdims, nf, 1, 200 + k)[..., 0] for k in range(nvec)])     # [nvec][Vf][nf] complex64
+    vc = syn.coarse_vector_np(cdims, nb, nrhs, 17)
+    f = syn.coarse_vector_np(fdims, nf, nrhs, 18)
+    tr = mrhs.Transfer(fdims, bdims, nvec, nrhs, dev(basis), nf=nf)
+    d_c = mrhs.coarse_field_import(cdims, nb, nrhs, mrhs.FULL, dev(vc))
+    d_f = mrhs.empty_field(fdims, nf, nrhs, mrhs.FULL)
+    tr.prolong(d_c, d_f)
+    torch.cuda.synchronize()
+    err = rel_l2_per_rhs(host(mrhs.coarse_field_export(fdims, nf, nrhs, mrhs.FULL, d_f)), otr.prolong_coarse(fdims, bdims, basis, vc))
+    assert err.max() < TOL, ("prolong", err)
+    d_f = mrhs.coarse_field_import(fdims, nf, nrhs, mrhs.FULL, dev(f))
+    d_c = mrhs.empty_field(cdims, nb, nrhs, mrhs.FULL)
+    tr.restrict(d_f, d_c)
+    torch.cuda.synchronize()
+    err = rel_l2_per_rhs(host(mrhs.coarse_field_export(cdims, nb, nrhs, mrhs.FULL, d_c)), otr.restrict_coarse(fdims, bdims, basis, f))
+    assert err.max() < TOL, ("restrict", err)
+    tr.close()
+
+
+def test_fine_level_transfer_with_six_basis_vectors():
+    """n_vec = 6 gives 12-component coarse vectors: through the explicit coarse layout entries they are site-contiguous."""
+    dims, bdims, nvec, nrhs = [8, 4, 4, 4], [4, 2, 2, 2], 6, 12
+    cdims = [d // b for d, b in zip(dims, bdims)]
+    V = syn.volume(dims)
+    basis = np.stack([syn.spinor_np(V, 1, 300 + k)[..., 0] for k in range(nvec)])
+    vc = syn.coarse_vector_np(cdims, 12, nrhs, 27)
+    f = syn.spinor_np(V, nrhs, 28)
+    tr = mrhs.Transfer(dims, bdims, nvec, nrhs, dev(basis))
+    d_f = mrhs.empty_field(dims, 12, nrhs, mrhs.FULL)
+    tr.prolong(mrhs.coarse_field_import(cdims, 12, nrhs, mrhs.FULL, dev(vc)), d_f)
+    torch.cuda.synchronize()
+    got = host(mrhs.field_export(dims, 12, nrhs, mrhs.FULL, d_f)).reshape(V, 4, 3, nrhs)
+    assert rel_l2_per_rhs(got, otr.prolong(dims, bdims, basis, vc)).max() < TOL
+    d_c = mrhs.empty_field(cdims, 12, nrhs, mrhs.FULL)
+    tr.restrict(mrhs.field_import(dims, 12, nrhs, mrhs.FULL, dev(f)), d_c)
+    torch.cuda.synchronize()
+    got = host(mrhs.coarse_field_export(cdims, 12, nrhs, mrhs.FULL, d_c))
+    assert rel_l2_per_rhs(got, otr.restrict(dims, bdims, basis, f)).max() < TOL
+    tr.close()
