@@ -19,10 +19,14 @@ All fields are resident in HBM in the library's native layout when the timed reg
 working set of every launch (>= 0.85 GB) is far larger than the 126 MB L2, so no flush is needed
 between iterations.  The metric is nominal GFLOP/s (1320 flops/site/RHS for the hop, 504 for the
 clover term, 72 nb^2 for the coarse apply); each kernel's algorithmic GB/s against the measured
-HBM copy bandwidth (MEASURED_PEAKS.json) is reported beside it.
+HBM copy bandwidth (MEASURED_PEAKS.json) is reported beside it, with mean, median and minimum
+launch time.  The line also carries `nrhs_sweep`: D_hop, M_eooe, M_ooee and the coarse apply (both
+math modes) at the N_rhs lists of BASELINE.json's configs 2-5 -- the metric is "GFLOP/s and % HBM
+roofline vs N_rhs" -- timed launch by launch with an L2 flush in between (--no-sweep leaves it out).
 
 --impl reference times the fp64 CPU oracle (oracle/), as it stands, on a bounded sample of the
-same workload.  --sweep writes one JSON line per (operator, lattice, N_rhs) for configs 2-5.
+same workload (named in its config.workload).  --sweep OUT.jsonl writes one JSON line per
+(operator, lattice, N_rhs) for every operator of the library over configs 2-5.
 """
 import argparse
 import json
@@ -45,11 +49,12 @@ NRHS = 12
 MASS, CSW = -0.05, 1.5
 SEED = 5
 
-# bounded sample of the same workload for the CPU oracle (cpu_baseline and --impl reference)
-CPU_FINE_DIMS = [16, 16, 16, 16]
-CPU_COARSE_DIMS = [6, 6, 6, 8]
-CPU_SAMPLE = ("same operators, distributions and N_rhs=12 on a 16^4 fine lattice (1/81 of the 48^4 sites) "
-              "and a 6^3x8 coarse lattice (1/4 of the 6^3x32 sites), fp64 oracle, OpenMP over sites")
+# bounded sample of the same workload for the CPU oracle (cpu_baseline and --impl reference): the fine operators full-field
+# on config 2's 24^4 lattice (1/16 of the sites of the 48^4 bench lattice, same N_rhs, same operators) and config 4 in full
+CPU_FINE_DIMS = [24, 24, 24, 24]
+CPU_COARSE_DIMS = [6, 6, 6, 32]
+CPU_SAMPLE = ("fp64 oracle, OpenMP over sites: the step's fine operators (D_hop, M_eooe x2, M_ooee, M_eooe M_ooee M_eooe) full-field on "
+              "config 2's 24^4 lattice at N_rhs=12 (1/16 of the 48^4 sites of the GPU step) + config 4's coarse apply in full (6^3x32, nbasis 40)")
 
 
 def coarse_flops(nb):
@@ -76,11 +81,15 @@ def vol(dims):
     return dims[0] * dims[1] * dims[2] * dims[3]
 
 
-def step_work(fdims, cdims, nb, N):
-    """Nominal flops and algorithmic bytes of each launch of one step, in launch order."""
+def step_work(fdims, cdims, nb, N, schur_fused=True):
+    """Nominal flops and algorithmic bytes of each launch of one step, in launch order.  The Schur-style sequence is
+    credited with the flops of its three operators and with the bytes of the path that runs: fused (sweep kernel, two
+    launches) the M_ooee stage moves only the clover blocks of the odd sites (288 B each) -- the intermediate field is
+    neither written nor re-read; unfused (gather kernel, three launches) it is a full M_ooee pass."""
     V, Vc = vol(fdims), vol(cdims)
     hop_f, hop_b = FLOPS_HOP * (V / 2) * N, bytes_meooe(V, N)
-    clv_h_f, clv_h_b = FLOPS_CLOVER * (V / 2) * N, bytes_mooee(V / 2, N)
+    clv_h_f = FLOPS_CLOVER * (V / 2) * N
+    clv_h_b = 288.0 * (V / 2) if schur_fused else bytes_mooee(V / 2, N)
     return [
         ("dhop", FLOPS_HOP * V * N, bytes_dhop(V, N)),
         ("meooe_oe", hop_f, hop_b),
@@ -217,7 +226,7 @@ def run_reference(args):
         "impl": "reference", "metric": "MRHS Wilson-clover stencil hot path, nominal GFLOP/s", "value": gf,
         "unit": "GFLOP/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(),
+        "config": reference_config(),
         "cpu_baseline": {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": CPU_SAMPLE},
         "e2e": {"value": gf, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -233,6 +242,16 @@ def workload_config():
             "precision": "complex64 fields, fp32 FMA",
             "l2": "every launch touches >= 0.85 GB, far above the 126 MB L2; no flush between iterations",
             "parallelism": "replicas only (one GPU per lattice, no collectives; north_star)"}
+
+
+def reference_config():
+    """The oracle arm times a bounded sample, and says so where the workload is named: its config is NOT the GPU arm's."""
+    cfg = workload_config()
+    cfg["workload"] = "SAMPLE of the GPU arm's workload -- " + CPU_SAMPLE
+    cfg["fine_dims"], cfg["coarse_dims"] = CPU_FINE_DIMS, CPU_COARSE_DIMS
+    cfg["precision"] = "complex128 (fp64 oracle)"
+    cfg["gpu_arm_workload"] = workload_config()["workload"]
+    return cfg
 
 
 # ------------------------------------------------------------------------ replicas (N > 1)
@@ -260,6 +279,7 @@ class Workload:
         self.torch, self.mrhs, self.fdims, self.cdims, self.nb, self.N = torch, mrhs, fdims, cdims, nb, N
         V = vol(fdims)
         U = syn.gauge_torch(fdims, SEED, device)
+        torch.cuda.synchronize()     # the inputs are generated on torch's current stream, the library works on `stream`
         self.w = mrhs.Wilson(fdims, N, MASS, CSW, U, stream=stream)
         del U
         psi = syn.spinor_torch(V, N, SEED, device)
@@ -271,6 +291,7 @@ class Workload:
         self.out_e, self.out_o = self.w.empty(mrhs.EVEN), self.w.empty(mrhs.ODD)
         self.t0, self.t1 = self.w.empty(mrhs.ODD), self.w.empty(mrhs.ODD)
         A = syn.coarse_links_torch(cdims, nb, 4, device)
+        torch.cuda.synchronize()
         self.c = mrhs.Coarse(cdims, nb, N, A, stream=stream)
         self.c_tc = mrhs.Coarse(cdims, nb, N, A, math_mode=mrhs.COARSE_TENSOR, stream=stream)
         del A
@@ -325,17 +346,18 @@ def run_gpu(args):
         if args.hop_tiling:
             t = [int(x) for x in args.hop_tiling.split(",")]
             mrhs.wilson_set_tiling(wl.w.h, which, t[:3], t[3:5])
-        if args.hop_prefetch is not None:
-            mrhs.wilson_set_prefetch(wl.w.h, which, args.hop_prefetch)
         if args.hop_kernel is not None:
             mrhs.wilson_set_hop_kernel(wl.w.h, which, {"gather": mrhs.HOP_GATHER, "sweep": mrhs.HOP_SWEEP}[args.hop_kernel])
         if args.hop_sweep:
             t = [int(x) for x in args.hop_sweep.split(",")]
             mrhs.wilson_set_sweep(wl.w.h, which, t[0], t[1:3])
+        if args.hop_prefetch is not None:
+            mrhs.wilson_set_prefetch(wl.w.h, which, args.hop_prefetch)
     if args.hop_tiling or args.hop_prefetch is not None or args.hop_kernel or args.hop_sweep:
         tiling_note = "override: kernel %s tiling %s prefetch %s sweep %s" % (args.hop_kernel, args.hop_tiling, args.hop_prefetch, args.hop_sweep)
     launches = wl.launches()
-    work = step_work(fdims, cdims, nb, N)
+    fused = mrhs.wilson_get_hop_kernel(wl.w.h, 1) == mrhs.HOP_SWEEP
+    work = step_work(fdims, cdims, nb, N, schur_fused=fused)
     flops_step = sum(w[1] for w in work)
     K, W = args.steps, args.warmup
 
@@ -360,7 +382,8 @@ def run_gpu(args):
     t_wall = time.perf_counter() - t_wall
     clocks = sampler.stop() if rank == 0 else None
     total_ms = evs[0][0].elapsed_time(evs[K - 1][nseg])
-    seg_ms = [sum(evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)) / K for i in range(nseg)]
+    seg_all = [sorted(evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(K)) for i in range(nseg)]
+    seg_ms = [sum(a) / K for a in seg_all]
     total_ms = max_over_ranks(total_ms, dist, device)
     ms_per_step = total_ms / K
     value = job_gflops(flops_step, world, ms_per_step)
@@ -377,25 +400,38 @@ def run_gpu(args):
     V = vol(fdims)
     seg_names = [n for n, _ in launches]
     kernels = {}
-    for name, ms in zip(seg_names, seg_ms):
+    for name, ms, allms in zip(seg_names, seg_ms, seg_all):
         if name == "schur":
             fl = sum(w[1] for w in work if w[0].startswith("schur"))
             by = sum(w[2] for w in work if w[0].startswith("schur"))
         else:
             fl, by = [(w[1], w[2]) for w in work if w[0] == name][0]
         gbs = by / (ms * 1e-3) / 1e9
-        kernels[name] = {"ms": ms, "gflops": fl / (ms * 1e-3) / 1e9, "gbs": gbs, "hbm_frac": gbs / peak,
-                         "share_of_step": ms / sum(seg_ms)}
+        kernels[name] = {"ms": ms, "ms_median": allms[len(allms) // 2], "ms_min": allms[0], "gflops": fl / (ms * 1e-3) / 1e9,
+                         "gbs": gbs, "hbm_frac": gbs / peak, "algorithmic_bytes": by, "share_of_step": ms / sum(seg_ms)}
+        if name == "schur":
+            # what three separate launches would have to move (22.2 GB), for comparison only
+            by3 = 2 * bytes_meooe(V, N) + bytes_mooee(V / 2, N)
+            kernels[name]["launches"] = 2 if fused else 3
+            kernels[name]["gbs_credited_with_unfused_bytes"] = by3 / (ms * 1e-3) / 1e9
     d = kernels["dhop"]
     kname = {mrhs.HOP_GATHER: "hop_kernel (gather)", mrhs.HOP_SWEEP: "hop_sweep_kernel (slice sweep)"}
     roofline = {"kernel": "%s: D_hop, full lattice %dx%dx%dx%d, N_rhs=%d" % (kname[mrhs.wilson_get_hop_kernel(wl.w.h, 0)], *fdims, N), "bound": "hbm",
                 "achieved": d["gbs"], "peak": peak, "unit": "GB/s", "frac": d["gbs"] / peak,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_dhop(V, N),
-                "avg_launch_ms": d["ms"], "traffic": ncu_traffic("dhop_48x48x48x48_n12") if not args.small else None}
+                "avg_launch_ms": d["ms"], "median_launch_ms": d["ms_median"], "min_launch_ms": d["ms_min"],
+                "traffic": ncu_traffic("dhop_48x48x48x48_n12") if not args.small else None,
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of this kernel in the committed ncu capture "
+                                  "(profiles/dram_traffic.csv; ncu cannot run inside the timed bench)"}
     cpu = None
     if not args.no_cpu:
         gf, ms, cores = time_oracle(args.cpu_steps, 1)
         cpu = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": CPU_SAMPLE, "ms_per_sample_step": ms}
+    nrhs_sweep = None
+    if not args.no_sweep and not args.small:
+        # release the step's fields first: the sweep builds its own handles (48^4 at N_rhs = 24 needs 12 GB per field)
+        wl = release_fields(wl)
+        nrhs_sweep = [r for r in sweep_records(torch, mrhs, syn, device, stream, peak, iters=args.inrun_sweep_iters, subset="north_star")]
     cfg = workload_config()
     def hop_cfg(which):
         k = mrhs.wilson_get_hop_kernel(wl.w.h, which)
@@ -413,12 +449,21 @@ def run_gpu(args):
         "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": cfg, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
-        "gpu_launches": (len(work) - (1 if mrhs.wilson_get_hop_kernel(wl.w.h, 1) == mrhs.HOP_SWEEP else 0)) * K, "kernels": kernels, "wall_ms_per_step": t_wall * 1e3 / K,
+        "gpu_launches": (len(work) - (1 if fused else 0)) * K, "kernels": kernels, "wall_ms_per_step": t_wall * 1e3 / K,
+        "nrhs_sweep": nrhs_sweep,
     }
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
     return 0
+
+
+def release_fields(wl):
+    """Drop the step's device fields (keeps the handles, whose tiling the report still reads)."""
+    for name in ("psi", "out_full", "in_e", "in_o", "out_e", "out_o", "t0", "t1", "v", "v_out"):
+        setattr(wl, name, None)
+    wl.torch.cuda.empty_cache()
+    return wl
 
 
 def run_e2e(torch, mrhs, wl, args, barrier, dist, device, world, flops_step):
@@ -471,20 +516,14 @@ def run_e2e(torch, mrhs, wl, args, barrier, dist, device, world, flops_step):
 
 # ------------------------------------------------------------------------ N_rhs sweep
 
-def run_sweep(args):
-    """One JSON line per (operator, lattice, N_rhs) for configs 2-5: median and min time of
-    individually timed launches, L2 flushed between launches (a 512 MB memset), GFLOP/s, GB/s,
-    fraction of the measured HBM peak, speed-up per RHS over N_rhs = 1."""
-    import torch
-    import paper_2211_13719_b200 as mrhs
-    import synth_inputs as syn
-    device = torch.device("cuda", 0)
-    torch.cuda.set_device(0)
-    peak, peak_src = measured_peaks()
-    stream = torch.cuda.Stream(device)
+def sweep_records(torch, mrhs, syn, device, stream, peak, iters, subset, warm=5, ops=("fine", "coarse")):
+    """Per (operator, lattice, N_rhs) records for configs 2-5: median and min time of individually timed launches on the
+    library's stream, L2 flushed between launches (a 512 MB memset), GFLOP/s, algorithmic GB/s, fraction of the measured
+    HBM peak, speed-up per RHS over the first N_rhs of the config.  subset "north_star": D_hop, M_eooe, M_ooee and the
+    coarse apply in both math modes at the N_rhs lists of BASELINE.json's configs (what the metric names);
+    "all": every operator of the library."""
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)
-    iters, warm = args.sweep_iters, 5
-    out = open(args.sweep, "w")
+    everything = subset == "all"
 
     def timeit(f):
         with torch.cuda.stream(stream):
@@ -502,29 +541,25 @@ def run_sweep(args):
         ts.sort()
         return ts[len(ts) // 2], ts[0]
 
-    def emit(cfg, op, dims, N, fl, by, med, mn, base, extra=None):
-        rec = {"config": cfg, "op": op, "dims": dims, "n_rhs": N, "ms_median": med, "ms_min": mn,
-               "gflops": fl / (med * 1e-3) / 1e9, "gbs": by / (med * 1e-3) / 1e9,
-               "hbm_frac": by / (med * 1e-3) / 1e9 / peak, "alg_bytes": by, "nominal_flops": fl}
-        key = (cfg, op)
-        if N == base.get(key, (N, None))[0] or key not in base:
-            base.setdefault(key, (N, med / N))
-        rec["speedup_per_rhs_vs_first_n"] = base[key][1] / (med / N)
-        if extra:
-            rec.update(extra)
-        out.write(json.dumps(rec) + "\n")
-        out.flush()
-        print("%-8s %-12s %-16s N=%-3d %8.4f ms  %9.1f GF/s  %7.1f GB/s  %5.1f%% HBM" %
-              (cfg, op, "x".join(map(str, dims)), N, med, rec["gflops"], rec["gbs"], 100 * rec["hbm_frac"]), flush=True)
-
     base = {}
+
+    def rec(cfg, op, dims, N, fl, by, t, extra=None):
+        med, mn = t
+        r = {"config": cfg, "op": op, "dims": dims, "n_rhs": N, "ms_median": med, "ms_min": mn,
+             "gflops": fl / (med * 1e-3) / 1e9, "gbs": by / (med * 1e-3) / 1e9,
+             "hbm_frac": by / (med * 1e-3) / 1e9 / peak, "alg_bytes": by, "nominal_flops": fl}
+        base.setdefault((cfg, op), med / N)
+        r["speedup_per_rhs_vs_first_n"] = base[(cfg, op)] / (med / N)
+        if extra:
+            r.update(extra)
+        return r
+
     fine = [("config2", [24, 24, 24, 24], [1, 4, 12, 24, 48], 2), ("config5", [48, 48, 48, 48], [1, 12, 24], 5)]
-    if "fine" not in args.sweep_ops.split(","):
-        fine = []
-    for cfg, dims, ns, seed in fine:
+    for cfg, dims, ns, seed in (fine if "fine" in ops else []):
         V = vol(dims)
         U = syn.gauge_torch(dims, seed, device)
         for N in ns:
+            torch.cuda.synchronize()
             w = mrhs.Wilson(dims, N, MASS, CSW, U, stream=stream)
             psi = w.import_field(syn.spinor_torch(V, N, seed, device), mrhs.FULL)
             o_full = w.empty(mrhs.FULL)
@@ -532,49 +567,53 @@ def run_sweep(args):
             mrhs.cb_split(dims, 12, N, psi, ie, io)
             oe, oo, t0 = w.empty(mrhs.EVEN), w.empty(mrhs.ODD), w.empty(mrhs.ODD)
             torch.cuda.synchronize()
-            m, mn = timeit(lambda: w.dhop(psi, o_full))
-            emit(cfg, "dhop", dims, N, FLOPS_HOP * V * N, bytes_dhop(V, N), m, mn, base)
-            m, mn = timeit(lambda: w.meooe(ie, oo, mrhs.ODD))
-            emit(cfg, "meooe", dims, N, FLOPS_HOP * V / 2 * N, bytes_meooe(V, N), m, mn, base)
-            m, mn = timeit(lambda: w.mooee(psi, o_full, mrhs.FULL))
-            emit(cfg, "mooee", dims, N, FLOPS_CLOVER * V * N, bytes_mooee(V, N), m, mn, base)
-            m, mn = timeit(lambda: w.schur_sequence(ie, oo, t0, oe))
-            emit(cfg, "schur_seq", dims, N, (2 * FLOPS_HOP + FLOPS_CLOVER) * V / 2 * N,
-                 2 * bytes_meooe(V, N) + bytes_mooee(V / 2, N), m, mn, base)
-            # the full Wilson-clover matrix M = M_ooee - D_hop / 2 in one fused launch (NEXT-2): gauge + clover + one field in, one out
-            m, mn = timeit(lambda: w.apply(psi, o_full))
-            emit(cfg, "wilson_M", dims, N, (FLOPS_HOP + FLOPS_CLOVER + 48) * V * N, V * (576.0 + 192.0 * N), m, mn, base)
-            # simultaneous inner products <psi_r, out_r> (NEXT-4): two fields read once, 8 flops per complex element
-            res = torch.empty(N, dtype=torch.complex128, device=device)
-            m, mn = timeit(lambda: mrhs.inner_products(dims, 12, N, mrhs.FULL, psi, o_full, res, stream=stream))
-            emit(cfg, "inner_products", dims, N, 8.0 * 12 * V * N, 2.0 * 96 * V * N, m, mn, base)
-            # intergrid operators (NEXT-3): 4^4 aggregates, 20 basis vectors (nbasis 40); basis 1920 B per site
-            if N in (12, 24) and cfg == "config5":
-                nvec, bd = 20, [4, 4, 4, 4]
-                cd = [d // b for d, b in zip(dims, bd)]
-                basis = syn.spinor_torch(V * nvec, 1, seed + 1, device).reshape(nvec, V, 4, 3)
-                tr = mrhs.Transfer(dims, bd, nvec, N, basis, stream=stream)
-                del basis
-                vc = mrhs.empty_field(cd, 2 * nvec, N, mrhs.FULL, device)
-                vc.normal_()
-                fl, by = 8.0 * 12 * nvec * V * N, V * (96.0 * nvec + 96.0 * N) + vol(cd) * 16.0 * nvec * N
-                m, mn = timeit(lambda: tr.prolong(vc, o_full))
-                emit(cfg, "prolong", dims, N, fl, by, m, mn, base, {"nvec": nvec, "block": bd})
-                m, mn = timeit(lambda: tr.restrict(psi, vc))
-                emit(cfg, "restrict", dims, N, fl, by, m, mn, base, {"nvec": nvec, "block": bd})
-                tr.close()
-                del vc
+            kern = {mrhs.HOP_GATHER: "gather", mrhs.HOP_SWEEP: "sweep"}[mrhs.wilson_get_hop_kernel(w.h, 0)]
+            yield rec(cfg, "dhop", dims, N, FLOPS_HOP * V * N, bytes_dhop(V, N), timeit(lambda: w.dhop(psi, o_full)), {"hop_kernel": kern})
+            yield rec(cfg, "meooe", dims, N, FLOPS_HOP * V / 2 * N, bytes_meooe(V, N), timeit(lambda: w.meooe(ie, oo, mrhs.ODD)), {"hop_kernel": kern})
+            yield rec(cfg, "mooee", dims, N, FLOPS_CLOVER * V * N, bytes_mooee(V, N), timeit(lambda: w.mooee(psi, o_full, mrhs.FULL)))
+            if everything or N == 12:
+                fused = kern == "sweep"
+                by = 2 * bytes_meooe(V, N) + (288.0 * V / 2 if fused else bytes_mooee(V / 2, N))
+                yield rec(cfg, "schur_seq", dims, N, (2 * FLOPS_HOP + FLOPS_CLOVER) * V / 2 * N, by,
+                          timeit(lambda: w.schur_sequence(ie, oo, t0, oe)), {"launches": 2 if fused else 3})
+                # the even-odd preconditioned operator C_e - H_eo C_o^-1 H_oe / 4 (NEXT-2): two hops, the even input read twice
+                yield rec(cfg, "schur_apply", dims, N, (2 * FLOPS_HOP + 2 * FLOPS_CLOVER + 24) * V / 2 * N,
+                          2 * bytes_meooe(V, N) + (V / 2) * (2 * 288.0 + 96.0 * N), timeit(lambda: w.schur_apply(ie, t0, oe)))
+                # the full Wilson-clover matrix M = M_ooee - D_hop / 2 in one launch: gauge + clover + one field in, one out
+                yield rec(cfg, "wilson_M", dims, N, (FLOPS_HOP + FLOPS_CLOVER + 48) * V * N, V * (576.0 + 192.0 * N), timeit(lambda: w.apply(psi, o_full)))
+                yield rec(cfg, "dhop_dag", dims, N, FLOPS_HOP * V * N, bytes_dhop(V, N), timeit(lambda: w.dhop_dag(psi, o_full)))
+            if everything:
+                # simultaneous inner products <psi_r, out_r> (NEXT-4): two fields read once, 8 flops per complex element
+                res = torch.empty(N, dtype=torch.complex128, device=device)
+                yield rec(cfg, "inner_products", dims, N, 8.0 * 12 * V * N, 2.0 * 96 * V * N,
+                          timeit(lambda: mrhs.inner_products(dims, 12, N, mrhs.FULL, psi, o_full, res, stream=stream)))
+                # intergrid operators (NEXT-3): 4^4 aggregates, 20 basis vectors (nbasis 40); basis 1920 B per site
+                if N in (12, 24) and cfg == "config5":
+                    nvec, bd = 20, [4, 4, 4, 4]
+                    cd = [d // b for d, b in zip(dims, bd)]
+                    basis = syn.spinor_torch(V * nvec, 1, seed + 1, device).reshape(nvec, V, 4, 3)
+                    torch.cuda.synchronize()
+                    tr = mrhs.Transfer(dims, bd, nvec, N, basis, stream=stream)
+                    del basis
+                    vc = mrhs.empty_field(cd, 2 * nvec, N, mrhs.FULL, device)
+                    vc.normal_()
+                    torch.cuda.synchronize()
+                    fl, by = 8.0 * 12 * nvec * V * N, V * (96.0 * nvec + 96.0 * N) + vol(cd) * 16.0 * nvec * N
+                    yield rec(cfg, "prolong", dims, N, fl, by, timeit(lambda: tr.prolong(vc, o_full)), {"nvec": nvec, "block": bd})
+                    yield rec(cfg, "restrict", dims, N, fl, by, timeit(lambda: tr.restrict(psi, vc)), {"nvec": nvec, "block": bd})
+                    tr.close()
+                    del vc
             w.close()
-            del psi, o_full, ie, io, oe, oo, t0
+            del w, psi, o_full, ie, io, oe, oo, t0
+            torch.cuda.empty_cache()
         del U
     coarse = [("config3", [8, 8, 8, 8], 24, [1, 12, 24, 64], 3), ("config4", [6, 6, 6, 32], 40, [12, 24, 48, 96], 4)]
-    if "coarse" not in args.sweep_ops.split(","):
-        coarse = []
-    for cfg, dims, nb, ns, seed in coarse:
+    for cfg, dims, nb, ns, seed in (coarse if "coarse" in ops else []):
         V = vol(dims)
         A = syn.coarse_links_torch(dims, nb, seed, device)
         for N in ns:
             for mode in mrhs.COARSE_MODES:
+                torch.cuda.synchronize()
                 try:
                     c = mrhs.Coarse(dims, nb, N, A, math_mode=mode, stream=stream)
                 except mrhs.MrhsError:
@@ -582,16 +621,57 @@ def run_sweep(args):
                 v = c.import_field(syn.spinor_torch(V, N, seed, device, ncomp=(nb,)))
                 vo = c.empty()
                 torch.cuda.synchronize()
-                m, mn = timeit(lambda: c.apply(v, vo))
-                emit(cfg, "coarse_mode%d" % mode, dims, N, coarse_flops(nb) * V * N, bytes_coarse(V, nb, N), m, mn, base,
-                     {"nbasis": nb, "fp32_fma_peak_frac": coarse_flops(nb) * V * N / (m * 1e-3) / 74.4e12})
-                # the 8-point coarse hopping term alone (what the paper's coarse-level figure measures, reading S12)
-                m, mn = timeit(lambda: c.apply(v, vo, mrhs.COARSE_HOP))
-                emit(cfg, "coarse_hop8_mode%d" % mode, dims, N, 64 * nb * nb * V * N, V * (64 * nb * nb + 16 * nb * N), m, mn, base,
-                     {"nbasis": nb})
+                fl = coarse_flops(nb) * V * N
+                t = timeit(lambda: c.apply(v, vo))
+                yield rec(cfg, "coarse_mode%d" % mode, dims, N, fl, bytes_coarse(V, nb, N), t,
+                          {"nbasis": nb, "fp32_fma_peak_frac": fl / (t[0] * 1e-3) / 74.4e12})
+                # the 8-point coarse hopping term alone (what the paper's coarse-level figure measures, reading S12) and coarse
+                # M_eooe (NEXT-1): the same term on one parity from the other (all link matrices of the output sites, half the vectors)
+                yield rec(cfg, "coarse_hop8_mode%d" % mode, dims, N, 64 * nb * nb * V * N, V * (64 * nb * nb + 16 * nb * N),
+                          timeit(lambda: c.apply(v, vo, mrhs.COARSE_HOP)), {"nbasis": nb})
+                if all(d % 2 == 0 for d in dims):
+                    ve, vod = c.empty(parity=mrhs.EVEN), c.empty(parity=mrhs.ODD)
+                    mrhs.coarse_cb_split(dims, nb, N, v, ve, vod)
+                    oe = c.empty(parity=mrhs.EVEN)
+                    torch.cuda.synchronize()
+                    yield rec(cfg, "coarse_meooe_mode%d" % mode, dims, N, 64 * nb * nb * (V / 2) * N, (V / 2) * (64 * nb * nb + 16 * nb * N),
+                              timeit(lambda: c.meooe(vod, oe, mrhs.EVEN)), {"nbasis": nb})
+                    del ve, vod, oe
                 c.close()
+                del c, v, vo
+        if everything and cfg == "config4":
+            # coarse -> coarser intergrid operators (NEXT-3): 40 -> 60 components, 3 x 3 x 3 x 2 aggregates
+            nf, nvec, bd, N = nb, 30, [3, 3, 3, 2], 12
+            cd = [d // b for d, b in zip(dims, bd)]
+            basis = syn.spinor_torch(V * nvec, 1, seed + 1, device, ncomp=(nf,)).reshape(nvec, V, nf)
+            torch.cuda.synchronize()
+            tr = mrhs.Transfer(dims, bd, nvec, N, basis, stream=stream, nf=nf)
+            del basis
+            vc = mrhs.empty_field(cd, 2 * nvec, N, mrhs.FULL, device).normal_()
+            vf = mrhs.empty_field(dims, nf, N, mrhs.FULL, device).normal_()
+            torch.cuda.synchronize()
+            fl, by = 8.0 * (nf / 2) * nvec * V * N * 2 / 2, V * (8.0 * nf * nvec + 8.0 * nf * N) + vol(cd) * 16.0 * nvec * N
+            yield rec(cfg, "prolong_coarse", dims, N, fl, by, timeit(lambda: tr.prolong(vc, vf)), {"nf": nf, "nvec": nvec, "block": bd})
+            yield rec(cfg, "restrict_coarse", dims, N, fl, by, timeit(lambda: tr.restrict(vf, vc)), {"nf": nf, "nvec": nvec, "block": bd})
+            tr.close()
         del A
-    out.close()
+
+
+def run_sweep(args):
+    """--sweep OUT.jsonl: every operator of the library over configs 2-5, one JSON line each (and a table on stdout)."""
+    import torch
+    import paper_2211_13719_b200 as mrhs
+    import synth_inputs as syn
+    device = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    peak, _ = measured_peaks()
+    stream = torch.cuda.Stream(device)
+    with open(args.sweep, "w") as out:
+        for r in sweep_records(torch, mrhs, syn, device, stream, peak, iters=args.sweep_iters, subset="all", ops=tuple(args.sweep_ops.split(","))):
+            out.write(json.dumps(r) + "\n")
+            out.flush()
+            print("%-8s %-20s %-16s N=%-3d %8.4f ms  %9.1f GF/s  %7.1f GB/s  %5.1f%% HBM" %
+                  (r["config"], r["op"], "x".join(map(str, r["dims"])), r["n_rhs"], r["ms_median"], r["gflops"], r["gbs"], 100 * r["hbm_frac"]), flush=True)
     return 0
 
 
@@ -608,6 +688,8 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=8, help="oracle sample steps timed for cpu_baseline")
     ap.add_argument("--sweep", default=None, help="write the per-operator N_rhs sweep to this .jsonl and exit")
     ap.add_argument("--sweep-iters", type=int, default=30)
+    ap.add_argument("--no-sweep", action="store_true", help="leave the N_rhs sweep (key nrhs_sweep) out of the bench line")
+    ap.add_argument("--inrun-sweep-iters", type=int, default=10, help="timed launches per point of the in-run N_rhs sweep")
     ap.add_argument("--sweep-ops", default="fine,coarse", help="which operator families the sweep covers")
     ap.add_argument("--hop-tiling", default=None, help="by,bz,bt,cy,cz for D_hop and M_eooe instead of the library default")
     ap.add_argument("--hop-prefetch", type=int, default=None, help="L2 prefetch distance in tiles (0 = off)")
