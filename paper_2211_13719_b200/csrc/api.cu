@@ -2,6 +2,7 @@
 // host-buffer (end-to-end) entries.  Every operator step runs in the kernels of fine_hop.cu,
 // clover.cu and coarse.cu; nothing here computes.
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "coarse.cuh"
@@ -39,10 +40,12 @@ struct mrhs_wilson {
     cudaStream_t st;
     FieldGeom gfull, gcb[2];
     float4 *gauge_full, *gauge_cb[2];
+    float4 *gauge_back[2];         // packed backward links of the sites of parity p (fine_sweep.cuh), the sweep kernel's second link stream
     float4 *clov_full, *clov_cb[2];
     float4 *cinv_full, *cinv_cb[2];   // inverse clover blocks, same packing and layouts
     HopParams hp_full, hp_cb[2];   // hp_cb[p]: output parity p
     SweepParams sp_full, sp_cb[2]; // the slice-sweep kernel's launch description (fine_sweep.cuh)
+    unsigned have;                 // SiteCopy bits: which derived site-data copies exist (api.cu wilson_ensure)
     int kern[2];                   // which kernel runs D_hop [0] / M_eooe [1]: MRHS_HOP_GATHER or MRHS_HOP_SWEEP
     int num_sms;
     size_t l2_bytes;
@@ -76,6 +79,7 @@ namespace {
 mrhs_status_t wilson_free(mrhs_wilson *h) {
     if (!h) return MRHS_OK;
     cudaFree(h->gauge_full); cudaFree(h->gauge_cb[0]); cudaFree(h->gauge_cb[1]);
+    cudaFree(h->gauge_back[0]); cudaFree(h->gauge_back[1]);
     cudaFree(h->clov_full); cudaFree(h->clov_cb[0]); cudaFree(h->clov_cb[1]);
     cudaFree(h->cinv_full); cudaFree(h->cinv_cb[0]); cudaFree(h->cinv_cb[1]);
     cudaFree(h->st_canon); cudaFree(h->st_in); cudaFree(h->st_out);
@@ -84,36 +88,82 @@ mrhs_status_t wilson_free(mrhs_wilson *h) {
     return MRHS_OK;
 }
 
+// Site data (gauge links, clover blocks, inverse clover blocks) is packed per layout that reads it: the full lattice and
+// the two checkerboards.  Only the full-lattice gauge and clover copies are made at create; every other copy is derived
+// from those on the handle's stream the first time an operator needs it (SiteCopy below), so a handle holds what its
+// launches actually read (at 48^4: 3.1 GB after create instead of 13.8 GB for all nine copies).
+enum SiteCopy { COPY_GAUGE_CB = 1, COPY_CLOV_CB = 2, COPY_CINV_FULL = 4, COPY_CINV_CB = 8 };
+
 mrhs_status_t wilson_build(mrhs_wilson *h, const void *d_gauge, const void *d_clover) {
     const size_t site_bytes = 72 * sizeof(float);
     const size_t V = (size_t)h->gfull.nsites;
     MRHS_CUDA(cudaMalloc(&h->gauge_full, V * site_bytes));
     MRHS_CUDA(cudaMalloc(&h->clov_full, V * site_bytes));
-    MRHS_CUDA(cudaMalloc(&h->cinv_full, V * site_bytes));
-    for (int p = 0; p < 2; p++) {
-        MRHS_CUDA(cudaMalloc(&h->gauge_cb[p], V / 2 * site_bytes));
-        MRHS_CUDA(cudaMalloc(&h->clov_cb[p], V / 2 * site_bytes));
-        MRHS_CUDA(cudaMalloc(&h->cinv_cb[p], V / 2 * site_bytes));
-    }
     // the canonical gauge field already is [lex][72 floats]
     mrhs_status_t s;
     if ((s = pack_site_data(h->gfull, (const float *)d_gauge, h->gauge_full, h->st)) != MRHS_OK) return s;
-    for (int p = 0; p < 2; p++)
-        if ((s = pack_site_data(h->gcb[p], (const float *)d_gauge, h->gauge_cb[p], h->st)) != MRHS_OK) return s;
     float *tmp = nullptr;
     MRHS_CUDA(cudaMalloc(&tmp, V * site_bytes));
     if (d_clover) s = pack_clover_blocks((long long)V, (const float2 *)d_clover, tmp, h->st);
     else s = build_clover(h->dims, h->mass, h->csw, (const float2 *)d_gauge, tmp, h->st);
     if (s == MRHS_OK) s = pack_site_data(h->gfull, tmp, h->clov_full, h->st);
-    for (int p = 0; p < 2 && s == MRHS_OK; p++) s = pack_site_data(h->gcb[p], tmp, h->clov_cb[p], h->st);
-    // inverse blocks, in place in tmp (pack_site_data above has been enqueued on the same stream)
-    if (s == MRHS_OK) s = invert_clover_blocks((long long)V, tmp, tmp, h->st);
-    if (s == MRHS_OK) s = pack_site_data(h->gfull, tmp, h->cinv_full, h->st);
-    for (int p = 0; p < 2 && s == MRHS_OK; p++) s = pack_site_data(h->gcb[p], tmp, h->cinv_cb[p], h->st);
     cudaError_t e = cudaStreamSynchronize(h->st);
     cudaFree(tmp);
     if (s != MRHS_OK) return s;
     MRHS_CUDA(e);
+    return MRHS_OK;
+}
+
+// Makes the copies in `want` (SiteCopy bits) that do not exist yet.  Source: the full-lattice packed copy, unpacked to the
+// canonical [lex][72] order in a temporary.  Synchronises the handle's stream when it had to build something.
+mrhs_status_t wilson_ensure(mrhs_wilson *h, unsigned want) {
+    want &= ~h->have;
+    if (!want) return MRHS_OK;
+    const size_t site_bytes = 72 * sizeof(float);
+    const size_t V = (size_t)h->gfull.nsites;
+    float *tmp = nullptr;
+    MRHS_CUDA(cudaMalloc(&tmp, V * site_bytes));
+    mrhs_status_t s = MRHS_OK;
+    auto alloc = [&](float4 **p, size_t bytes) {
+        if (s != MRHS_OK || *p) return;
+        cudaError_t e = cudaMalloc(p, bytes);
+        if (e != cudaSuccess) s = cuda_fail(e, "cudaMalloc(site data)", __FILE__, __LINE__);
+    };
+    if (want & COPY_GAUGE_CB) {
+        for (int p = 0; p < 2; p++) alloc(&h->gauge_cb[p], V / 2 * site_bytes);
+        if (s == MRHS_OK) s = unpack_site_data(h->gfull, h->gauge_full, tmp, h->st);
+        for (int p = 0; p < 2 && s == MRHS_OK; p++) s = pack_site_data(h->gcb[p], tmp, h->gauge_cb[p], h->st);
+        if (h->sp_cb[0].grid) {      // the sweep kernel can run this geometry
+            for (int p = 0; p < 2; p++) alloc(&h->gauge_back[p], (size_t)h->gcb[p].nblocks() * kBackF4 * h->gcb[p].XB * sizeof(float4));
+            for (int p = 0; p < 2 && s == MRHS_OK; p++) s = pack_back_links(h->gcb[p], tmp, h->gauge_back[p], h->st);
+        }
+    }
+    if (want & (COPY_CLOV_CB | COPY_CINV_FULL | COPY_CINV_CB)) {
+        if (want & COPY_CLOV_CB) for (int p = 0; p < 2; p++) alloc(&h->clov_cb[p], V / 2 * site_bytes);
+        if (want & COPY_CINV_FULL) alloc(&h->cinv_full, V * site_bytes);
+        if (want & COPY_CINV_CB) for (int p = 0; p < 2; p++) alloc(&h->cinv_cb[p], V / 2 * site_bytes);
+        if (s == MRHS_OK) s = unpack_site_data(h->gfull, h->clov_full, tmp, h->st);
+        if (want & COPY_CLOV_CB)
+            for (int p = 0; p < 2 && s == MRHS_OK; p++) s = pack_site_data(h->gcb[p], tmp, h->clov_cb[p], h->st);
+        if (want & (COPY_CINV_FULL | COPY_CINV_CB)) {
+            // inverse blocks, in place in tmp (the packs above have been enqueued on the same stream)
+            if (s == MRHS_OK) s = invert_clover_blocks((long long)V, tmp, tmp, h->st);
+            if ((want & COPY_CINV_FULL) && s == MRHS_OK) s = pack_site_data(h->gfull, tmp, h->cinv_full, h->st);
+            if (want & COPY_CINV_CB)
+                for (int p = 0; p < 2 && s == MRHS_OK; p++) s = pack_site_data(h->gcb[p], tmp, h->cinv_cb[p], h->st);
+        }
+    }
+    cudaError_t e = cudaStreamSynchronize(h->st);
+    cudaFree(tmp);
+    if (s != MRHS_OK) return s;
+    MRHS_CUDA(e);
+    h->have |= want;
+    if (want & COPY_GAUGE_CB)
+        for (int p = 0; p < 2; p++) {
+            h->hp_cb[p].gauge_out = h->gauge_cb[p];     h->sp_cb[p].gauge_out = h->gauge_cb[p];
+            h->hp_cb[p].gauge_in = h->gauge_cb[1 - p];  h->sp_cb[p].gauge_in = h->gauge_cb[1 - p];
+            h->sp_cb[p].gauge_back = h->gauge_back[p];
+        }
     return MRHS_OK;
 }
 
@@ -145,12 +195,37 @@ mrhs_status_t wilson_set_default_tiling(mrhs_wilson *h) {
         for (int p = 0; p < 2; p++) ok = ok && build_sweep_params(h->gcb[p], p, default_sweep_tiling(h->gcb[p], h->num_sms), h->sp_cb[p]);
         if (ok) {
             h->sp_full.gauge_out = h->sp_full.gauge_in = h->gauge_full;
-            for (int p = 0; p < 2; p++) { h->sp_cb[p].gauge_out = h->gauge_cb[p]; h->sp_cb[p].gauge_in = h->gauge_cb[1 - p]; }
+            for (int p = 0; p < 2; p++) { h->sp_cb[p].gauge_out = h->gauge_cb[p]; h->sp_cb[p].gauge_in = h->gauge_cb[1 - p]; h->sp_cb[p].gauge_back = h->gauge_back[p]; }
             // measured cross-over (profiles/r1d_kernel_choice.md): the sweep kernel wins from N_rhs = 12 on lattices of 32^4
             // sites and more; below that the gather kernel's many small blocks hide latency better
             if (h->nrhs >= 12 && h->gfull.nsites >= (1ll << 20)) h->kern[0] = h->kern[1] = MRHS_HOP_SWEEP;
         }
     }
+    return MRHS_OK;
+}
+
+// One private stream-ordered memory pool per device for per-call scratch (mrhs_inner_products).  Freed blocks stay in the
+// pool (release threshold = max), so a call does not go back to the driver; created once per device under a mutex.
+mrhs_status_t scratch_pool(int dev, cudaMemPool_t *out) {
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static cudaMemPool_t pools[kMaxDev] = {};
+    if (dev < 0 || dev >= kMaxDev) { set_error("scratch pool: device ordinal %d out of range", dev); return MRHS_ERR_UNSUPPORTED; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!pools[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t p = nullptr;
+        MRHS_CUDA(cudaMemPoolCreate(&p, &props));
+        unsigned long long keep = ~0ull;
+        cudaError_t e = cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep);
+        if (e != cudaSuccess) { cudaMemPoolDestroy(p); return cuda_fail(e, "cudaMemPoolSetAttribute", __FILE__, __LINE__); }
+        pools[dev] = p;
+    }
+    *out = pools[dev];
     return MRHS_OK;
 }
 
@@ -213,6 +288,10 @@ mrhs_status_t mrhs_wilson_create(mrhs_wilson_t **out, const int dims[4], int nrh
 // dagger = the adjoint; clover / aux = the fused epilogues of the sweep kernel (fine_sweep.cuh), sweep kernel only.
 static mrhs_status_t hop_launch(mrhs_wilson_t *h, int parity, int dagger, const float4 *clover, const void *aux, const void *d_in, void *d_out) {
     const int which = parity < 0 ? 0 : 1;
+    if (parity >= 0) {
+        mrhs_status_t s = wilson_ensure(h, COPY_GAUGE_CB);
+        if (s != MRHS_OK) return s;
+    }
     if (h->kern[which] == MRHS_HOP_SWEEP) {
         SweepParams p = parity < 0 ? h->sp_full : h->sp_cb[parity];
         p.dagger = dagger;
@@ -263,13 +342,15 @@ mrhs_status_t mrhs_schur_apply(mrhs_wilson_t *h, const void *d_in, void *d_tmp, 
     MRHS_REQUIRE(d_in != d_out && d_in != d_tmp && d_tmp != d_out, "schur apply: the three buffers must be distinct");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_tmp) && aligned16(d_out), "schur apply: buffers must be 16-byte aligned");
     // S = C_e - H_eo C_o^-1 H_oe / 4 (the daggered hops for S^+; the clover blocks are Hermitian)
+    mrhs_status_t s = wilson_ensure(h, COPY_GAUGE_CB | COPY_CLOV_CB | COPY_CINV_CB);
+    if (s != MRHS_OK) return s;
     if (h->kern[1] == MRHS_HOP_SWEEP) {
         // two launches: tmp = C_o^-1 H_oe in;  out = C_e in - H_eo tmp / 4 (the input is read again by the second epilogue)
-        mrhs_status_t s = hop_launch(h, MRHS_ODD, dagger, h->cinv_cb[MRHS_ODD], nullptr, d_in, d_tmp);
+        s = hop_launch(h, MRHS_ODD, dagger, h->cinv_cb[MRHS_ODD], nullptr, d_in, d_tmp);
         if (s == MRHS_OK) s = hop_launch(h, MRHS_EVEN, dagger, h->clov_cb[MRHS_EVEN], d_in, d_tmp, d_out);
         return s;
     }
-    mrhs_status_t s = hop_launch(h, MRHS_ODD, dagger, nullptr, nullptr, d_in, d_tmp);
+    s = hop_launch(h, MRHS_ODD, dagger, nullptr, nullptr, d_in, d_tmp);
     if (s == MRHS_OK) s = launch_mooee(h->gcb[MRHS_ODD], h->cinv_cb[MRHS_ODD], d_tmp, d_tmp, h->st);
     if (s == MRHS_OK) s = hop_launch(h, MRHS_EVEN, dagger, nullptr, nullptr, d_tmp, d_out);
     if (s == MRHS_OK) s = launch_mooee(h->gcb[MRHS_EVEN], h->clov_cb[MRHS_EVEN], d_in, d_out, h->st, -0.25f);
@@ -284,6 +365,8 @@ static mrhs_status_t mooee_impl(mrhs_wilson_t *h, const void *d_in, void *d_out,
     MRHS_REQUIRE(parity >= 0 && parity <= 2, "mooee: parity must be 0, 1 or 2");
     MRHS_REQUIRE(d_in != d_out, "mooee: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "mooee: buffers must be 16-byte aligned");
+    const mrhs_status_t s = wilson_ensure(h, parity == MRHS_FULL ? (inverse ? COPY_CINV_FULL : 0u) : (inverse ? COPY_CINV_CB : COPY_CLOV_CB));
+    if (s != MRHS_OK) return s;
     if (parity == MRHS_FULL) return launch_mooee(h->gfull, inverse ? h->cinv_full : h->clov_full, d_in, d_out, h->st);
     return launch_mooee(h->gcb[parity], inverse ? h->cinv_cb[parity] : h->clov_cb[parity], d_in, d_out, h->st);
 }
@@ -296,11 +379,13 @@ static mrhs_status_t meooe_mooee_impl(mrhs_wilson_t *h, const void *d_in, void *
     MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "meooe_mooee: out_parity must be 0 or 1");
     MRHS_REQUIRE(d_in != d_out, "meooe_mooee: in and out must not alias");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "meooe_mooee: buffers must be 16-byte aligned");
+    mrhs_status_t s = wilson_ensure(h, COPY_GAUGE_CB | (inverse ? COPY_CINV_CB : COPY_CLOV_CB));
+    if (s != MRHS_OK) return s;
     const float4 *blocks = inverse ? h->cinv_cb[out_parity] : h->clov_cb[out_parity];
     // sweep kernel: one launch, the clover blocks of the output sites are applied to the hop result before it is stored
     if (h->kern[1] == MRHS_HOP_SWEEP) return hop_launch(h, out_parity, 0, blocks, nullptr, d_in, d_out);
     // gather kernel: two launches, the second in place
-    mrhs_status_t s = hop_launch(h, out_parity, 0, nullptr, nullptr, d_in, d_out);
+    s = hop_launch(h, out_parity, 0, nullptr, nullptr, d_in, d_out);
     if (s == MRHS_OK) s = launch_mooee(h->gcb[out_parity], blocks, d_out, d_out, h->st);
     return s;
 }
@@ -407,6 +492,7 @@ mrhs_status_t mrhs_wilson_set_sweep(mrhs_wilson_t *h, int which, int lt, const i
             MRHS_REQUIRE(build_sweep_params(h->gcb[q], q, t, p[q]), "set sweep: segment / chunk does not fit the checkerboarded lattice (or odd N_rhs)");
             p[q].gauge_out = h->gauge_cb[q];
             p[q].gauge_in = h->gauge_cb[1 - q];
+            p[q].gauge_back = h->gauge_back[q];
             p[q].pf = h->sp_cb[q].pf;
         }
         h->sp_cb[0] = p[0];
@@ -674,17 +760,13 @@ mrhs_status_t mrhs_inner_products(const int dims[4], int ncomp, int nrhs, int pa
     MRHS_CUDA(cudaGetDevice(&dev));
     MRHS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     const int grid = inner_grid(sms);
-    // the scratch comes from the device's stream-ordered pool; keep freed blocks in the pool so that the
-    // allocation does not go back to the driver on every call
-    static bool pool_ready = false;
-    if (!pool_ready) {
-        cudaMemPool_t pool;
-        unsigned long long keep = ~0ull;
-        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        pool_ready = true;
-    }
+    // the scratch comes from a stream-ordered pool of the library's own (one per device, made on first use, kept warm);
+    // the device's default pool and its settings are the caller's and are not touched
+    cudaMemPool_t pool = nullptr;
+    mrhs_status_t ps = scratch_pool(dev, &pool);
+    if (ps != MRHS_OK) return ps;
     double2 *partial = nullptr;
-    MRHS_CUDA(cudaMallocAsync(&partial, (size_t)grid * nrhs * sizeof(double2), st));
+    MRHS_CUDA(cudaMallocFromPoolAsync((void **)&partial, (size_t)grid * nrhs * sizeof(double2), pool, st));
     mrhs_status_t s = launch_inner_products((long long)(bytes / 4), nrhs, d_x, d_y, partial, grid, (double2 *)d_result, st);
     cudaError_t e = cudaFreeAsync(partial, st);
     if (s != MRHS_OK) return s;

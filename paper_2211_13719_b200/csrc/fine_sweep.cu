@@ -38,16 +38,19 @@ static_assert(BY == 2 && BZ == 2, "every tile row has exactly one halo row in y 
 
 // Byte sizes of the shared-memory regions for a layout block of XB sites and NP RHS pairs.
 struct SweepSmem {
-    uint32_t RB, GO, GW, GROW;              // tile row, own links of a row, one link window, all links of one row
+    uint32_t RB, GO, GW, GBK, GROW;         // tile row, own links of a row, one link window, backward links of a row (checkerboarded), all links of one row
     uint32_t I_BYTES, G_BYTES;              // per buffer (two buffers each)
     uint32_t H_BYTES, XH_BYTES;             // halo rows in y and z (ROWS each); x halo slots [side][row][component][pair]
     uint32_t C_BYTES;                       // packed clover blocks of the tile rows (fused epilogues), per buffer
     uint32_t off_G, off_H, off_XH, off_C, off_bar, total;
-    __host__ __device__ SweepSmem(int XB, int NP, bool clov) {
+    __host__ __device__ SweepSmem(int XB, int NP, bool clov, bool cb) {
         RB = 12u * XB * NP * 16u;
         GO = 18u * XB * 16u;
         GW = 5u * XB * 16u;
-        GROW = GO + 5u * GW;
+        GBK = (uint32_t)kBackF4 * XB * 16u;
+        // full lattice: the backward links are other sites' own links, three windows of them (x-block before, y-1, z-1);
+        // checkerboarded: the packed backward links of the row (fine_sweep.cuh)
+        GROW = cb ? GO + GBK : GO + 3u * GW;
         I_BYTES = ROWS * RB;
         G_BYTES = ROWS * GROW;
         H_BYTES = 2u * ROWS * RB;
@@ -84,14 +87,14 @@ struct SplitOperands {
 
 // nb: component 0 of the neighbour's element for this unit; os / op: offsets of colour 0 of the two spin rows; st: component
 // stride; g: float4 0 of the link's site data
-template <int MU>
+template <int MU, int LMU = MU>
 __device__ __forceinline__ void split_load(SplitOperands &o, const float4 *nb, int os, int op, int st, const float4 *g, int XB) {
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         o.ps[c] = nb[os + c * st];
         o.pp[c] = nb[op + c * st];
     }
-    load_link_s<MU>(g, XB, o.u);
+    load_link_s<LMU>(g, XB, o.u);
 }
 
 // This lane's row of the projected half spinor and of r = U h (FWD) or U^+ h.  Spin row s (e = +1 for s = 0, -1 for s = 1):
@@ -189,7 +192,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     const int cs = XB * NP;                       // units (site, RHS pair) per tile row = elements of one row component
     const int WPR = (cs + 15) >> 4;               // consumer warps per tile row: sixteen units x two spin rows each
     const int NWC = ROWS * WPR;
-    const SweepSmem L(XB, NP, CLOV);
+    const SweepSmem L(XB, NP, CLOV, CB);
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + L.off_bar);
     uint64_t *fullI = bars, *freeI = bars + 2, *fullG = bars + 4, *freeG = bars + 6, *fullH = bars + 8, *freeH = bars + 10;
@@ -249,7 +252,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
                     if (q < ROWS) bulk_prefetch_l2(in + bb * 12 * cs, L.RB);
                     else if (jp < lt) {
                         bulk_prefetch_l2(p.gauge_out + bb * kSiteF4 * XB, L.GO);
-                        if (CB) bulk_prefetch_l2(p.gauge_in + bb * kSiteF4 * XB, L.GO);      // the backward links live on the input sites
+                        if (CB) bulk_prefetch_l2(p.gauge_back + bb * kBackF4 * XB, L.GBK);
                     }
                 }
             };
@@ -289,29 +292,36 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
                 const int t = tw(j);
                 const uint32_t b = (uint32_t)(j + 1) & 1u;
                 const bool mid = j >= 0 && j < lt;
-                // link copies per row: on the full lattice U_x and U_t of the input row are the own links
-                constexpr int NG = CB ? 6 : 4;
                 unsigned char *Gb = smem + L.off_G + b * L.G_BYTES;
                 if (mid || j == -1) {
-                    if (lane == 0) mbar_expect_tx(&fullG[b], mid ? (ROWS / 2) * (L.GO + (NG - 1) * L.GW + (CLOV ? L.GO : 0u)) : (ROWS / 2) * (CB ? L.GW : L.GO));
-                    __syncwarp();
-                    for (int idx = lane; idx < (ROWS / 2) * 6; idx += 32) {
-                        const int r = r_lo + idx / 6, w = idx % 6;
-                        if (!CB && (w == 1 || w == 5)) continue;
-                        if (j == -1 && w != (CB ? 5 : 0)) continue;
-                        const int y = y0 + r % BY, z = z0 + r / BY;
-                        unsigned char *dst = Gb + r * L.GROW;
-                        const float4 *src;
-                        uint32_t bytes = L.GW;
-                        switch (w) {
-                            case 0: src = p.gauge_out + blk(xb, y, z, t) * kSiteF4 * XB; bytes = L.GO; break;                       // own links
-                            case 1: src = p.gauge_in + blk(xb, y, z, t) * kSiteF4 * XB; dst += L.GO; break;                        // U_x at the -x neighbours in this x-block
-                            case 2: src = p.gauge_in + blk(xbm, y, z, t) * kSiteF4 * XB; dst += L.GO + L.GW; break;                // ... and in the x-block before it
-                            case 3: src = p.gauge_in + (blk(xb, wrap(y - 1, Y), z, t) * kSiteF4 + 4) * XB; dst += L.GO + 2 * L.GW; break;   // U_y at y-1
-                            case 4: src = p.gauge_in + (blk(xb, y, wrap(z - 1, Z), t) * kSiteF4 + 9) * XB; dst += L.GO + 3 * L.GW; break;   // U_z at z-1
-                            default: src = p.gauge_in + (blk(xb, y, z, t) * kSiteF4 + 13) * XB; dst += L.GO + 4 * L.GW; break;     // U_t of the input row (carry)
+                    if constexpr (CB) {
+                        // per row: the own links and the packed backward links (one contiguous copy each); for slice -1 only the
+                        // t-links of the input row, which the carry of the first step needs
+                        if (lane == 0) mbar_expect_tx(&fullG[b], mid ? (ROWS / 2) * (L.GO + L.GBK + (CLOV ? L.GO : 0u)) : (ROWS / 2) * L.GW);
+                        __syncwarp();
+                        if (lane < ROWS) {
+                            const int r = r_lo + (lane >> 1), w = lane & 1;
+                            const size_t bb = blk(xb, y0 + r % BY, z0 + r / BY, t);
+                            unsigned char *dst = Gb + r * L.GROW;
+                            if (mid && w == 0) bulk_g2s(dst, p.gauge_out + bb * kSiteF4 * XB, L.GO, &fullG[b]);
+                            else if (mid) bulk_g2s(dst + L.GO, p.gauge_back + bb * kBackF4 * XB, L.GBK, &fullG[b]);
+                            else if (w == 1) bulk_g2s(dst + L.GO + kBackT * XB * 16, p.gauge_back + (bb * kBackF4 + kBackT) * XB, L.GW, &fullG[b]);
                         }
-                        bulk_g2s(dst, src, bytes, &fullG[b]);
+                    } else {
+                        // per row: the own links (U_x and U_t of the input row are own links too) and three windows of other rows'
+                        // links; for slice -1 only the own links
+                        if (lane == 0) mbar_expect_tx(&fullG[b], mid ? (ROWS / 2) * (L.GO + 3 * L.GW + (CLOV ? L.GO : 0u)) : (ROWS / 2) * L.GO);
+                        __syncwarp();
+                        if (lane < (ROWS / 2) * 4) {
+                            const int r = r_lo + (lane >> 2), w = lane & 3;
+                            const int y = y0 + r % BY, z = z0 + r / BY;
+                            unsigned char *dst = Gb + r * L.GROW;
+                            if (w == 0) bulk_g2s(dst, p.gauge_out + blk(xb, y, z, t) * kSiteF4 * XB, L.GO, &fullG[b]);                                     // own links
+                            else if (!mid) {}
+                            else if (w == 1) bulk_g2s(dst + L.GO, p.gauge_in + blk(xbm, y, z, t) * kSiteF4 * XB, L.GW, &fullG[b]);                        // U_x in the x-block before
+                            else if (w == 2) bulk_g2s(dst + L.GO + L.GW, p.gauge_in + (blk(xb, wrap(y - 1, Y), z, t) * kSiteF4 + 4) * XB, L.GW, &fullG[b]);      // U_y at y-1
+                            else bulk_g2s(dst + L.GO + 2 * L.GW, p.gauge_in + (blk(xb, y, wrap(z - 1, Z), t) * kSiteF4 + 9) * XB, L.GW, &fullG[b]);              // U_z at z-1
+                        }
                     }
                     if (CLOV && mid && lane >= 32 - ROWS / 2) {
                         const int r = r_lo + lane - (32 - ROWS / 2);
@@ -358,14 +368,19 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     const int zm_o = tz == 0 ? oHz : own - BY * rowlen, zm_bs = tz == 0 ? 0 : IB4;
     const bool edge_p = xin + 1 == XB, edge_m = xin == 0;
     const int hxp = oXH + ((ROWS + r) * 12) * NP + pair, hxm = oXH + (r * 12) * NP + pair;
-    // links (float4 units): row r of the link buffer; windows are addressed through the base of a virtual 18-row site
+    // links (float4 units), row r of the link buffer: the own links, then
+    //   checkerboarded: the packed backward links of this row's sites (the link of the hop from x-mu sits at site x; the t-links of
+    //   the input row follow from float4 kBackT on)
+    //   full lattice: windows of other sites' own links (last site of the x-block before, row y-1, row z-1), addressed through the
+    //   base of a virtual 18-row site
     const int Gr = (int)(L.off_G / 16) + r * (int)(L.GROW / 16);
     const int g_own = Gr + xin;
     const int g_bx_same = CB ? Gr + 18 * XB + xin : g_own;
-    const int g_bx_step = edge_m ? Gr + 23 * XB + XB - 1 : (CB ? Gr + 18 * XB + xin - 1 : g_own - 1);
-    const int g_by = Gr + 28 * XB - 4 * XB + xin;
-    const int g_bz = Gr + 33 * XB - 9 * XB + xin;
-    const int g_bt = CB ? Gr + 38 * XB - 13 * XB + xin : g_own;
+    const int g_bx_step = CB ? g_bx_same : (edge_m ? Gr + 18 * XB + XB - 1 : g_own - 1);
+    const int g_by = CB ? g_bx_same : Gr + 23 * XB - 4 * XB + xin;
+    const int g_bz = CB ? g_bx_same : Gr + 28 * XB - 9 * XB + xin;
+    const int g_bt = CB ? Gr + (18 + kBackT) * XB + xin : g_own;
+    constexpr int LT = CB ? 0 : 3;      // where the t-link starts inside its site data: float4 0 of the packed t-links, or link 3 of the own links
 
     CVec<2> up[3], la[3], lb[3];   // output spin row s; rows 3 - s (from the x and y hops) and 2 + s (from the z and t hops)
     // this lane's row of U_t^+ (1 + gamma_t) psi of the slice before the centre slice.  The own rows of a slice are read from
@@ -406,7 +421,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     // prologue (slice -1 in buffer 0, slice 0 in buffer 1): the carry of the first step, and the own rows of slice 0 in registers
     mbar_wait(&fullI[0], 0);
     mbar_wait(&fullG[0], 0);
-    split_load<3>(A, Sown, os, ob, cs, S + g_bt, XB);
+    split_load<3, LT>(A, Sown, os, ob, cs, S + g_bt, XB);
     split_half<3, false>(A, d, ed, c1);
     __syncwarp();
     if (lane == 0) { mbar_arrive(&freeI[0]); mbar_arrive(&freeG[0]); }
@@ -428,7 +443,7 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
         for (int c = 0; c < 3; c++) { up[c] = c1[c]; lb[c] = c1[c]; la[c] = czero<2>(); }    // the -t hop (S = -1): up += r, out_{2+s} += d r (lb holds d times its value)
         if (more) {
             // A still holds the own rows of this slice (loaded as the +t neighbour of the step before): the -t hop of the next slice
-            load_link_s<3>(G + g_bt, XB, A.u);
+            load_link_s<LT>(G + g_bt, XB, A.u);
             split_half<3, false>(A, d, ed, c1);
         }
         // y hops
@@ -536,13 +551,60 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
 
 }  // namespace
 
+namespace {
+// one thread per float of the packed backward-link array (layout: fine_sweep.cuh)
+__global__ void pack_back_kernel(FieldGeom g, const float *__restrict__ src, float *__restrict__ dst, long long total) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    const int k = (int)(idx & 3);
+    long long q = idx >> 2;
+    const int xin = (int)(q % g.XB); q /= g.XB;
+    const int j = (int)(q % kBackF4);
+    long long b = q / kBackF4;
+    const int xb = (int)(b % g.nxb); b /= g.nxb;
+    const int y = (int)(b % g.Y); b /= g.Y;
+    const int z = (int)(b % g.Z);
+    const int t = (int)(b / g.Z);
+    const int xe = xb * g.XB + xin;
+    auto lex = [&](int x, int yy, int zz, int tt) { return x + (long long)g.X * (yy + (long long)g.Y * (zz + (long long)g.Z * tt)); };
+    float v = 0.f;
+    if (j < kBackT) {
+        const int f = 4 * j + k;                       // floats 0..53: U_mu(x - mu), mu = 0, 1, 2
+        if (f < 54) {
+            const int mu = f / 18, e = f % 18;
+            int c[4] = {x_of(g, xe, y, z, t), y, z, t};
+            const int ext[4] = {g.X, g.Y, g.Z, g.T};
+            c[mu] = c[mu] == 0 ? ext[mu] - 1 : c[mu] - 1;
+            v = src[lex(c[0], c[1], c[2], c[3]) * 72 + 18 * mu + e];
+        }
+    } else {
+        const int f = 4 * (j - kBackT) + k;            // floats 56..73: U_t of the other parity's site with the same index
+        if (f < 18) {
+            FieldGeom o = g;
+            o.parity = 1 - g.parity;
+            v = src[lex(x_of(o, xe, y, z, t), y, z, t) * 72 + 54 + f];
+        }
+    }
+    dst[idx] = v;
+}
+
+}  // namespace
+
+mrhs_status_t pack_back_links(const FieldGeom &g, const float *d_gauge_canonical, float4 *d_dst, cudaStream_t st) {
+    if (!g.cb) { set_error("pack_back_links: checkerboarded geometry expected"); return MRHS_ERR_INVALID_ARG; }
+    const long long total = g.nblocks() * kBackF4 * g.XB * 4;
+    pack_back_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(g, d_gauge_canonical, (float *)d_dst, total);
+    MRHS_CUDA(cudaGetLastError());
+    return MRHS_OK;
+}
+
 // ------------------------------------------------------------------ host side
 bool sweep_supported(const FieldGeom &g) {
     if (g.N & 1) return false;                       // RHS pairs in FFMA2 lanes; bulk copies need 16-byte pieces
     if (g.Y < 2 || g.Z < 2 || (g.Y % BY) || (g.Z % BZ)) return false;
     const int np = threads_per_site(g.N);
     if (g.XB * np > 48) return false;                // three consumer warps per tile row, twelve per block, plus the producer warps
-    const SweepSmem L(g.XB, np, true);
+    const SweepSmem L(g.XB, np, true, g.cb != 0);
     return L.total <= 227u * 1024u;
 }
 
@@ -603,7 +665,7 @@ bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t
     ok &= make_fastdiv(p.ntseg, grid, p.d_ntseg);
     ok &= make_fastdiv(nty / t.cy, grid, p.d_ncy);
     if (!ok) return false;
-    p.gauge_out = p.gauge_in = nullptr;
+    p.gauge_out = p.gauge_in = p.gauge_back = nullptr;
     p.clover = nullptr;
     p.aux = nullptr;
     p.dagger = 0;
@@ -611,8 +673,8 @@ bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t
     const int wpr = (g.XB * np + 15) / 16;
     p.threads = (unsigned)(ROWS * wpr + kSweepProducerWarps) * 32u;
     p.grid = (unsigned)grid;
-    p.smem_bytes = SweepSmem(g.XB, np, false).total;
-    p.smem_bytes_clover = SweepSmem(g.XB, np, true).total;
+    p.smem_bytes = SweepSmem(g.XB, np, false, g.cb != 0).total;
+    p.smem_bytes_clover = SweepSmem(g.XB, np, true, g.cb != 0).total;
     return true;
 }
 

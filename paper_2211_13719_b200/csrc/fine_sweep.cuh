@@ -18,6 +18,15 @@ constexpr int kSweepProducerWarps = 4;                          // tile rows, ha
 constexpr int kSweepConsumerRegs = 152, kSweepProducerRegs = 40;
 constexpr int kSweepMaxThreads = (kSweepRows * 3 + 4) * 32;   // three consumer warps per tile row, the producer warps, rounded to four warps per SM sub-partition (128 registers)
 
+// Packed backward links of a checkerboarded field (the sweep kernel's second link stream): per site of parity p, in that field's
+// block order, [block][kBackF4][xin] float4 =
+//   floats 0..53   U_mu(x - mu), mu = x, y, z, each at the position it has in the own-link site data (18 floats per link)
+//   floats 56..73  U_t of the site of the OTHER parity with the same checkerboarded index (x-block, xin, y, z, t): the link of the
+//                  hop from that site into the slice after it (the kernel carries that hop from step to step)
+// so that one contiguous bulk copy per tile row brings every backward link of the step; floats 54, 55, 74, 75 are padding.
+constexpr int kBackF4 = 19, kBackT = 14;
+mrhs_status_t pack_back_links(const FieldGeom &g, const float *d_gauge_canonical, float4 *d_dst, cudaStream_t st);
+
 struct SweepTiling {
     int lt;          // t-slices one thread block sweeps (divides T)
     int cy, cz;      // tiles per concurrently scheduled chunk in y and z
@@ -32,7 +41,8 @@ struct SweepParams {
     int cy, cz;
     FastDiv d_nxb, d_cy, d_cz, d_ntseg, d_ncy;   // block index -> (x-block, tile in chunk, segment, chunk)
     const float4 *gauge_out;      // links on the sites of the output field, [block][18][xin] float4
-    const float4 *gauge_in;       // links on the sites of the input field
+    const float4 *gauge_in;       // links on the sites of the input field (full lattice: the same array)
+    const float4 *gauge_back;     // checkerboarded: the packed backward links of the output sites (pack_back_links)
     const float4 *clover;         // packed clover blocks on the sites of the output field: non-null => out = C H (checkerboarded) or C in - H/2 (full lattice)
     const float4 *aux;            // with clover on checkerboarded fields: non-null => out = C aux - H/4 (Schur complement, second launch)
     int dagger;                   // 1: the adjoint hopping term (gamma_5 D_hop gamma_5)

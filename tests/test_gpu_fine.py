@@ -323,6 +323,60 @@ def test_inner_products_match_oracle(dims, ncomp, nrhs, parity):
     assert np.max(np.abs(nrm.imag)) == 0.0 and np.all(nrm.real > 0)
 
 
+def test_inner_products_leave_the_default_mempool_alone():
+    """The per-call scratch comes from a pool of the library's own: the release threshold of the device's default
+    stream-ordered pool (a process-wide setting that belongs to the caller) is what it was before the call."""
+    import ctypes
+    rt = ctypes.CDLL("libcudart.so.12")
+    pool, thr0, thr1 = ctypes.c_void_p(), ctypes.c_uint64(), ctypes.c_uint64()
+    torch.zeros(1).cuda()
+    assert rt.cudaDeviceGetDefaultMemPool(ctypes.byref(pool), 0) == 0
+    kReleaseThreshold = 4     # cudaMemPoolAttrReleaseThreshold
+    assert rt.cudaMemPoolGetAttribute(pool, kReleaseThreshold, ctypes.byref(thr0)) == 0
+    dims, nrhs = [4, 4, 4, 4], 4
+    x = (np.random.default_rng(5).standard_normal((256, 4, 3, nrhs)) + 0j).astype(np.complex64)
+    dx = mrhs.field_import(dims, 12, nrhs, mrhs.FULL, dev(x))
+    for _ in range(3):
+        mrhs.inner_products(dims, 12, nrhs, mrhs.FULL, dx, dx)
+    torch.cuda.synchronize()
+    assert rt.cudaMemPoolGetAttribute(pool, kReleaseThreshold, ctypes.byref(thr1)) == 0
+    assert thr1.value == thr0.value, (thr0.value, thr1.value)
+
+
+def test_site_data_copies_are_made_on_first_use_in_any_order():
+    """A handle packs gauge and clover per layout on first use (checkerboarded links, backward links of the sweep kernel, clover
+    and inverse clover per parity): a fresh handle whose FIRST call is the last operator of the list matches the oracle."""
+    dims, nrhs = [16, 4, 4, 4], 12
+    U = syn.gauge_np(dims, 81)
+    psi = syn.spinor_np(syn.volume(dims), nrhs, 81)
+    C, _ = oracle.clover_blocks(dims, U, -0.05, 1.5)
+    Ci = oracle.clover_inverse(C)
+    src = oracle.cb_split(dims, psi)
+    Cp, Cip = oracle.cb_split(dims, C), oracle.cb_split(dims, Ci)
+    for kern in (mrhs.HOP_GATHER, mrhs.HOP_SWEEP):
+        w = make_wilson(dims, nrhs, -0.05, 1.5, U)
+        mrhs.wilson_set_hop_kernel(w.h, 1, kern)
+        # first call: the fused inverse launch (needs checkerboarded links + inverse blocks of one parity)
+        d_in = w.import_field(dev(src[0]), mrhs.EVEN)
+        d_out = w.empty(mrhs.ODD)
+        d_out.fill_(float("nan"))
+        torch.cuda.synchronize()
+        w.meooe_mooee_inv(d_in, d_out, mrhs.ODD)
+        torch.cuda.synchronize()
+        want = oracle.mooee(Cip[1], oracle.meooe(dims, U, src[0], 1))
+        assert rel_l2_per_rhs(host(w.export_field(d_out, mrhs.ODD)), want).max() < TOL, kern
+        # then the full-lattice inverse and a checkerboarded clover apply
+        d_f = w.import_field(dev(psi), mrhs.FULL)
+        d_o = w.empty(mrhs.FULL)
+        d_o.fill_(float("nan"))
+        torch.cuda.synchronize()
+        w.mooee_inv(d_f, d_o, mrhs.FULL)
+        torch.cuda.synchronize()
+        assert rel_l2_per_rhs(host(w.export_field(d_o, mrhs.FULL)), oracle.mooee(Ci, psi)).max() < TOL, kern
+        assert rel_l2_per_rhs(gpu_mooee(w, src[0], mrhs.EVEN), oracle.mooee(Cp[0], src[0])).max() < TOL, kern
+        w.close()
+
+
 @pytest.mark.parametrize("dims,nrhs,seed", [([8, 4, 4, 6], 12, 75), ([4, 4, 4, 4], 3, 76), ([16, 2, 4, 4], 24, 77), ([2, 2, 2, 2], 4, 78),
                                             ([16, 4, 4, 4], 12, 79), ([48, 2, 4, 2], 12, 80)])
 def test_full_wilson_clover_matrix(dims, nrhs, seed):
