@@ -191,8 +191,8 @@ mrhs_status_t wilson_set_default_tiling(mrhs_wilson *h) {
     if (sweep_supported(h->gfull) && sweep_supported(h->gcb[0])) {
         mrhs_status_t s = sweep_prepare();
         if (s != MRHS_OK) return s;
-        bool ok = build_sweep_params(h->gfull, 0, default_sweep_tiling(h->gfull, h->num_sms), h->sp_full);
-        for (int p = 0; p < 2; p++) ok = ok && build_sweep_params(h->gcb[p], p, default_sweep_tiling(h->gcb[p], h->num_sms), h->sp_cb[p]);
+        bool ok = build_sweep_params(h->gfull, 0, default_sweep_tiling(h->gfull, h->num_sms), h->num_sms, h->sp_full);
+        for (int p = 0; p < 2; p++) ok = ok && build_sweep_params(h->gcb[p], p, default_sweep_tiling(h->gcb[p], h->num_sms), h->num_sms, h->sp_cb[p]);
         if (ok) {
             h->sp_full.gauge_out = h->sp_full.gauge_in = h->gauge_full;
             for (int p = 0; p < 2; p++) { h->sp_cb[p].gauge_out = h->gauge_cb[p]; h->sp_cb[p].gauge_in = h->gauge_cb[1 - p]; h->sp_cb[p].gauge_back = h->gauge_back[p]; }
@@ -482,14 +482,14 @@ mrhs_status_t mrhs_wilson_set_sweep(mrhs_wilson_t *h, int which, int lt, const i
     SweepTiling t = {lt, chunk[0], chunk[1]};
     if (which == 0) {
         SweepParams p;
-        MRHS_REQUIRE(build_sweep_params(h->gfull, 0, t, p), "set sweep: segment / chunk does not fit the full lattice (or odd N_rhs)");
+        MRHS_REQUIRE(build_sweep_params(h->gfull, 0, t, h->num_sms, p), "set sweep: segment / chunk does not fit the full lattice (or odd N_rhs)");
         p.gauge_out = p.gauge_in = h->gauge_full;
         p.pf = h->sp_full.pf;
         h->sp_full = p;
     } else {
         SweepParams p[2];
         for (int q = 0; q < 2; q++) {
-            MRHS_REQUIRE(build_sweep_params(h->gcb[q], q, t, p[q]), "set sweep: segment / chunk does not fit the checkerboarded lattice (or odd N_rhs)");
+            MRHS_REQUIRE(build_sweep_params(h->gcb[q], q, t, h->num_sms, p[q]), "set sweep: segment / chunk does not fit the checkerboarded lattice (or odd N_rhs)");
             p[q].gauge_out = h->gauge_cb[q];
             p[q].gauge_in = h->gauge_cb[1 - q];
             p[q].gauge_back = h->gauge_back[q];

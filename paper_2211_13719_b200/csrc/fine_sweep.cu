@@ -29,6 +29,10 @@
 #include "async_copy.cuh"
 #include "hop_math.cuh"
 
+#include <algorithm>
+#include <queue>
+#include <vector>
+
 namespace mrhs {
 
 namespace {
@@ -198,16 +202,26 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     uint64_t *fullI = bars, *freeI = bars + 2, *fullG = bars + 4, *freeG = bars + 6, *fullH = bars + 8, *freeH = bars + 10;
 
     const int tid = threadIdx.x, wid = tid >> 5, lane = tid & 31;
-    const int Y = p.Y, Z = p.Z, T = p.T, nxb = p.nxb, lt = p.lt;
+    const int Y = p.Y, Z = p.Z, T = p.T, nxb = p.nxb;
 
-    // block -> (x-block, tile, t-segment): x-blocks fastest, then the tiles of a chunk, then segments, then chunks
+    // block -> (x-block, tile, t-segment): x-blocks fastest, then the tiles of a chunk, then segments, then chunks.  The last
+    // p.tail_tiles tiles of that order are cut into p.tail_seg segments each (blocks n_whole, n_whole + 1, ...: the segments of a
+    // tile follow one another), so that the blocks of the last, partly filled wave are short ones (build_sweep_params)
+    uint32_t bi = blockIdx.x, tseg = 0;
+    int lt = p.lt;
+    if (bi >= p.n_whole) {
+        const uint32_t j = bi - p.n_whole, q = j / (uint32_t)p.tail_seg;
+        tseg = j - q * (uint32_t)p.tail_seg;
+        bi = p.n_whole + q;
+        lt = p.T / p.tail_seg;
+    }
     uint32_t xb, yc, zc, seg, chy, chz, q0;
-    p.d_nxb.divmod(blockIdx.x, q0, xb);
+    p.d_nxb.divmod(bi, q0, xb);
     p.d_cy.divmod(q0, q0, yc);
     p.d_cz.divmod(q0, q0, zc);
     p.d_ntseg.divmod(q0, q0, seg);
     p.d_ncy.divmod(q0, chz, chy);
-    const int y0 = (int)(chy * p.cy + yc) * BY, z0 = (int)(chz * p.cz + zc) * BZ, t0 = (int)seg * lt;
+    const int y0 = (int)(chy * p.cy + yc) * BY, z0 = (int)(chz * p.cz + zc) * BZ, t0 = (int)(seg + tseg) * lt;
 
     if (tid == 0) {
         for (int i = 0; i < 2; i++) {
@@ -645,14 +659,52 @@ SweepTiling default_sweep_tiling(const FieldGeom &g, int num_sms) {
     return t;
 }
 
-bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t, SweepParams &p) {
+namespace {
+// Time at which the last of `workers` SMs finishes when each takes the next block of the list as soon as it is free: n_whole
+// blocks of cost c_whole, then n_short of cost c_short (costs in slice steps).
+double sweep_makespan(long long n_whole, double c_whole, long long n_short, double c_short, int workers) {
+    // after the whole blocks: n_whole % workers SMs have done one more than the others
+    std::priority_queue<double, std::vector<double>, std::greater<double>> free_at;
+    const long long q = n_whole / workers, r = n_whole % workers;
+    for (int i = 0; i < workers; i++) free_at.push((q + (i < r ? 1 : 0)) * c_whole);
+    double end = (q + (r ? 1 : 0)) * c_whole;
+    for (long long i = 0; i < n_short; i++) {
+        const double t = free_at.top() + c_short;
+        free_at.pop();
+        free_at.push(t);
+        if (t > end) end = t;
+    }
+    return end;
+}
+}  // namespace
+
+bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t, int num_sms, SweepParams &p) {
     if (!sweep_supported(g)) return false;
     if (t.lt < 1 || g.T % t.lt || t.cy < 1 || t.cz < 1) return false;
     const int nty = g.Y / BY, ntz = g.Z / BZ;
     if (nty % t.cy || ntz % t.cz) return false;
     const int np = threads_per_site(g.N);
-    const long long grid = (long long)g.nxb * nty * ntz * (g.T / t.lt);
+    long long grid = (long long)g.nxb * nty * ntz * (g.T / t.lt);
     if (grid >= (1ll << 31)) return false;
+    // Whole-line sweeps: the grid is rarely a multiple of the SM count, and a last wave of a few whole-line blocks keeps most SMs
+    // idle for a full sweep (48^4, N = 12: 3456 tiles on 148 SMs = 23.35 waves).  Cut the last tail_tiles tiles into tail_seg
+    // segments each; every segment costs about three extra slice steps (two extra slices, pipeline fill).  Pick the pair with
+    // the shortest simulated schedule.
+    p.n_whole = (unsigned)grid; p.tail_tiles = 0; p.tail_seg = 1;
+    if (t.lt == g.T && num_sms > 0 && grid > num_sms) {
+        const double extra = 3.0;
+        double best = sweep_makespan(grid, g.T + extra, 0, 0.0, num_sms) * 0.995;     // a split has to win by more than the model's noise
+        const long long max_tail = std::min<long long>(grid, 3ll * num_sms), step = std::max(1, num_sms / 37);
+        for (int ts = 2; ts <= 8; ts++) {
+            if (g.T % ts || g.T / ts < 6) continue;
+            for (long long tt = step; tt <= max_tail; tt += step) {
+                const double m = sweep_makespan(grid - tt, g.T + extra, tt * ts, g.T / ts + extra, num_sms);
+                if (m < best) { best = m; p.tail_tiles = (int)tt; p.tail_seg = ts; }
+            }
+        }
+        p.n_whole = (unsigned)(grid - p.tail_tiles);
+        grid = (long long)p.n_whole + (long long)p.tail_tiles * p.tail_seg;
+    }
     p.Y = g.Y; p.Z = g.Z; p.T = g.T;
     p.XB = g.XB; p.nxb = g.nxb; p.NP = np;
     p.cb = g.cb; p.out_parity = out_parity;

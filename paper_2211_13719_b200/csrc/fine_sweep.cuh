@@ -37,6 +37,8 @@ struct SweepParams {
     int XB, nxb, NP;              // layout block, blocks per x-line, threads per site (= RHS pairs)
     int cb, out_parity;
     int lt, ntseg;                // slices per segment, segments per t-line
+    unsigned n_whole;             // blocks before the tail: the last tail_tiles tiles are cut into tail_seg segments each (whole-line sweeps only)
+    int tail_tiles, tail_seg;
     int pf;                       // L2 prefetch distance of the producer, in slices (0 = off)
     int cy, cz;
     FastDiv d_nxb, d_cy, d_cz, d_ntseg, d_ncy;   // block index -> (x-block, tile in chunk, segment, chunk)
@@ -53,7 +55,8 @@ struct SweepParams {
 // true if the sweep kernel can run this geometry (even N_rhs, shared memory fits)
 bool sweep_supported(const FieldGeom &g);
 SweepTiling default_sweep_tiling(const FieldGeom &g, int num_sms);
-bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t, SweepParams &p);
+// num_sms: thread blocks resident at the same time (one per SM); 0 = do not balance the last wave
+bool build_sweep_params(const FieldGeom &g, int out_parity, const SweepTiling &t, int num_sms, SweepParams &p);
 mrhs_status_t sweep_prepare();    // opt in to large dynamic shared memory for every instantiation
 mrhs_status_t launch_sweep(const SweepParams &p, const void *d_in, void *d_out, cudaStream_t st);
 
