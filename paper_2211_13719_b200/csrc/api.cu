@@ -196,7 +196,7 @@ mrhs_status_t wilson_set_default_tiling(mrhs_wilson *h) {
         if (ok) {
             h->sp_full.gauge_out = h->sp_full.gauge_in = h->gauge_full;
             for (int p = 0; p < 2; p++) { h->sp_cb[p].gauge_out = h->gauge_cb[p]; h->sp_cb[p].gauge_in = h->gauge_cb[1 - p]; h->sp_cb[p].gauge_back = h->gauge_back[p]; }
-            // measured cross-over (profiles/r1d_kernel_choice.md): the sweep kernel wins from N_rhs = 12 on lattices of 32^4
+            // measured cross-over (round 1): the sweep kernel wins from N_rhs = 12 on lattices of 32^4
             // sites and more; below that the gather kernel's many small blocks hide latency better
             if (h->nrhs >= 12 && h->gfull.nsites >= (1ll << 20)) h->kern[0] = h->kern[1] = MRHS_HOP_SWEEP;
         }

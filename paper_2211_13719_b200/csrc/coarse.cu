@@ -28,10 +28,11 @@ constexpr int largest_ks(int nb, int groups) {
 }
 
 // Register tile of (rows, RHS lanes) per thread, chosen from measurements at nbasis 24 / 40: up to
-// N_rhs = 24 the small 2 x 1 tile with many column slices keeps more warps busy per site (few lanes to spread over
-// threads); from N_rhs = 32 the 4-row tile with 2 or 3 lanes (per column 2 + TP shared-memory loads of 16 bytes feed
+// N_rhs = 16 the small 2 x 1 tile with many column slices keeps more warps busy per site (few lanes to spread over
+// threads; 4 x 1, 2 x 2, 4 x 2, 2 x 3, 4 x 3 and 8-row tiles all measured slower there); at N_rhs = 24 a 4 x 1 tile (10 % faster
+// at nbasis 24 and 40); from N_rhs = 32 the 4-row tile with 2 or 3 lanes (per column 2 + TP shared-memory loads of 16 bytes feed
 // 16 TP FFMA2) relieves the shared-memory pipe, as long as the block keeps at least six warps.
-constexpr int pick_ti(int nb, int np, int r) { return np * r >= 32 || nb * np / 2 > 256 ? 4 : 2; }
+constexpr int pick_ti(int nb, int np, int r) { return np * r >= 24 || nb * np / 2 > 256 ? 4 : 2; }
 constexpr int pick_tp(int nb, int np, int r) {
     if (np * r < 32) return (nb * np / 2 > 256 && np % 2 == 0) ? 2 : 1;
     return (np % 3 == 0 && nb / 4 * (np / 3) >= 192) ? 3 : 2;

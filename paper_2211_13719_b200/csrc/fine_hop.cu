@@ -212,7 +212,7 @@ HopTiling default_tiling(const FieldGeom &g, size_t l2_budget) {
     const int per_row = g.XB * np;
     // Small thread blocks (about three warps, several resident per SM) measured faster than one large
     // block per SM at 48^4: their load and arithmetic phases drift apart instead of all warps of an
-    // SM waiting on the same neighbour rows at once (profiles/r1b_tiling.md).
+    // SM waiting on the same neighbour rows at once (measured in round 1).
     int rows_max = kHopTargetThreads / per_row;
     if (rows_max < 1) rows_max = 1;
     HopTiling best = {1, 1, 1, 1, 1};
