@@ -2,6 +2,7 @@
 // right-hand sides at once (reading S9).  First correct version:
 // FP32 FMA (FFMA2 over RHS pairs), operands through L1/L2; fields in the library's native layouts.
 #include "transfer.cuh"
+#include "async_copy.cuh"
 
 namespace mrhs {
 
@@ -255,6 +256,221 @@ restrict_kernel(TransferGeom g, int NP, int PC, int S, const float4 *__restrict_
 }
 
 
+// Restriction with both operands staged in shared memory (even N_rhs, block extent in x dividing the layout block XB).
+// A thread block owns the XB / bx aggregates that share an x-block and walks their by x bz x bt rows; a row is ONE contiguous run in
+// the field (the layout block row: 12 components x XB sites x NP lanes) and ONE in the basis (XB sites x n_vec x 96 bytes), brought
+// in by two bulk async copies per row into a ring of stages (a producer warp, mbarriers), so each SM has tens of KB of both streams
+// in flight.  A consumer warp is one slice of the sites (position of the site inside its aggregate's x-run, row index modulo RS);
+// its lanes are the (aggregate, chirality, group of KT basis vectors, group of LT lanes) tiles, each summing KT x LT coefficients in
+// registers: per site and tile 3 KT + 6 LT shared-memory loads of 16 bytes feed 24 KT LT FFMA2.  Slices are added through shared
+// memory in a fixed order (bit-reproducible).
+constexpr int kRestrictStages = 4;
+template <int KT, int LT>
+__global__ void __launch_bounds__(288, 2)
+restrict_staged_kernel(TransferGeom g, int NP, int RS, const float4 *__restrict__ basis, const float4 *__restrict__ fine, float4 *__restrict__ coarse) {
+    extern __shared__ __align__(128) unsigned char sm[];
+    const int XB = g.XB, CS = XB * NP;
+    const uint32_t f_bytes = 12u * CS * 16u, b_bytes = (uint32_t)XB * g.nvec * 96u, st_bytes = f_bytes + b_bytes;
+    uint64_t *full = reinterpret_cast<uint64_t *>(sm + (size_t)kRestrictStages * st_bytes), *empty = full + kRestrictStages;
+    const int agx = XB / g.bx;                                  // aggregates per block
+    const int kgs = g.nvec / KT, lgs = NP / LT, tiles = agx * 2 * kgs * lgs;   // tiles = lanes with work in a consumer warp (<= 32)
+    const int S = g.bx * RS, NR = g.by * g.bz * g.bt;           // site slices = consumer warps; rows
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // block -> (x-block, coarse y, z, t)
+    long long q = blockIdx.x;
+    const int xb = (int)(q % g.nxb); q /= g.nxb;
+    const int cy = (int)(q % g.cY); q /= g.cY;
+    const int cz = (int)(q % g.cZ);
+    const int ct = (int)(q / g.cZ);
+    if (tid == 0) {
+        for (int i = 0; i < kRestrictStages; i++) { mbar_init(&full[i], 1); mbar_init(&empty[i], S); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (warp == S) {
+        // ------------------------------------------------ producer
+        if (lane == 0) {
+            for (int r = 0; r < NR; r++) {
+                const int st = r % kRestrictStages;
+                if (r >= kRestrictStages) mbar_wait(&empty[st], ((r / kRestrictStages) - 1) & 1);
+                int w = r;
+                const int iy = w % g.by; w /= g.by;
+                const int iz = w % g.bz;
+                const int it = w / g.bz;
+                const long long yzt = (cy * g.by + iy) + (long long)g.Y * ((cz * g.bz + iz) + (long long)g.Z * (ct * g.bt + it));
+                unsigned char *dst = sm + (size_t)st * st_bytes;
+                mbar_expect_tx(&full[st], st_bytes);
+                bulk_g2s(dst, fine + ((size_t)xb + (size_t)g.nxb * yzt) * 12 * CS, f_bytes, &full[st]);
+                bulk_g2s(dst + f_bytes, basis + ((size_t)xb * XB + (size_t)g.X * yzt) * g.nvec * 6, b_bytes, &full[st]);
+            }
+        }
+    } else if (warp < S) {
+        // ------------------------------------------------ consumers
+        const int xs = warp % g.bx, rp = warp / g.bx;          // position in the aggregate's x-run, row class
+        // lane -> tile; the aggregate and the chirality are the high bits so that the eight lanes of a quarter-warp share them
+        // (their field rows are a multiple of 128 bytes apart: the same banks)
+        const bool has = lane < tiles;
+        const int tl = has ? lane : 0;
+        const int a = tl / (2 * kgs * lgs), chi = (tl / (kgs * lgs)) & 1, kg = (tl / lgs) % kgs, lg = tl % lgs;
+        const int xin = a * g.bx + xs;
+        CVec<2> acc[KT][LT];
+#pragma unroll
+        for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+            for (int l = 0; l < LT; l++) acc[kk][l] = czero_t<2>();
+        for (int r = 0; r < NR; r++) {
+            const int st = r % kRestrictStages;
+            // every warp waits for every row, also the rows of other row classes: a warp that ran ahead would arrive twice in one
+            // phase of the stage's empty barrier
+            mbar_wait(&full[st], (r / kRestrictStages) & 1);
+            if (r % RS == rp) {
+                const float4 *sf = reinterpret_cast<const float4 *>(sm + (size_t)st * st_bytes) + ((size_t)(chi * 6) * XB + xin) * NP + lg * LT;
+                const float4 *sb = reinterpret_cast<const float4 *>(sm + (size_t)st * st_bytes + f_bytes) + ((size_t)xin * g.nvec + kg * KT) * 6 + chi * 3;
+#pragma unroll
+                for (int j = 0; j < 3; j++) {
+                    CVec<2> f0[LT], f1[LT];
+#pragma unroll
+                    for (int l = 0; l < LT; l++) {
+                        f0[l] = to_cvec(sf[(size_t)(2 * j) * CS + l]);
+                        f1[l] = to_cvec(sf[(size_t)(2 * j + 1) * CS + l]);
+                    }
+#pragma unroll
+                    for (int kk = 0; kk < KT; kk++) {
+                        const float4 p = sb[kk * 6 + j];           // components 2j, 2j+1 of this chirality
+#pragma unroll
+                        for (int l = 0; l < LT; l++) {
+                            acc[kk][l] = cfma_conj(p.x, p.y, f0[l], acc[kk][l]);
+                            acc[kk][l] = cfma_conj(p.z, p.w, f1[l], acc[kk][l]);
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]);
+        }
+        // every row has been consumed by every warp (the arrivals above): the ring is free for the slice sums
+        // [slice][tile][KT LT] float4
+        float4 *red = reinterpret_cast<float4 *>(sm);
+        asm volatile("bar.sync 1, %0;" ::"r"(S * 32) : "memory");
+        if (has && warp > 0) {
+            float4 *rp4 = red + ((size_t)(warp - 1) * tiles + tl) * KT * LT;
+#pragma unroll
+            for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+                for (int l = 0; l < LT; l++) rp4[kk * LT + l] = from_cvec(acc[kk][l]);
+        }
+        asm volatile("bar.sync 1, %0;" ::"r"(S * 32) : "memory");
+        if (has && warp == 0) {
+            for (int w = 1; w < S; w++) {
+                const float4 *rp4 = red + ((size_t)(w - 1) * tiles + tl) * KT * LT;
+#pragma unroll
+                for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+                    for (int l = 0; l < LT; l++) acc[kk][l] = cadd(acc[kk][l], to_cvec(rp4[kk * LT + l]));
+            }
+            const long long B = (xb * agx + a) + (long long)g.cX * (cy + (long long)g.cY * (cz + (long long)g.cZ * ct));
+            float4 *po = coarse + ((size_t)B * 2 * g.nvec + (size_t)chi * g.nvec + kg * KT) * NP + lg * LT;
+#pragma unroll
+            for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+                for (int l = 0; l < LT; l++) po[(size_t)kk * NP + l] = from_cvec(acc[kk][l]);
+        }
+    }
+}
+
+
+// Prolongation with the basis streamed through a ring of shared-memory stages (even N_rhs, block extent in x dividing XB): the same
+// block / row decomposition as restrict_staged_kernel.  The 2 n_vec coefficient vectors of the block's XB / bx aggregates are staged
+// once; a basis row (XB sites x n_vec x 96 bytes, contiguous) arrives by one bulk async copy per row.  A consumer warp takes every
+// NW-th row; its lanes are the (site of the row, chirality, group of LT lanes) tiles, each producing the six components of its
+// chirality for LT lanes: per basis vector 3 + LT shared-memory loads of 16 bytes feed 24 LT FFMA2.
+template <int LT>
+__global__ void __launch_bounds__(160, 3)
+prolong_staged_kernel(TransferGeom g, int NP, int NW, const float4 *__restrict__ basis, const float4 *__restrict__ coarse, float4 *__restrict__ fine) {
+    extern __shared__ __align__(128) unsigned char sm[];
+    const int XB = g.XB, CS = XB * NP;
+    const uint32_t b_bytes = (uint32_t)XB * g.nvec * 96u;
+    const int agx = XB / g.bx, lgs = NP / LT, tiles = XB * 2 * lgs, NR = g.by * g.bz * g.bt;
+    const uint32_t c_bytes = (uint32_t)agx * 2u * g.nvec * NP * 16u;
+    float4 *sc = reinterpret_cast<float4 *>(sm + (size_t)kRestrictStages * b_bytes);                    // [aggregate][2 n_vec][NP]
+    uint64_t *full = reinterpret_cast<uint64_t *>(sm + (size_t)kRestrictStages * b_bytes + c_bytes), *empty = full + kRestrictStages, *cfull = empty + kRestrictStages;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    long long q = blockIdx.x;
+    const int xb = (int)(q % g.nxb); q /= g.nxb;
+    const int cy = (int)(q % g.cY); q /= g.cY;
+    const int cz = (int)(q % g.cZ);
+    const int ct = (int)(q / g.cZ);
+    if (tid == 0) {
+        for (int i = 0; i < kRestrictStages; i++) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
+        mbar_init(cfull, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto row_yzt = [&](int r) {
+        const int iy = r % g.by; r /= g.by;
+        const int iz = r % g.bz;
+        const int it = r / g.bz;
+        return (long long)(cy * g.by + iy) + (long long)g.Y * ((cz * g.bz + iz) + (long long)g.Z * (ct * g.bt + it));
+    };
+    if (warp == NW) {
+        // ------------------------------------------------ producer
+        if (lane == 0) {
+            mbar_expect_tx(cfull, c_bytes);
+            for (int a = 0; a < agx; a++) {
+                const long long B = (xb * agx + a) + (long long)g.cX * (cy + (long long)g.cY * (cz + (long long)g.cZ * ct));
+                bulk_g2s(sc + (size_t)a * 2 * g.nvec * NP, coarse + (size_t)B * 2 * g.nvec * NP, c_bytes / agx, cfull);
+            }
+            for (int r = 0; r < NR; r++) {
+                const int st = r % kRestrictStages;
+                if (r >= kRestrictStages) mbar_wait(&empty[st], ((r / kRestrictStages) - 1) & 1);
+                mbar_expect_tx(&full[st], b_bytes);
+                bulk_g2s(sm + (size_t)st * b_bytes, basis + ((size_t)xb * XB + (size_t)g.X * row_yzt(r)) * g.nvec * 6, b_bytes, &full[st]);
+            }
+        }
+    } else if (warp < NW) {
+        // ------------------------------------------------ consumers: warp w takes rows w, w + NW, ...; each row is read by one warp only
+        const bool has = lane < tiles;
+        const int tl = has ? lane : 0;
+        const int chi = tl / (XB * lgs), xin = (tl / lgs) % XB, lg = tl % lgs;
+        const float4 *vc = sc + ((size_t)(xin / g.bx) * 2 * g.nvec + (size_t)chi * g.nvec) * NP + lg * LT;
+        mbar_wait(cfull, 0);
+        for (int r = warp; r < NR; r += NW) {
+            const int st = r % kRestrictStages;
+            mbar_wait(&full[st], (r / kRestrictStages) & 1);
+            const float4 *sb = reinterpret_cast<const float4 *>(sm + (size_t)st * b_bytes) + (size_t)xin * g.nvec * 6 + chi * 3;
+            CVec<2> acc[6][LT];
+#pragma unroll
+            for (int c = 0; c < 6; c++)
+#pragma unroll
+                for (int l = 0; l < LT; l++) acc[c][l] = czero_t<2>();
+#pragma unroll 4
+            for (int k = 0; k < g.nvec; k++) {
+                CVec<2> v[LT];
+#pragma unroll
+                for (int l = 0; l < LT; l++) v[l] = to_cvec(vc[(size_t)k * NP + l]);
+#pragma unroll
+                for (int j = 0; j < 3; j++) {
+                    const float4 p = sb[k * 6 + j];
+#pragma unroll
+                    for (int l = 0; l < LT; l++) {
+                        acc[2 * j][l] = cfma(p.x, p.y, v[l], acc[2 * j][l]);
+                        acc[2 * j + 1][l] = cfma(p.z, p.w, v[l], acc[2 * j + 1][l]);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]);
+            if (has) {
+                float4 *po = fine + ((size_t)xb + (size_t)g.nxb * row_yzt(r)) * 12 * CS + ((size_t)(chi * 6) * XB + xin) * NP + lg * LT;
+#pragma unroll
+                for (int c = 0; c < 6; c++)
+#pragma unroll
+                    for (int l = 0; l < LT; l++) __stcs(po + (size_t)c * CS + l, from_cvec(acc[c][l]));
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------ coarse -> coarser
 __global__ void pack_basis_coarse_kernel(int nvec, int nf, long long V, const float2 *__restrict__ src, float2 *__restrict__ dst, long long total) {
     long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // native order [x][k][c]
@@ -386,8 +602,34 @@ mrhs_status_t pack_basis(const TransferGeom &g, const float2 *d_canonical, float
     return MRHS_OK;
 }
 
+namespace {
+template <int LT>
+bool try_prolong_staged(const TransferGeom &g, int np, const float2 *d_basis, const void *d_coarse, void *d_fine, cudaStream_t st, mrhs_status_t *status) {
+    if ((g.N & 1) || g.XB % g.bx || np % LT) return false;
+    const int tiles = g.XB * 2 * (np / LT);
+    if (tiles > 32 || tiles < 16) return false;
+    const int agx = g.XB / g.bx, NR = g.by * g.bz * g.bt;
+    const int NW = NR < 4 ? NR : 4;      // four consumer warps + the producer: three blocks per SM at 136 registers
+    const size_t smem = (size_t)kRestrictStages * g.XB * g.nvec * 96 + (size_t)agx * 2 * g.nvec * np * 16 + (2 * kRestrictStages + 1) * 8;
+    if (smem > 72 * 1024) return false;
+    *status = MRHS_OK;
+    cudaError_t e = cudaFuncSetAttribute(prolong_staged_kernel<LT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 72 * 1024);
+    if (e != cudaSuccess) { *status = cuda_fail(e, "cudaFuncSetAttribute", __FILE__, __LINE__); return true; }
+    const long long grid = (long long)g.nxb * g.cY * g.cZ * g.cT;
+    prolong_staged_kernel<LT><<<(unsigned)grid, (NW + 1) * 32, smem, st>>>(g, np, NW, (const float4 *)d_basis, (const float4 *)d_coarse, (float4 *)d_fine);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) *status = cuda_fail(e, "prolong_staged_kernel", __FILE__, __LINE__);
+    return true;
+}
+}  // namespace
+
 mrhs_status_t launch_prolong(const TransferGeom &g, const float2 *d_basis, const void *d_coarse, void *d_fine, cudaStream_t st) {
     const int np = threads_per_site(g.N);
+    {
+        mrhs_status_t status = MRHS_OK;
+        if (try_prolong_staged<3>(g, np, d_basis, d_coarse, d_fine, st, &status)) return status;
+        if (try_prolong_staged<2>(g, np, d_basis, d_coarse, d_fine, st, &status)) return status;
+    }
     const long long nthreads = g.nsites * np;
     // shared-memory staging when at least two blocks fit an SM; the plain kernel otherwise
     const int cs = g.XB * np;
@@ -414,9 +656,43 @@ mrhs_status_t launch_prolong(const TransferGeom &g, const float2 *d_basis, const
     return MRHS_OK;
 }
 
+namespace {
+// the staged kernel where its tiling fits: even N_rhs, whole aggregate x-runs inside a layout block, at most 32 tiles per slice
+// and 8 slices, four stages + the slice sums in shared memory.  Returns false if it does not apply (nothing launched).
+template <int KT, int LT>
+bool try_restrict_staged(const TransferGeom &g, int np, const float2 *d_basis, const void *d_fine, void *d_coarse, cudaStream_t st, mrhs_status_t *status) {
+    if ((g.N & 1) || g.XB % g.bx || g.nvec % KT || np % LT) return false;
+    const int agx = g.XB / g.bx, tiles = agx * 2 * (g.nvec / KT) * (np / LT);
+    if (tiles > 32 || tiles < 16 || g.bx > 8) return false;
+    const int NR = g.by * g.bz * g.bt;
+    int RS = 8 / g.bx;
+    while (RS > 1 && NR % RS) RS--;
+    const int S = g.bx * RS;
+    const size_t st_bytes = (size_t)12 * g.XB * np * 16 + (size_t)g.XB * g.nvec * 96;
+    const size_t red = (size_t)(S - 1) * tiles * KT * LT * 16;
+    const size_t smem = kRestrictStages * st_bytes + 2 * kRestrictStages * 8;
+    if (smem > 110 * 1024 || red > kRestrictStages * st_bytes) return false;
+    *status = MRHS_OK;
+    cudaError_t e = cudaFuncSetAttribute(restrict_staged_kernel<KT, LT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);
+    if (e != cudaSuccess) { *status = cuda_fail(e, "cudaFuncSetAttribute", __FILE__, __LINE__); return true; }
+    const long long grid = (long long)g.nxb * g.cY * g.cZ * g.cT;
+    restrict_staged_kernel<KT, LT><<<(unsigned)grid, (S + 1) * 32, smem, st>>>(g, np, RS, (const float4 *)d_basis, (const float4 *)d_fine, (float4 *)d_coarse);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) *status = cuda_fail(e, "restrict_staged_kernel", __FILE__, __LINE__);
+    return true;
+}
+}  // namespace
+
 mrhs_status_t launch_restrict(const TransferGeom &g, const float2 *d_basis, const void *d_fine, void *d_coarse, cudaStream_t st) {
     const int np = threads_per_site(g.N);
     if (g.nvec > 256) { set_error("restrict: nvec = %d exceeds 256", g.nvec); return MRHS_ERR_UNSUPPORTED; }
+    {
+        mrhs_status_t status = MRHS_OK;
+        if (try_restrict_staged<5, 3>(g, np, d_basis, d_fine, d_coarse, st, &status)) return status;
+        if (try_restrict_staged<4, 3>(g, np, d_basis, d_fine, d_coarse, st, &status)) return status;
+        if (try_restrict_staged<4, 2>(g, np, d_basis, d_fine, d_coarse, st, &status)) return status;
+        if (try_restrict_staged<3, 3>(g, np, d_basis, d_fine, d_coarse, st, &status)) return status;
+    }
     const int kt = g.nvec % 4 == 0 ? 4 : (g.nvec % 2 == 0 ? 2 : 1);   // basis vectors per thread
     const int lt = np % 2 == 0 ? 2 : 1;                              // RHS lanes per thread
     const int groups = g.nvec / kt, lgroups = np / lt;

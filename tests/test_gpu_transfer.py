@@ -25,6 +25,9 @@ CASES = [
     ([8, 8, 8, 8], [4, 4, 4, 4], 20, 24),     # 4^4 aggregates as in the paper, nbasis 40
     ([12, 6, 4, 4], [2, 3, 2, 2], 5, 3),      # odd N_rhs, block extent 3
     ([8, 4, 4, 4], [2, 2, 2, 2], 20, 96),
+    ([16, 8, 4, 4], [4, 4, 2, 2], 20, 12),    # staged kernels: two aggregates per x-block, 5 x 3 tiles
+    ([16, 4, 6, 4], [8, 2, 3, 2], 12, 12),    # staged kernels: block extent 8 = the x-block, odd number of rows, 4 x 3 tiles
+    ([8, 4, 4, 4], [2, 2, 2, 2], 8, 8),       # staged kernels: four aggregates per x-block, 4 x 2 tiles
 ]
 
 
@@ -47,6 +50,8 @@ def test_prolong_restrict_match_oracle(dims, bdims, nvec, nrhs):
     # restriction
     d_f = mrhs.field_import(dims, 12, nrhs, mrhs.FULL, dev(f))
     d_c = mrhs.empty_field(cdims, nb, nrhs, mrhs.FULL)
+    d_c.fill_(float("nan"))
+    torch.cuda.synchronize()
     tr.restrict(d_f, d_c)
     torch.cuda.synchronize()
     got = host(mrhs.field_export(cdims, nb, nrhs, mrhs.FULL, d_c)).reshape(Vc, nb, nrhs)
