@@ -321,6 +321,17 @@ mrhs_status_t mrhs_inner_products(const int dims[4], int ncomp, int nrhs, int pa
 mrhs_status_t mrhs_wilson_apply_host(mrhs_wilson_t *h, int op, int parity,
                                      const void *h_in, void *h_out);
 mrhs_status_t mrhs_coarse_apply_host(mrhs_coarse_t *h, const void *h_in, void *h_out);
+/* The same without the final synchronise: the call returns once its copies and kernels are enqueued, and
+ * mrhs_*_host_wait blocks until every enqueued call of the handle has delivered its result.  h_in and h_out must stay
+ * valid (and should be pinned, else the copies serialise) until then; results of different calls must not alias.
+ * The handle cycles through three staging slots: the host->device copy of a call runs under the kernels and the
+ * device->host copy of the call before (one copy stream per direction, events in between), so a sequence of calls
+ * uses both directions of the link at once.  Calls are executed in the order they were made. */
+mrhs_status_t mrhs_wilson_apply_host_async(mrhs_wilson_t *h, int op, int parity,
+                                           const void *h_in, void *h_out);
+mrhs_status_t mrhs_wilson_host_wait(mrhs_wilson_t *h);
+mrhs_status_t mrhs_coarse_apply_host_async(mrhs_coarse_t *h, const void *h_in, void *h_out);
+mrhs_status_t mrhs_coarse_host_wait(mrhs_coarse_t *h);
 
 /* ------------------------------------------------------------------- errors */
 

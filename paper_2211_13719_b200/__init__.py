@@ -78,6 +78,10 @@ _SIGNATURES = {
     "mrhs_coarse_cb_merge": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
     "mrhs_wilson_apply_host": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _vp, _vp]),
     "mrhs_coarse_apply_host": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_wilson_apply_host_async": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _vp, _vp]),
+    "mrhs_wilson_host_wait": (ctypes.c_int, [_vp]),
+    "mrhs_coarse_apply_host_async": (ctypes.c_int, [_vp, _vp, _vp]),
+    "mrhs_coarse_host_wait": (ctypes.c_int, [_vp]),
     "mrhs_last_error": (ctypes.c_char_p, []),
     "mrhs_version": (ctypes.c_char_p, []),
 }
@@ -345,6 +349,15 @@ def wilson_apply_host(h, op, parity, h_in, h_out):
     _check(lib().mrhs_wilson_apply_host(h, int(op), int(parity), _ptr(h_in), _ptr(h_out)))
 
 
+def wilson_apply_host_async(h, op, parity, h_in, h_out):
+    """Enqueue only; h_in / h_out (pinned HOST tensors) must stay alive until wilson_host_wait(h)."""
+    _check(lib().mrhs_wilson_apply_host_async(h, int(op), int(parity), _ptr(h_in), _ptr(h_out)))
+
+
+def wilson_host_wait(h):
+    _check(lib().mrhs_wilson_host_wait(h))
+
+
 def wilson_destroy(h):
     _check(lib().mrhs_wilson_destroy(h))
 
@@ -372,6 +385,14 @@ def coarse_meooe(h, d_in, d_out, out_parity):
 
 def coarse_apply_host(h, h_in, h_out):
     _check(lib().mrhs_coarse_apply_host(h, _ptr(h_in), _ptr(h_out)))
+
+
+def coarse_apply_host_async(h, h_in, h_out):
+    _check(lib().mrhs_coarse_apply_host_async(h, _ptr(h_in), _ptr(h_out)))
+
+
+def coarse_host_wait(h):
+    _check(lib().mrhs_coarse_host_wait(h))
 
 
 def coarse_destroy(h):

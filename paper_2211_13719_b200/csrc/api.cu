@@ -33,6 +33,20 @@ static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 
 
 using namespace mrhs;
 
+// Staging of the host-buffer entries: kPipeSlots slots, each with a canonical buffer (host data lands there and results leave from
+// there) and native in / out fields; host->device copies run on one stream, device->host copies on another, the operator on
+// the handle's stream, chained by events.  While call k computes or copies out, call k + 1 can already copy in: PCIe carries
+// both directions at once.
+constexpr int kPipeSlots = 3;
+struct HostPipe {
+    void *canon[kPipeSlots], *din[kPipeSlots], *dout[kPipeSlots];
+    size_t bytes[kPipeSlots];
+    cudaStream_t s_in, s_out;
+    cudaEvent_t ev_in[kPipeSlots], ev_out[kPipeSlots], ev_free[kPipeSlots];
+    bool used[kPipeSlots], ready;
+    unsigned next;
+};
+
 struct mrhs_wilson {
     int dims[4];
     int nrhs;
@@ -49,9 +63,7 @@ struct mrhs_wilson {
     int kern[2];                   // which kernel runs D_hop [0] / M_eooe [1]: MRHS_HOP_GATHER or MRHS_HOP_SWEEP
     int num_sms;
     size_t l2_bytes;
-    // staging for the host-buffer entry
-    void *st_canon, *st_in, *st_out;
-    size_t st_bytes;
+    HostPipe pipe;                 // staging of the host-buffer entries
     void *st_tmp[2];               // odd-parity temporaries of the Schur sequence
     size_t st_tmp_bytes;
 };
@@ -70,19 +82,76 @@ struct mrhs_coarse {
     cudaStream_t st;
     float2 *links;                 // math_mode 0: [site][p][col][row] complex; math_mode 1: the tensor-core order (coarse.cuh)
     int tc_grid;                   // persistent grid of the tensor-core kernel
-    void *st_canon, *st_in, *st_out;
-    size_t st_bytes;
+    HostPipe pipe;
 };
 
 namespace {
 
+void pipe_free(HostPipe &p) {
+    if (p.ready) {
+        cudaStreamSynchronize(p.s_in); cudaStreamSynchronize(p.s_out);
+        cudaStreamDestroy(p.s_in); cudaStreamDestroy(p.s_out);
+        for (int b = 0; b < kPipeSlots; b++) { cudaEventDestroy(p.ev_in[b]); cudaEventDestroy(p.ev_out[b]); cudaEventDestroy(p.ev_free[b]); }
+    }
+    for (int b = 0; b < kPipeSlots; b++) { cudaFree(p.canon[b]); cudaFree(p.din[b]); cudaFree(p.dout[b]); }
+    memset(&p, 0, sizeof(p));
+}
+
+// next slot with room for `bytes`, its previous use finished as far as the copy-in stream is concerned
+mrhs_status_t pipe_acquire(HostPipe &p, size_t bytes, int *slot) {
+    if (!p.ready) {
+        MRHS_CUDA(cudaStreamCreateWithFlags(&p.s_in, cudaStreamNonBlocking));
+        MRHS_CUDA(cudaStreamCreateWithFlags(&p.s_out, cudaStreamNonBlocking));
+        for (int b = 0; b < kPipeSlots; b++) {
+            MRHS_CUDA(cudaEventCreateWithFlags(&p.ev_in[b], cudaEventDisableTiming));
+            MRHS_CUDA(cudaEventCreateWithFlags(&p.ev_out[b], cudaEventDisableTiming));
+            MRHS_CUDA(cudaEventCreateWithFlags(&p.ev_free[b], cudaEventDisableTiming));
+        }
+        p.ready = true;
+    }
+    const int b = (int)(p.next++ % kPipeSlots);
+    if (p.bytes[b] < bytes) {
+        if (p.used[b]) MRHS_CUDA(cudaEventSynchronize(p.ev_free[b]));
+        cudaFree(p.canon[b]); cudaFree(p.din[b]); cudaFree(p.dout[b]);
+        p.canon[b] = p.din[b] = p.dout[b] = nullptr; p.bytes[b] = 0;
+        MRHS_CUDA(cudaMalloc(&p.canon[b], bytes));
+        MRHS_CUDA(cudaMalloc(&p.din[b], bytes));
+        MRHS_CUDA(cudaMalloc(&p.dout[b], bytes));
+        p.bytes[b] = bytes;
+    }
+    if (p.used[b]) MRHS_CUDA(cudaStreamWaitEvent(p.s_in, p.ev_free[b], 0));     // the copy-out of the slot's previous use has finished
+    *slot = b;
+    return MRHS_OK;
+}
+mrhs_status_t pipe_copy_in(HostPipe &p, int b, const void *h_in, size_t bytes, cudaStream_t st) {
+    MRHS_CUDA(cudaMemcpyAsync(p.canon[b], h_in, bytes, cudaMemcpyHostToDevice, p.s_in));
+    MRHS_CUDA(cudaEventRecord(p.ev_in[b], p.s_in));
+    MRHS_CUDA(cudaStreamWaitEvent(st, p.ev_in[b], 0));
+    return MRHS_OK;
+}
+mrhs_status_t pipe_copy_out(HostPipe &p, int b, void *h_out, size_t bytes, cudaStream_t st) {
+    MRHS_CUDA(cudaEventRecord(p.ev_out[b], st));
+    MRHS_CUDA(cudaStreamWaitEvent(p.s_out, p.ev_out[b], 0));
+    MRHS_CUDA(cudaMemcpyAsync(h_out, p.canon[b], bytes, cudaMemcpyDeviceToHost, p.s_out));
+    MRHS_CUDA(cudaEventRecord(p.ev_free[b], p.s_out));
+    p.used[b] = true;
+    return MRHS_OK;
+}
+mrhs_status_t pipe_wait(HostPipe &p, cudaStream_t st) {
+    if (!p.ready) return MRHS_OK;
+    MRHS_CUDA(cudaStreamSynchronize(p.s_in));
+    MRHS_CUDA(cudaStreamSynchronize(st));
+    MRHS_CUDA(cudaStreamSynchronize(p.s_out));
+    return MRHS_OK;
+}
+
 mrhs_status_t wilson_free(mrhs_wilson *h) {
     if (!h) return MRHS_OK;
+    pipe_free(h->pipe);
     cudaFree(h->gauge_full); cudaFree(h->gauge_cb[0]); cudaFree(h->gauge_cb[1]);
     cudaFree(h->gauge_back[0]); cudaFree(h->gauge_back[1]);
     cudaFree(h->clov_full); cudaFree(h->clov_cb[0]); cudaFree(h->clov_cb[1]);
     cudaFree(h->cinv_full); cudaFree(h->cinv_cb[0]); cudaFree(h->cinv_cb[1]);
-    cudaFree(h->st_canon); cudaFree(h->st_in); cudaFree(h->st_out);
     cudaFree(h->st_tmp[0]); cudaFree(h->st_tmp[1]);
     delete h;
     return MRHS_OK;
@@ -233,17 +302,6 @@ bool fine_dims_ok(const int dims[4]) {
     for (int i = 0; i < 4; i++)
         if (dims[i] < 2 || (dims[i] & 1)) return false;
     return true;
-}
-
-mrhs_status_t ensure_stage(void **canon, void **in, void **out, size_t *have, size_t need) {
-    if (*have >= need) return MRHS_OK;
-    cudaFree(*canon); cudaFree(*in); cudaFree(*out);
-    *canon = *in = *out = nullptr; *have = 0;
-    MRHS_CUDA(cudaMalloc(canon, need));
-    MRHS_CUDA(cudaMalloc(in, need));
-    MRHS_CUDA(cudaMalloc(out, need));
-    *have = need;
-    return MRHS_OK;
 }
 
 }  // namespace
@@ -520,7 +578,7 @@ mrhs_status_t mrhs_wilson_get_tiling(mrhs_wilson_t *h, int which, int tile[3], i
 
 mrhs_status_t mrhs_wilson_destroy(mrhs_wilson_t *h) { return wilson_free(h); }
 
-mrhs_status_t mrhs_wilson_apply_host(mrhs_wilson_t *h, int op, int parity, const void *h_in, void *h_out) {
+mrhs_status_t mrhs_wilson_apply_host_async(mrhs_wilson_t *h, int op, int parity, const void *h_in, void *h_out) {
     MRHS_REQUIRE(h && h_in && h_out, "apply host: NULL argument");
     MRHS_REQUIRE(op >= 0 && op <= 3, "apply host: op must be 0 (D_hop), 1 (M_eooe), 2 (M_ooee) or 3 (Schur sequence)");
     int in_par = MRHS_FULL, out_par = MRHS_FULL;
@@ -533,28 +591,38 @@ mrhs_status_t mrhs_wilson_apply_host(mrhs_wilson_t *h, int op, int parity, const
         in_par = out_par = parity;
     }
     const size_t bytes = mrhs_field_bytes(h->dims, 12, h->nrhs, in_par != MRHS_FULL);
-    mrhs_status_t s = ensure_stage(&h->st_canon, &h->st_in, &h->st_out, &h->st_bytes, bytes);
-    if (s != MRHS_OK) return s;
     if (op == 3 && h->st_tmp_bytes < bytes) {
+        MRHS_CUDA(cudaStreamSynchronize(h->st));
         cudaFree(h->st_tmp[0]); cudaFree(h->st_tmp[1]);
         h->st_tmp[0] = h->st_tmp[1] = nullptr; h->st_tmp_bytes = 0;
         MRHS_CUDA(cudaMalloc(&h->st_tmp[0], bytes));
         MRHS_CUDA(cudaMalloc(&h->st_tmp[1], bytes));
         h->st_tmp_bytes = bytes;
     }
-    MRHS_CUDA(cudaMemcpyAsync(h->st_canon, h_in, bytes, cudaMemcpyHostToDevice, h->st));
-    s = mrhs_field_import(h->dims, 12, h->nrhs, in_par, h->st_canon, h->st_in, h->st);
+    HostPipe &p = h->pipe;
+    int b = 0;
+    mrhs_status_t s = pipe_acquire(p, bytes, &b);
+    if (s == MRHS_OK) s = pipe_copy_in(p, b, h_in, bytes, h->st);
+    if (s == MRHS_OK) s = mrhs_field_import(h->dims, 12, h->nrhs, in_par, p.canon[b], p.din[b], h->st);
     if (s != MRHS_OK) return s;
-    if (op == 3) s = mrhs_schur_sequence(h, h->st_in, h->st_tmp[0], h->st_tmp[1], h->st_out);
-    else if (op == 0) s = mrhs_dhop(h, h->st_in, h->st_out);
-    else if (op == 1) s = mrhs_meooe(h, h->st_in, h->st_out, out_par);
-    else s = mrhs_mooee(h, h->st_in, h->st_out, parity);
-    if (s != MRHS_OK) return s;
-    s = mrhs_field_export(h->dims, 12, h->nrhs, out_par, h->st_out, h->st_canon, h->st);
-    if (s != MRHS_OK) return s;
-    MRHS_CUDA(cudaMemcpyAsync(h_out, h->st_canon, bytes, cudaMemcpyDeviceToHost, h->st));
-    MRHS_CUDA(cudaStreamSynchronize(h->st));
-    return MRHS_OK;
+    if (op == 3) s = mrhs_schur_sequence(h, p.din[b], h->st_tmp[0], h->st_tmp[1], p.dout[b]);
+    else if (op == 0) s = mrhs_dhop(h, p.din[b], p.dout[b]);
+    else if (op == 1) s = mrhs_meooe(h, p.din[b], p.dout[b], out_par);
+    else s = mrhs_mooee(h, p.din[b], p.dout[b], parity);
+    if (s == MRHS_OK) s = mrhs_field_export(h->dims, 12, h->nrhs, out_par, p.dout[b], p.canon[b], h->st);
+    if (s == MRHS_OK) s = pipe_copy_out(p, b, h_out, bytes, h->st);
+    return s;
+}
+
+mrhs_status_t mrhs_wilson_host_wait(mrhs_wilson_t *h) {
+    MRHS_REQUIRE(h, "host wait: NULL handle");
+    return pipe_wait(h->pipe, h->st);
+}
+
+mrhs_status_t mrhs_wilson_apply_host(mrhs_wilson_t *h, int op, int parity, const void *h_in, void *h_out) {
+    mrhs_status_t s = mrhs_wilson_apply_host_async(h, op, parity, h_in, h_out);
+    if (s == MRHS_OK) s = mrhs_wilson_host_wait(h);
+    return s;
 }
 
 /* ---------------------------------------------------------------- coarse level */
@@ -633,25 +701,35 @@ mrhs_status_t mrhs_coarse_apply(mrhs_coarse_t *h, const void *d_in, void *d_out)
 mrhs_status_t mrhs_coarse_destroy(mrhs_coarse_t *h) {
     if (!h) return MRHS_OK;
     cudaFree(h->links);
-    cudaFree(h->st_canon); cudaFree(h->st_in); cudaFree(h->st_out);
+    pipe_free(h->pipe);
     delete h;
     return MRHS_OK;
 }
 
-mrhs_status_t mrhs_coarse_apply_host(mrhs_coarse_t *h, const void *h_in, void *h_out) {
+mrhs_status_t mrhs_coarse_apply_host_async(mrhs_coarse_t *h, const void *h_in, void *h_out) {
     MRHS_REQUIRE(h && h_in && h_out, "coarse apply host: NULL argument");
     const int dims[4] = {h->g.X, h->g.Y, h->g.Z, h->g.T};
     const size_t bytes = mrhs_field_bytes(dims, h->g.nb, h->g.N, 0);
-    mrhs_status_t s = ensure_stage(&h->st_canon, &h->st_in, &h->st_out, &h->st_bytes, bytes);
-    if (s != MRHS_OK) return s;
-    MRHS_CUDA(cudaMemcpyAsync(h->st_canon, h_in, bytes, cudaMemcpyHostToDevice, h->st));
-    s = mrhs_field_import(dims, h->g.nb, h->g.N, MRHS_FULL, h->st_canon, h->st_in, h->st);
-    if (s == MRHS_OK) s = mrhs_coarse_apply(h, h->st_in, h->st_out);
-    if (s == MRHS_OK) s = mrhs_field_export(dims, h->g.nb, h->g.N, MRHS_FULL, h->st_out, h->st_canon, h->st);
-    if (s != MRHS_OK) return s;
-    MRHS_CUDA(cudaMemcpyAsync(h_out, h->st_canon, bytes, cudaMemcpyDeviceToHost, h->st));
-    MRHS_CUDA(cudaStreamSynchronize(h->st));
-    return MRHS_OK;
+    HostPipe &p = h->pipe;
+    int b = 0;
+    mrhs_status_t s = pipe_acquire(p, bytes, &b);
+    if (s == MRHS_OK) s = pipe_copy_in(p, b, h_in, bytes, h->st);
+    if (s == MRHS_OK) s = mrhs_field_import(dims, h->g.nb, h->g.N, MRHS_FULL, p.canon[b], p.din[b], h->st);
+    if (s == MRHS_OK) s = mrhs_coarse_apply(h, p.din[b], p.dout[b]);
+    if (s == MRHS_OK) s = mrhs_field_export(dims, h->g.nb, h->g.N, MRHS_FULL, p.dout[b], p.canon[b], h->st);
+    if (s == MRHS_OK) s = pipe_copy_out(p, b, h_out, bytes, h->st);
+    return s;
+}
+
+mrhs_status_t mrhs_coarse_host_wait(mrhs_coarse_t *h) {
+    MRHS_REQUIRE(h, "host wait: NULL handle");
+    return pipe_wait(h->pipe, h->st);
+}
+
+mrhs_status_t mrhs_coarse_apply_host(mrhs_coarse_t *h, const void *h_in, void *h_out) {
+    mrhs_status_t s = mrhs_coarse_apply_host_async(h, h_in, h_out);
+    if (s == MRHS_OK) s = mrhs_coarse_host_wait(h);
+    return s;
 }
 
 mrhs_status_t mrhs_transfer_create(mrhs_transfer_t **out, const int dims[4], const int bdims[4], int nvec, int nrhs,

@@ -65,6 +65,13 @@ def test_config4_coarsest_level(nrhs):
     mrhs.coarse_apply_host(c.h, h_in, h_out)
     err = rel_l2_per_rhs(h_out.numpy(), oracle.coarse_apply(cdims, A, v))
     assert err.max() < TOL, err
+    # asynchronous entry: five calls in flight over the three staging slots, one wait
+    outs = [torch.full_like(h_in, float("nan")).pin_memory() for _ in range(5)]
+    for o in outs:
+        mrhs.coarse_apply_host_async(c.h, h_in, o)
+    mrhs.coarse_host_wait(c.h)
+    for o in outs:
+        assert np.array_equal(o.numpy(), h_out.numpy())
     c.close()
 
 

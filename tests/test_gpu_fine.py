@@ -224,6 +224,20 @@ def test_schur_sequence_and_host_entry():
     mrhs.wilson_apply_host(w.h, mrhs.OP_MEOOE, 0, h_in, h_out)
     err = rel_l2_per_rhs(h_out.numpy(), oracle.meooe(dims, U, po, 0))
     assert err.max() < TOL, err
+    # the asynchronous entries: five calls of four operators in flight over the three staging slots, one wait
+    h_psi, h_pe, h_po = (torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (psi, pe, po))
+    outs = [torch.full_like(h_psi, float("nan")).pin_memory(), torch.full_like(h_pe, float("nan")).pin_memory(),
+            torch.full_like(h_po, float("nan")).pin_memory(), torch.full_like(h_psi, float("nan")).pin_memory(),
+            torch.full_like(h_pe, float("nan")).pin_memory()]
+    mrhs.wilson_apply_host_async(w.h, mrhs.OP_DHOP, 0, h_psi, outs[0])
+    mrhs.wilson_apply_host_async(w.h, mrhs.OP_MEOOE, mrhs.EVEN, h_po, outs[1])
+    mrhs.wilson_apply_host_async(w.h, mrhs.OP_MEOOE, mrhs.ODD, h_pe, outs[2])
+    mrhs.wilson_apply_host_async(w.h, mrhs.OP_MOOEE, mrhs.FULL, h_psi, outs[3])
+    mrhs.wilson_apply_host_async(w.h, mrhs.OP_SCHUR, 0, h_pe, outs[4])
+    mrhs.wilson_host_wait(w.h)
+    wants = [oracle.dhop(dims, U, psi), oracle.meooe(dims, U, po, 0), oracle.meooe(dims, U, pe, 1), oracle.mooee(C, psi), want]
+    for i, (o, wnt) in enumerate(zip(outs, wants)):
+        assert rel_l2_per_rhs(o.numpy(), wnt).max() < TOL, ("async host entry", i)
     w.close()
 
 
