@@ -265,9 +265,13 @@ mrhs_status_t wilson_set_default_tiling(mrhs_wilson *h) {
         if (ok) {
             h->sp_full.gauge_out = h->sp_full.gauge_in = h->gauge_full;
             for (int p = 0; p < 2; p++) { h->sp_cb[p].gauge_out = h->gauge_cb[p]; h->sp_cb[p].gauge_in = h->gauge_cb[1 - p]; h->sp_cb[p].gauge_back = h->gauge_back[p]; }
-            // measured cross-over (round 1): the sweep kernel wins from N_rhs = 12 on lattices of 32^4
-            // sites and more; below that the gather kernel's many small blocks hide latency better
-            if (h->nrhs >= 12 && h->gfull.nsites >= (1ll << 20)) h->kern[0] = h->kern[1] = MRHS_HOP_SWEEP;
+            // measured cross-over (round 2, after the packed backward links and the tail split; D_hop / M_eooe, L2 flushed):
+            // 16^4: the sweep kernel wins from N_rhs = 24 (0.098 / 0.055 ms vs 0.100 / 0.056), 24^4: from N_rhs = 12 (0.197 / 0.131 vs
+            // 0.226 / 0.142 ms; N_rhs = 4: 0.106 / 0.060 vs 0.094 / 0.057), 32^4: from N_rhs = 4 (0.253 / 0.144 vs 0.265 / 0.147);
+            // below that the gather kernel's many small blocks hide latency better
+            const long long V = h->gfull.nsites;
+            if ((h->nrhs >= 24 && V >= (1ll << 16)) || (h->nrhs >= 12 && V >= (1ll << 18)) || (h->nrhs >= 4 && V >= (1ll << 20)))
+                h->kern[0] = h->kern[1] = MRHS_HOP_SWEEP;
         }
     }
     return MRHS_OK;

@@ -389,7 +389,9 @@ __global__ void __launch_bounds__(160, 3)
 prolong_staged_kernel(TransferGeom g, int NP, int NW, const float4 *__restrict__ basis, const float4 *__restrict__ coarse, float4 *__restrict__ fine) {
     extern __shared__ __align__(128) unsigned char sm[];
     const int XB = g.XB, CS = XB * NP;
-    const uint32_t b_bytes = (uint32_t)XB * g.nvec * 96u;
+    // a site's basis (n_vec x 96 bytes) is copied on its own and lands one float4 further than a dense row would put it: the lanes of
+    // a quarter-warp read four sites at the same (k, component), 1920 bytes apart in a dense row = the same banks
+    const uint32_t site_bytes = (uint32_t)g.nvec * 96u, site_pitch = site_bytes + 16u, b_bytes = (uint32_t)XB * site_pitch;
     const int agx = XB / g.bx, lgs = NP / LT, tiles = XB * 2 * lgs, NR = g.by * g.bz * g.bt;
     const uint32_t c_bytes = (uint32_t)agx * 2u * g.nvec * NP * 16u;
     float4 *sc = reinterpret_cast<float4 *>(sm + (size_t)kRestrictStages * b_bytes);                    // [aggregate][2 n_vec][NP]
@@ -420,12 +422,14 @@ prolong_staged_kernel(TransferGeom g, int NP, int NW, const float4 *__restrict__
                 const long long B = (xb * agx + a) + (long long)g.cX * (cy + (long long)g.cY * (cz + (long long)g.cZ * ct));
                 bulk_g2s(sc + (size_t)a * 2 * g.nvec * NP, coarse + (size_t)B * 2 * g.nvec * NP, c_bytes / agx, cfull);
             }
-            for (int r = 0; r < NR; r++) {
-                const int st = r % kRestrictStages;
-                if (r >= kRestrictStages) mbar_wait(&empty[st], ((r / kRestrictStages) - 1) & 1);
-                mbar_expect_tx(&full[st], b_bytes);
-                bulk_g2s(sm + (size_t)st * b_bytes, basis + ((size_t)xb * XB + (size_t)g.X * row_yzt(r)) * g.nvec * 6, b_bytes, &full[st]);
-            }
+        }
+        for (int r = 0; r < NR; r++) {
+            const int st = r % kRestrictStages;
+            if (r >= kRestrictStages) mbar_wait(&empty[st], ((r / kRestrictStages) - 1) & 1);
+            if (lane == 0) mbar_expect_tx(&full[st], XB * site_bytes);
+            __syncwarp();
+            if (lane < XB)
+                bulk_g2s(sm + (size_t)st * b_bytes + (size_t)lane * site_pitch, basis + ((size_t)xb * XB + lane + (size_t)g.X * row_yzt(r)) * g.nvec * 6, site_bytes, &full[st]);
         }
     } else if (warp < NW) {
         // ------------------------------------------------ consumers: warp w takes rows w, w + NW, ...; each row is read by one warp only
@@ -437,7 +441,7 @@ prolong_staged_kernel(TransferGeom g, int NP, int NW, const float4 *__restrict__
         for (int r = warp; r < NR; r += NW) {
             const int st = r % kRestrictStages;
             mbar_wait(&full[st], (r / kRestrictStages) & 1);
-            const float4 *sb = reinterpret_cast<const float4 *>(sm + (size_t)st * b_bytes) + (size_t)xin * g.nvec * 6 + chi * 3;
+            const float4 *sb = reinterpret_cast<const float4 *>(sm + (size_t)st * b_bytes + (size_t)xin * site_pitch) + chi * 3;
             CVec<2> acc[6][LT];
 #pragma unroll
             for (int c = 0; c < 6; c++)
@@ -610,7 +614,7 @@ bool try_prolong_staged(const TransferGeom &g, int np, const float2 *d_basis, co
     if (tiles > 32 || tiles < 16) return false;
     const int agx = g.XB / g.bx, NR = g.by * g.bz * g.bt;
     const int NW = NR < 4 ? NR : 4;      // four consumer warps + the producer: three blocks per SM at 136 registers
-    const size_t smem = (size_t)kRestrictStages * g.XB * g.nvec * 96 + (size_t)agx * 2 * g.nvec * np * 16 + (2 * kRestrictStages + 1) * 8;
+    const size_t smem = (size_t)kRestrictStages * g.XB * (g.nvec * 96 + 16) + (size_t)agx * 2 * g.nvec * np * 16 + (2 * kRestrictStages + 1) * 8;
     if (smem > 72 * 1024) return false;
     *status = MRHS_OK;
     cudaError_t e = cudaFuncSetAttribute(prolong_staged_kernel<LT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 72 * 1024);
