@@ -127,11 +127,11 @@ struct TcCfg {
     static constexpr int KS = NB / 8;                         // MMA K steps per stencil point
     static constexpr int THREADS = NT <= 64 ? 128 : 256;
     static constexpr int A_LBO = 2 * NB * 16;                 // bytes between K chunks of the A operand: only the 2 nb used rows are stored
-    static constexpr int B_LBO = NT * 16;
+    static constexpr int B_LBO = NT * 16 + 16;                 // + 16: consecutive K chunks of the B operand start in different banks (operand stores of one warp span several chunks)
     static constexpr int A_BYTES = KC * A_LBO;                // one of hi / lo
     static constexpr int B_BYTES = KC * B_LBO;
     static constexpr int OPER_BYTES = 2 * A_BYTES + 2 * B_BYTES;
-    static constexpr int S_PITCH = 129;                       // epilogue scratch S[col][lane], floats
+    static constexpr int S_PITCH = 128 + (32 + NP - 1) / NP;  // epilogue scratch S[col][lane], floats; the combine reads NP columns x 32 / NP lanes per warp: distinct banks
     static constexpr int S_BYTES = NT * S_PITCH * 4;
     static constexpr int DATA_BYTES = OPER_BYTES > S_BYTES ? OPER_BYTES : S_BYTES;
     static constexpr int SMEM_BYTES = DATA_BYTES + 32;        // + mbarrier + TMEM address slot
