@@ -58,9 +58,9 @@
 extern "C" {
 #endif
 
-typedef struct mrhs_wilson mrhs_wilson_t;   /* opaque: owns packed gauge + clover  */
-typedef struct mrhs_coarse mrhs_coarse_t;
-typedef struct mrhs_transfer mrhs_transfer_t;   /* opaque, owns the repacked multigrid basis vectors */   /* opaque: owns packed coarse links    */
+typedef struct mrhs_wilson mrhs_wilson_t;       /* opaque: owns packed gauge + clover */
+typedef struct mrhs_coarse mrhs_coarse_t;       /* opaque: owns packed coarse links */
+typedef struct mrhs_transfer mrhs_transfer_t;   /* opaque: owns the repacked multigrid basis vectors */
 
 typedef enum {
     MRHS_OK = 0,
@@ -173,7 +173,7 @@ mrhs_status_t mrhs_wilson_get_tiling(mrhs_wilson_t *h, int which, int tile[3], i
  * asks the copy engine to bring the rows of the tile distance_tiles later into L2 (0 = off).
  * set_tiling resets it to the default (296 tiles: half of the tiles resident on 148 SMs at four per SM).
  * While the sweep kernel is selected for `which`, the call sets ITS prefetch distance instead, in t-slices
- * (default 2; set_sweep resets it).  The environment variable MRHS_DEBUG=1 makes create calls print
+ * (default 0 = off: measured to add DRAM traffic and no speed; set_sweep keeps it).  The environment variable MRHS_DEBUG=1 makes create calls print
  * their launch geometry to stderr; nothing else in the library reads the environment. */
 mrhs_status_t mrhs_wilson_set_prefetch(mrhs_wilson_t *h, int which, int distance_tiles);
 
@@ -183,10 +183,12 @@ mrhs_status_t mrhs_wilson_set_prefetch(mrhs_wilson_t *h, int which, int distance
  *                    (any N_rhs; the only kernel for odd N_rhs);
  *   MRHS_HOP_SWEEP   a thread block sweeps a t-segment of an XB x 2 x 2 tile with the current slice,
  *                    its halo and the links staged in shared memory by TMA bulk copies (even N_rhs;
- *                    the default where supported).
+ *                    the default where it measured faster: from N_rhs = 24 at 16^4 sites, 12 at 24^4, 4 at 32^4).
  * which: 0 = D_hop, 1 = M_eooe.  UNSUPPORTED if the sweep kernel is asked for with odd N_rhs.
  * set_sweep: lt = t-slices one thread block sweeps (divides T); chunk = {cy, cz}: tiles (of 2 x 2
- * sites in y,z) per concurrently scheduled patch; INVALID_ARG if they do not divide the lattice. */
+ * sites in y,z) per concurrently scheduled patch; INVALID_ARG if they do not divide the lattice.
+ * With lt = T the last tiles of the dispatch order are cut into shorter t-segments by the library so that the
+ * last wave of thread blocks is balanced; results do not depend on any of these settings (bit-identical). */
 #define MRHS_HOP_GATHER 0
 #define MRHS_HOP_SWEEP 1
 mrhs_status_t mrhs_wilson_set_hop_kernel(mrhs_wilson_t *h, int which, int kernel);
