@@ -122,3 +122,48 @@ def test_fine_level_transfer_with_six_basis_vectors():
     got = host(mrhs.coarse_field_export(cdims, 12, nrhs, mrhs.FULL, d_c))
     assert rel_l2_per_rhs(got, otr.restrict(dims, bdims, basis, f)).max() < TOL
     tr.close()
+
+
+@pytest.mark.parametrize("nrhs", [12, 24])
+def test_intergrid_operators_at_48_4_on_sampled_aggregates(nrhs):
+    """The size bench.py --sweep times (48^4, 4^4 aggregates, n_vec = 20: the staged kernels in their default launch geometry):
+    restriction and prolongation on sampled aggregates, each handed to the oracle as a 4^4 lattice of its own (one block).
+    Inputs are gathered from the device inputs, never from outputs."""
+    dims, bdims, nvec = [48] * 4, [4] * 4, 20
+    cdims = [12] * 4
+    V, Vc, nb = syn.volume(dims), syn.volume(cdims), 2 * nvec
+    d = torch.device("cuda", 0)
+    basis = syn.spinor_torch(V * nvec, 1, 411, d).reshape(nvec, V, 4, 3)
+    f = syn.spinor_torch(V, nrhs, 412, d)
+    vc = syn.spinor_torch(Vc, nrhs, 413, d, ncomp=(nb,))
+    tr = mrhs.Transfer(dims, bdims, nvec, nrhs, basis)
+    rng = np.random.default_rng(77)
+    cc = rng.integers(0, 12, size=(24, 4))
+    cc[0], cc[1], cc[2] = (0, 0, 0, 0), (11, 11, 11, 11), (11, 0, 11, 0)      # corners of the coarse lattice
+    # fine sites of an aggregate in the lexicographic order of a 4^4 lattice
+    i = np.arange(256)
+    off = np.stack([i % 4, (i // 4) % 4, (i // 16) % 4, i // 64], axis=1)
+    d_f = mrhs.field_import(dims, 12, nrhs, mrhs.FULL, f)
+    d_c = mrhs.empty_field(cdims, nb, nrhs, mrhs.FULL)
+    d_c.fill_(float("nan"))
+    torch.cuda.synchronize()
+    tr.restrict(d_f, d_c)
+    torch.cuda.synchronize()
+    got_c = mrhs.coarse_field_export(cdims, nb, nrhs, mrhs.FULL, d_c)
+    del d_f
+    d_p = mrhs.empty_field(dims, 12, nrhs, mrhs.FULL)
+    d_p.fill_(float("nan"))
+    torch.cuda.synchronize()
+    tr.prolong(mrhs.coarse_field_import(cdims, nb, nrhs, mrhs.FULL, vc), d_p)
+    torch.cuda.synchronize()
+    got_p = mrhs.field_export(dims, 12, nrhs, mrhs.FULL, d_p).reshape(V, 4, 3, nrhs)
+    for c in cc:
+        x = 4 * c[None, :] + off
+        lex = torch.from_numpy(x[:, 0] + 48 * (x[:, 1] + 48 * (x[:, 2] + 48 * x[:, 3]))).to(d)
+        B = int(c[0] + 12 * (c[1] + 12 * (c[2] + 12 * c[3])))
+        b_sub, f_sub = host(basis[:, lex]), host(f[lex])
+        want = otr.restrict([4] * 4, [4] * 4, b_sub, f_sub)[0]
+        assert rel_l2_per_rhs(host(got_c[B]), want).max() < TOL, ("restrict", c)
+        want = otr.prolong([4] * 4, [4] * 4, b_sub, host(vc[B])[None])
+        assert rel_l2_per_rhs(host(got_p[lex]), want).max() < TOL, ("prolong", c)
+    tr.close()
