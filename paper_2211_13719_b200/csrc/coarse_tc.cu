@@ -21,30 +21,16 @@
 // back on an mbarrier via tcgen05.commit.  Several CTAs share an SM, so one CTA's operand conversion
 // overlaps another's MMAs.
 #include "coarse.cuh"
+#include "async_copy.cuh"
 #include <cstdlib>
 
 namespace mrhs {
 
 namespace {
 
-__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
-    uint32_t ok;
-    do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(ok)
-                     : "r"(smem_addr(bar)), "r"(parity)
-                     : "memory");
-    } while (!ok);
-}
-
 // ---- tcgen05 wrappers (PTX ISA 8.6+, sm_100a)
 template <int COLS> __device__ __forceinline__ void tmem_alloc(uint32_t *slot) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_addr(slot)), "n"(COLS) : "memory");
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "n"(COLS) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
 }
 template <int COLS> __device__ __forceinline__ void tmem_free(uint32_t taddr) {
@@ -65,7 +51,7 @@ __device__ __forceinline__ void mma_tf32(uint32_t d_tmem, uint64_t a_desc, uint6
 }
 // arrive on bar once every MMA issued so far by this thread has completed
 __device__ __forceinline__ void mma_commit(uint64_t *bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_addr(bar)) : "memory");
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 // 16 consecutive fp32 columns of this thread's TMEM lane
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
@@ -163,7 +149,7 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
     // one-time setup: barrier, zeroed operand area (so that the unused MMA rows / columns never see NaN patterns), TMEM accumulator
     if (tid == 0) {
         mbar_init(bar, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
     }
     for (int i = tid; i < C::OPER_BYTES / 16; i += C::THREADS) reinterpret_cast<float4 *>(smem)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (warp == 0) tmem_alloc<C::TMEM_COLS>(tslot);
@@ -188,8 +174,8 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
     // contiguous block), so that the register loads of that stage find them there
     auto prefetch_stage = [&](long long osite, int p) {
         const long long site = coarse_site_lex(sites, osite);
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(links + ((size_t)site * 9 + p) * C::A_UNITS), "r"(C::A_UNITS * 16) : "memory");
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(in + (size_t)neighbour(site, p) * NB * C::NP), "r"(NB * C::NP * 16) : "memory");
+        bulk_prefetch_l2(links + ((size_t)site * 9 + p) * C::A_UNITS, C::A_UNITS * 16);
+        bulk_prefetch_l2(in + (size_t)neighbour(site, p) * NB * C::NP, NB * C::NP * 16);
     };
     auto load_stage = [&](long long osite, int p) {
         const long long site = coarse_site_lex(sites, osite);
@@ -263,7 +249,7 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
             __syncthreads();
             if (tid == 0) {
                 tc_fence_after();
-                const uint32_t ah = smem_addr(a_hi), al = smem_addr(a_lo), bh = smem_addr(b_hi), bl = smem_addr(b_lo);
+                const uint32_t ah = smem_u32(a_hi), al = smem_u32(a_lo), bh = smem_u32(b_hi), bl = smem_u32(b_lo);
 #pragma unroll
                 for (int ks = 0; ks < C::KS; ks++) {
                     const uint64_t dah = smem_desc(ah + ks * 2 * C::A_LBO, C::A_LBO, 128);

@@ -89,19 +89,13 @@ prolong_smem_kernel(TransferGeom g, int NP, int rows, long long nblk, const floa
         return (long long)xb * g.XB + (long long)g.X * (y + (long long)g.Y * (z + (long long)g.Z * t));
     };
     if (tid == 0) {
-        const uint32_t bs = (uint32_t)__cvta_generic_to_shared(&bar);
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bs) : "memory");
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_init(&bar, 1);
+        mbar_fence_init();
         int nrow = 0;
         for (int r = 0; r < rows; r++) nrow += b0 + r < nblk;
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bs), "r"(nrow * row_bytes) : "memory");
-        for (int r = 0; r < nrow; r++) {
-            const float4 *src = basis + (size_t)row_lex0(b0 + r) * g.nvec * 6;
-            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                             (uint32_t)__cvta_generic_to_shared(sm + (size_t)r * row_bytes)),
-                         "l"(src), "r"(row_bytes), "r"(bs)
-                         : "memory");
-        }
+        mbar_expect_tx(&bar, nrow * row_bytes);
+        for (int r = 0; r < nrow; r++)
+            bulk_g2s(sm + (size_t)r * row_bytes, basis + (size_t)row_lex0(b0 + r) * g.nvec * 6, row_bytes, &bar);
     }
     __syncthreads();
     const int row = tid / CS, rem = tid - row * CS;
@@ -120,13 +114,7 @@ prolong_smem_kernel(TransferGeom g, int NP, int rows, long long nblk, const floa
         const long long B = (x / g.bx) + (long long)g.cX * ((y / g.by) + (long long)g.cY * ((z / g.bz) + (long long)g.cZ * (t / g.bt)));
         vc = coarse + (size_t)B * 2 * g.nvec * NP + pair;
     }
-    {   // wait for the basis rows
-        const uint32_t bs = (uint32_t)__cvta_generic_to_shared(&bar);
-        uint32_t ok;
-        do {
-            asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}" : "=r"(ok) : "r"(bs), "r"(0u) : "memory");
-        } while (!ok);
-    }
+    mbar_wait(&bar, 0);      // the basis rows have landed
     if (!active) return;
     const int site = row * g.XB + xin;
     const float4 *ph = sb + (size_t)site * g.nvec * 6;
