@@ -522,7 +522,7 @@ def run_e2e(torch, mrhs, wl, args, barrier, dist, device, world, flops_step):
 
 # ------------------------------------------------------------------------ N_rhs sweep
 
-def sweep_records(torch, mrhs, syn, device, stream, peak, iters, subset, warm=5, ops=("fine", "coarse")):
+def sweep_records(torch, mrhs, syn, device, stream, peak, iters, subset, warm=10, ops=("fine", "coarse")):
     """Per (operator, lattice, N_rhs) records for configs 2-5: median and min time of individually timed launches on the
     library's stream, L2 flushed between launches (a 512 MB memset), GFLOP/s, algorithmic GB/s, fraction of the measured
     HBM peak, speed-up per RHS over the first N_rhs of the config.  subset "north_star": D_hop, M_eooe, M_ooee and the
@@ -681,6 +681,63 @@ def run_sweep(args):
     return 0
 
 
+def run_oracle_table(args):
+    """--oracle-table OUT.jsonl: the fp64 oracle as it stands, timed per operator (SURVEY.md Sec. 8(d) "Oracle beside it"):
+    full-field on configs 1-4 and on config 5 at N_rhs = 1, single-threaded and with OpenMP over sites on all cores the
+    process may use.  A reported baseline (needs no GPU); one JSON line per (config, operator, N_rhs, threads)."""
+    import numpy as np
+    import oracle
+    import synth_inputs as syn
+    cores = len(os.sched_getaffinity(0))
+
+    def timed(f, reps):
+        f()
+        ts = []
+        for _ in range(reps):
+            t0 = time.perf_counter(); f(); ts.append(time.perf_counter() - t0)
+        ts.sort()
+        return ts[len(ts) // 2]
+
+    fine = [("config1", [4, 4, 4, 4], [4], -0.1, 1.0, 0, 5), ("config2", [24, 24, 24, 24], [1, 4, 12, 24, 48], MASS, CSW, 2, 1),
+            ("config5", [48, 48, 48, 48], [1], MASS, CSW, 5, 1)]
+    coarse = [("config3", [8, 8, 8, 8], 24, [1, 12, 24, 64], 3), ("config4", [6, 6, 6, 32], 40, [12, 24, 48, 96], 4)]
+    with open(args.oracle_table, "w") as out:
+        def emit(cfg, op, dims, N, fl, t, thr):
+            r = {"config": cfg, "op": op, "dims": dims, "n_rhs": N, "threads": thr, "ms": t * 1e3, "gflops": fl / t / 1e9,
+                 "site_rhs_per_s": vol(dims) * N / t, "kind": "oracle", "dtype": "f64"}
+            out.write(json.dumps(r) + "\n"); out.flush()
+            print("%-8s %-10s %-14s N=%-3d threads=%-3d %10.2f ms %8.2f GF/s" % (cfg, op, "x".join(map(str, dims)), N, thr, r["ms"], r["gflops"]), flush=True)
+        for cfg, dims, ns, mass, csw, seed, reps in fine:
+            V = vol(dims)
+            U = syn.gauge_np(dims, seed).astype(np.complex128)
+            oracle.set_threads(cores)
+            C, _ = oracle.clover_blocks(dims, U, mass, csw)
+            for N in ns:
+                psi = syn.spinor_np(V, N, seed).astype(np.complex128)
+                pe, _po = oracle.cb_split(dims, psi)
+                for thr in (cores, 1):
+                    if thr == 1 and V * N > 24 ** 4 * 12:
+                        continue          # single-threaded only where it ends in seconds
+                    oracle.set_threads(thr)
+                    emit(cfg, "dhop", dims, N, 1320.0 * V * N, timed(lambda: oracle.dhop(dims, U, psi), reps), thr)
+                    emit(cfg, "meooe", dims, N, 1320.0 * (V / 2) * N, timed(lambda: oracle.meooe(dims, U, pe, 1), reps), thr)
+                    emit(cfg, "mooee", dims, N, 504.0 * V * N, timed(lambda: oracle.mooee(C, psi), reps), thr)
+                del psi, pe, _po
+            del U, C
+        for cfg, dims, nb, ns, seed in coarse:
+            A = syn.coarse_links_np(dims, nb, seed).astype(np.complex128)
+            for N in ns:
+                v = syn.coarse_vector_np(dims, nb, N, seed).astype(np.complex128)
+                for thr in (cores, 1):
+                    if thr == 1 and N > 24:
+                        continue
+                    oracle.set_threads(thr)
+                    emit(cfg, "coarse", dims, N, coarse_flops(nb) * vol(dims) * N, timed(lambda: oracle.coarse_apply(dims, A, v), 1), thr)
+            del A
+    oracle.set_threads(cores)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -693,7 +750,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-steps", type=int, default=8, help="oracle sample steps timed for cpu_baseline")
     ap.add_argument("--sweep", default=None, help="write the per-operator N_rhs sweep to this .jsonl and exit")
-    ap.add_argument("--sweep-iters", type=int, default=30)
+    ap.add_argument("--sweep-iters", type=int, default=50)
+    ap.add_argument("--oracle-table", default=None, help="time the fp64 oracle per operator on configs 1-5 (host cores, no GPU), write this .jsonl and exit")
     ap.add_argument("--no-sweep", action="store_true", help="leave the N_rhs sweep (key nrhs_sweep) out of the bench line")
     ap.add_argument("--inrun-sweep-iters", type=int, default=10, help="timed launches per point of the in-run N_rhs sweep")
     ap.add_argument("--sweep-ops", default="fine,coarse", help="which operator families the sweep covers")
@@ -706,6 +764,8 @@ def main():
         args.warmup = 3   # timing rule: at least 3 warm-up steps
     if args.impl == "reference":
         return run_reference(args)
+    if args.oracle_table:
+        return run_oracle_table(args)
     if args.sweep:
         return run_sweep(args)
     return run_gpu(args)
