@@ -64,7 +64,7 @@ typedef struct mrhs_transfer mrhs_transfer_t;   /* opaque: owns the repacked mul
 
 typedef enum {
     MRHS_OK = 0,
-    MRHS_ERR_INVALID_ARG = 1,   /* NULL pointer, odd or < 2 extent, bad parity, misalignment, aliasing */
+    MRHS_ERR_INVALID_ARG = 1,   /* NULL pointer, odd or < 2 extent, bad parity, misalignment, overlapping in and out buffers */
     MRHS_ERR_UNSUPPORTED = 2,   /* N_rhs or nbasis without a compiled specialisation */
     MRHS_ERR_ALLOC = 3,         /* device or host allocation failed */
     MRHS_ERR_CUDA = 4           /* a CUDA runtime call or kernel launch failed */

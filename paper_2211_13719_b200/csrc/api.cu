@@ -28,6 +28,11 @@ mrhs_status_t cuda_fail(cudaError_t e, const char *what, const char *file, int l
 }
 
 static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+// true if the byte ranges [a, a + na) and [b, b + nb) share a byte
+static bool overlap(const void *a, size_t na, const void *b, size_t nb) {
+    const uintptr_t x = reinterpret_cast<uintptr_t>(a), y = reinterpret_cast<uintptr_t>(b);
+    return x < y + nb && y < x + na;
+}
 
 }  // namespace mrhs
 
@@ -67,6 +72,9 @@ struct mrhs_wilson {
     void *st_tmp[2];               // odd-parity temporaries of the Schur sequence
     size_t st_tmp_bytes;
 };
+
+static size_t full_bytes(const mrhs_wilson *h) { return h ? mrhs_field_bytes(h->dims, 12, h->nrhs, 0) : 0; }
+static size_t cb_bytes(const mrhs_wilson *h) { return h ? mrhs_field_bytes(h->dims, 12, h->nrhs, 1) : 0; }
 
 struct mrhs_transfer {
     int coarse_level;        // 0: fine spinors (12 components, x-blocked layout) -> first coarse level; 1: coarse -> coarser
@@ -368,7 +376,7 @@ static mrhs_status_t hop_launch(mrhs_wilson_t *h, int parity, int dagger, const 
 
 static mrhs_status_t dhop_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int dagger) {
     MRHS_REQUIRE(h && d_in && d_out, "dhop: NULL argument");
-    MRHS_REQUIRE(d_in != d_out, "dhop: in and out must not alias");
+    MRHS_REQUIRE(!overlap(d_in, full_bytes(h), d_out, full_bytes(h)), "dhop: in and out must not overlap");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "dhop: buffers must be 16-byte aligned");
     return hop_launch(h, -1, dagger, nullptr, nullptr, d_in, d_out);
 }
@@ -378,7 +386,7 @@ mrhs_status_t mrhs_dhop_dag(mrhs_wilson_t *h, const void *d_in, void *d_out) { r
 static mrhs_status_t meooe_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity, int dagger) {
     MRHS_REQUIRE(h && d_in && d_out, "meooe: NULL argument");
     MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "meooe: out_parity must be 0 or 1");
-    MRHS_REQUIRE(d_in != d_out, "meooe: in and out must not alias");
+    MRHS_REQUIRE(!overlap(d_in, cb_bytes(h), d_out, cb_bytes(h)), "meooe: in and out must not overlap");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "meooe: buffers must be 16-byte aligned");
     return hop_launch(h, out_parity, dagger, nullptr, nullptr, d_in, d_out);
 }
@@ -387,7 +395,7 @@ mrhs_status_t mrhs_meooe_dag(mrhs_wilson_t *h, const void *d_in, void *d_out, in
 
 static mrhs_status_t wilson_apply_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int dagger) {
     MRHS_REQUIRE(h && d_in && d_out, "wilson apply: NULL argument");
-    MRHS_REQUIRE(d_in != d_out, "wilson apply: in and out must not alias");
+    MRHS_REQUIRE(!overlap(d_in, full_bytes(h), d_out, full_bytes(h)), "wilson apply: in and out must not overlap");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "wilson apply: buffers must be 16-byte aligned");
     // sweep kernel: one launch, C in(x) is formed from the centre slice in shared memory and the eight hops are added to it
     if (h->kern[0] == MRHS_HOP_SWEEP) return hop_launch(h, -1, dagger, h->clov_full, nullptr, d_in, d_out);
@@ -401,7 +409,8 @@ mrhs_status_t mrhs_wilson_apply_dag(mrhs_wilson_t *h, const void *d_in, void *d_
 mrhs_status_t mrhs_schur_apply(mrhs_wilson_t *h, const void *d_in, void *d_tmp, void *d_out, int dagger) {
     MRHS_REQUIRE(h && d_in && d_tmp && d_out, "schur apply: NULL argument");
     MRHS_REQUIRE(dagger == 0 || dagger == 1, "schur apply: dagger must be 0 or 1");
-    MRHS_REQUIRE(d_in != d_out && d_in != d_tmp && d_tmp != d_out, "schur apply: the three buffers must be distinct");
+    MRHS_REQUIRE(!overlap(d_in, cb_bytes(h), d_out, cb_bytes(h)) && !overlap(d_in, cb_bytes(h), d_tmp, cb_bytes(h)) && !overlap(d_tmp, cb_bytes(h), d_out, cb_bytes(h)),
+                 "schur apply: the three buffers must not overlap");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_tmp) && aligned16(d_out), "schur apply: buffers must be 16-byte aligned");
     // S = C_e - H_eo C_o^-1 H_oe / 4 (the daggered hops for S^+; the clover blocks are Hermitian)
     mrhs_status_t s = wilson_ensure(h, COPY_GAUGE_CB | COPY_CLOV_CB | COPY_CINV_CB);
@@ -425,7 +434,7 @@ mrhs_status_t mrhs_mooee_inv(mrhs_wilson_t *h, const void *d_in, void *d_out, in
 static mrhs_status_t mooee_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int parity, bool inverse) {
     MRHS_REQUIRE(h && d_in && d_out, "mooee: NULL argument");
     MRHS_REQUIRE(parity >= 0 && parity <= 2, "mooee: parity must be 0, 1 or 2");
-    MRHS_REQUIRE(d_in != d_out, "mooee: in and out must not alias");
+    MRHS_REQUIRE(!overlap(d_in, parity == MRHS_FULL ? full_bytes(h) : cb_bytes(h), d_out, parity == MRHS_FULL ? full_bytes(h) : cb_bytes(h)), "mooee: in and out must not overlap");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "mooee: buffers must be 16-byte aligned");
     const mrhs_status_t s = wilson_ensure(h, parity == MRHS_FULL ? (inverse ? COPY_CINV_FULL : 0u) : (inverse ? COPY_CINV_CB : COPY_CLOV_CB));
     if (s != MRHS_OK) return s;
@@ -439,7 +448,7 @@ mrhs_status_t mrhs_meooe_mooee_inv(mrhs_wilson_t *h, const void *d_in, void *d_o
 static mrhs_status_t meooe_mooee_impl(mrhs_wilson_t *h, const void *d_in, void *d_out, int out_parity, bool inverse) {
     MRHS_REQUIRE(h && d_in && d_out, "meooe_mooee: NULL argument");
     MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "meooe_mooee: out_parity must be 0 or 1");
-    MRHS_REQUIRE(d_in != d_out, "meooe_mooee: in and out must not alias");
+    MRHS_REQUIRE(!overlap(d_in, cb_bytes(h), d_out, cb_bytes(h)), "meooe_mooee: in and out must not overlap");
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "meooe_mooee: buffers must be 16-byte aligned");
     mrhs_status_t s = wilson_ensure(h, COPY_GAUGE_CB | (inverse ? COPY_CINV_CB : COPY_CLOV_CB));
     if (s != MRHS_OK) return s;
@@ -454,8 +463,12 @@ static mrhs_status_t meooe_mooee_impl(mrhs_wilson_t *h, const void *d_in, void *
 
 mrhs_status_t mrhs_schur_sequence(mrhs_wilson_t *h, const void *d_in, void *d_tmp0, void *d_tmp1, void *d_out) {
     MRHS_REQUIRE(h && d_in && d_tmp0 && d_tmp1 && d_out, "schur sequence: NULL argument");
-    MRHS_REQUIRE(d_in != d_out && d_tmp0 != d_tmp1 && d_in != d_tmp0 && d_in != d_tmp1 && d_out != d_tmp0 && d_out != d_tmp1,
-                 "schur sequence: the four buffers must be distinct");
+    {
+        const void *bufs[4] = {d_in, d_tmp0, d_tmp1, d_out};
+        for (int i = 0; i < 4; i++)
+            for (int j = i + 1; j < 4; j++)
+                MRHS_REQUIRE(!overlap(bufs[i], cb_bytes(h), bufs[j], cb_bytes(h)), "schur sequence: the four buffers must not overlap");
+    }
     mrhs_status_t s;
     if (h->kern[1] == MRHS_HOP_SWEEP) {
         // M_ooee rides in the epilogue of the first hop: two launches, d_tmp0 is not touched
@@ -678,7 +691,11 @@ mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nb
 
 mrhs_status_t mrhs_coarse_apply_points(mrhs_coarse_t *h, const void *d_in, void *d_out, int point_mask) {
     MRHS_REQUIRE(h && d_in && d_out, "coarse apply: NULL argument");
-    MRHS_REQUIRE(d_in != d_out, "coarse apply: in and out must not alias");
+    {
+        const int cd[4] = {h->g.X, h->g.Y, h->g.Z, h->g.T};
+        const size_t nb = mrhs_field_bytes(cd, h->g.nb, h->g.N, 0);
+        MRHS_REQUIRE(!overlap(d_in, nb, d_out, nb), "coarse apply: in and out must not overlap");
+    }
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "coarse apply: buffers must be 16-byte aligned");
     MRHS_REQUIRE(point_mask > 0 && point_mask <= 0x1FF, "coarse apply: point_mask must select at least one of the nine stencil points");
     const CoarseSites sites = coarse_sites_full(h->g);
@@ -690,6 +707,10 @@ mrhs_status_t mrhs_coarse_meooe(mrhs_coarse_t *h, const void *d_in, void *d_out,
     MRHS_REQUIRE(h && d_in && d_out, "coarse meooe: NULL argument");
     MRHS_REQUIRE(out_parity == 0 || out_parity == 1, "coarse meooe: out_parity must be 0 or 1");
     MRHS_REQUIRE(d_in != d_out, "coarse meooe: in and out must not alias");
+    {
+        const size_t nb = (size_t)h->g.nsites / 2 * h->g.nb * h->g.N * 8;
+        MRHS_REQUIRE(!overlap(d_in, nb, d_out, nb), "coarse meooe: in and out must not overlap");
+    }
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "coarse meooe: buffers must be 16-byte aligned");
     MRHS_REQUIRE(!((h->g.X | h->g.Y | h->g.Z | h->g.T) & 1), "coarse meooe: checkerboarded coarse fields need even extents");
     // the 8-point hopping term at the sites of one parity: same kernels, same link field, parity site map

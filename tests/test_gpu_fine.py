@@ -196,6 +196,16 @@ def test_argument_errors():
         w.mooee(f, w.empty(mrhs.FULL), 3)
     with pytest.raises(mrhs.MrhsError):
         w.dhop(f[1:], w.empty(mrhs.FULL))       # misaligned
+    # overlapping (not just identical) buffers are rejected: out starts inside in
+    big = torch.empty(2 * f.numel(), dtype=torch.float32, device=f.device)
+    with pytest.raises(mrhs.MrhsError) as e:
+        w.dhop(big[:f.numel()], big[f.numel() // 2: f.numel() // 2 + f.numel()])
+    assert e.value.status == mrhs.ERR_INVALID_ARG
+    half = w.empty(mrhs.EVEN).numel()
+    with pytest.raises(mrhs.MrhsError):
+        w.meooe(big[:half], big[half - 4: 2 * half - 4], mrhs.ODD)
+    w.dhop(big[:f.numel()], big[f.numel():])    # adjacent halves are fine
+    torch.cuda.synchronize()
     w.close()
 
 
