@@ -198,6 +198,16 @@ mrhs_status_t mrhs_wilson_get_sweep(mrhs_wilson_t *h, int which, int *lt, int ch
 
 mrhs_status_t mrhs_wilson_destroy(mrhs_wilson_t *h);
 
+/* Launch plan of the sweep kernel for a lattice, computed on the host (no device needed; what a handle on a device with
+ * num_sms multiprocessors would launch with its default settings).  parity: MRHS_FULL = D_hop, 0 / 1 = M_eooe with that
+ * output parity.  plan[0..8] = {thread blocks, threads per block, tiles (XB x 2 x 2 sites each), whole-line blocks,
+ * tail tiles, t-segments per tail tile, slices per whole block (lt), cy, cz}.  UNSUPPORTED if the sweep kernel cannot
+ * run the geometry (odd N_rhs, shared memory).  mrhs_sweep_blocks: the tile segments that blocks first .. first + count - 1
+ * of that plan sweep, coords[5 i ..] = {x-block, first y, first z, first t, slices}: the same index function the kernel
+ * evaluates. */
+mrhs_status_t mrhs_sweep_plan(const int dims[4], int nrhs, int parity, int num_sms, int plan[9]);
+mrhs_status_t mrhs_sweep_blocks(const int dims[4], int nrhs, int parity, int num_sms, int first, int count, int *coords);
+
 /* ---------------------------------------------------------------- coarse level */
 
 /* Coarse-level handle (reading S8; PAPER.md:61 nbasis, PAPER.md:75 coarse hopping).

@@ -55,6 +55,8 @@ _SIGNATURES = {
     "mrhs_wilson_set_sweep": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _int2]),
     "mrhs_wilson_get_sweep": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int), _int2]),
     "mrhs_wilson_destroy": (ctypes.c_int, [_vp]),
+    "mrhs_sweep_plan": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int * 9]),
+    "mrhs_sweep_blocks": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]),
     "mrhs_coarse_create": (ctypes.c_int, [ctypes.POINTER(_vp), _int4, ctypes.c_int, ctypes.c_int, _vp, ctypes.c_int, _vp]),
     "mrhs_coarse_apply": (ctypes.c_int, [_vp, _vp, _vp]),
     "mrhs_coarse_apply_points": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int]),
@@ -356,6 +358,20 @@ def wilson_apply_host_async(h, op, parity, h_in, h_out):
 
 def wilson_host_wait(h):
     _check(lib().mrhs_wilson_host_wait(h))
+
+
+def sweep_plan(dims, nrhs, parity, num_sms):
+    """Host-only: (blocks, threads, tiles, whole-line blocks, tail tiles, segments per tail tile, lt, cy, cz) of the sweep kernel."""
+    plan = (ctypes.c_int * 9)()
+    _check(lib().mrhs_sweep_plan(_dims(dims), int(nrhs), int(parity), int(num_sms), plan))
+    return list(plan)
+
+
+def sweep_blocks(dims, nrhs, parity, num_sms, first, count):
+    """Host-only: [(x-block, first y, first z, first t, slices)] of the tile segments blocks first .. first + count - 1 sweep."""
+    c = (ctypes.c_int * (5 * int(count)))()
+    _check(lib().mrhs_sweep_blocks(_dims(dims), int(nrhs), int(parity), int(num_sms), int(first), int(count), c))
+    return [tuple(c[5 * i:5 * i + 5]) for i in range(int(count))]
 
 
 def wilson_destroy(h):

@@ -595,6 +595,42 @@ mrhs_status_t mrhs_wilson_get_tiling(mrhs_wilson_t *h, int which, int tile[3], i
 
 mrhs_status_t mrhs_wilson_destroy(mrhs_wilson_t *h) { return wilson_free(h); }
 
+static mrhs_status_t sweep_plan_params(const int dims[4], int nrhs, int parity, int num_sms, SweepParams &p) {
+    MRHS_REQUIRE(dims, "sweep plan: NULL argument");
+    MRHS_REQUIRE(fine_dims_ok(dims), "sweep plan: extents must be even and >= 2");
+    MRHS_REQUIRE(nrhs >= 1 && nrhs <= 128, "sweep plan: nrhs must be 1..128");
+    MRHS_REQUIRE(parity >= 0 && parity <= 2, "sweep plan: parity must be 0, 1 or 2");
+    MRHS_REQUIRE(num_sms >= 1, "sweep plan: num_sms must be positive");
+    const FieldGeom g = make_geom(dims, 12, nrhs, parity);
+    if (!sweep_supported(g) || !build_sweep_params(g, parity == MRHS_FULL ? 0 : parity, default_sweep_tiling(g, num_sms), num_sms, p)) {
+        set_error("sweep plan: the slice-sweep kernel cannot run this geometry (even N_rhs, tile rows of at most 48 units)");
+        return MRHS_ERR_UNSUPPORTED;
+    }
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_sweep_plan(const int dims[4], int nrhs, int parity, int num_sms, int plan[9]) {
+    MRHS_REQUIRE(plan, "sweep plan: NULL argument");
+    SweepParams p;
+    mrhs_status_t s = sweep_plan_params(dims, nrhs, parity, num_sms, p);
+    if (s != MRHS_OK) return s;
+    const int tiles = p.nxb * (p.Y / kSweepBY) * (p.Z / kSweepBZ);
+    const int out[9] = {(int)p.grid, (int)p.threads, tiles, (int)p.n_whole, p.tail_tiles, p.tail_seg, p.lt, p.cy, p.cz};
+    for (int i = 0; i < 9; i++) plan[i] = out[i];
+    return MRHS_OK;
+}
+
+mrhs_status_t mrhs_sweep_blocks(const int dims[4], int nrhs, int parity, int num_sms, int first, int count, int *coords) {
+    MRHS_REQUIRE(coords, "sweep blocks: NULL argument");
+    SweepParams p;
+    mrhs_status_t s = sweep_plan_params(dims, nrhs, parity, num_sms, p);
+    if (s != MRHS_OK) return s;
+    MRHS_REQUIRE(first >= 0 && count >= 0 && (unsigned long long)first + (unsigned long long)count <= p.grid, "sweep blocks: block range out of the grid");
+    for (int i = 0; i < count; i++)
+        sweep_block_coords(p, (uint32_t)(first + i), coords[5 * i], coords[5 * i + 1], coords[5 * i + 2], coords[5 * i + 3], coords[5 * i + 4]);
+    return MRHS_OK;
+}
+
 mrhs_status_t mrhs_wilson_apply_host_async(mrhs_wilson_t *h, int op, int parity, const void *h_in, void *h_out) {
     MRHS_REQUIRE(h && h_in && h_out, "apply host: NULL argument");
     MRHS_REQUIRE(op >= 0 && op <= 3, "apply host: op must be 0 (D_hop), 1 (M_eooe), 2 (M_ooee) or 3 (Schur sequence)");

@@ -40,7 +40,7 @@ struct FastDiv {
 #ifdef __CUDA_ARCH__
         return div == 1 ? n : __umulhi(n, mul);
 #else
-        return n / div;
+        return div == 1 ? n : (uint32_t)(((uint64_t)n * mul) >> 32);     // the same multiply as on the device (host-side plan checks)
 #endif
     }
     // n -> (n / d, n % d)

@@ -204,24 +204,10 @@ hop_sweep_kernel(const SweepParams p, const float4 *__restrict__ in, float4 *__r
     const int tid = threadIdx.x, wid = tid >> 5, lane = tid & 31;
     const int Y = p.Y, Z = p.Z, T = p.T, nxb = p.nxb;
 
-    // block -> (x-block, tile, t-segment): x-blocks fastest, then the tiles of a chunk, then segments, then chunks.  The last
-    // p.tail_tiles tiles of that order are cut into p.tail_seg segments each (blocks n_whole, n_whole + 1, ...: the segments of a
-    // tile follow one another), so that the blocks of the last, partly filled wave are short ones (build_sweep_params)
-    uint32_t bi = blockIdx.x, tseg = 0;
-    int lt = p.lt;
-    if (bi >= p.n_whole) {
-        const uint32_t j = bi - p.n_whole, q = j / (uint32_t)p.tail_seg;
-        tseg = j - q * (uint32_t)p.tail_seg;
-        bi = p.n_whole + q;
-        lt = p.T / p.tail_seg;
-    }
-    uint32_t xb, yc, zc, seg, chy, chz, q0;
-    p.d_nxb.divmod(bi, q0, xb);
-    p.d_cy.divmod(q0, q0, yc);
-    p.d_cz.divmod(q0, q0, zc);
-    p.d_ntseg.divmod(q0, q0, seg);
-    p.d_ncy.divmod(q0, chz, chy);
-    const int y0 = (int)(chy * p.cy + yc) * BY, z0 = (int)(chz * p.cz + zc) * BZ, t0 = (int)(seg + tseg) * lt;
+    // block -> (x-block, tile, t-segment)
+    int xb_i, y0, z0, t0, lt;
+    sweep_block_coords(p, blockIdx.x, xb_i, y0, z0, t0, lt);
+    const uint32_t xb = (uint32_t)xb_i;
 
     if (tid == 0) {
         for (int i = 0; i < 2; i++) {

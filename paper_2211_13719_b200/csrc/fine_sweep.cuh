@@ -52,6 +52,31 @@ struct SweepParams {
     unsigned smem_bytes, smem_bytes_clover;   // dynamic shared memory without / with the clover blocks of the fused epilogues
 };
 
+// Thread block -> (x-block, first y, first z, first t, slices) of the tile segment it sweeps.  x-blocks fastest, then the tiles of a
+// chunk, then segments, then chunks; the last p.tail_tiles tiles of that order are cut into p.tail_seg segments each (blocks
+// n_whole, n_whole + 1, ...: the segments of a tile follow one another), so that the blocks of the last, partly filled wave are
+// short ones (build_sweep_params).  Shared by the kernel and the host-side plan check (mrhs_sweep_block).
+__host__ __device__ __forceinline__ void sweep_block_coords(const SweepParams &p, uint32_t block, int &xb, int &y0, int &z0, int &t0, int &lt) {
+    uint32_t bi = block, tseg = 0;
+    lt = p.lt;
+    if (bi >= p.n_whole) {
+        const uint32_t j = bi - p.n_whole, q = j / (uint32_t)p.tail_seg;
+        tseg = j - q * (uint32_t)p.tail_seg;
+        bi = p.n_whole + q;
+        lt = p.T / p.tail_seg;
+    }
+    uint32_t x, yc, zc, seg, chy, chz, q0;
+    p.d_nxb.divmod(bi, q0, x);
+    p.d_cy.divmod(q0, q0, yc);
+    p.d_cz.divmod(q0, q0, zc);
+    p.d_ntseg.divmod(q0, q0, seg);
+    p.d_ncy.divmod(q0, chz, chy);
+    xb = (int)x;
+    y0 = (int)(chy * p.cy + yc) * kSweepBY;
+    z0 = (int)(chz * p.cz + zc) * kSweepBZ;
+    t0 = (int)(seg + tseg) * lt;
+}
+
 // true if the sweep kernel can run this geometry (even N_rhs, shared memory fits)
 bool sweep_supported(const FieldGeom &g);
 SweepTiling default_sweep_tiling(const FieldGeom &g, int num_sms);
