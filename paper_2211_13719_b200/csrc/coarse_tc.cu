@@ -113,15 +113,25 @@ struct TcCfg {
     static constexpr int KS = NB / 8;                         // MMA K steps per stencil point
     static constexpr int THREADS = NT <= 64 ? 128 : 256;
     static constexpr int A_LBO = 2 * NB * 16;                 // bytes between K chunks of the A operand: only the 2 nb used rows are stored
-    static constexpr int B_LBO = NT * 16 + 16;                 // + 16: consecutive K chunks of the B operand start in different banks (operand stores of one warp span several chunks)
+    // Stacked B operand (2 NT <= 256 columns): the hi and lo parts of the vectors are the columns 0..NT-1 and NT..2NT-1 of ONE operand,
+    // so A_hi x [B_hi | B_lo] is one MMA of 2 NT columns and A_lo x B_hi a second one of NT columns on the same buffer: two
+    // instructions per K step instead of three (an MMA of this size costs a fixed ~77 cycles + ~0.6 per column);
+    // hi*hi and lo*hi land in accumulator columns 0..NT-1, hi*lo in NT..2NT-1, summed in the epilogue.
+    // Used where it measured faster (6^3x32: nb = 40, N = 12: 0.270 -> 0.252 ms): the doubled accumulator must not cost resident blocks
+    // (N = 24: 128 instead of 64 TMEM columns, N = 48: 256 instead of 128: 0.31 -> 0.52 and 0.43 -> 0.60 ms), and with the three K steps
+    // of nb = 24 there is nothing to gain (0.109 -> 0.113 ms).
+    static constexpr bool STK = NT <= 32 && NB >= 40;
+    static constexpr int B_ROWS = STK ? 2 * NT : NT;          // rows of one K chunk of the B operand
+    static constexpr int D_COLS = STK ? 2 * NT : NT;          // accumulator columns
+    static constexpr int B_LBO = B_ROWS * 16 + 16;                 // + 16: consecutive K chunks of the B operand start in different banks (operand stores of one warp span several chunks)
     static constexpr int A_BYTES = KC * A_LBO;                // one of hi / lo
-    static constexpr int B_BYTES = KC * B_LBO;
-    static constexpr int OPER_BYTES = 2 * A_BYTES + 2 * B_BYTES;
+    static constexpr int B_BYTES = KC * B_LBO;                // stacked: hi and lo together; else one of hi / lo
+    static constexpr int OPER_BYTES = 2 * A_BYTES + (STK ? 1 : 2) * B_BYTES;
     static constexpr int S_PITCH = 128 + (32 + NP - 1) / NP;  // epilogue scratch S[col][lane], floats; the combine reads NP columns x 32 / NP lanes per warp: distinct banks
     static constexpr int S_BYTES = NT * S_PITCH * 4;
     static constexpr int DATA_BYTES = OPER_BYTES > S_BYTES ? OPER_BYTES : S_BYTES;
     static constexpr int SMEM_BYTES = DATA_BYTES + 32;        // + mbarrier + TMEM address slot
-    static constexpr int TMEM_COLS = pow2_cols(NT);
+    static constexpr int TMEM_COLS = pow2_cols(D_COLS);
     static constexpr int A_UNITS = 2 * KC * NB;               // 16-byte units of one link matrix
     static constexpr int B_UNITS = KC * NP;                   // (K chunk, RHS pair) work items of one vector
     static_assert(NT <= 256, "MMA N limit");
@@ -139,7 +149,7 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
     constexpr int B_IT = (C::B_UNITS + C::THREADS - 1) / C::THREADS;
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char *a_hi = smem, *a_lo = smem + C::A_BYTES;
-    unsigned char *b_hi = smem + 2 * C::A_BYTES, *b_lo = b_hi + C::B_BYTES;
+    unsigned char *b_hi = smem + 2 * C::A_BYTES, *b_lo = b_hi + (C::STK ? C::NT * 16 : C::B_BYTES);     // stacked: the lo rows follow the hi rows inside every K chunk
     float *S = reinterpret_cast<float *>(smem);
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem + C::DATA_BYTES);
     uint32_t *tslot = reinterpret_cast<uint32_t *>(smem + C::DATA_BYTES + 8);
@@ -157,7 +167,7 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tslot;
-    constexpr uint32_t idesc = instr_desc_tf32(128, C::NT);
+    constexpr uint32_t idesc = instr_desc_tf32(128, C::NT), idesc2 = instr_desc_tf32(128, 2 * C::NT);
 
     uint32_t nstage = 0;   // operand stages handed to the tensor core so far (same in every thread)
     // raw fp32 operands of one stage (stencil point p of a site) in registers; loaded one stage ahead, right after
@@ -256,9 +266,14 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
                     const uint64_t dal = smem_desc(al + ks * 2 * C::A_LBO, C::A_LBO, 128);
                     const uint64_t dbh = smem_desc(bh + ks * 2 * C::B_LBO, C::B_LBO, 128);
                     const uint64_t dbl = smem_desc(bl + ks * 2 * C::B_LBO, C::B_LBO, 128);
-                    mma_tf32(tmem, dal, dbh, idesc, (sp | ks) != 0);
-                    mma_tf32(tmem, dah, dbl, idesc, 1);
-                    mma_tf32(tmem, dah, dbh, idesc, 1);
+                    if (C::STK) {
+                        mma_tf32(tmem, dah, dbh, idesc2, (sp | ks) != 0);     // hi x [hi | lo]
+                        mma_tf32(tmem, dal, dbh, idesc, 1);                    // lo x hi
+                    } else {
+                        mma_tf32(tmem, dal, dbh, idesc, (sp | ks) != 0);
+                        mma_tf32(tmem, dah, dbl, idesc, 1);
+                        mma_tf32(tmem, dah, dbh, idesc, 1);
+                    }
                 }
                 mma_commit(bar);
                 // L2 prefetch kPfAhead stages ahead (possibly into the next site of this block)
@@ -281,6 +296,12 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
             for (int ch = warp >> 2; ch < C::NT / 16; ch += C::THREADS / 128) {
                 float v[16];
                 tmem_ld16(tmem + ((uint32_t)(quarter * 32) << 16) + ch * 16, v);
+                if (C::STK) {       // the hi*lo part sits NT columns further
+                    float w[16];
+                    tmem_ld16(tmem + ((uint32_t)(quarter * 32) << 16) + C::NT + ch * 16, w);
+#pragma unroll
+                    for (int k = 0; k < 16; k++) v[k] += w[k];
+                }
 #pragma unroll
                 for (int k = 0; k < 16; k++) S[(ch * 16 + k) * C::S_PITCH + quarter * 32 + lane] = v[k];
             }
@@ -290,11 +311,12 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
         for (int idx = tid; idx < NB * C::NP; idx += C::THREADS) {
             const int i = idx / C::NP, q = idx - i * C::NP;
             const int n0 = q, n1 = C::NP + q;   // column order of D: Re even RHS | Re odd RHS | Im even | Im odd (conflict-free operand stores)
+            auto d = [&](int col, int row) { return S[col * C::S_PITCH + row]; };
             float4 o;
-            o.x = S[n0 * C::S_PITCH + i] - S[(N + n0) * C::S_PITCH + NB + i];
-            o.y = S[n1 * C::S_PITCH + i] - S[(N + n1) * C::S_PITCH + NB + i];
-            o.z = S[(N + n0) * C::S_PITCH + i] + S[n0 * C::S_PITCH + NB + i];
-            o.w = S[(N + n1) * C::S_PITCH + i] + S[n1 * C::S_PITCH + NB + i];
+            o.x = d(n0, i) - d(N + n0, NB + i);
+            o.y = d(n1, i) - d(N + n1, NB + i);
+            o.z = d(N + n0, i) + d(n0, NB + i);
+            o.w = d(N + n1, i) + d(n1, NB + i);
             out[((size_t)site * NB + i) * C::NP + q] = o;
         }
         __syncthreads();   // S (aliasing the operand buffer) is free for the next site
