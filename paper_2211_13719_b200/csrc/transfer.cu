@@ -4,6 +4,8 @@
 #include "transfer.cuh"
 #include "async_copy.cuh"
 
+#include <cooperative_groups.h>
+
 namespace mrhs {
 
 namespace {
@@ -515,18 +517,22 @@ prolong_coarse_kernel(CoarseTransferGeom g, int NP, int items, long long nthread
     for (int l = 0; l < TP; l++) { po[l] = from_cvec(acc[0][l]); po[NP + l] = from_cvec(acc[1][l]); }
 }
 
-// One thread block = one aggregate; a thread owns one (site slice, chirality, KT basis vectors, LT RHS lanes) and sums its slice of
-// the aggregate's sites over the nf / 2 components of its chirality; slices are added through shared memory in a fixed order.
+// One thread block cluster of G blocks = one aggregate (a coarse level has few aggregates: 128 at 6^3x32 / 3x3x3x2, fewer than SMs);
+// a thread owns one (site slice, chirality, KT basis vectors, LT RHS lanes) and sums its slice of the aggregate's sites over the
+// nf / 2 components of its chirality; the slices of a block are added through shared memory, the blocks of the cluster through
+// distributed shared memory by block 0, both in a fixed order (bit-reproducible).
 template <int R, int KT, int LT>
 __global__ void __launch_bounds__(256)
-restrict_coarse_kernel(CoarseTransferGeom g, int NP, int S, const float2 *__restrict__ basis,
+restrict_coarse_kernel(CoarseTransferGeom g, int NP, int S, int G, const float2 *__restrict__ basis,
                        const typename Elem<R>::type *__restrict__ fine, typename Elem<R>::type *__restrict__ coarse) {
     typedef typename Elem<R>::type E;
     extern __shared__ __align__(16) unsigned char sm[];
-    E *red = reinterpret_cast<E *>(sm);                                   // [S-1][items][KT LT]
     const int nagg = g.bx * g.by * g.bz * g.bt, h = g.nf / 2;
     const int kgs = g.nvec / KT, lgs = NP / LT, items = 2 * kgs * lgs;
-    const long long B = blockIdx.x;
+    E *part = reinterpret_cast<E *>(sm);                                  // [items][KT LT]: this block's sums, read by block 0 of the cluster
+    E *red = part + (size_t)items * KT * LT;                              // [S-1][items][KT LT]
+    const long long B = blockIdx.x / G;
+    const int crank = (int)(blockIdx.x - B * G);                          // rank in the cluster: blocks B G .. B G + G - 1
     const int c0x = (int)(B % g.cX) * g.bx, c0y = (int)((B / g.cX) % g.cY) * g.by, c0z = (int)((B / ((long long)g.cX * g.cY)) % g.cZ) * g.bz;
     const int c0t = (int)(B / ((long long)g.cX * g.cY * g.cZ)) * g.bt;
     const int tid = threadIdx.x, s = tid / items, item = tid - s * items;
@@ -538,7 +544,7 @@ restrict_coarse_kernel(CoarseTransferGeom g, int NP, int S, const float2 *__rest
 #pragma unroll
         for (int l = 0; l < LT; l++) acc[kk][l] = czero_t<R>();
     if (active) {
-        for (int i = s; i < nagg; i += S) {
+        for (int i = crank * S + s; i < nagg; i += S * G) {
             int q = i;
             const int ix = q % g.bx; q /= g.bx;
             const int iy = q % g.by; q /= g.by;
@@ -577,6 +583,29 @@ restrict_coarse_kernel(CoarseTransferGeom g, int NP, int S, const float2 *__rest
 #pragma unroll
                 for (int l = 0; l < LT; l++) acc[kk][l] = cadd(acc[kk][l], to_cvec(rp[kk * LT + l]));
         }
+        if (G > 1) {
+#pragma unroll
+            for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+                for (int l = 0; l < LT; l++) part[(size_t)item * KT * LT + kk * LT + l] = from_cvec(acc[kk][l]);
+        }
+    }
+    if (G > 1) {
+        namespace cg = cooperative_groups;
+        cg::cluster_group cluster = cg::this_cluster();
+        cluster.sync();                                    // every block of the cluster has written its sums
+        if (crank == 0 && active && s == 0) {
+            for (int r = 1; r < G; r++) {
+                const E *rp = cluster.map_shared_rank(part, r) + (size_t)item * KT * LT;
+#pragma unroll
+                for (int kk = 0; kk < KT; kk++)
+#pragma unroll
+                    for (int l = 0; l < LT; l++) acc[kk][l] = cadd(acc[kk][l], to_cvec(rp[kk * LT + l]));
+            }
+        }
+        cluster.sync();                                    // block 0 has read them: the other blocks may exit
+    }
+    if (crank == 0 && active && s == 0) {
         E *po = coarse + ((size_t)B * 2 * g.nvec + (size_t)chi * g.nvec + k0) * NP + lane;
 #pragma unroll
         for (int kk = 0; kk < KT; kk++)
@@ -746,9 +775,22 @@ mrhs_status_t launch_restrict_coarse(const CoarseTransferGeom &g, const float2 *
     if (S > nagg) S = nagg;
     const int threads = S * items;
     const int esz = (g.N & 1) ? 8 : 16;
-    const size_t smem = (size_t)(S - 1) * items * kt * lt * esz;
+    // blocks per aggregate (one cluster): enough to give every SM work when the coarse lattice has few aggregates
+    int G = 1;
+    while (G < 8 && nagg >= 2 * G * S && g.ncoarse * G < 1024) G *= 2;
+    const size_t smem = (size_t)S * items * kt * lt * esz;
     if (smem > 48 * 1024) { set_error("restrict (coarse level): %zu bytes of shared memory needed (max 48 KB)", smem); return MRHS_ERR_UNSUPPORTED; }
-#define MRHS_RC(RR, KT, LT, ET) restrict_coarse_kernel<RR, KT, LT><<<(unsigned)g.ncoarse, threads, smem, st>>>(g, np, S, d_basis, (const ET *)d_fine, (ET *)d_coarse)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(g.ncoarse * G));
+    cfg.blockDim = dim3((unsigned)threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)G; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+#define MRHS_RC(RR, KT, LT, ET) MRHS_CUDA(cudaLaunchKernelEx(&cfg, restrict_coarse_kernel<RR, KT, LT>, g, np, S, G, d_basis, (const ET *)d_fine, (ET *)d_coarse))
 #define MRHS_RC_LT(RR, KT, ET) do { if (lt == 3) MRHS_RC(RR, KT, 3, ET); else if (lt == 2) MRHS_RC(RR, KT, 2, ET); else MRHS_RC(RR, KT, 1, ET); } while (0)
     if (g.N & 1) { if (kt == 2) MRHS_RC_LT(1, 2, float2); else MRHS_RC_LT(1, 1, float2); }
     else         { if (kt == 2) MRHS_RC_LT(2, 2, float4); else MRHS_RC_LT(2, 1, float4); }
