@@ -14,6 +14,7 @@ N_rhs = 12):
     Schur sequence M_eooe, M_ooee, M_eooe                  row a7 (M_ooee fused into the first hop: 2 launches)
     coarse 9-point apply, FP32 FMA                         row a5
     coarse 9-point apply, tensor cores (3xTF32, tcgen05)    row a6
+    coarse 9-point apply, tensor cores (fp16 hi + lo split, kind::f16; column-maximum and split passes included)  row a6
 
 All fields are resident in HBM in the library's native layout when the timed region starts; the
 working set of every launch (>= 0.85 GB) is far larger than the 126 MB L2, so no flush is needed
@@ -100,6 +101,7 @@ def step_work(fdims, cdims, nb, N, schur_fused=True):
         ("schur_meooe_eo", hop_f, hop_b),
         ("coarse_fma", coarse_flops(nb) * Vc * N, bytes_coarse(Vc, nb, N)),
         ("coarse_tc", coarse_flops(nb) * Vc * N, bytes_coarse(Vc, nb, N)),
+        ("coarse_tc_f16", coarse_flops(nb) * Vc * N, bytes_coarse(Vc, nb, N)),
     ]
 
 
@@ -201,7 +203,8 @@ def oracle_step(s):
     t = oracle.meooe(s["fd"], s["U"], s["pe"], 1)
     t = oracle.mooee(s["Co"], t)
     oracle.meooe(s["fd"], s["U"], t, 0)
-    oracle.coarse_apply(s["cd"], s["A"], s["v"])
+    for _ in range(3):      # the GPU step applies the coarse operator once per math mode (FP32 FMA, tf32 split, fp16 split)
+        oracle.coarse_apply(s["cd"], s["A"], s["v"])
 
 
 def time_oracle(steps, warmup):
@@ -294,6 +297,7 @@ class Workload:
         torch.cuda.synchronize()
         self.c = mrhs.Coarse(cdims, nb, N, A, stream=stream)
         self.c_tc = mrhs.Coarse(cdims, nb, N, A, math_mode=mrhs.COARSE_TENSOR, stream=stream)
+        self.c_h16 = mrhs.Coarse(cdims, nb, N, A, math_mode=mrhs.COARSE_TENSOR_F16, stream=stream)
         del A
         v = syn.spinor_torch(vol(cdims), N, 4, device, ncomp=(nb,))
         self.v = self.c.import_field(v)
@@ -310,6 +314,7 @@ class Workload:
             ("schur", lambda: w.schur_sequence(self.in_e, self.t0, self.t1, self.out_e)),
             ("coarse_fma", lambda: c.apply(self.v, self.v_out)),
             ("coarse_tc", lambda: self.c_tc.apply(self.v, self.v_out)),
+            ("coarse_tc_f16", lambda: self.c_h16.apply(self.v, self.v_out)),
         ]
 
 
@@ -449,7 +454,8 @@ def run_gpu(args):
         "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": cfg, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
-        "gpu_launches": (len(work) - (1 if fused else 0)) * K, "kernels": kernels, "wall_ms_per_step": t_wall * 1e3 / K,
+        # + 2: the column-maximum and split passes of the fp16-split coarse apply
+        "gpu_launches": (len(work) - (1 if fused else 0) + 2) * K, "kernels": kernels, "wall_ms_per_step": t_wall * 1e3 / K,
         "nrhs_sweep": nrhs_sweep,
     }
     print(json.dumps(line))
@@ -486,9 +492,10 @@ def run_e2e(torch, mrhs, wl, args, barrier, dist, device, world, flops_step):
     h_half_out = [torch.empty(half_shape, dtype=torch.complex64).pin_memory() for _ in range(3)]
     h_v_in = torch.empty((vol(cdims), nb, N), dtype=torch.complex64).pin_memory()
     h_v_in.copy_(wl.c.export_field(wl.v))
-    h_v_out = torch.empty_like(h_v_in).pin_memory()
+    h_v_out = [torch.empty_like(h_v_in).pin_memory() for _ in range(3)]
     torch.cuda.synchronize()
-    w, c = wl.w.h, wl.c.h
+    w = wl.w.h
+    coarse = (wl.c.h, wl.c_tc.h, wl.c_h16.h)     # one coarse apply per math mode, as in the device-timed step
 
     def step():
         # the asynchronous host entries: every call's host->device copy, kernels and device->host copy are enqueued, the copy-in
@@ -498,13 +505,15 @@ def run_e2e(torch, mrhs, wl, args, barrier, dist, device, world, flops_step):
         mrhs.wilson_apply_host_async(w, mrhs.OP_MEOOE, mrhs.EVEN, h_o_in, h_half_out[1])
         mrhs.wilson_apply_host_async(w, mrhs.OP_MOOEE, mrhs.FULL, h_full_in, h_full_out[1])
         mrhs.wilson_apply_host_async(w, mrhs.OP_SCHUR, 0, h_e_in, h_half_out[2])
-        mrhs.coarse_apply_host_async(c, h_v_in, h_v_out)
+        for c, o in zip(coarse, h_v_out):
+            mrhs.coarse_apply_host_async(c, h_v_in, o)
         mrhs.wilson_host_wait(w)
-        mrhs.coarse_host_wait(c)
+        for c in coarse:
+            mrhs.coarse_host_wait(c)
 
     fb, hb, cb = h_full_in.numel() * 8, h_e_in.numel() * 8, h_v_in.numel() * 8
-    h2d = 2 * fb + 3 * hb + cb
-    d2h = 2 * fb + 3 * hb + cb
+    h2d = 2 * fb + 3 * hb + 3 * cb
+    d2h = 2 * fb + 3 * hb + 3 * cb
     E = max(1, min(args.steps, args.e2e_steps))
     step()   # warm-up: allocates the handle's staging buffers
     barrier()

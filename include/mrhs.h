@@ -214,7 +214,13 @@ mrhs_status_t mrhs_sweep_blocks(const int dims[4], int nrhs, int parity, int num
  *   cdims: coarse lattice extents (>= 2; need not be even), nbasis in {24, 40},
  *   nrhs in {1,2,4,8,12,16,24,32,48,64,96};
  *   d_links: device, canonical A[lex][9][nb][nb];
- *   math_mode: 0 = FP32 FMA, 1 = tensor-core split precision (same tolerance). */
+ *   math_mode: 0 = FP32 FMA; 1 = tensor cores, tf32 split precision (three kind::tf32 MMAs per K step on hi / lo parts made in
+ *   the kernel); 2 = tensor cores, fp16 split precision (kind::f16 on hi + lo fp16 parts after an exact power-of-two scaling:
+ *   the link field is split once here, one scale per site, and keeps its size; every apply first splits its input vector into
+ *   a scratch image owned by the handle (2 nbasis (2 N_rhs rounded up to 16) fp16 per site), one scale per right-hand side
+ *   taken from that RHS's largest magnitude over the field).  Modes 1 and 2 need even nrhs and are held to the same 1e-5
+ *   tolerance per RHS (reading S15); in mode 2 an element smaller than 2^-17 of the largest element of its RHS (or, for the
+ *   links, of its site) carries an absolute error of 2^-40 of that largest element instead of a relative one. */
 mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nbasis, int nrhs,
                                  const void *d_links, int math_mode, void *cuda_stream);
 

@@ -22,10 +22,10 @@ _lib = None
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA = 0, 1, 2, 3, 4
 EVEN, ODD, FULL = 0, 1, 2
 OP_DHOP, OP_MEOOE, OP_MOOEE, OP_SCHUR = 0, 1, 2, 3
-COARSE_FMA, COARSE_TENSOR = 0, 1
+COARSE_FMA, COARSE_TENSOR, COARSE_TENSOR_F16 = 0, 1, 2
 HOP_GATHER, HOP_SWEEP = 0, 1
 COARSE_SELF, COARSE_HOP, COARSE_ALL = 0x001, 0x1FE, 0x1FF
-COARSE_MODES = (COARSE_FMA, COARSE_TENSOR)
+COARSE_MODES = (COARSE_FMA, COARSE_TENSOR, COARSE_TENSOR_F16)
 
 _vp = ctypes.c_void_p
 _int4 = ctypes.c_int * 4

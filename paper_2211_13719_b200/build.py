@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmrhs.so")
-SOURCES = ["api.cu", "layout.cu", "fine_hop.cu", "fine_sweep.cu", "clover.cu", "coarse.cu", "coarse_tc.cu", "blas.cu", "transfer.cu"]
+SOURCES = ["api.cu", "layout.cu", "fine_hop.cu", "fine_sweep.cu", "clover.cu", "coarse.cu", "coarse_tc.cu", "coarse_h16.cu", "blas.cu", "transfer.cu"]
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

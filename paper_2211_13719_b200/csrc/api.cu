@@ -88,8 +88,10 @@ struct mrhs_coarse {
     CoarseGeom g;
     int mode;
     cudaStream_t st;
-    float2 *links;                 // math_mode 0: [site][p][col][row] complex; math_mode 1: the tensor-core order (coarse.cuh)
-    int tc_grid;                   // persistent grid of the tensor-core kernel
+    float2 *links;                 // math_mode 0: [site][p][col][row] complex; math_mode 1 / 2: the tensor-core orders (coarse.cuh)
+    int tc_grid;                   // persistent grid of the tensor-core kernels
+    float *site_scale;             // math_mode 2: 1 / scale of the site's matrices, then 128 floats for the column maxima of an apply
+    void *vec16;                   // math_mode 2: the split input vector of an apply
     HostPipe pipe;
 };
 
@@ -687,13 +689,14 @@ mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nb
     MRHS_REQUIRE(cdims && d_links, "coarse create: NULL argument");
     for (int i = 0; i < 4; i++) MRHS_REQUIRE(cdims[i] >= 2, "coarse create: extents must be >= 2");
     MRHS_REQUIRE(nbasis >= 1 && nrhs >= 1, "coarse create: nbasis and nrhs must be positive");
-    MRHS_REQUIRE(math_mode == 0 || math_mode == 1, "coarse create: math_mode must be 0 or 1");
+    MRHS_REQUIRE(math_mode >= 0 && math_mode <= 2, "coarse create: math_mode must be 0, 1 or 2");
+    MRHS_REQUIRE((long long)cdims[0] * cdims[1] * cdims[2] * cdims[3] < (1ll << 30), "coarse create: more than 2^30 coarse sites");
     MRHS_REQUIRE(aligned16(d_links), "coarse create: links must be 16-byte aligned");
     if (!coarse_fma_supported(nbasis, nrhs)) {
         set_error("coarse create: no specialisation for nbasis=%d nrhs=%d (nbasis 24|40, nrhs 1,2,4,8,12,16,24,32,48,64,96)", nbasis, nrhs);
         return MRHS_ERR_UNSUPPORTED;
     }
-    if (math_mode == 1 && !coarse_tc_supported(nbasis, nrhs)) {
+    if ((math_mode == 1 && !coarse_tc_supported(nbasis, nrhs)) || (math_mode == 2 && !coarse_h16_supported(nbasis, nrhs))) {
         set_error("coarse create: no tensor-core specialisation for nbasis=%d nrhs=%d (nbasis 24|40, even nrhs in 2,4,8,12,16,24,32,48,64,96)", nbasis, nrhs);
         return MRHS_ERR_UNSUPPORTED;
     }
@@ -709,7 +712,13 @@ mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nb
     cudaError_t e = cudaMalloc(&h->links, bytes);
     if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaMalloc(links)", __FILE__, __LINE__); }
     mrhs_status_t s;
-    if (math_mode == 1) {
+    if (math_mode == 2) {
+        e = cudaMalloc(&h->site_scale, ((size_t)h->g.nsites + 128) * sizeof(float));
+        if (e == cudaSuccess) e = cudaMalloc(&h->vec16, coarse_h16_vec_bytes(h->g));
+        if (e != cudaSuccess) { cudaFree(h->site_scale); cudaFree(h->links); delete h; return cuda_fail(e, "cudaMalloc(split operands)", __FILE__, __LINE__); }
+        s = pack_coarse_links_h16(h->g, (const float2 *)d_links, h->links, h->site_scale, h->st);
+        if (s == MRHS_OK) s = coarse_h16_prepare(h->g, &h->tc_grid);
+    } else if (math_mode == 1) {
         s = pack_coarse_links_tc(h->g, (const float2 *)d_links, (float *)h->links, h->st);
         if (s == MRHS_OK) s = coarse_tc_prepare(h->g, &h->tc_grid);
     } else {
@@ -720,7 +729,7 @@ mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nb
         e = cudaStreamSynchronize(h->st);
         if (e != cudaSuccess) s = cuda_fail(e, "cudaStreamSynchronize", __FILE__, __LINE__);
     }
-    if (s != MRHS_OK) { cudaFree(h->links); delete h; return s; }
+    if (s != MRHS_OK) { cudaFree(h->links); cudaFree(h->site_scale); cudaFree(h->vec16); delete h; return s; }
     *out = h;
     return MRHS_OK;
 }
@@ -735,6 +744,8 @@ mrhs_status_t mrhs_coarse_apply_points(mrhs_coarse_t *h, const void *d_in, void 
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "coarse apply: buffers must be 16-byte aligned");
     MRHS_REQUIRE(point_mask > 0 && point_mask <= 0x1FF, "coarse apply: point_mask must select at least one of the nine stencil points");
     const CoarseSites sites = coarse_sites_full(h->g);
+    if (h->mode == 2)
+        return launch_coarse_h16(h->g, sites, h->tc_grid, (unsigned)point_mask, h->links, h->site_scale, d_in, h->vec16, h->site_scale + h->g.nsites, d_out, h->st);
     if (h->mode == 1) return launch_coarse_tc(h->g, sites, h->tc_grid, (unsigned)point_mask, (const float *)h->links, d_in, d_out, h->st);
     return launch_coarse_fma(h->g, sites, (unsigned)point_mask, h->links, d_in, d_out, h->st);
 }
@@ -751,6 +762,8 @@ mrhs_status_t mrhs_coarse_meooe(mrhs_coarse_t *h, const void *d_in, void *d_out,
     MRHS_REQUIRE(!((h->g.X | h->g.Y | h->g.Z | h->g.T) & 1), "coarse meooe: checkerboarded coarse fields need even extents");
     // the 8-point hopping term at the sites of one parity: same kernels, same link field, parity site map
     const CoarseSites sites = coarse_sites_parity(h->g, out_parity);
+    if (h->mode == 2)
+        return launch_coarse_h16(h->g, sites, h->tc_grid, MRHS_COARSE_HOP, h->links, h->site_scale, d_in, h->vec16, h->site_scale + h->g.nsites, d_out, h->st);
     if (h->mode == 1) return launch_coarse_tc(h->g, sites, h->tc_grid, MRHS_COARSE_HOP, (const float *)h->links, d_in, d_out, h->st);
     return launch_coarse_fma(h->g, sites, MRHS_COARSE_HOP, h->links, d_in, d_out, h->st);
 }
@@ -762,6 +775,8 @@ mrhs_status_t mrhs_coarse_apply(mrhs_coarse_t *h, const void *d_in, void *d_out)
 mrhs_status_t mrhs_coarse_destroy(mrhs_coarse_t *h) {
     if (!h) return MRHS_OK;
     cudaFree(h->links);
+    cudaFree(h->site_scale);
+    cudaFree(h->vec16);
     pipe_free(h->pipe);
     delete h;
     return MRHS_OK;

@@ -80,10 +80,11 @@ coarse_fma_kernel(const CoarseSites sites, unsigned mask, const float2 *__restri
     const int ks = tid / C::GROUPS;
 
     const long long osite = blockIdx.x;                       // output site; its links live at lex
-    const long long site = coarse_site_lex(sites, osite);
+    const CoarseSite32 sc = coarse_site32(sites, osite);
+    const long long site = sc.lex;
     // vector index of the neighbour at stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t
     auto neighbour = [&](int p) -> long long {
-        const long long n = coarse_neighbour_lex(sites, site, p);
+        const int n = coarse_neighbour32(sites, sc, p);
         return sites.cb ? n >> 1 : n;
     };
     // the stencil points of this apply: bit p of mask (all nine for the full operator, bit 0 = self term alone,

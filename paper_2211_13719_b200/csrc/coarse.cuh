@@ -46,6 +46,30 @@ __device__ __forceinline__ long long coarse_neighbour_lex(const CoarseSites &g, 
     else c3 = (c3 + d + g.T) % g.T;
     return c0 + (long long)g.X * (c1 + (long long)g.Y * (c2 + (long long)g.Z * c3));
 }
+// The same two maps in 32-bit arithmetic without a division per neighbour (coarse lattices have fewer than 2^31 sites; checked at
+// create): the kernels evaluate them per stencil point on the thread that issues the copies, where the 64-bit divisions of the
+// functions above cost more than the copy itself.
+struct CoarseSite32 { int lex, x, y, z, t; };
+__device__ __forceinline__ CoarseSite32 coarse_site32(const CoarseSites &g, long long idx) {
+    CoarseSite32 c;
+    unsigned s = g.cb ? 2u * (unsigned)idx : (unsigned)idx;
+    c.lex = (int)s;
+    c.x = (int)(s % (unsigned)g.X); s /= (unsigned)g.X;
+    c.y = (int)(s % (unsigned)g.Y); s /= (unsigned)g.Y;
+    c.z = (int)(s % (unsigned)g.Z);
+    c.t = (int)(s / (unsigned)g.Z);
+    if (g.cb && (((c.x + c.y + c.z + c.t) & 1) != g.parity)) { c.lex += 1; c.x += 1; }   // the pair (2 idx, 2 idx + 1) differs in x only (X even)
+    return c;
+}
+__device__ __forceinline__ int coarse_neighbour32(const CoarseSites &g, const CoarseSite32 &c, int p) {
+    if (p == 0) return c.lex;
+    const int mu = (p - 1) & 3;
+    const int coord = mu == 0 ? c.x : mu == 1 ? c.y : mu == 2 ? c.z : c.t;
+    const int ext = mu == 0 ? g.X : mu == 1 ? g.Y : mu == 2 ? g.Z : g.T;
+    const int stride = mu == 0 ? 1 : mu == 1 ? g.X : mu == 2 ? g.X * g.Y : g.X * g.Y * g.Z;
+    const int d = p <= 4 ? (coord + 1 == ext ? -(ext - 1) : 1) : (coord == 0 ? ext - 1 : -1);
+    return c.lex + d * stride;
+}
 #endif
 inline CoarseSites coarse_sites_full(const CoarseGeom &g) { return {g.X, g.Y, g.Z, g.T, 0, 0, g.nsites}; }
 inline CoarseSites coarse_sites_parity(const CoarseGeom &g, int parity) { return {g.X, g.Y, g.Z, g.T, 1, parity, g.nsites / 2}; }
@@ -69,5 +93,15 @@ mrhs_status_t pack_coarse_links_tc(const CoarseGeom &g, const float2 *d_canonica
 // opt in to large dynamic shared memory and size the persistent grid (CTAs per SM limited by shared memory and TMEM)
 mrhs_status_t coarse_tc_prepare(const CoarseGeom &g, int *grid);
 mrhs_status_t launch_coarse_tc(const CoarseGeom &g, const CoarseSites &sites, int grid, unsigned mask, const float *d_links, const void *d_in, void *d_out, cudaStream_t st);
+
+// ---- tensor-core variant 2 (row a6, math_mode 2): tcgen05 kind::f16 on operands split into fp16 hi + lo after a power-of-two
+// scaling (coarse_h16.cu).  The links are split at create time (same bytes as fp32) with one scale per site; the input vector is
+// split per apply into a scratch image of coarse_h16_vec_bytes() bytes, with one scale per right-hand side (d_colmax: 128 floats).
+bool coarse_h16_supported(int nb, int nrhs);
+size_t coarse_h16_vec_bytes(const CoarseGeom &g);
+mrhs_status_t pack_coarse_links_h16(const CoarseGeom &g, const float2 *d_canonical, void *d_links16, float *d_site_scale, cudaStream_t st);
+mrhs_status_t coarse_h16_prepare(const CoarseGeom &g, int *grid);
+mrhs_status_t launch_coarse_h16(const CoarseGeom &g, const CoarseSites &sites, int grid, unsigned mask, const void *d_links16, const float *d_site_scale,
+                                const void *d_in, void *d_vec16, float *d_colmax, void *d_out, cudaStream_t st);
 
 }  // namespace mrhs

@@ -176,21 +176,19 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
     float4 rb[B_IT][4];
     const long long nsites = sites.nout;       // output sites, enumerated by osite; the links of output site osite live at its lex
     // vector index of the neighbour at stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
-    auto neighbour = [&](long long lex, int p) -> long long {
-        const long long n = coarse_neighbour_lex(sites, lex, p);
+    auto neighbour = [&](const CoarseSite32 &c, int p) -> long long {
+        const int n = coarse_neighbour32(sites, c, p);
         return sites.cb ? n >> 1 : n;
     };
     // one thread asks the copy engine to bring a later stage's matrix and neighbour vector into L2 (each is one
     // contiguous block), so that the register loads of that stage find them there
-    auto prefetch_stage = [&](long long osite, int p) {
-        const long long site = coarse_site_lex(sites, osite);
-        bulk_prefetch_l2(links + ((size_t)site * 9 + p) * C::A_UNITS, C::A_UNITS * 16);
-        bulk_prefetch_l2(in + (size_t)neighbour(site, p) * NB * C::NP, NB * C::NP * 16);
+    auto prefetch_stage = [&](const CoarseSite32 &c, int p) {
+        bulk_prefetch_l2(links + ((size_t)c.lex * 9 + p) * C::A_UNITS, C::A_UNITS * 16);
+        bulk_prefetch_l2(in + (size_t)neighbour(c, p) * NB * C::NP, NB * C::NP * 16);
     };
-    auto load_stage = [&](long long osite, int p) {
-        const long long site = coarse_site_lex(sites, osite);
-        const float4 *lp = links + ((size_t)site * 9 + p) * C::A_UNITS;
-        const float4 *vp = in + (size_t)neighbour(site, p) * NB * C::NP;
+    auto load_stage = [&](const CoarseSite32 &c, int p) {
+        const float4 *lp = links + ((size_t)c.lex * 9 + p) * C::A_UNITS;
+        const float4 *vp = in + (size_t)neighbour(c, p) * NB * C::NP;
 #pragma unroll
         for (int it = 0; it < A_IT; it++) {
             const int u = tid + it * C::THREADS;
@@ -213,11 +211,14 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
     // the stencil points of this apply: bit p of mask; stage s of a site handles the s-th set bit
     const int npts = ALL ? 9 : __popc(mask);
     auto point = [&](int s) { return ALL ? s : (int)__fns(mask, 0, s + 1); };
-    if (AHEAD && (long long)blockIdx.x < nsites) load_stage(blockIdx.x, point(0));
+    // site coordinates once per site (this site and the block's next one), neighbours from them without divisions
+    CoarseSite32 cur = coarse_site32(sites, blockIdx.x), nxt = cur;
+    if (AHEAD && (long long)blockIdx.x < nsites) load_stage(cur, point(0));
     for (long long site = blockIdx.x; site < nsites; site += gridDim.x) {
+        if (site + gridDim.x < nsites) nxt = coarse_site32(sites, site + gridDim.x);
         for (int sp = 0; sp < npts; sp++) {
             const int p = point(sp);
-            if (!AHEAD) load_stage(site, p);
+            if (!AHEAD) load_stage(cur, p);
             // the single operand buffer is free once the previous stage's MMAs have completed
             if (nstage > 0) mbar_wait(bar, (nstage - 1) & 1);
 #pragma unroll
@@ -280,12 +281,13 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
                 int sp2 = sp + kPfAhead;
                 long long site2 = site;
                 while (sp2 >= npts) { sp2 -= npts; site2 += gridDim.x; }
-                if (site2 < nsites) prefetch_stage(site2, point(sp2));
+                if (site2 == site) prefetch_stage(cur, point(sp2));
+                else if (site2 == site + gridDim.x && site2 < nsites) prefetch_stage(nxt, point(sp2));
             }
             nstage++;
             if (AHEAD) {
-                if (sp + 1 < npts) load_stage(site, point(sp + 1));
-                else if (site + gridDim.x < nsites) load_stage(site + gridDim.x, point(0));
+                if (sp + 1 < npts) load_stage(cur, point(sp + 1));
+                else if (site + gridDim.x < nsites) load_stage(nxt, point(0));
             }
         }
         // all nine points accumulated: TMEM -> shared scratch S[col][lane] -> combine -> global
@@ -320,6 +322,7 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
             out[((size_t)site * NB + i) * C::NP + q] = o;
         }
         __syncthreads();   // S (aliasing the operand buffer) is free for the next site
+        cur = nxt;
     }
 
     tc_fence_before();

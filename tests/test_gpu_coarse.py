@@ -75,17 +75,20 @@ def test_config4_coarsest_level(nrhs):
     c.close()
 
 
-# ---- row a6: the tensor-core variant (tcgen05 kind::tf32, hi/lo split operands) is held to the same tolerance
+# ---- row a6: the tensor-core variants (tcgen05 kind::tf32 with hi/lo tf32 operands split in the kernel; kind::f16 with hi/lo
+# fp16 operands split beforehand after a power-of-two scaling) are held to the same tolerance
+TC_MODES = [mrhs.COARSE_TENSOR, mrhs.COARSE_TENSOR_F16]
 TC_SMALL = [([2, 2, 2, 2], 24, n) for n in (2, 4, 8, 12, 16, 24, 32, 48, 64, 96)] + \
            [([3, 2, 4, 2], 40, n) for n in (2, 4, 8, 12, 16, 24, 32, 48, 64, 96)] + \
            [([5, 3, 2, 4], 24, 12), ([4, 4, 4, 6], 40, 12), ([7, 5, 3, 11], 40, 24)]
 
 
+@pytest.mark.parametrize("mode", TC_MODES)
 @pytest.mark.parametrize("cdims,nb,nrhs", TC_SMALL)
-def test_coarse_tensor_core_matches_oracle_small(cdims, nb, nrhs):
+def test_coarse_tensor_core_matches_oracle_small(cdims, nb, nrhs, mode):
     A = syn.coarse_links_np(cdims, nb, 3)
     v = syn.coarse_vector_np(cdims, nb, nrhs, 3)
-    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=1)
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=mode)
     want = oracle.coarse_apply(cdims, A, v)
     err = rel_l2_per_rhs(gpu_coarse(c, v), want)
     assert err.max() < TOL, err
@@ -105,6 +108,13 @@ def test_config4_tensor_core(nrhs):
     err_tc = rel_l2_per_rhs(gpu_coarse(c, v), want)
     assert err_tc.max() < TOL, err_tc
     c.close()
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=2)
+    err_h16 = rel_l2_per_rhs(gpu_coarse(c, v), want)
+    assert err_h16.max() < TOL, err_h16
+    # a second apply reuses the split-vector scratch, the column maxima and the barrier phases
+    err_h16 = rel_l2_per_rhs(gpu_coarse(c, v), want)
+    assert err_h16.max() < TOL, err_h16
+    c.close()
     # the two math modes agree with each other far inside the tolerance
     c0 = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=0)
     err_fma = rel_l2_per_rhs(gpu_coarse(c0, v), want)
@@ -113,27 +123,55 @@ def test_config4_tensor_core(nrhs):
     assert err_tc.max() < 20 * max(err_fma.max(), 1e-7), (err_tc.max(), err_fma.max())
 
 
+@pytest.mark.parametrize("mode", TC_MODES)
 @pytest.mark.parametrize("nrhs", [12, 64])
-def test_config3_tensor_core(nrhs):
+def test_config3_tensor_core(nrhs, mode):
     cdims, nb = [8, 8, 8, 8], 24
     A = syn.coarse_links_np(cdims, nb, 3)
     v = syn.coarse_vector_np(cdims, nb, nrhs, 3)
-    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=1)
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=mode)
     err = rel_l2_per_rhs(gpu_coarse(c, v), oracle.coarse_apply(cdims, A, v))
     assert err.max() < TOL, err
     c.close()
 
 
-def test_coarse_tensor_core_rejects_odd_nrhs():
+@pytest.mark.parametrize("mode", TC_MODES)
+def test_coarse_tensor_core_rejects_odd_nrhs(mode):
     cdims, nb = [2, 2, 2, 2], 24
     A = dev(syn.coarse_links_np(cdims, nb, 3))
     with pytest.raises(mrhs.MrhsError) as e:
-        mrhs.Coarse(cdims, nb, 1, A, math_mode=1)
+        mrhs.Coarse(cdims, nb, 1, A, math_mode=mode)
     assert e.value.status == mrhs.ERR_UNSUPPORTED
 
 
+@pytest.mark.parametrize("cdims,nb,nrhs", [([4, 2, 6, 2], 24, 12), ([3, 2, 4, 2], 40, 24)])
+def test_coarse_fp16_split_scales(cdims, nb, nrhs):
+    """math_mode 2 represents every number as two fp16 parts after a power-of-two scaling: per site for the links, per RHS for
+    the vectors.  Right-hand sides and sites of very different magnitudes (1e-12 .. 1e+12, far outside the fp16 range), a zero
+    RHS and a RHS that is a point source must come out within the tolerance per RHS."""
+    rng = np.random.default_rng(11)
+    A = syn.coarse_links_np(cdims, nb, 3)
+    nsites = int(np.prod(cdims))
+    site_mag = (10.0 ** rng.uniform(-6, 6, size=nsites)).astype(np.float32)
+    A = (A.reshape(nsites, -1) * site_mag[:, None]).reshape(A.shape).astype(np.complex64)
+    v = syn.coarse_vector_np(cdims, nb, nrhs, 3)
+    col_mag = (10.0 ** np.linspace(-12, 12, nrhs)).astype(np.float32)
+    v = (v * col_mag).astype(np.complex64)
+    v[..., 3] = 0                                   # a zero right-hand side
+    v[..., 5] = 0
+    v.reshape(nsites, nb, nrhs)[nsites // 2, 7, 5] = 3.0e-5 - 2.0e-5j     # a point source
+    c = mrhs.Coarse(cdims, nb, nrhs, dev(A), math_mode=2)
+    got = gpu_coarse(c, v)
+    want = oracle.coarse_apply(cdims, A, v)
+    assert np.all(got[..., 3] == 0)
+    keep = [n for n in range(nrhs) if n != 3]
+    err = rel_l2_per_rhs(got[..., keep], want[..., keep])
+    assert err.max() < TOL, err
+    c.close()
+
+
 # ---- subsets of the stencil (NEXT-1): stand-alone self term, 8-point hopping term, single points; both math modes
-@pytest.mark.parametrize("mode", [mrhs.COARSE_FMA, mrhs.COARSE_TENSOR])
+@pytest.mark.parametrize("mode", mrhs.COARSE_MODES)
 @pytest.mark.parametrize("cdims,nb,nrhs", [([4, 2, 6, 2], 24, 12), ([3, 4, 2, 5], 40, 24), ([2, 2, 2, 2], 40, 96)])
 def test_coarse_point_subsets_match_oracle(cdims, nb, nrhs, mode):
     A = syn.coarse_links_np(cdims, nb, 7)
@@ -165,11 +203,11 @@ def test_coarse_errors():
 MEOOE_CASES = [([4, 2, 6, 2], 24, 12), ([2, 4, 2, 6], 40, 24), ([2, 2, 2, 2], 40, 96), ([6, 4, 2, 4], 24, 1), ([8, 4, 4, 6], 40, 12)]
 
 
-@pytest.mark.parametrize("mode", [mrhs.COARSE_FMA, mrhs.COARSE_TENSOR])
+@pytest.mark.parametrize("mode", mrhs.COARSE_MODES)
 @pytest.mark.parametrize("cdims,nb,nrhs", MEOOE_CASES)
 def test_coarse_meooe_matches_oracle(cdims, nb, nrhs, mode):
-    if mode == mrhs.COARSE_TENSOR and nrhs % 2:
-        pytest.skip("the tensor-core variant needs an even N_rhs")
+    if mode != mrhs.COARSE_FMA and nrhs % 2:
+        pytest.skip("the tensor-core variants need an even N_rhs")
     A = syn.coarse_links_np(cdims, nb, 8)
     v = syn.coarse_vector_np(cdims, nb, nrhs, 8)
     src = oracle.cb_split(cdims, v)
