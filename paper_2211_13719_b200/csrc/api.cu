@@ -715,6 +715,7 @@ mrhs_status_t mrhs_coarse_create(mrhs_coarse_t **out, const int cdims[4], int nb
     if (math_mode == 2) {
         e = cudaMalloc(&h->site_scale, ((size_t)h->g.nsites + 128) * sizeof(float));
         if (e == cudaSuccess) e = cudaMalloc(&h->vec16, coarse_h16_vec_bytes(h->g));
+        if (e == cudaSuccess) e = cudaMemsetAsync(h->vec16, 0, coarse_h16_vec_bytes(h->g), h->st);     // its last K chunk stays zero
         if (e != cudaSuccess) { cudaFree(h->site_scale); cudaFree(h->links); delete h; return cuda_fail(e, "cudaMalloc(split operands)", __FILE__, __LINE__); }
         s = pack_coarse_links_h16(h->g, (const float2 *)d_links, h->links, h->site_scale, h->st);
         if (s == MRHS_OK) s = coarse_h16_prepare(h->g, &h->tc_grid);

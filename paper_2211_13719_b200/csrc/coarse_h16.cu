@@ -109,8 +109,11 @@ struct H16Cfg {
     static constexpr int NP = N / 2;                          // float4 elements per component
     static constexpr int NT = ((2 * N + 15) / 16) * 16;       // columns of one of v_hi / v_lo: Re at 0, Im at NT / 2
     static constexpr int KC = NB / 8;                         // 16-byte K chunks (8 fp16) per stencil point
-    static constexpr int KCP = (KC + 1) / 2 * 2;              // in shared memory: padded to whole MMAs (K = 16 = two chunks)
-    static constexpr int KS = KCP / 2;                        // MMAs K steps per stencil point
+    // An MMA takes K = 16 = two chunks.  With an odd chunk count per point (nbasis = 24, 40) a stage holds TWO stencil points whose
+    // chunks follow each other (2 KC chunks = KC MMA steps for two points); a site's last, single point is followed by one chunk of
+    // zeros in the B operand (copied from a zero buffer, not stored per site): nbasis 40: 23 K steps per site instead of 27.
+    static constexpr int PP = KC % 2 ? 2 : 1;                 // stencil points per operand stage
+    static constexpr int KCP = PP * KC;                       // chunks of one stage in shared memory (even)
     static constexpr int NG = (NB + 15) / 16;                 // 16-component groups = TMEM lane quarters with rows
     static constexpr int ROWS = 2 * NB;                       // stored rows of the A operand
     static constexpr bool STK = 2 * NT <= 256;                // stacked B operand: two MMAs per K step
@@ -128,16 +131,19 @@ struct H16Cfg {
     static constexpr int SMEM_BYTES = NSTAGE * STAGE + TAIL;
     static constexpr int THREADS = 6 * 32;                    // copy, MMA, four epilogue warps
     static_assert(NSTAGE >= 2, "operand ring needs two stages");
+    static_assert(KCP % 2 == 0, "whole MMAs per stage");
     static_assert(NT <= 256 && 2 * D_COLS <= 512 && N <= 128, "MMA N / TMEM limit");
 };
 
 // links16: [site][p][hi | lo][K chunk][row][8 fp16]; site_scale[site] = 1 / s_A; vec16: [site][K chunk][2 NT columns][8 fp16];
+// zeros: one K chunk of the B operand (2 NT x 16 bytes) of zeros;
 // colmax[n] = max |v| of RHS n (both written by the passes below); out: coarse vectors [site][component][RHS pair] float4.
 // ALL: the nine-point operator (mask ignored)
 template <int NB, int N, bool ALL>
 __global__ void __launch_bounds__(H16Cfg<NB, N>::THREADS, 1)
 coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *__restrict__ links16, const float *__restrict__ site_scale,
-                  const unsigned char *__restrict__ vec16, const float *__restrict__ colmax, float4 *__restrict__ out) {
+                  const unsigned char *__restrict__ vec16, const unsigned char *__restrict__ zeros, const float *__restrict__ colmax,
+                  float4 *__restrict__ out) {
     typedef H16Cfg<NB, N> C;
     extern __shared__ __align__(128) unsigned char smem[];
     float *cinv = reinterpret_cast<float *>(smem + C::NSTAGE * C::STAGE);
@@ -173,18 +179,22 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
             for (long long site = blockIdx.x; site < nsites; site += gridDim.x) {
                 const CoarseSite32 sc = coarse_site32(sites, site);
                 const long long lex = sc.lex;
-                for (int sp = 0; sp < npts; sp++) {
-                    const int p = point(sp);
+                for (int sp = 0; sp < npts; sp += C::PP) {
                     if (wrapped) mbar_wait(&empty[s], ph);
-                    // vector index of the neighbour at stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
-                    long long nbr = coarse_neighbour32(sites, sc, p);
-                    if (sites.cb) nbr >>= 1;
                     unsigned char *dst = smem + (size_t)s * C::STAGE;
-                    const unsigned char *a = links16 + ((size_t)lex * 9 + p) * (2 * C::A_HALF);
-                    mbar_expect_tx(&full[s], 2 * C::A_HALF + C::B_COPY);
-                    bulk_g2s(dst, a, C::A_HALF, &full[s]);
-                    bulk_g2s(dst + C::A_SLOT, a + C::A_HALF, C::A_HALF, &full[s]);
-                    bulk_g2s(dst + 2 * C::A_SLOT, vec16 + (size_t)nbr * C::B_COPY, C::B_COPY, &full[s]);
+                    const bool two = C::PP == 2 && sp + 1 < npts;
+                    mbar_expect_tx(&full[s], (two ? 2 : 1) * (2 * C::A_HALF + C::B_COPY) + (C::PP == 2 && !two ? C::B_LBO : 0));
+                    for (int k = 0; k < (two ? 2 : 1); k++) {
+                        const int p = point(sp + k);
+                        // vector index of the neighbour at stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
+                        long long nbr = coarse_neighbour32(sites, sc, p);
+                        if (sites.cb) nbr >>= 1;
+                        const unsigned char *a = links16 + ((size_t)lex * 9 + p) * (2 * C::A_HALF);
+                        bulk_g2s(dst + k * C::A_HALF, a, C::A_HALF, &full[s]);
+                        bulk_g2s(dst + C::A_SLOT + k * C::A_HALF, a + C::A_HALF, C::A_HALF, &full[s]);
+                        bulk_g2s(dst + 2 * C::A_SLOT + k * C::B_COPY, vec16 + (size_t)nbr * C::B_COPY, C::B_COPY, &full[s]);
+                    }
+                    if (C::PP == 2 && !two) bulk_g2s(dst + 2 * C::A_SLOT + C::B_COPY, zeros, C::B_LBO, &full[s]);     // K padding of a single point
                     if (++s == (uint32_t)C::NSTAGE) { s = 0; ph ^= 1u; wrapped = true; }
                 }
             }
@@ -198,13 +208,13 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
             if (sl >= 2) mbar_wait(&accfree[a], ((sl >> 1) - 1) & 1u);      // the epilogue has read this accumulator set
             tc_fence_after();
             const uint32_t d = tmem + a * C::D_COLS;
-            for (int sp = 0; sp < npts; sp++) {
+            for (int sp = 0; sp < npts; sp += C::PP) {
                 mbar_wait(&full[s], ph);
                 tc_fence_after();
+                const int steps = C::PP == 2 && sp + 1 >= npts ? (C::KC + 1) / 2 : C::KCP / 2;
                 if (elect_one()) {
                     const uint32_t ah = smem_u32(smem + (size_t)s * C::STAGE), al = ah + C::A_SLOT, bh = ah + 2 * C::A_SLOT, bl = bh + C::NT * 16;
-#pragma unroll
-                    for (int ks = 0; ks < C::KS; ks++) {
+                    for (int ks = 0; ks < steps; ks++) {
                         const uint64_t dah = smem_desc(ah + ks * 2 * C::A_LBO, C::A_LBO, 128);
                         const uint64_t dal = smem_desc(al + ks * 2 * C::A_LBO, C::A_LBO, 128);
                         const uint64_t dbh = smem_desc(bh + ks * 2 * C::B_LBO, C::B_LBO, 128);
@@ -219,7 +229,7 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
                         }
                     }
                     mma_commit(&empty[s]);                           // the operand stage is free once these MMAs have read it
-                    if (sp == npts - 1) mma_commit(&accfull[a]);     // all points of the site accumulated
+                    if (sp + C::PP >= npts) mma_commit(&accfull[a]); // all points of the site accumulated
                 }
                 __syncwarp();
                 if (++s == (uint32_t)C::NSTAGE) { s = 0; ph ^= 1u; }
@@ -401,15 +411,15 @@ mrhs_status_t h16_prepare_t() {
 }
 template <int NB, int N>
 mrhs_status_t h16_launch_t(const CoarseSites &sites, int grid, unsigned mask, const void *links16, const float *site_scale, const void *vec16,
-                           const float *colmax, void *out, cudaStream_t st) {
+                           const void *zeros, const float *colmax, void *out, cudaStream_t st) {
     typedef H16Cfg<NB, N> C;
     if ((long long)grid > sites.nout) grid = (int)sites.nout;
     if (mask == 0x1FFu)
         coarse_h16_kernel<NB, N, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(sites, mask, (const unsigned char *)links16, site_scale,
-                                                                                 (const unsigned char *)vec16, colmax, (float4 *)out);
+                                                                                 (const unsigned char *)vec16, (const unsigned char *)zeros, colmax, (float4 *)out);
     else
         coarse_h16_kernel<NB, N, false><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(sites, mask, (const unsigned char *)links16, site_scale,
-                                                                                  (const unsigned char *)vec16, colmax, (float4 *)out);
+                                                                                  (const unsigned char *)vec16, (const unsigned char *)zeros, colmax, (float4 *)out);
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
 }
@@ -426,9 +436,14 @@ bool coarse_h16_supported(int nb, int nrhs) {
     return false;
 }
 
-size_t coarse_h16_vec_bytes(const CoarseGeom &g) {
+// the split image of a full-lattice vector, followed by one K chunk of zeros (the caller clears the buffer once)
+static size_t h16_image_bytes(const CoarseGeom &g) {
     const int nt = (2 * g.N + 15) / 16 * 16;
     return (size_t)g.nsites * (g.nb / 8) * 2 * nt * 16;
+}
+size_t coarse_h16_vec_bytes(const CoarseGeom &g) {
+    const int nt = (2 * g.N + 15) / 16 * 16;
+    return h16_image_bytes(g) + (size_t)2 * nt * 16;
 }
 
 mrhs_status_t coarse_h16_prepare(const CoarseGeom &g, int *grid) {
@@ -477,7 +492,8 @@ mrhs_status_t launch_coarse_h16(const CoarseGeom &g, const CoarseSites &sites, i
         h16_split_vec_kernel<<<(unsigned)((items + 255) / 256), 256, 0, st>>>((const float4 *)d_in, nin, g.nb, np, nt, d_colmax, (uint4 *)d_vec16);
         MRHS_CUDA(cudaGetLastError());
     }
-#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return h16_launch_t<NB, NN>(sites, grid, mask, d_links16, d_site_scale, d_vec16, d_colmax, d_out, st);
+    const void *zeros = (const unsigned char *)d_vec16 + h16_image_bytes(g);
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return h16_launch_t<NB, NN>(sites, grid, mask, d_links16, d_site_scale, d_vec16, zeros, d_colmax, d_out, st);
     MRHS_H16_N_LIST(MRHS_CASE, 24)
     MRHS_H16_N_LIST(MRHS_CASE, 40)
 #undef MRHS_CASE
