@@ -13,7 +13,7 @@
 //   * vectors: two small passes per apply (column maxima; split into the operand image, 2 x 2 N_rhs (rounded) fp16 per component),
 //     instead of converting each vector nine times, once per stencil point that reads it.
 // The stencil kernel is then a plain TMA -> tcgen05 -> epilogue pipeline: one persistent block per SM, one copy warp (three bulk
-// copies per stencil point), one MMA warp, four epilogue warps, operand ring of up to eight stages, two accumulator sets in
+// copies per stencil point), one MMA warp, four epilogue warps, operand ring of two to eight stages, two accumulator sets in
 // tensor memory so that the epilogue of a site runs under the MMAs of the next.
 //
 // Per site the complex contraction is ONE real GEMM accumulated over the stencil points, D[128 x cols] += Aop[128 x 16] Bop[16 x cols]:
@@ -23,7 +23,8 @@
 //   stacked (2 NT <= 256): A_hi x [v_hi | v_lo] and A_lo x v_hi, two MMAs per K step, hi*lo in accumulator columns NT..2NT-1;
 //   otherwise three MMAs per K step into columns 0..NT-1.
 //   Re out = D[Re i][n] - D[Im i][NT/2 + n],  Im out = D[Re i][NT/2 + n] + D[Im i][n]   (one warp shuffle per value).
-// nbasis / 8 K chunks of 16 bytes per point; an odd count is padded in SHARED memory by a chunk that stays zero (not in HBM).
+// nbasis / 8 K chunks of 16 bytes per point, an MMA takes two: with an odd count a stage holds two stencil points back to back and a
+// site's last single point is followed by one chunk of zeros copied from a zero buffer (nothing is padded in HBM).
 #include "coarse.cuh"
 #include "async_copy.cuh"
 #include <cuda_fp16.h>
