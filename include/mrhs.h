@@ -328,6 +328,21 @@ mrhs_status_t mrhs_transfer_destroy(mrhs_transfer_t *h);
 mrhs_status_t mrhs_inner_products(const int dims[4], int ncomp, int nrhs, int parity,
                                   const void *d_x, const void *d_y, void *d_result, void *cuda_stream);
 
+/* The same operation for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): no cudaMalloc / cudaMallocAsync / cudaFree and no allocating library routine is called.  The per-block
+ * partial sums live in a static __device__ array of the library (2 MiB = 131072 complex128 partial sums, held by every GPU
+ * that loads the library until the process exits) instead of stream-ordered scratch.  Same arguments, same kernels, same
+ * thread-block count and summation order as mrhs_inner_products: the results are bit-identical.
+ *   Limit: (8 x SM count) x nrhs <= 131072, i.e. nrhs <= 110 on a 148-SM B200; beyond it MRHS_ERR_UNSUPPORTED with a message
+ *   naming both numbers (nothing is launched).  The lattice size is not limited.
+ *   Every call on a device shares the one array: calls that overlap on the GPU (different streams, no ordering between
+ *   them) RACE on it; calls on one stream, or ordered by events, are safe.  The array keeps the last call's contents;
+ *   nothing needs clearing, because a call writes every partial sum it later reads.
+ *   The first call on a device looks the array's device address up (cudaGetSymbolAddress, no allocation) and caches it;
+ *   make that first call outside a graph capture.  Asynchronous on cuda_stream. */
+mrhs_status_t mrhs_inner_products_noalloc(const int dims[4], int ncomp, int nrhs, int parity,
+                                          const void *d_x, const void *d_y, void *d_result, void *cuda_stream);
+
 /* ------------------------------------------- host-buffer (end-to-end) entries */
 
 /* One operator apply with HOST buffers in CANONICAL layout: host->device copy,

@@ -68,6 +68,7 @@ _SIGNATURES = {
     "mrhs_restrict": (ctypes.c_int, [_vp, _vp, _vp]),
     "mrhs_transfer_destroy": (ctypes.c_int, [_vp]),
     "mrhs_inner_products": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
+    "mrhs_inner_products_noalloc": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
     "mrhs_xblock": (ctypes.c_int, [ctypes.c_int, ctypes.c_int]),
     "mrhs_field_bytes": (ctypes.c_size_t, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
     "mrhs_field_import": (ctypes.c_int, [_int4, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]),
@@ -203,6 +204,13 @@ def inner_products(dims, ncomp, nrhs, parity, x, y, result=None, stream=None):
     if result is None:
         result = torch.empty(nrhs, dtype=torch.complex128, device=x.device)
     _check(lib().mrhs_inner_products(_dims(dims), ncomp, nrhs, parity, _ptr(x), _ptr(y), _ptr(result), _stream_ptr(stream)))
+    return result
+
+
+def inner_products_noalloc(dims, ncomp, nrhs, parity, x, y, result, stream=None):
+    """inner_products through the entry that allocates nothing (static device scratch, (8 x SMs) x nrhs <= 131072);
+    result: caller-provided complex128 device tensor [nrhs].  Calls that overlap on the GPU race on the shared scratch."""
+    _check(lib().mrhs_inner_products_noalloc(_dims(dims), ncomp, nrhs, parity, _ptr(x), _ptr(y), _ptr(result), _stream_ptr(stream)))
     return result
 
 

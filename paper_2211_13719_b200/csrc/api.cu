@@ -929,6 +929,21 @@ mrhs_status_t mrhs_inner_products(const int dims[4], int ncomp, int nrhs, int pa
     return MRHS_OK;
 }
 
+mrhs_status_t mrhs_inner_products_noalloc(const int dims[4], int ncomp, int nrhs, int parity, const void *d_x, const void *d_y,
+                                          void *d_result, void *cuda_stream) {
+    MRHS_REQUIRE(dims && d_x && d_y && d_result, "inner products (no alloc): NULL argument");
+    MRHS_REQUIRE(parity >= 0 && parity <= 2, "inner products (no alloc): parity must be 0, 1 or 2");
+    MRHS_REQUIRE(nrhs >= 1 && nrhs <= 256, "inner products (no alloc): nrhs must be 1..256");
+    MRHS_REQUIRE(aligned16(d_x) && aligned16(d_y) && aligned16(d_result), "inner products (no alloc): buffers must be 16-byte aligned");
+    const size_t bytes = mrhs_field_bytes(dims, ncomp, nrhs, parity != MRHS_FULL);
+    MRHS_REQUIRE(bytes > 0, "inner products (no alloc): invalid lattice (extents >= 2, even for checkerboarded fields)");
+    int dev = 0, sms = 0;
+    MRHS_CUDA(cudaGetDevice(&dev));
+    MRHS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    // same grid as mrhs_inner_products, so the same summation order and the same bits
+    return launch_inner_products_static((long long)(bytes / 4), nrhs, d_x, d_y, inner_grid(sms), (double2 *)d_result, (cudaStream_t)cuda_stream);
+}
+
 const char *mrhs_last_error(void) { return g_err; }
 
 const char *mrhs_version(void) { return "mrhs-wilson-b200 0.1 (sm_100a)"; }

@@ -6,6 +6,13 @@
 // fields (HBM-bound: 2 x field bytes), products and sums in fp64, two kernels so that the result is deterministic:
 // per-block partial sums, then one block adds the partials in a fixed order.
 #include "blas.cuh"
+#include <mutex>
+
+// Scratch of the allocation-free entry (mrhs_inner_products_noalloc): the per-block partial sums live in this file-scope array
+// instead of a stream-ordered allocation.  2 MiB on every GPU that loads the library, until the process exits.  In host code
+// this NAME is a host-side stand-in, not a device address: the host passes kernels the address cudaGetSymbolAddress returns.
+static constexpr size_t kInnerStaticPartials = 131072;     // double2 elements: thread blocks x N_rhs of one call at most
+static __device__ __align__(256) double2 g_mrhs_inner_scratch[kInnerStaticPartials];
 
 namespace mrhs {
 
@@ -89,6 +96,38 @@ mrhs_status_t launch_inner_products(long long nfloats, int nrhs, const void *d_x
     inner_final_kernel<<<nrhs, 256, 0, st>>>(d_partial, grid, nrhs, d_out);
     MRHS_CUDA(cudaGetLastError());
     return MRHS_OK;
+}
+
+size_t inner_static_capacity() { return kInnerStaticPartials; }
+
+// The same two kernels with the partial sums in g_mrhs_inner_scratch.  No allocation: the device address of the array is
+// looked up once per device (with that device current: it is the caller's current device) and cached.  Nothing has to be
+// cleared between calls: the first kernel writes every one of the grid * nrhs partials the second one reads.
+mrhs_status_t launch_inner_products_static(long long nfloats, int nrhs, const void *d_x, const void *d_y, int grid,
+                                           double2 *d_out, cudaStream_t st) {
+    if ((size_t)grid * (size_t)nrhs > kInnerStaticPartials) {
+        set_error("inner products (no alloc): %d thread blocks x %d right-hand sides = %zu partial sums exceed the static scratch of %zu",
+                  grid, nrhs, (size_t)grid * (size_t)nrhs, kInnerStaticPartials);
+        return MRHS_ERR_UNSUPPORTED;
+    }
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static double2 *addr[kMaxDev] = {};
+    int dev = 0;
+    MRHS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDev) { set_error("inner products (no alloc): device ordinal %d out of range", dev); return MRHS_ERR_UNSUPPORTED; }
+    double2 *partial = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (!addr[dev]) {
+            void *p = nullptr;
+            MRHS_CUDA(cudaGetSymbolAddress(&p, g_mrhs_inner_scratch));
+            if (!p) { set_error("inner products (no alloc): cudaGetSymbolAddress returned NULL"); return MRHS_ERR_CUDA; }
+            addr[dev] = (double2 *)p;
+        }
+        partial = addr[dev];
+    }
+    return launch_inner_products(nfloats, nrhs, d_x, d_y, partial, grid, d_out, st);
 }
 
 }  // namespace mrhs

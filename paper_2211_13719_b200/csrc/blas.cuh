@@ -10,4 +10,10 @@ int inner_grid(int num_sms);
 mrhs_status_t launch_inner_products(long long nfloats, int nrhs, const void *d_x, const void *d_y, double2 *d_partial,
                                     int grid, double2 *d_out, cudaStream_t st);
 
+// The same with the partial sums in a file-scope __device__ array of inner_static_capacity() double2 (blas.cu): allocates
+// nothing; MRHS_ERR_UNSUPPORTED if grid * nrhs exceeds the capacity.  Calls share the array: calls that overlap on the GPU race.
+size_t inner_static_capacity();
+mrhs_status_t launch_inner_products_static(long long nfloats, int nrhs, const void *d_x, const void *d_y, int grid,
+                                           double2 *d_out, cudaStream_t st);
+
 }  // namespace mrhs
