@@ -13,15 +13,17 @@
 //   * vectors: two small passes per apply (column maxima; split into the operand image, 2 x 2 N_rhs (rounded) fp16 per component),
 //     instead of converting each vector nine times, once per stencil point that reads it.
 // The stencil kernel is then a plain TMA -> tcgen05 -> epilogue pipeline: one persistent block per SM, one copy warp (three bulk
-// copies per stencil point), one MMA warp, four epilogue warps, operand ring of two to eight stages, two accumulator sets in
+// copies per stencil point), one MMA warp, eight epilogue warps, operand ring of two to eight stages, two accumulator sets in
 // tensor memory so that the epilogue of a site runs under the MMAs of the next.
 //
 // Per site the complex contraction is ONE real GEMM accumulated over the stencil points, D[128 x cols] += Aop[128 x 16] Bop[16 x cols]:
 //   Aop rows (TMEM lanes): groups of 16 components, each group 16 rows of Re A followed by the same 16 rows of Im A (a last group of
 //                          8 + 8 if nbasis mod 16 = 8), so Re and Im of an output component sit in the same 32-lane quarter;
 //   Bop cols 0..N-1 = Re v_hi, NT/2..NT/2+N-1 = Im v_hi, NT..2NT-1 the same for v_lo     (NT = 2 N rounded up to 16)
-//   stacked (2 NT <= 256): A_hi x [v_hi | v_lo] and A_lo x v_hi, two MMAs per K step, hi*lo in accumulator columns NT..2NT-1;
-//   otherwise three MMAs per K step into columns 0..NT-1.
+//   stacked B (2 NT <= 256): A_hi x [v_hi | v_lo] and A_lo x v_hi, two MMAs per K step, hi*lo in accumulator columns NT..2NT-1;
+//   otherwise three MMAs per K step into columns 0..NT-1;
+//   stacked A (4 nbasis <= 128, i.e. nbasis 24): the A_lo rows follow the A_hi rows of the same 8 components inside a lane quarter,
+//   [A_hi ; A_lo] x [v_hi | v_lo] is ONE MMA per K step (two without the stacked B), hi and lo rows added by a warp shuffle.
 //   Re out = D[Re i][n] - D[Im i][NT/2 + n],  Im out = D[Re i][NT/2 + n] + D[Im i][n]   (one warp shuffle per value).
 // nbasis / 8 K chunks of 16 bytes per point, an MMA takes two: with an odd count a stage holds two stencil points back to back and a
 // site's last single point is followed by one chunk of zeros copied from a zero buffer (nothing is padded in HBM).
@@ -45,6 +47,9 @@ template <int COLS> __device__ __forceinline__ void tmem_free(uint32_t taddr) {
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// programmatic dependent launch: wait for the preceding kernel of the stream (no-op in a normal launch); let the next one start early
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;
     asm volatile("{\n .reg .pred p;\n elect.sync _|p, 0xffffffff;\n selp.u32 %0, 1, 0, p;\n}" : "=r"(pred));
@@ -62,17 +67,15 @@ __device__ __forceinline__ void mma_f16(uint32_t d_tmem, uint64_t a_desc, uint64
 __device__ __forceinline__ void mma_commit(uint64_t *bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-// 8 consecutive fp32 columns of this thread's TMEM lane (no wait: several loads are in flight before tmem_ld_wait)
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, float (&v)[8]) {
-    uint32_t r[8];
+// 8 consecutive fp32 columns of this thread's TMEM lane.  Asynchronous: the registers hold the values only after tmem_ld_wait(),
+// so that the loads of one chunk (two to four) are in flight together.
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8]) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
                  : "r"(taddr)
                  : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-    for (int i = 0; i < 8; i++) v[i] = __uint_as_float(r[i]);
 }
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // Shared-memory matrix descriptor, K-major, no swizzle: core matrix = 8 rows x 16 bytes stored as 128 contiguous bytes; SBO =
 // distance between 8-row groups, LBO = distance between the two 16-byte K chunks of one MMA (K = 16 fp16 = 32 bytes).
@@ -115,28 +118,34 @@ struct H16Cfg {
     // zeros in the B operand (copied from a zero buffer, not stored per site): nbasis 40: 23 K steps per site instead of 27.
     static constexpr int PP = KC % 2 ? 2 : 1;                 // stencil points per operand stage
     static constexpr int KCP = PP * KC;                       // chunks of one stage in shared memory (even)
-    static constexpr int NG = (NB + 15) / 16;                 // 16-component groups = TMEM lane quarters with rows
-    static constexpr int ROWS = 2 * NB;                       // stored rows of the A operand
+    // Stacked A operand (4 nbasis <= 128 rows, i.e. nbasis 24): the rows of A_lo follow those of A_hi in the SAME operand, so one MMA
+    // forms A_hi x B and A_lo x B at once (an MMA of this size costs a fixed ~77 cycles + ~0.6 per column whatever its row count):
+    // with the stacked B operand ONE MMA per K step, all four hi / lo products (lo x lo is exact too and is simply kept).
+    static constexpr bool SA = 4 * NB <= 128;
+    static constexpr int NA = SA ? 1 : 2;                     // A operands per stencil point
+    static constexpr int GW = SA ? 8 : 16;                    // components per TMEM lane quarter
+    static constexpr int NG = (NB + GW - 1) / GW;             // TMEM lane quarters with rows
+    static constexpr int ROWS = (SA ? 4 : 2) * NB;            // stored rows of one A operand
     static constexpr bool STK = 2 * NT <= 256;                // stacked B operand: two MMAs per K step
     static constexpr int D_COLS = STK ? 2 * NT : NT;          // accumulator columns of one set
     static constexpr int TMEM_COLS = pow2_cols(2 * D_COLS);   // two sets
     static constexpr int A_LBO = ROWS * 16;
     static constexpr int B_LBO = 2 * NT * 16;
-    static constexpr int A_HALF = KC * A_LBO;                 // bytes of A_hi (or A_lo) of one matrix in HBM
+    static constexpr int A_HALF = KC * A_LBO;                 // bytes of one A operand (A_hi or A_lo; stacked: both) of one matrix in HBM
     static constexpr int A_SLOT = KCP * A_LBO;                // and in shared memory
     static constexpr int B_COPY = KC * B_LBO;                 // bytes of one split vector [chunk][hi cols | lo cols][8]
     static constexpr int B_SLOT = KCP * B_LBO;
-    static constexpr int STAGE = 2 * A_SLOT + B_SLOT;
+    static constexpr int STAGE = NA * A_SLOT + B_SLOT;
     static constexpr int TAIL = 512 + 256;                    // column scales (N <= 128 floats), mbarriers + TMEM slot
     static constexpr int NSTAGE = (int)((kH16SmemLimit - TAIL) / STAGE) < kH16MaxStages ? (int)((kH16SmemLimit - TAIL) / STAGE) : kH16MaxStages;
     static constexpr int SMEM_BYTES = NSTAGE * STAGE + TAIL;
-    static constexpr int THREADS = 6 * 32;                    // copy, MMA, four epilogue warps
+    static constexpr int THREADS = 10 * 32;                   // copy, MMA, eight epilogue warps (two per TMEM lane quarter)
     static_assert(NSTAGE >= 2, "operand ring needs two stages");
     static_assert(KCP % 2 == 0, "whole MMAs per stage");
     static_assert(NT <= 256 && 2 * D_COLS <= 512 && N <= 128, "MMA N / TMEM limit");
 };
 
-// links16: [site][p][hi | lo][K chunk][row][8 fp16]; site_scale[site] = 1 / s_A; vec16: [site][K chunk][2 NT columns][8 fp16];
+// links16: [site][p][hi | lo][K chunk][row][8 fp16] (stacked A: [site][p][K chunk][row of hi or lo][8 fp16]); site_scale[site] = 1 / s_A; vec16: [site][K chunk][2 NT columns][8 fp16];
 // zeros: one K chunk of the B operand (2 NT x 16 bytes) of zeros;
 // colmax[n] = max |v| of RHS n (both written by the passes below); out: coarse vectors [site][component][RHS pair] float4.
 // ALL: the nine-point operator (mask ignored)
@@ -144,7 +153,7 @@ template <int NB, int N, bool ALL>
 __global__ void __launch_bounds__(H16Cfg<NB, N>::THREADS, 1)
 coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *__restrict__ links16, const float *__restrict__ site_scale,
                   const unsigned char *__restrict__ vec16, const unsigned char *__restrict__ zeros, const float *__restrict__ colmax,
-                  float4 *__restrict__ out) {
+                  float *__restrict__ colmax_next, float4 *__restrict__ out) {
     typedef H16Cfg<NB, N> C;
     extern __shared__ __align__(128) unsigned char smem[];
     float *cinv = reinterpret_cast<float *>(smem + C::NSTAGE * C::STAGE);
@@ -155,14 +164,18 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
         for (int s = 0; s < C::NSTAGE; s++) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
-        for (int a = 0; a < 2; a++) { mbar_init(&accfull[a], 1); mbar_init(&accfree[a], C::NG); }
+        for (int a = 0; a < 2; a++) { mbar_init(&accfull[a], 1); mbar_init(&accfree[a], 2 * C::NG); }
         mbar_fence_init();
     }
     // the padding chunks (and, before the first fill, everything else) read as zero
     for (int i = tid; i < C::NSTAGE * C::STAGE / 16; i += C::THREADS) reinterpret_cast<float4 *>(smem)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int n = tid; n < N; n += C::THREADS) cinv[n] = ldexpf(1.f, -scale_exp(colmax[n]));
     fence_async_smem();
     if (warp == 0) tmem_alloc<C::TMEM_COLS>(tslot);
+    // the column maxima of the NEXT apply start from zero (the handle alternates between two buffers, so nobody reads this one now)
+    if (blockIdx.x == 0 && tid < 128) colmax_next[tid] = 0.f;
+    // Launched with programmatic stream serialization: everything above overlaps the tail of the split pass; what follows reads its output
+    grid_dependency_wait();
+    for (int n = tid; n < N; n += C::THREADS) cinv[n] = ldexpf(1.f, -scale_exp(colmax[n]));
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -184,18 +197,18 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
                     if (wrapped) mbar_wait(&empty[s], ph);
                     unsigned char *dst = smem + (size_t)s * C::STAGE;
                     const bool two = C::PP == 2 && sp + 1 < npts;
-                    mbar_expect_tx(&full[s], (two ? 2 : 1) * (2 * C::A_HALF + C::B_COPY) + (C::PP == 2 && !two ? C::B_LBO : 0));
+                    mbar_expect_tx(&full[s], (two ? 2 : 1) * (C::NA * C::A_HALF + C::B_COPY) + (C::PP == 2 && !two ? C::B_LBO : 0));
                     for (int k = 0; k < (two ? 2 : 1); k++) {
                         const int p = point(sp + k);
                         // vector index of the neighbour at stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
                         long long nbr = coarse_neighbour32(sites, sc, p);
                         if (sites.cb) nbr >>= 1;
-                        const unsigned char *a = links16 + ((size_t)lex * 9 + p) * (2 * C::A_HALF);
+                        const unsigned char *a = links16 + ((size_t)lex * 9 + p) * (C::NA * C::A_HALF);
                         bulk_g2s(dst + k * C::A_HALF, a, C::A_HALF, &full[s]);
-                        bulk_g2s(dst + C::A_SLOT + k * C::A_HALF, a + C::A_HALF, C::A_HALF, &full[s]);
-                        bulk_g2s(dst + 2 * C::A_SLOT + k * C::B_COPY, vec16 + (size_t)nbr * C::B_COPY, C::B_COPY, &full[s]);
+                        if (!C::SA) bulk_g2s(dst + C::A_SLOT + k * C::A_HALF, a + C::A_HALF, C::A_HALF, &full[s]);
+                        bulk_g2s(dst + C::NA * C::A_SLOT + k * C::B_COPY, vec16 + (size_t)nbr * C::B_COPY, C::B_COPY, &full[s]);
                     }
-                    if (C::PP == 2 && !two) bulk_g2s(dst + 2 * C::A_SLOT + C::B_COPY, zeros, C::B_LBO, &full[s]);     // K padding of a single point
+                    if (C::PP == 2 && !two) bulk_g2s(dst + C::NA * C::A_SLOT + C::B_COPY, zeros, C::B_LBO, &full[s]);     // K padding of a single point
                     if (++s == (uint32_t)C::NSTAGE) { s = 0; ph ^= 1u; wrapped = true; }
                 }
             }
@@ -214,12 +227,15 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
                 tc_fence_after();
                 const int steps = C::PP == 2 && sp + 1 >= npts ? (C::KC + 1) / 2 : C::KCP / 2;
                 if (elect_one()) {
-                    const uint32_t ah = smem_u32(smem + (size_t)s * C::STAGE), al = ah + C::A_SLOT, bh = ah + 2 * C::A_SLOT, bl = bh + C::NT * 16;
+                    const uint32_t ah = smem_u32(smem + (size_t)s * C::STAGE), al = ah + C::A_SLOT, bh = ah + C::NA * C::A_SLOT, bl = bh + C::NT * 16;
                     for (int ks = 0; ks < steps; ks++) {
                         const uint64_t dah = smem_desc(ah + ks * 2 * C::A_LBO, C::A_LBO, 128);
                         const uint64_t dal = smem_desc(al + ks * 2 * C::A_LBO, C::A_LBO, 128);
                         const uint64_t dbh = smem_desc(bh + ks * 2 * C::B_LBO, C::B_LBO, 128);
-                        if (C::STK) {
+                        if (C::SA) {
+                            mma_f16(d, dah, dbh, idesc2, (sp | ks) != 0);     // [hi ; lo] x [hi | lo], or [hi ; lo] x hi
+                            if (!C::STK) mma_f16(d, dah, smem_desc(bl + ks * 2 * C::B_LBO, C::B_LBO, 128), idesc, 1);    // [hi ; lo] x lo, same columns
+                        } else if (C::STK) {
                             mma_f16(d, dah, dbh, idesc2, (sp | ks) != 0);     // hi x [hi | lo]
                             mma_f16(d, dal, dbh, idesc, 1);                    // lo x hi
                         } else {
@@ -237,11 +253,13 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
             }
         }
     } else {
-        // ------------------------------------------------------------------ epilogue warps: a warp reads the TMEM lane quarter warp & 3
-        const int g = warp & 3;
+        // ------------------------------------------------------------------ epilogue warps: a warp reads the TMEM lane quarter warp & 3;
+        // the two warps of a quarter take the even and the odd chunks of eight columns
+        const int g = warp & 3, half = (warp - 2) >> 2;
         if (g < C::NG) {
-            const int w = NB - 16 * g < 16 ? NB - 16 * g : 16;       // components of this group
-            const int part = lane / w, i = 16 * g + lane % w;
+            // rows of a quarter: w components x (Re, Im); stacked A: 8 components x (Re, Im) of A_hi, then the same of A_lo
+            const int w = C::SA ? 8 : (NB - 16 * g < 16 ? NB - 16 * g : 16);
+            const int part = (lane / w) & 1, i = C::GW * g + lane % w;
             const bool live = lane < 2 * w;
             uint32_t sl = 0;
             for (long long site = blockIdx.x; site < nsites; site += gridDim.x, sl++) {
@@ -251,35 +269,49 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
                 tc_fence_after();
                 float *o = reinterpret_cast<float *>(out + ((size_t)site * NB + (live ? i : 0)) * C::NP) + 2 * part;
                 const uint32_t t0 = tmem + ((uint32_t)(g * 32) << 16) + a * C::D_COLS;
-                constexpr int NCH = (N + 7) / 8;
+                constexpr int NCH = (N + 7) / 8, NCHW = (NCH + 1) / 2;
 #pragma unroll
-                for (int ch = 0; ch < NCH; ch++) {
-                    float x[8], y[8];
-                    tmem_ld8(t0 + ch * 8, x);
-                    tmem_ld8(t0 + C::NT / 2 + ch * 8, y);
-                    if (C::STK) {
-                        float xa[8], ya[8];
-                        tmem_ld8(t0 + C::NT + ch * 8, xa);
-                        tmem_ld8(t0 + C::NT + C::NT / 2 + ch * 8, ya);
-#pragma unroll
-                        for (int k = 0; k < 8; k++) { x[k] += xa[k]; y[k] += ya[k]; }
+                for (int c = 0; c < NCHW; c++) {
+                    const int ch = 2 * c + half;
+                    uint32_t rx[8], ry[8], rxa[8], rya[8];
+                    if (ch < NCH) {
+                        tmem_ld8(t0 + ch * 8, rx);
+                        tmem_ld8(t0 + C::NT / 2 + ch * 8, ry);
+                        if (C::STK) {
+                            tmem_ld8(t0 + C::NT + ch * 8, rxa);
+                            tmem_ld8(t0 + C::NT + C::NT / 2 + ch * 8, rya);
+                        }
+                        tmem_ld_wait();
                     }
-                    if (ch == NCH - 1) {
+                    if (c == NCHW - 1) {
                         // the accumulator has been read: hand it back before the arithmetic and the stores
                         tc_fence_before();
                         __syncwarp();
                         if (lane == 0) mbar_arrive(&accfree[a]);
                     }
+                    if (ch < NCH) {
+                        float x[8], y[8];
 #pragma unroll
-                    for (int k = 0; k < 8; k += 2) {
-                        const int n = ch * 8 + k;
-                        const float r0 = __shfl_xor_sync(0xffffffffu, y[k], w);          // the partner row's Im-column value
-                        const float r1 = __shfl_xor_sync(0xffffffffu, y[k + 1], w);
-                        if (n < N && live) {
-                            // Re row: Re out = D[Re i][n] - D[Im i][NT/2 + n];  Im row: Im out = D[Re i][NT/2 + n] + D[Im i][n]
-                            const float v0 = (part ? r0 + x[k] : x[k] - r0) * sa * cinv[n];          // two exact power-of-two factors, applied one after the other
-                            const float v1 = (part ? r1 + x[k + 1] : x[k + 1] - r1) * sa * cinv[n + 1];
-                            *reinterpret_cast<float2 *>(o + 2 * n) = make_float2(v0, v1);      // element n / 2 = (re0 re1 im0 im1)
+                        for (int k = 0; k < 8; k++) {
+                            x[k] = __uint_as_float(rx[k]);
+                            y[k] = __uint_as_float(ry[k]);
+                            if (C::STK) { x[k] += __uint_as_float(rxa[k]); y[k] += __uint_as_float(rya[k]); }
+                            if (C::SA) {      // the A_lo rows sit 16 lanes further
+                                x[k] += __shfl_xor_sync(0xffffffffu, x[k], 16);
+                                y[k] += __shfl_xor_sync(0xffffffffu, y[k], 16);
+                            }
+                        }
+#pragma unroll
+                        for (int k = 0; k < 8; k += 2) {
+                            const int n = ch * 8 + k;
+                            const float r0 = __shfl_xor_sync(0xffffffffu, y[k], w);          // the partner row's Im-column value
+                            const float r1 = __shfl_xor_sync(0xffffffffu, y[k + 1], w);
+                            if (n < N && live) {
+                                // Re row: Re out = D[Re i][n] - D[Im i][NT/2 + n];  Im row: Im out = D[Re i][NT/2 + n] + D[Im i][n]
+                                const float v0 = (part ? r0 + x[k] : x[k] - r0) * sa * cinv[n];          // two exact power-of-two factors, applied one after the other
+                                const float v1 = (part ? r1 + x[k + 1] : x[k + 1] - r1) * sa * cinv[n + 1];
+                                *reinterpret_cast<float2 *>(o + 2 * n) = make_float2(v0, v1);      // element n / 2 = (re0 re1 im0 im1)
+                            }
                         }
                     }
                 }
@@ -298,6 +330,7 @@ __device__ __forceinline__ void atomic_max_abs(float *addr, float m) {
 }
 // grid * block is a multiple of np, so a thread sees one RHS pair only
 __global__ void h16_colmax_kernel(const float4 *__restrict__ in, long long total, int np, float *__restrict__ colmax) {
+    grid_launch_dependents();      // the split pass may be scheduled now; it waits for this grid before it reads colmax
     const long long stride = (long long)gridDim.x * blockDim.x;
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int q = (int)(e % np);
@@ -325,6 +358,8 @@ union H8 { uint4 u; __half h[8]; };
 // pairs past N_rhs are the zero padding of the operand
 __global__ void h16_split_vec_kernel(const float4 *__restrict__ in, long long nsites, int nb, int np, int nt, const float *__restrict__ colmax,
                                      uint4 *__restrict__ vec16) {
+    grid_launch_dependents();      // the stencil kernel may start its set-up; it waits for this grid before it reads vec16
+    grid_dependency_wait();        // launched with programmatic stream serialization after the column-maximum pass
     const int kcn = nb / 8, qn = nt / 4;
     const long long total = nsites * kcn * qn;
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -379,13 +414,14 @@ __global__ void h16_pack_links_kernel(int nb, const float2 *__restrict__ src, ui
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= total) return;
     const int kcn = nb / 8, rows = 2 * nb;
+    const bool sa = 4 * nb <= 128;         // stacked A operand (H16Cfg::SA)
     const int u = (int)(idx % (kcn * rows));
     const long long mat = idx / (kcn * rows);
     const long long site = mat / 9;
     const int kc = u / rows, rr = u - kc * rows;
-    // operand row rr -> (part, component)
-    const int g = rr >> 5, w = nb - 16 * g < 16 ? nb - 16 * g : 16;
-    const int part = (rr - 32 * g) / w, i = 16 * g + (rr - 32 * g) % w;
+    // operand row rr -> (part, component); stacked: rr enumerates the hi rows, (part, component) = (rr / 8 & 1, 8 (rr / 16) + rr % 8)
+    const int g = sa ? rr >> 4 : rr >> 5, w = sa ? 8 : (nb - 16 * g < 16 ? nb - 16 * g : 16);
+    const int part = sa ? (rr >> 3) & 1 : (rr - 32 * g) / w, i = sa ? 8 * g + (rr & 7) : 16 * g + (rr - 32 * g) % w;
     const int k = scale_exp(site_scale[site]);
     const float s = ldexpf(1.f, k);
     H8 hi, lo;
@@ -395,8 +431,14 @@ __global__ void h16_pack_links_kernel(int nb, const float2 *__restrict__ src, ui
         split_h16((part ? a.y : a.x) * s, hi.h[j], lo.h[j]);
     }
     uint4 *d = dst + (size_t)mat * 2 * kcn * rows;
-    d[kc * rows + rr] = hi.u;
-    d[(kcn + kc) * rows + rr] = lo.u;
+    if (sa) {       // [K chunk][quarter: 8 Re hi, 8 Im hi, 8 Re lo, 8 Im lo][8 fp16]
+        const int r4 = 32 * g + 8 * part + (rr & 7);
+        d[kc * 2 * rows + r4] = hi.u;
+        d[kc * 2 * rows + r4 + 16] = lo.u;
+    } else {
+        d[kc * rows + rr] = hi.u;
+        d[(kcn + kc) * rows + rr] = lo.u;
+    }
 }
 __global__ void h16_site_scale_kernel(float *__restrict__ site_scale, long long nsites) {
     const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -412,16 +454,24 @@ mrhs_status_t h16_prepare_t() {
 }
 template <int NB, int N>
 mrhs_status_t h16_launch_t(const CoarseSites &sites, int grid, unsigned mask, const void *links16, const float *site_scale, const void *vec16,
-                           const void *zeros, const float *colmax, void *out, cudaStream_t st) {
+                           const void *zeros, const float *colmax, float *colmax_next, void *out, cudaStream_t st) {
     typedef H16Cfg<NB, N> C;
     if ((long long)grid > sites.nout) grid = (int)sites.nout;
-    if (mask == 0x1FFu)
-        coarse_h16_kernel<NB, N, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(sites, mask, (const unsigned char *)links16, site_scale,
-                                                                                 (const unsigned char *)vec16, (const unsigned char *)zeros, colmax, (float4 *)out);
-    else
-        coarse_h16_kernel<NB, N, false><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(sites, mask, (const unsigned char *)links16, site_scale,
-                                                                                  (const unsigned char *)vec16, (const unsigned char *)zeros, colmax, (float4 *)out);
-    MRHS_CUDA(cudaGetLastError());
+    // programmatic stream serialization: the kernel's set-up (shared memory, barriers, tensor memory) runs under the tail of the split pass
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(C::THREADS);
+    cfg.dynamicSmemBytes = C::SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const unsigned char *l = (const unsigned char *)links16, *v = (const unsigned char *)vec16, *z = (const unsigned char *)zeros;
+    float4 *o = (float4 *)out;
+    if (mask == 0x1FFu) MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, true>, sites, mask, l, site_scale, v, z, colmax, colmax_next, o));
+    else                MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, false>, sites, mask, l, site_scale, v, z, colmax, colmax_next, o));
     return MRHS_OK;
 }
 
@@ -475,11 +525,11 @@ mrhs_status_t pack_coarse_links_h16(const CoarseGeom &g, const float2 *d_canonic
 }
 
 mrhs_status_t launch_coarse_h16(const CoarseGeom &g, const CoarseSites &sites, int grid, unsigned mask, const void *d_links16, const float *d_site_scale,
-                                const void *d_in, void *d_vec16, float *d_colmax, void *d_out, cudaStream_t st) {
+                                const void *d_in, void *d_vec16, float *d_colmax, float *d_colmax_next, void *d_out, cudaStream_t st) {
     const int np = g.N / 2, nt = (2 * g.N + 15) / 16 * 16;
     const long long nin = sites.cb ? g.nsites / 2 : g.nsites;      // sites of the input vector
     const long long total = nin * g.nb * np;
-    MRHS_CUDA(cudaMemsetAsync(d_colmax, 0, 128 * sizeof(float), st));
+    // d_colmax is zero: cleared at create or by the stencil kernel of the apply before the last (two buffers, used alternately)
     {
         // a multiple of 3 blocks of 256 threads: the thread count is a multiple of every supported N_rhs / 2
         long long blocks = (total + 255) / 256;
@@ -490,11 +540,19 @@ mrhs_status_t launch_coarse_h16(const CoarseGeom &g, const CoarseSites &sites, i
     }
     {
         const long long items = nin * (g.nb / 8) * (nt / 4);
-        h16_split_vec_kernel<<<(unsigned)((items + 255) / 256), 256, 0, st>>>((const float4 *)d_in, nin, g.nb, np, nt, d_colmax, (uint4 *)d_vec16);
-        MRHS_CUDA(cudaGetLastError());
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)((items + 255) / 256));
+        cfg.blockDim = dim3(256);
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        MRHS_CUDA(cudaLaunchKernelEx(&cfg, h16_split_vec_kernel, (const float4 *)d_in, nin, g.nb, np, nt, (const float *)d_colmax, (uint4 *)d_vec16));
     }
     const void *zeros = (const unsigned char *)d_vec16 + h16_image_bytes(g);
-#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return h16_launch_t<NB, NN>(sites, grid, mask, d_links16, d_site_scale, d_vec16, zeros, d_colmax, d_out, st);
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return h16_launch_t<NB, NN>(sites, grid, mask, d_links16, d_site_scale, d_vec16, zeros, d_colmax, d_colmax_next, d_out, st);
     MRHS_H16_N_LIST(MRHS_CASE, 24)
     MRHS_H16_N_LIST(MRHS_CASE, 40)
 #undef MRHS_CASE
