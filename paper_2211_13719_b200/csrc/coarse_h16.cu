@@ -28,7 +28,7 @@
 // nbasis / 8 K chunks of 16 bytes per point, an MMA takes two: with an odd count a stage holds two stencil points back to back and a
 // site's last single point is followed by one chunk of zeros copied from a zero buffer (nothing is padded in HBM).
 #include "coarse.cuh"
-#include "async_copy.cuh"
+#include "tcgen05.cuh"
 #include <cuda_fp16.h>
 #include <cstdlib>
 
@@ -36,37 +36,9 @@ namespace mrhs {
 
 namespace {
 
-// ---- tcgen05 wrappers (PTX ISA 8.6+, sm_100a)
-template <int COLS> __device__ __forceinline__ void tmem_alloc(uint32_t *slot) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "n"(COLS) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-template <int COLS> __device__ __forceinline__ void tmem_free(uint32_t taddr) {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(COLS) : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // programmatic dependent launch: wait for the preceding kernel of the stream (no-op in a normal launch); let the next one start early
 __device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-__device__ __forceinline__ bool elect_one() {
-    uint32_t pred;
-    asm volatile("{\n .reg .pred p;\n elect.sync _|p, 0xffffffff;\n selp.u32 %0, 1, 0, p;\n}" : "=r"(pred));
-    return pred != 0;
-}
-// D[tmem] (+)= A[smem] * B[smem], fp16 inputs, fp32 accumulate, issued by one thread for the CTA
-__device__ __forceinline__ void mma_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n"
-        " tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
-        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
-// arrive on bar once every MMA issued so far by this thread has completed
-__device__ __forceinline__ void mma_commit(uint64_t *bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
 // 8 consecutive fp32 columns of this thread's TMEM lane.  Asynchronous: the registers hold the values only after tmem_ld_wait(),
 // so that the loads of one chunk (two to four) are in flight together.
 __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8]) {
@@ -77,23 +49,6 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8]) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
-// Shared-memory matrix descriptor, K-major, no swizzle: core matrix = 8 rows x 16 bytes stored as 128 contiguous bytes; SBO =
-// distance between 8-row groups, LBO = distance between the two 16-byte K chunks of one MMA (K = 16 fp16 = 32 bytes).
-// Bits: [0,14) address >> 4, [16,30) LBO >> 4, [32,46) SBO >> 4, [46,48) descriptor version (1 on sm_100), [61,64) swizzle (0 = none).
-__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-    uint64_t d = 0;
-    d |= (uint64_t)((addr & 0x3FFFFu) >> 4);
-    d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16;
-    d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32;
-    d |= (uint64_t)1 << 46;
-    return d;
-}
-// Instruction descriptor, kind::f16: [4,6) D format (1 = f32), [7,10) A format (0 = f16), [10,13) B format (0 = f16),
-// bit 15 / 16 A / B major (0 = K-major), [17,23) N >> 3, [24,29) M >> 4.
-__host__ __device__ constexpr uint32_t instr_desc_f16(int M, int N) {
-    return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
-}
-
 // Exponent k of the scale 2^k that brings a largest magnitude m into [2^14, 2^15) (fp16 overflows at 65504); 0 for m = 0.
 __device__ __forceinline__ int scale_exp(float m) {
     if (!(m > 0.f) || !(m <= 3.0e38f)) return 0;      // zero field, or Inf / NaN in the input: no scaling (the result is Inf / NaN as in fp32)
@@ -102,7 +57,6 @@ __device__ __forceinline__ int scale_exp(float m) {
     return 14 - e;
 }
 
-constexpr int pow2_cols(int n) { return n <= 32 ? 32 : n <= 64 ? 64 : n <= 128 ? 128 : n <= 256 ? 256 : 512; }
 constexpr unsigned kH16SmemLimit = 227u * 1024u;
 constexpr int kH16MaxStages = 8;
 

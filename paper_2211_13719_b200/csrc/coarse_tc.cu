@@ -21,38 +21,13 @@
 // back on an mbarrier via tcgen05.commit.  Several CTAs share an SM, so one CTA's operand conversion
 // overlaps another's MMAs.
 #include "coarse.cuh"
-#include "async_copy.cuh"
+#include "tcgen05.cuh"
 #include <cstdlib>
 
 namespace mrhs {
 
 namespace {
 
-// ---- tcgen05 wrappers (PTX ISA 8.6+, sm_100a)
-template <int COLS> __device__ __forceinline__ void tmem_alloc(uint32_t *slot) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "n"(COLS) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-template <int COLS> __device__ __forceinline__ void tmem_free(uint32_t taddr) {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(COLS) : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-// generic-proxy writes to shared memory -> visible to the async proxy (the MMA's operand reads)
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
-// D[tmem] (+)= A[smem] * B[smem], tf32 inputs, fp32 accumulate, issued by one thread for the CTA
-__device__ __forceinline__ void mma_tf32(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n"
-        " tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
-        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
-// arrive on bar once every MMA issued so far by this thread has completed
-__device__ __forceinline__ void mma_commit(uint64_t *bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
 // 16 consecutive fp32 columns of this thread's TMEM lane
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
     uint32_t r[16];
@@ -65,24 +40,6 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
     for (int i = 0; i < 16; i++) v[i] = __uint_as_float(r[i]);
-}
-
-// Shared-memory matrix descriptor, K-major, no swizzle: core matrix = 8 rows x 16 bytes stored as
-// 128 contiguous bytes; SBO = distance between 8-row groups, LBO = distance between the two
-// 16-byte K chunks of one MMA (K = 8 tf32 = 32 bytes).  Bits: [0,14) address >> 4, [16,30) LBO >> 4,
-// [32,46) SBO >> 4, [46,48) descriptor version (1 on sm_100), [61,64) swizzle mode (0 = none).
-__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-    uint64_t d = 0;
-    d |= (uint64_t)((addr & 0x3FFFFu) >> 4);
-    d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16;
-    d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32;
-    d |= (uint64_t)1 << 46;
-    return d;
-}
-// Instruction descriptor, kind::tf32: [4,6) D format (1 = f32), [7,10) A format (2 = tf32), [10,13) B
-// format (2 = tf32), bit 15 / 16 A / B major (0 = K-major), [17,23) N >> 3, [24,29) M >> 4.
-__host__ __device__ constexpr uint32_t instr_desc_tf32(int M, int N) {
-    return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 
 // round-to-nearest tf32 (low 13 mantissa bits cleared) and the remainder, itself rounded to tf32
@@ -100,8 +57,6 @@ __device__ __forceinline__ void split4(float4 x, float4 &hi, float4 &lo) {
     split_tf32(x.z, hi.z, lo.z);
     split_tf32(x.w, hi.w, lo.w);
 }
-
-constexpr int pow2_cols(int n) { return n <= 32 ? 32 : n <= 64 ? 64 : n <= 128 ? 128 : n <= 256 ? 256 : 512; }
 
 template <int NB, int N>
 struct TcCfg {
