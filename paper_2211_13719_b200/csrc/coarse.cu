@@ -90,8 +90,9 @@ coarse_fma_kernel(const CoarseSites sites, unsigned mask, const float2 *__restri
     // the stencil points of this apply: bit p of mask (all nine for the full operator, bit 0 = self term alone,
     // bits 1..8 = the 8-point hopping term); stage s handles the s-th set bit
     const int npts = ALL ? 9 : __popc(mask);
+    const unsigned long long plist = ALL ? 0ull : coarse_point_list(mask);
     auto issue = [&](int s) {
-        const int p = ALL ? s : (int)__fns(mask, 0, s + 1);
+        const int p = ALL ? s : coarse_point(plist, s);
         const int slot = s % C::NSTAGE;
         unsigned char *dst = smem + (size_t)slot * C::STAGE_BYTES;
         mbar_expect_tx(&full[slot], C::STAGE_BYTES);

@@ -70,6 +70,16 @@ __device__ __forceinline__ int coarse_neighbour32(const CoarseSites &g, const Co
     const int d = p <= 4 ? (coord + 1 == ext ? -(ext - 1) : 1) : (coord == 0 ? ext - 1 : -1);
     return c.lex + d * stride;
 }
+// The stencil points selected by a mask as a list of 4-bit entries (s-th entry = the s-th set bit), made once per kernel:
+// __fns (n-th set bit) is a software loop, too slow for the thread that issues the copies of every stage.
+__device__ __forceinline__ unsigned long long coarse_point_list(unsigned mask) {
+    unsigned long long l = 0;
+    int n = 0;
+    for (int p = 0; p < 9; p++)
+        if ((mask >> p) & 1u) { l |= (unsigned long long)p << (4 * n); n++; }
+    return l;
+}
+__device__ __forceinline__ int coarse_point(unsigned long long list, int s) { return (int)((list >> (4 * s)) & 15ull); }
 #endif
 inline CoarseSites coarse_sites_full(const CoarseGeom &g) { return {g.X, g.Y, g.Z, g.T, 0, 0, g.nsites}; }
 inline CoarseSites coarse_sites_parity(const CoarseGeom &g, int parity) { return {g.X, g.Y, g.Z, g.T, 1, parity, g.nsites / 2}; }

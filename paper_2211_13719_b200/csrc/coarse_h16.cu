@@ -102,8 +102,17 @@ struct H16Cfg {
 // links16: [site][p][hi | lo][K chunk][row][8 fp16] (stacked A: [site][p][K chunk][row of hi or lo][8 fp16]); site_scale[site] = 1 / s_A; vec16: [site][K chunk][2 NT columns][8 fp16];
 // zeros: one K chunk of the B operand (2 NT x 16 bytes) of zeros;
 // colmax[n] = max |v| of RHS n (both written by the passes below); out: coarse vectors [site][component][RHS pair] float4.
-// ALL: the nine-point operator (mask ignored)
-template <int NB, int N, bool ALL>
+// CM: the point mask at compile time (0x1FF the nine-point operator, 0x1FE the hopping term: the argument is ignored, the loops over
+// the points unroll and every point index folds into the address arithmetic of the thread that issues the copies), or 0: the
+// argument `mask` at run time (any subset; the point list is unpacked once)
+__host__ __device__ constexpr int h16_nth_point(unsigned m, int n) {
+    int c = 0;
+    for (int p = 0; p < 9; p++)
+        if ((m >> p) & 1u) { if (c == n) return p; c++; }
+    return 0;
+}
+__host__ __device__ constexpr int h16_popc(unsigned m) { int c = 0; for (int p = 0; p < 9; p++) c += (m >> p) & 1u; return c; }
+template <int NB, int N, unsigned CM>
 __global__ void __launch_bounds__(H16Cfg<NB, N>::THREADS, 1)
 coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *__restrict__ links16, const float *__restrict__ site_scale,
                   const unsigned char *__restrict__ vec16, const unsigned char *__restrict__ zeros, const float *__restrict__ colmax,
@@ -136,8 +145,9 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
     const uint32_t tmem = *tslot;
 
     const long long nsites = sites.nout;       // output sites, enumerated by osite; the links of output site osite live at its lex
-    const int npts = ALL ? 9 : __popc(mask);
-    auto point = [&](int s) { return ALL ? s : (int)__fns(mask, 0, s + 1); };
+    const int npts = CM ? h16_popc(CM) : __popc(mask);
+    const unsigned long long plist = CM ? 0ull : coarse_point_list(mask);
+    auto point = [&](int s) { return CM ? h16_nth_point(CM, s) : coarse_point(plist, s); };
 
     if (warp == 0) {
         // ------------------------------------------------------------------ copy warp
@@ -147,12 +157,15 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
             for (long long site = blockIdx.x; site < nsites; site += gridDim.x) {
                 const CoarseSite32 sc = coarse_site32(sites, site);
                 const long long lex = sc.lex;
+#pragma unroll
                 for (int sp = 0; sp < npts; sp += C::PP) {
                     if (wrapped) mbar_wait(&empty[s], ph);
                     unsigned char *dst = smem + (size_t)s * C::STAGE;
                     const bool two = C::PP == 2 && sp + 1 < npts;
                     mbar_expect_tx(&full[s], (two ? 2 : 1) * (C::NA * C::A_HALF + C::B_COPY) + (C::PP == 2 && !two ? C::B_LBO : 0));
-                    for (int k = 0; k < (two ? 2 : 1); k++) {
+#pragma unroll
+                    for (int k = 0; k < C::PP; k++) {
+                        if (k == 1 && !two) break;
                         const int p = point(sp + k);
                         // vector index of the neighbour at stencil point p: 0 self, 1..4 = +x..+t, 5..8 = -x..-t (periodic)
                         long long nbr = coarse_neighbour32(sites, sc, p);
@@ -402,8 +415,9 @@ __global__ void h16_site_scale_kernel(float *__restrict__ site_scale, long long 
 template <int NB, int N>
 mrhs_status_t h16_prepare_t() {
     typedef H16Cfg<NB, N> C;
-    MRHS_CUDA(cudaFuncSetAttribute(coarse_h16_kernel<NB, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-    MRHS_CUDA(cudaFuncSetAttribute(coarse_h16_kernel<NB, N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_h16_kernel<NB, N, 0x1FFu>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_h16_kernel<NB, N, 0x1FEu>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    MRHS_CUDA(cudaFuncSetAttribute(coarse_h16_kernel<NB, N, 0u>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
     return MRHS_OK;
 }
 template <int NB, int N>
@@ -424,8 +438,9 @@ mrhs_status_t h16_launch_t(const CoarseSites &sites, int grid, unsigned mask, co
     cfg.numAttrs = 1;
     const unsigned char *l = (const unsigned char *)links16, *v = (const unsigned char *)vec16, *z = (const unsigned char *)zeros;
     float4 *o = (float4 *)out;
-    if (mask == 0x1FFu) MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, true>, sites, mask, l, site_scale, v, z, colmax, colmax_next, o));
-    else                MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, false>, sites, mask, l, site_scale, v, z, colmax, colmax_next, o));
+    if (mask == 0x1FFu)      MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, 0x1FFu>, sites, mask, l, site_scale, v, z, colmax, colmax_next, o));
+    else if (mask == 0x1FEu) MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, 0x1FEu>, sites, mask, l, site_scale, v, z, colmax, colmax_next, o));
+    else                     MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, 0u>, sites, mask, l, site_scale, v, z, colmax, colmax_next, o));
     return MRHS_OK;
 }
 

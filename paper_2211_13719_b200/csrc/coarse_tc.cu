@@ -165,7 +165,8 @@ coarse_tc_kernel(const CoarseSites sites, unsigned mask, const float4 *__restric
     constexpr int kPfAhead = AHEAD ? 3 : 2;
     // the stencil points of this apply: bit p of mask; stage s of a site handles the s-th set bit
     const int npts = ALL ? 9 : __popc(mask);
-    auto point = [&](int s) { return ALL ? s : (int)__fns(mask, 0, s + 1); };
+    const unsigned long long plist = ALL ? 0ull : coarse_point_list(mask);
+    auto point = [&](int s) { return ALL ? s : coarse_point(plist, s); };
     // site coordinates once per site (this site and the block's next one), neighbours from them without divisions
     CoarseSite32 cur = coarse_site32(sites, blockIdx.x), nxt = cur;
     if (AHEAD && (long long)blockIdx.x < nsites) load_stage(cur, point(0));
