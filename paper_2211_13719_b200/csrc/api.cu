@@ -90,8 +90,7 @@ struct mrhs_coarse {
     cudaStream_t st;
     float2 *links;                 // math_mode 0: [site][p][col][row] complex; math_mode 1 / 2: the tensor-core orders (coarse.cuh)
     int tc_grid;                   // persistent grid of the tensor-core kernels
-    float *site_scale;             // math_mode 2: 1 / scale of the site's matrices, then 2 x 128 floats for the column maxima of an apply (used alternately)
-    unsigned h16_calls;            // math_mode 2: applies so far (selects the column-maximum buffer)
+    float *site_scale;             // math_mode 2: 1 / scale of the site's matrices, then 128 floats for the column maxima of an apply and the block counter of its stencil kernel (zero between applies)
     void *vec16;                   // math_mode 2: the split input vector of an apply
     HostPipe pipe;
 };
@@ -747,11 +746,8 @@ mrhs_status_t mrhs_coarse_apply_points(mrhs_coarse_t *h, const void *d_in, void 
     MRHS_REQUIRE(aligned16(d_in) && aligned16(d_out), "coarse apply: buffers must be 16-byte aligned");
     MRHS_REQUIRE(point_mask > 0 && point_mask <= 0x1FF, "coarse apply: point_mask must select at least one of the nine stencil points");
     const CoarseSites sites = coarse_sites_full(h->g);
-    if (h->mode == 2) {
-        float *cm = h->site_scale + h->g.nsites;
-        const unsigned k = h->h16_calls++ & 1u;
-        return launch_coarse_h16(h->g, sites, h->tc_grid, (unsigned)point_mask, h->links, h->site_scale, d_in, h->vec16, cm + 128 * k, cm + 128 * (k ^ 1u), d_out, h->st);
-    }
+    if (h->mode == 2)
+        return launch_coarse_h16(h->g, sites, h->tc_grid, (unsigned)point_mask, h->links, h->site_scale, d_in, h->vec16, h->site_scale + h->g.nsites, d_out, h->st);
     if (h->mode == 1) return launch_coarse_tc(h->g, sites, h->tc_grid, (unsigned)point_mask, (const float *)h->links, d_in, d_out, h->st);
     return launch_coarse_fma(h->g, sites, (unsigned)point_mask, h->links, d_in, d_out, h->st);
 }
@@ -768,11 +764,8 @@ mrhs_status_t mrhs_coarse_meooe(mrhs_coarse_t *h, const void *d_in, void *d_out,
     MRHS_REQUIRE(!((h->g.X | h->g.Y | h->g.Z | h->g.T) & 1), "coarse meooe: checkerboarded coarse fields need even extents");
     // the 8-point hopping term at the sites of one parity: same kernels, same link field, parity site map
     const CoarseSites sites = coarse_sites_parity(h->g, out_parity);
-    if (h->mode == 2) {
-        float *cm = h->site_scale + h->g.nsites;
-        const unsigned k = h->h16_calls++ & 1u;
-        return launch_coarse_h16(h->g, sites, h->tc_grid, MRHS_COARSE_HOP, h->links, h->site_scale, d_in, h->vec16, cm + 128 * k, cm + 128 * (k ^ 1u), d_out, h->st);
-    }
+    if (h->mode == 2)
+        return launch_coarse_h16(h->g, sites, h->tc_grid, MRHS_COARSE_HOP, h->links, h->site_scale, d_in, h->vec16, h->site_scale + h->g.nsites, d_out, h->st);
     if (h->mode == 1) return launch_coarse_tc(h->g, sites, h->tc_grid, MRHS_COARSE_HOP, (const float *)h->links, d_in, d_out, h->st);
     return launch_coarse_fma(h->g, sites, MRHS_COARSE_HOP, h->links, d_in, d_out, h->st);
 }

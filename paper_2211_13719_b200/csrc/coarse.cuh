@@ -106,13 +106,13 @@ mrhs_status_t launch_coarse_tc(const CoarseGeom &g, const CoarseSites &sites, in
 
 // ---- tensor-core variant 2 (row a6, math_mode 2): tcgen05 kind::f16 on operands split into fp16 hi + lo after a power-of-two
 // scaling (coarse_h16.cu).  The links are split at create time (same bytes as fp32) with one scale per site; the input vector is
-// split per apply into a scratch image of coarse_h16_vec_bytes() bytes (cleared once by the caller: its tail is a chunk of zeros), with one scale per right-hand side (d_colmax: 128 floats that are zero on entry; the apply clears
-// d_colmax_next, the buffer of the next apply on this handle: the caller alternates between two).
+// split per apply into a scratch image of coarse_h16_vec_bytes() bytes (cleared once by the caller: its tail is a chunk of zeros), with one scale per right-hand side (d_colmax: 128 floats and one unsigned counter behind
+// them, all zero on entry and zero again when the apply has finished).
 bool coarse_h16_supported(int nb, int nrhs);
 size_t coarse_h16_vec_bytes(const CoarseGeom &g);
 mrhs_status_t pack_coarse_links_h16(const CoarseGeom &g, const float2 *d_canonical, void *d_links16, float *d_site_scale, cudaStream_t st);
 mrhs_status_t coarse_h16_prepare(const CoarseGeom &g, int *grid);
 mrhs_status_t launch_coarse_h16(const CoarseGeom &g, const CoarseSites &sites, int grid, unsigned mask, const void *d_links16, const float *d_site_scale,
-                                const void *d_in, void *d_vec16, float *d_colmax, float *d_colmax_next, void *d_out, cudaStream_t st);
+                                const void *d_in, void *d_vec16, float *d_colmax, void *d_out, cudaStream_t st);
 
 }  // namespace mrhs

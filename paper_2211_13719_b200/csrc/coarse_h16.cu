@@ -101,7 +101,7 @@ struct H16Cfg {
 
 // links16: [site][p][hi | lo][K chunk][row][8 fp16] (stacked A: [site][p][K chunk][row of hi or lo][8 fp16]); site_scale[site] = 1 / s_A; vec16: [site][K chunk][2 NT columns][8 fp16];
 // zeros: one K chunk of the B operand (2 NT x 16 bytes) of zeros;
-// colmax[n] = max |v| of RHS n (both written by the passes below); out: coarse vectors [site][component][RHS pair] float4.
+// colmax[n] = max |v| of RHS n (both written by the passes below; 128 floats, cleared again by this kernel), blocks_done: a zero counter; out: coarse vectors [site][component][RHS pair] float4.
 // CM: the point mask at compile time (0x1FF the nine-point operator, 0x1FE the hopping term: the argument is ignored, the loops over
 // the points unroll and every point index folds into the address arithmetic of the thread that issues the copies), or 0: the
 // argument `mask` at run time (any subset; the point list is unpacked once)
@@ -115,8 +115,8 @@ __host__ __device__ constexpr int h16_popc(unsigned m) { int c = 0; for (int p =
 template <int NB, int N, unsigned CM>
 __global__ void __launch_bounds__(H16Cfg<NB, N>::THREADS, 1)
 coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *__restrict__ links16, const float *__restrict__ site_scale,
-                  const unsigned char *__restrict__ vec16, const unsigned char *__restrict__ zeros, const float *__restrict__ colmax,
-                  float *__restrict__ colmax_next, float4 *__restrict__ out) {
+                  const unsigned char *__restrict__ vec16, const unsigned char *__restrict__ zeros, float *colmax,
+                  unsigned *blocks_done, float4 *__restrict__ out) {
     typedef H16Cfg<NB, N> C;
     extern __shared__ __align__(128) unsigned char smem[];
     float *cinv = reinterpret_cast<float *>(smem + C::NSTAGE * C::STAGE);
@@ -134,14 +134,21 @@ coarse_h16_kernel(const CoarseSites sites, unsigned mask, const unsigned char *_
     for (int i = tid; i < C::NSTAGE * C::STAGE / 16; i += C::THREADS) reinterpret_cast<float4 *>(smem)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     fence_async_smem();
     if (warp == 0) tmem_alloc<C::TMEM_COLS>(tslot);
-    // the column maxima of the NEXT apply start from zero (the handle alternates between two buffers, so nobody reads this one now)
-    if (blockIdx.x == 0 && tid < 128) colmax_next[tid] = 0.f;
     // Launched with programmatic stream serialization: everything above overlaps the tail of the split pass; what follows reads its output
     grid_dependency_wait();
     for (int n = tid; n < N; n += C::THREADS) cinv[n] = ldexpf(1.f, -scale_exp(colmax[n]));
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    // The column maxima must be zero again when the next apply starts: the last block to have read them clears them (and the
+    // counter), so every apply leaves the handle as it found it (no memset launch, and safe under graph replay).
+    if (tid == 64) {
+        __threadfence();
+        if (atomicAdd(blocks_done, 1u) == gridDim.x - 1) {
+            for (int n = 0; n < 128; n++) colmax[n] = 0.f;
+            *blocks_done = 0u;
+        }
+    }
     const uint32_t tmem = *tslot;
 
     const long long nsites = sites.nout;       // output sites, enumerated by osite; the links of output site osite live at its lex
@@ -422,7 +429,7 @@ mrhs_status_t h16_prepare_t() {
 }
 template <int NB, int N>
 mrhs_status_t h16_launch_t(const CoarseSites &sites, int grid, unsigned mask, const void *links16, const float *site_scale, const void *vec16,
-                           const void *zeros, const float *colmax, float *colmax_next, void *out, cudaStream_t st) {
+                           const void *zeros, float *colmax, unsigned *blocks_done, void *out, cudaStream_t st) {
     typedef H16Cfg<NB, N> C;
     if ((long long)grid > sites.nout) grid = (int)sites.nout;
     // programmatic stream serialization: the kernel's set-up (shared memory, barriers, tensor memory) runs under the tail of the split pass
@@ -438,9 +445,9 @@ mrhs_status_t h16_launch_t(const CoarseSites &sites, int grid, unsigned mask, co
     cfg.numAttrs = 1;
     const unsigned char *l = (const unsigned char *)links16, *v = (const unsigned char *)vec16, *z = (const unsigned char *)zeros;
     float4 *o = (float4 *)out;
-    if (mask == 0x1FFu)      MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, 0x1FFu>, sites, mask, l, site_scale, v, z, colmax, colmax_next, o));
-    else if (mask == 0x1FEu) MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, 0x1FEu>, sites, mask, l, site_scale, v, z, colmax, colmax_next, o));
-    else                     MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, 0u>, sites, mask, l, site_scale, v, z, colmax, colmax_next, o));
+    if (mask == 0x1FFu)      MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, 0x1FFu>, sites, mask, l, site_scale, v, z, colmax, blocks_done, o));
+    else if (mask == 0x1FEu) MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, 0x1FEu>, sites, mask, l, site_scale, v, z, colmax, blocks_done, o));
+    else                     MRHS_CUDA(cudaLaunchKernelEx(&cfg, coarse_h16_kernel<NB, N, 0u>, sites, mask, l, site_scale, v, z, colmax, blocks_done, o));
     return MRHS_OK;
 }
 
@@ -494,11 +501,11 @@ mrhs_status_t pack_coarse_links_h16(const CoarseGeom &g, const float2 *d_canonic
 }
 
 mrhs_status_t launch_coarse_h16(const CoarseGeom &g, const CoarseSites &sites, int grid, unsigned mask, const void *d_links16, const float *d_site_scale,
-                                const void *d_in, void *d_vec16, float *d_colmax, float *d_colmax_next, void *d_out, cudaStream_t st) {
+                                const void *d_in, void *d_vec16, float *d_colmax, void *d_out, cudaStream_t st) {
     const int np = g.N / 2, nt = (2 * g.N + 15) / 16 * 16;
     const long long nin = sites.cb ? g.nsites / 2 : g.nsites;      // sites of the input vector
     const long long total = nin * g.nb * np;
-    // d_colmax is zero: cleared at create or by the stencil kernel of the apply before the last (two buffers, used alternately)
+    // d_colmax (128 floats + the block counter behind them) is zero: cleared at create and by the stencil kernel of every apply
     {
         // a multiple of 3 blocks of 256 threads: the thread count is a multiple of every supported N_rhs / 2
         long long blocks = (total + 255) / 256;
@@ -521,7 +528,7 @@ mrhs_status_t launch_coarse_h16(const CoarseGeom &g, const CoarseSites &sites, i
         MRHS_CUDA(cudaLaunchKernelEx(&cfg, h16_split_vec_kernel, (const float4 *)d_in, nin, g.nb, np, nt, (const float *)d_colmax, (uint4 *)d_vec16));
     }
     const void *zeros = (const unsigned char *)d_vec16 + h16_image_bytes(g);
-#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return h16_launch_t<NB, NN>(sites, grid, mask, d_links16, d_site_scale, d_vec16, zeros, d_colmax, d_colmax_next, d_out, st);
+#define MRHS_CASE(NB, NN) if (g.nb == NB && g.N == NN) return h16_launch_t<NB, NN>(sites, grid, mask, d_links16, d_site_scale, d_vec16, zeros, d_colmax, reinterpret_cast<unsigned *>(d_colmax + 128), d_out, st);
     MRHS_H16_N_LIST(MRHS_CASE, 24)
     MRHS_H16_N_LIST(MRHS_CASE, 40)
 #undef MRHS_CASE

@@ -167,6 +167,13 @@ def test_coarse_fp16_split_scales(cdims, nb, nrhs):
     keep = [n for n in range(nrhs) if n != 3]
     err = rel_l2_per_rhs(got[..., keep], want[..., keep])
     assert err.max() < TOL, err
+    # the column maxima of an apply do not leak into the next one on the handle: a much smaller input afterwards keeps its accuracy
+    # (with stale maxima its fp16 parts would underflow to zero), and so does the first input once more
+    small = (v * np.float32(1e-20)).astype(np.complex64)
+    err = rel_l2_per_rhs(gpu_coarse(c, small)[..., keep], oracle.coarse_apply(cdims, A, small)[..., keep])
+    assert err.max() < TOL, err
+    err = rel_l2_per_rhs(gpu_coarse(c, v)[..., keep], want[..., keep])
+    assert err.max() < TOL, err
     c.close()
 
 
