@@ -55,7 +55,7 @@ SEED = 5
 CPU_FINE_DIMS = [24, 24, 24, 24]
 CPU_COARSE_DIMS = [6, 6, 6, 32]
 CPU_SAMPLE = ("fp64 oracle, OpenMP over sites: the step's fine operators (D_hop, M_eooe x2, M_ooee, M_eooe M_ooee M_eooe) full-field on "
-              "config 2's 24^4 lattice at N_rhs=12 (1/16 of the 48^4 sites of the GPU step) + config 4's coarse apply in full (6^3x32, nbasis 40)")
+              "config 2's 24^4 lattice at N_rhs=12 (1/16 of the 48^4 sites of the GPU step) + config 4's coarse apply in full (6^3x32, nbasis 40), three times as in the GPU step (once per math mode)")
 
 
 def coarse_flops(nb):
@@ -240,7 +240,7 @@ def run_reference(args):
 
 def workload_config():
     return {"workload": "config 5 (48^4 fine, N_rhs=12, mass -0.05, c_sw 1.5: D_hop, M_eooe x2, M_ooee, Schur sequence) "
-                        "+ config 4 (6^3x32 coarse, nbasis 40, N_rhs=12: 9-point apply, FP32 FMA and tensor-core variants)",
+                        "+ config 4 (6^3x32 coarse, nbasis 40, N_rhs=12: 9-point apply in the three math modes: FP32 FMA, tf32 split, fp16 split)",
             "fine_dims": FINE_DIMS, "coarse_dims": COARSE_DIMS, "nbasis": NBASIS, "n_rhs": NRHS,
             "precision": "complex64 fields, fp32 FMA",
             "l2": "every launch touches >= 0.85 GB, far above the 126 MB L2; no flush between iterations",
