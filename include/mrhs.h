@@ -153,8 +153,8 @@ mrhs_status_t mrhs_wilson_apply_dag(mrhs_wilson_t *h, const void *d_in, void *d_
 /* The even-odd preconditioned operator (Schur complement of M on the even sites; PAPER.md:43,
  * :53 "precomputed clover term"; reading S6 with M_eo = -M_eooe / 2):
  *   out = S in,  S = M_ee - M_eo M_oo^-1 M_oe = C_e - M_eooe(e<-o) C_o^-1 M_eooe(o<-e) / 4,    dagger != 0: S^+ (daggered hops).
- * d_in, d_out: native EVEN fields; d_tmp: native ODD scratch field (overwritten); all three distinct.  Sweep kernel: two
- * launches (C_o^-1 rides in the first hop's epilogue, C_e in - ... / 4 in the second's); gather kernel: four. */
+ * d_in, d_out: native EVEN fields; d_tmp: native ODD scratch field (overwritten); all three distinct.  Sweep kernel: three
+ * launches (C_o^-1 rides in the first hop's epilogue; plain hop; clover kernel forming C_e in - ... / 4); gather kernel: four. */
 mrhs_status_t mrhs_schur_apply(mrhs_wilson_t *h, const void *d_in, void *d_tmp, void *d_out, int dagger);
 
 /* Copy the handle's native clover blocks back in canonical form

@@ -237,3 +237,50 @@ def test_config5_full_matrix_sampled_sites(config5, kernel):
     want = oracle.mooee(C, psi[t_lex].cpu().numpy()) - 0.5 * oracle.dhop_sites(links, nbrs)
     err = rel_l2_per_rhs(got, want)
     assert err.max() < TOL, err
+
+
+def test_config5_sweep_kernels_repeat_bitwise_and_match_gather_on_the_whole_field(config5):
+    """Sampled sites cannot see a race that spoils a few tile rows per launch (one did: the sweep kernel's `C aux - H / 4`
+    epilogue at 48^4, N_rhs = 12, 0.05 % of the elements, different ones in every call).  Every operator of the sweep path is
+    therefore run twice on NaN-filled outputs and must repeat bit for bit, and must agree on the WHOLE field with the gather
+    kernels (an independent kernel family, itself checked against the oracle above) to fp32 rounding."""
+    U, psi, w = config5
+    if w.nrhs % 2:
+        pytest.skip("the sweep kernel needs an even N_rhs")
+    if w.nrhs > 12:
+        pytest.skip("N_rhs = 24: the fields of both kernel families do not fit beside each other")
+    d_in = w.import_field(psi, mrhs.FULL)
+    ie, io = w.empty(mrhs.EVEN), w.empty(mrhs.ODD)
+    mrhs.cb_split(DIMS, 12, w.nrhs, d_in, ie, io)
+    full, t0, t1 = w.empty(mrhs.FULL), w.empty(mrhs.ODD), w.empty(mrhs.ODD)
+    oe, oo = w.empty(mrhs.EVEN), w.empty(mrhs.ODD)
+    ops = [
+        ("dhop", 0, lambda: w.dhop(d_in, full), full),
+        ("dhop_dag", 0, lambda: w.dhop_dag(d_in, full), full),
+        ("meooe_dag odd", 1, lambda: w.meooe_dag(ie, oo, mrhs.ODD), oo),
+        ("wilson_apply", 0, lambda: w.apply(d_in, full), full),
+        ("meooe odd", 1, lambda: w.meooe(ie, oo, mrhs.ODD), oo),
+        ("meooe even", 1, lambda: w.meooe(io, oe, mrhs.EVEN), oe),
+        ("meooe_mooee odd", 1, lambda: w.meooe_mooee(ie, oo, mrhs.ODD), oo),
+        ("meooe_mooee even", 1, lambda: w.meooe_mooee(io, oe, mrhs.EVEN), oe),
+        ("meooe_mooee_inv odd", 1, lambda: w.meooe_mooee_inv(ie, oo, mrhs.ODD), oo),
+        ("schur_sequence", 1, lambda: w.schur_sequence(ie, t0, t1, oe), oe),
+        ("schur_apply", 1, lambda: w.schur_apply(ie, t0, oe), oe),
+        ("schur_apply dagger", 1, lambda: w.schur_apply(ie, t0, oe, True), oe),
+    ]
+    for name, which, run, buf in ops:
+        res = []
+        for kernel in (mrhs.HOP_SWEEP, mrhs.HOP_SWEEP, mrhs.HOP_SWEEP, mrhs.HOP_GATHER):
+            mrhs.wilson_set_hop_kernel(w.h, which, kernel)
+            buf.fill_(float("nan"))
+            run()
+            torch.cuda.synchronize()
+            res.append(buf.clone())
+        assert not bool(torch.isnan(res[0]).any()), name
+        assert torch.equal(res[0], res[1]) and torch.equal(res[0], res[2]), "%s: the sweep kernel does not repeat bit for bit" % name
+        scale = float(res[3].abs().max())
+        diff = float((res[0] - res[3]).abs().max())
+        assert diff < 2e-5 * scale, "%s: sweep and gather kernels differ on the whole field: %g of %g" % (name, diff, scale)
+        del res
+    mrhs.wilson_set_hop_kernel(w.h, 0, mrhs.HOP_SWEEP)
+    mrhs.wilson_set_hop_kernel(w.h, 1, mrhs.HOP_SWEEP)
