@@ -247,8 +247,7 @@ def test_config5_sweep_kernels_repeat_bitwise_and_match_gather_on_the_whole_fiel
     U, psi, w = config5
     if w.nrhs % 2:
         pytest.skip("the sweep kernel needs an even N_rhs")
-    if w.nrhs > 12:
-        pytest.skip("N_rhs = 24: the fields of both kernel families do not fit beside each other")
+    with_gather = w.nrhs <= 12       # N_rhs = 24: repeatability only (keeps the device memory of the test below 120 GB)
     d_in = w.import_field(psi, mrhs.FULL)
     ie, io = w.empty(mrhs.EVEN), w.empty(mrhs.ODD)
     mrhs.cb_split(DIMS, 12, w.nrhs, d_in, ie, io)
@@ -270,7 +269,7 @@ def test_config5_sweep_kernels_repeat_bitwise_and_match_gather_on_the_whole_fiel
     ]
     for name, which, run, buf in ops:
         res = []
-        for kernel in (mrhs.HOP_SWEEP, mrhs.HOP_SWEEP, mrhs.HOP_SWEEP, mrhs.HOP_GATHER):
+        for kernel in (mrhs.HOP_SWEEP, mrhs.HOP_SWEEP, mrhs.HOP_SWEEP) + ((mrhs.HOP_GATHER,) if with_gather else ()):
             mrhs.wilson_set_hop_kernel(w.h, which, kernel)
             buf.fill_(float("nan"))
             run()
@@ -278,9 +277,10 @@ def test_config5_sweep_kernels_repeat_bitwise_and_match_gather_on_the_whole_fiel
             res.append(buf.clone())
         assert not bool(torch.isnan(res[0]).any()), name
         assert torch.equal(res[0], res[1]) and torch.equal(res[0], res[2]), "%s: the sweep kernel does not repeat bit for bit" % name
-        scale = float(res[3].abs().max())
-        diff = float((res[0] - res[3]).abs().max())
-        assert diff < 2e-5 * scale, "%s: sweep and gather kernels differ on the whole field: %g of %g" % (name, diff, scale)
+        if with_gather:
+            scale = float(res[3].abs().max())
+            diff = float((res[0] - res[3]).abs().max())
+            assert diff < 2e-5 * scale, "%s: sweep and gather kernels differ on the whole field: %g of %g" % (name, diff, scale)
         del res
     mrhs.wilson_set_hop_kernel(w.h, 0, mrhs.HOP_SWEEP)
     mrhs.wilson_set_hop_kernel(w.h, 1, mrhs.HOP_SWEEP)
